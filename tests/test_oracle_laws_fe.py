@@ -1,0 +1,301 @@
+"""Pins for the oracle's constitutive laws, FE nodal force, force points and projection (no GPU).
+
+SURVEY.md §8(c) pins 1-4, 11 and readings A2, A3, A6, A9-A13: closed-form stresses, P = dPsi/dF
+and B = -dE/dx by central differences, objectivity, HO -> neo-Hookean reduction, fibre terms
+switching off in compression, zero force under rigid motion, zero net force/torque, patch test,
+single-cube closed form, lumped weights summing to the volume, prolong/restrict transposes.
+"""
+import os
+
+import numpy as np
+import pytest
+
+from helpers import distorted_block, rotation
+from paper_2503_22695_b200 import workloads as W
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+NH = W.material(W.LAW_NEOHOOKEAN, a=1e4, kappa=1e6)
+HO = W.material(W.LAW_HO, **W.HO_LV)
+# PAPER.md Table 2 (L351-366) parameter set, dyn/cm^2 -- a free extra test vector (A8)
+HO_T2 = W.material(W.LAW_HO, a=2244.87, b=1.6215, af=24267.0, bf=1.8268, as_=5562.38, bs=0.7746,
+                   afs=3905.16, bfs=1.695, kappa=1e6)
+
+
+def _fd_P(orc, mat, F, ef, es, eps=1e-6):
+    P = np.zeros((3, 3))
+    for c in range(3):
+        for K in range(3):
+            Fp, Fm = F.copy(), F.copy()
+            Fp[c, K] += eps
+            Fm[c, K] -= eps
+            P[c, K] = (orc.pk1(mat, Fp, ef, es)[1] - orc.pk1(mat, Fm, ef, es)[1]) / (2 * eps)
+    return P
+
+
+def test_neo_hookean_closed_forms(orc):
+    rows = {}
+    for line in open(os.path.join(GOLD, "nh_closed_form.txt")):
+        if not line.startswith("#"):
+            p = line.split()
+            rows[p[0]] = list(map(float, p[1:]))
+    l = 1.2
+    P, psi = orc.pk1(W.material(0, a=1e4, kappa=123.0), np.diag([l, l ** -0.5, l ** -0.5]))
+    assert np.allclose(np.diag(P), rows["isochoric_uniaxial_l1.2_mu1e4"], rtol=1e-13)
+    assert np.max(np.abs(P - np.diag(np.diag(P)))) < 1e-9
+    assert abs(psi - 0.5e4 * (l * l + 2 / l - 3)) < 1e-10 * psi          # mu/2 (Ibar1 - 3), J = 1
+    P, psi = orc.pk1(NH, np.diag([1.1, 1.0, 1.0]))
+    assert np.allclose(np.diag(P), rows["diag_1.1_1_1_mu1e4_kappa1e6"], rtol=1e-13)
+    # pure dilation: Ibar1 = 3 -> only U(J) = kappa/2 (ln J)^2; P = kappa lnJ / lam I
+    lam = 1.05
+    P, psi = orc.pk1(NH, lam * np.eye(3))
+    assert abs(psi - 0.5e6 * (3 * np.log(lam)) ** 2) < 1e-12 * psi
+    assert np.allclose(P, 1e6 * 3 * np.log(lam) / lam * np.eye(3), rtol=1e-12, atol=1e-7)
+    # identity is stress free
+    P, psi = orc.pk1(NH, np.eye(3))
+    assert np.max(np.abs(P)) < 1e-9 and abs(psi) < 1e-12
+
+
+def test_ho_closed_forms(orc):
+    m = HO
+    ex, ey = np.array([1.0, 0, 0]), np.array([0, 1.0, 0])
+    # isochoric uniaxial stretch along the fibre: I4f = l^2, I4s = 1/l < 1 (switched off, A9), I8 = 0
+    l = 1.15
+    F = np.diag([l, l ** -0.5, l ** -0.5])
+    I1 = l * l + 2 / l
+    P, psi = orc.pk1(m, F, ex, ey)
+    e_iso = np.exp(m["b"] * (I1 - 3))
+    e_f = np.exp(m["bf"] * (l * l - 1) ** 2)
+    assert abs(psi - (m["a"] / (2 * m["b"]) * e_iso + m["af"] / (2 * m["bf"]) * (e_f - 1))) < 1e-14 * psi
+    P11 = m["a"] * e_iso * (l - I1 / (3 * l)) + 2 * m["af"] * (l * l - 1) * e_f * l
+    P22 = m["a"] * e_iso * (l ** -0.5 - I1 / 3 * l ** 0.5)
+    assert np.allclose(np.diag(P), [P11, P22, P22], rtol=1e-13)
+    # simple shear F = I + g ex (x) ey: F ef = ex, F es = g ex + ey -> I8 = g, I4s = 1 + g^2, J = 1
+    gam = 0.3
+    F = np.eye(3)
+    F[0, 1] = gam
+    P, psi = orc.pk1(m, F, ex, ey)
+    I1 = 3 + gam * gam
+    e_iso = np.exp(m["b"] * gam * gam)
+    e_s = np.exp(m["bs"] * gam ** 4)
+    e_fs = np.exp(m["bfs"] * gam * gam)
+    psi_exp = (m["a"] / (2 * m["b"]) * e_iso + m["as_"] / (2 * m["bs"]) * (e_s - 1)
+               + m["afs"] / (2 * m["bfs"]) * (e_fs - 1))
+    assert abs(psi - psi_exp) < 1e-14 * psi
+    Finv_T = np.eye(3)
+    Finv_T[1, 0] = -gam
+    Fs = np.array([gam, 1.0, 0])
+    P_exp = (m["a"] * e_iso * (F - I1 / 3 * Finv_T) + 2 * m["as_"] * gam * gam * e_s * np.outer(Fs, ey)
+             + m["afs"] * gam * e_fs * (np.outer(ex, ey) + np.outer(Fs, ex)))
+    assert np.allclose(P, P_exp, rtol=1e-13, atol=1e-15)
+
+
+@pytest.mark.parametrize("mat", [NH, HO, HO_T2], ids=["NH", "HO", "HO_table2"])
+def test_P_is_dPsi_dF_and_objective(orc, mat):
+    rng = np.random.default_rng(0)
+    for trial in range(6):
+        F = np.eye(3) + 0.25 * rng.normal(size=(3, 3))
+        if np.linalg.det(F) < 0.3:
+            continue
+        ef = rng.normal(size=3)
+        ef /= np.linalg.norm(ef)
+        es = np.cross(ef, rng.normal(size=3))
+        es /= np.linalg.norm(es)
+        P, psi = orc.pk1(mat, F, ef, es)
+        Pfd = _fd_P(orc, mat, F, ef, es)
+        assert np.max(np.abs(P - Pfd)) < 2e-8 * np.max(np.abs(P)), trial        # A2, A3
+        # P F^T symmetric (Cauchy stress symmetric; fails for the cross term as printed, A3)
+        S = P @ F.T
+        assert np.max(np.abs(S - S.T)) < 1e-13 * np.max(np.abs(S))
+        # spatial objectivity: Psi(QF) = Psi(F), P(QF) = Q P(F)
+        Q = rotation(trial)
+        Pq, psiq = orc.pk1(mat, Q @ F, ef, es)
+        assert abs(psiq - psi) < 1e-13 * abs(psi)
+        assert np.max(np.abs(Pq - Q @ P)) < 1e-12 * np.max(np.abs(P))
+        # material frame (A11): rotating F and the fibres together leaves Psi unchanged
+        R = rotation(trial + 100)
+        _, psir = orc.pk1(mat, F @ R.T, R @ ef, R @ es)
+        assert abs(psir - psi) < 1e-13 * abs(psi)
+
+
+def test_ho_reduces_to_neo_hookean_and_compression_switch(orc):
+    rng = np.random.default_rng(1)
+    F = np.eye(3) + 0.2 * rng.normal(size=(3, 3))
+    ef, es = np.array([0, 0, 1.0]), np.array([1.0, 0, 0])
+    # A6: HO with b=0 and no fibre constants == NH
+    P1, w1 = orc.pk1(W.material(W.LAW_HO, a=1e4, b=0.0, kappa=1e6), F, ef, es)
+    P0, w0 = orc.pk1(NH, F)
+    assert np.array_equal(P1, P0) and w1 == w0
+    # b -> 0 limit is continuous
+    P2, _ = orc.pk1(W.material(W.LAW_HO, a=1e4, b=1e-9, kappa=1e6), F, ef, es)
+    assert np.max(np.abs(P2 - P0)) < 1e-7 * np.max(np.abs(P0))
+    # A9: fibres in compression (I4 < 1) contribute exactly nothing
+    Fc = np.diag([1.3, 1.0, 0.7])                    # ef = ez compressed, es = ex stretched
+    m_f = W.material(W.LAW_HO, a=0.24, b=5.08, af=1.46, bf=4.15, kappa=1e3)
+    m_0 = W.material(W.LAW_HO, a=0.24, b=5.08, kappa=1e3)
+    Pf, wf = orc.pk1(m_f, Fc, ef, es)
+    Pn, wn = orc.pk1(m_0, Fc, ef, es)
+    assert np.array_equal(Pf, Pn) and wf == wn
+    # inverted element is an error (A10)
+    with pytest.raises(ValueError):
+        orc.pk1(NH, np.diag([1.0, 1.0, -1.0]))
+
+
+def test_single_cube_element_closed_form(orc):
+    # one unit-cube element under homogeneous x = F0 X: B_a,c = -sum_I P_cI xi_a,I / 4
+    conn = np.arange(8, dtype=np.int32).reshape(1, 8)
+    X = np.array([[a & 1, (a >> 1) & 1, (a >> 2) & 1] for a in range(8)], dtype=np.float64).T
+    F0 = np.array([[1.1, 0.3, 0.0], [0.0, 0.9, -0.2], [0.1, 0.0, 1.05]])
+    x = F0 @ X + np.array([[0.3], [0.1], [-0.2]])
+    ef, es = np.array([0.6, 0.8, 0.0]), np.array([-0.8, 0.6, 0.0])
+    fib = np.concatenate([ef, es]).reshape(6, 1)
+    for mat in (NH, HO):
+        r = orc.fe_force(conn, X, x, fib, np.zeros(1, np.int32), [mat])
+        P, psi = orc.pk1(mat, F0, ef, es)
+        xi = 2 * X - 1
+        Bexp = -(P @ xi) / 4
+        assert np.max(np.abs(r["B"] - Bexp)) < 1e-13 * np.max(np.abs(Bexp))
+        assert abs(r["energy"] - psi) < 1e-13 * abs(psi)
+        assert abs(r["minJ"] - np.linalg.det(F0)) < 1e-14
+
+
+@pytest.mark.parametrize("mat", [NH, HO], ids=["NH", "HO"])
+def test_force_is_minus_energy_gradient(orc, mat):
+    # pin 1: B = -dE/dx by central differences on a distorted mesh
+    conn, X, x, fib = distorted_block(3, 3, 2, seed=1)
+    mid = np.zeros(conn.shape[0], np.int32)
+    B = orc.fe_force(conn, X, x, fib, mid, [mat])["B"]
+    d = 0.1 * 1e-6
+    rng = np.random.default_rng(0)
+    nn = X.shape[1]
+    worst = 0.0
+    for _ in range(25):
+        c, n = int(rng.integers(3)), int(rng.integers(nn))
+        xp_, xm_ = x.copy(), x.copy()
+        xp_[c, n] += d
+        xm_[c, n] -= d
+        Ep = orc.fe_force(conn, X, xp_, fib, mid, [mat])["energy"]
+        Em = orc.fe_force(conn, X, xm_, fib, mid, [mat])["energy"]
+        fd = -(Ep - Em) / (2 * d)
+        worst = max(worst, abs(fd - B[c, n]) / np.max(np.abs(B)))
+    assert worst < 5e-8, worst
+
+
+def test_rigid_motion_balance_and_patch(orc):
+    conn, X, x, fib = distorted_block(4, 3, 3, seed=2)
+    ne, nn = conn.shape[0], X.shape[1]
+    mid = np.zeros(ne, np.int32)
+    h = 0.1
+    for mat in (NH, HO):
+        kappa = mat["kappa"]
+        # pin 2: rigid translation + rotation of the reference -> no force
+        Q = rotation(5)
+        xr = Q @ X + np.array([[0.4], [-0.2], [0.7]])
+        # fibres are material vectors, they do not rotate with the body
+        B = orc.fe_force(conn, X, xr, fib, mid, [mat])["B"]
+        assert np.max(np.abs(B)) < 1e-12 * kappa * h * h
+        # zero net force and torque for ANY deformation (internal forces)
+        B = orc.fe_force(conn, X, x, fib, mid, [mat])["B"]
+        scale = np.abs(B).sum()
+        assert np.max(np.abs(B.sum(axis=1))) < 1e-14 * scale
+        tq = np.cross(x.T, B.T).sum(axis=0)
+        assert np.max(np.abs(tq)) < 1e-14 * scale
+    # pin 4 (A12): homogeneous x = F0 X on a distorted mesh, homogeneous material (constant fibres)
+    # -> interior nodal forces vanish
+    F0 = np.array([[1.2, 0.1, 0.0], [0.05, 0.95, 0.1], [0.0, -0.1, 1.1]])
+    fibc = np.tile(np.array([[0.6], [0.0], [0.8], [0.0], [1.0], [0.0]]), (1, ne))
+    B = orc.fe_force(conn, X, F0 @ X, fibc, mid, [HO])["B"]
+    cnt = np.bincount(conn.ravel(), minlength=nn)
+    interior = cnt == 8
+    assert interior.sum() > 0
+    assert np.max(np.abs(B[:, interior])) < 1e-12 * np.max(np.abs(B[:, ~interior]))
+    # A10: an inverted element is reported with its id
+    xi = x.copy()
+    n0 = conn[7, 0]
+    xi[:, n0] = x[:, conn[7, 7]] + (x[:, conn[7, 7]] - x[:, n0])       # push node 0 through node 7
+    r = orc.fe_force(conn, X, xi, fib, mid, [NH])
+    assert r["rc"] == 1 and r["first_bad"] >= 0
+
+
+def test_points_weights_prolong_restrict(orc):
+    conn, X, x, fib = distorted_block(3, 2, 2, seed=3)
+    ne, nn = conn.shape[0], X.shape[1]
+    rng = np.random.default_rng(0)
+    nsub = rng.integers(1, 5, size=(ne, 3)).astype(np.int32)
+    xp, Wp, wa = orc.points(conn, X, x, nsub)
+    P = int(np.prod(nsub, axis=1).sum())
+    assert xp.shape == (3, P) and orc.num_points(nn, ne, nsub) == P
+    # pin 11: sum w_a = sum W_s; with a 2x2x2 midpoint-free check on an undistorted box it is the volume
+    assert abs(wa.sum() - Wp.sum()) < 1e-14 * Wp.sum()
+    cb, Xb, _, _ = distorted_block(3, 2, 2, seed=3, ref_noise=0.0, cur_noise=0.0)
+    _, Wb, wb = orc.points(cb, Xb, Xb, nsub)
+    assert abs(Wb.sum() - 0.3 * 0.3 * 0.2) < 1e-15
+    interior_w = wb[np.bincount(cb.ravel(), minlength=nn) == 8]
+    assert interior_w.size == 0 or np.allclose(interior_w, 0.1 * 0.15 * 0.1)
+    # affine map is reproduced at every sub-point: x_s = A X_s + c  (X_s from the same routine)
+    A = np.array([[1.1, 0.2, 0.0], [0.0, 0.9, 0.1], [0.3, 0.0, 1.2]])
+    Xs, _, _ = orc.points(conn, X, X, nsub)
+    xs, _, _ = orc.points(conn, X, A @ X + 0.5, nsub)
+    assert np.max(np.abs(xs - (A @ Xs + 0.5))) < 1e-15
+    # sub-point ordering s = m1 + n1 (m2 + n2 m3) on the unit cube: X_s is the cell midpoint
+    c1 = np.arange(8, dtype=np.int32).reshape(1, 8)
+    X1 = np.array([[a & 1, (a >> 1) & 1, (a >> 2) & 1] for a in range(8)], dtype=np.float64).T
+    ns = np.array([[2, 3, 4]], dtype=np.int32)
+    Xs1, W1, _ = orc.points(c1, X1, X1, ns)
+    m3, m2, m1 = np.meshgrid(np.arange(4), np.arange(3), np.arange(2), indexing="ij")
+    exp = np.stack([(m1.ravel() + .5) / 2, (m2.ravel() + .5) / 3, (m3.ravel() + .5) / 4])
+    assert np.max(np.abs(Xs1 - exp)) < 1e-16 and np.allclose(W1, 1 / 24, rtol=1e-15)
+    # prolongation conserves the total force (partition of unity); a constant force density is exact
+    B = rng.normal(size=(3, nn))
+    Gp = orc.prolong(conn, nsub, wa, Wp, B)
+    assert np.max(np.abs(Gp.sum(axis=1) - B.sum(axis=1))) < 1e-13 * np.abs(B).sum()
+    Gc = orc.prolong(conn, nsub, wa, Wp, wa[None, :] * np.array([[2.0], [-1.0], [0.5]]))
+    assert np.max(np.abs(Gc - Wp[None, :] * np.array([[2.0], [-1.0], [0.5]]))) < 1e-15
+    # restriction is the transpose: sum_s G_s.U_s = sum_a B_a.U_a ; constants are preserved
+    Up = rng.normal(size=(3, P))
+    Un = orc.restrict(conn, nsub, wa, Wp, Up)
+    assert abs(np.sum(Gp * Up) - np.sum(B * Un)) < 1e-13 * abs(np.sum(B * Un))
+    Uc = orc.restrict(conn, nsub, wa, Wp, np.tile(np.array([[1.5], [0.0], [-2.0]]), (1, P)))
+    assert np.max(np.abs(Uc - np.array([[1.5], [0.0], [-2.0]]))) < 1e-15
+    # nodal rule of PAPER.md L241: w_q = int phi_q, sums to the volume of the mesh
+    wq = orc.nodal_weights(cb, Xb)
+    assert abs(wq.sum() - 0.3 * 0.3 * 0.2) < 1e-15
+
+
+def test_coupling_step_composition_and_node_level_adjointness(orc):
+    conn, X, x, fib = distorted_block(3, 3, 2, size=(0.3, 0.3, 0.2), origin=(0.35, 0.3, 0.4), seed=4)
+    ne, nn = conn.shape[0], X.shape[1]
+    nsub = np.tile(np.array([[2, 3, 2]], np.int32), (ne, 1))
+    mid = np.zeros(ne, np.int32)
+    n, h = 16, 1.0 / 16
+    g = orc.make_grid(n, n, n, h)
+    rng = np.random.default_rng(0)
+    u, v, w = rng.normal(size=(3, n ** 3))
+    out = orc.coupling_step(g, conn, X, fib, mid, nsub, [HO], x, u, v, w)
+    # pieces
+    B = orc.fe_force(conn, X, x, fib, mid, [HO])["B"]
+    assert np.array_equal(out["B"], B)
+    # pin 7: total spread force = total Lagrangian force = 0 for internal forces
+    for f in (out["fu"], out["fv"], out["fw"]):
+        assert abs(h ** 3 * f.sum()) < 1e-12 * np.abs(B).sum()
+    # pin 6 (node level, A13): h^3 sum f.u = sum_a B_a . Un_a
+    lhs = h ** 3 * (out["fu"] @ u + out["fv"] @ v + out["fw"] @ w)
+    rhs = np.sum(B * out["Un"])
+    assert abs(lhs - rhs) < 1e-12 * abs(rhs)
+    # nodal mode reproduces PAPER.md L253-257 literally: points = nodes, spread B itself
+    outn = orc.coupling_step(g, conn, X, fib, mid, None, [HO], x, u, v, w)
+    fN = orc.spread(g, x, B)
+    UN = orc.interp(g, x, u, v, w)
+    assert np.array_equal(outn["fu"], fN[0]) and np.array_equal(outn["Un"], UN)
+
+
+def test_generated_configs_are_valid(orc):
+    # every synthetic config has positive Jacobians and moderate deformation
+    for wl in (W.config1(), W.config2(), W.lv_small()):
+        r = orc.fe_force(wl.conn, wl.X, wl.x, wl.fibers, wl.mat_id, wl.mats)
+        assert r["rc"] == 0 and r["minJ"] > 0.2, (wl.name, r["minJ"])
+        ef, es = wl.fibers[:3], wl.fibers[3:]
+        assert np.allclose(np.linalg.norm(ef, axis=0), 1) and np.allclose(np.linalg.norm(es, axis=0), 1)
+        assert np.max(np.abs(np.sum(ef * es, axis=0))) < 1e-9
+        lo = np.array(wl.origin) + 5 * wl.h
+        hi = np.array(wl.origin) + (np.array([wl.nx, wl.ny, wl.nz]) - 5) * wl.h
+        assert np.all(wl.x.min(axis=1) > lo) and np.all(wl.x.max(axis=1) < hi)
