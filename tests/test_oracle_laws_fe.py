@@ -296,6 +296,6 @@ def test_generated_configs_are_valid(orc):
         ef, es = wl.fibers[:3], wl.fibers[3:]
         assert np.allclose(np.linalg.norm(ef, axis=0), 1) and np.allclose(np.linalg.norm(es, axis=0), 1)
         assert np.max(np.abs(np.sum(ef * es, axis=0))) < 1e-9
-        lo = np.array(wl.origin) + 5 * wl.h
-        hi = np.array(wl.origin) + (np.array([wl.nx, wl.ny, wl.nz]) - 5) * wl.h
+        lo = np.array(wl.origin) + 4 * wl.h   # full-size 6h margins: tests/test_workloads.py
+        hi = np.array(wl.origin) + (np.array([wl.nx, wl.ny, wl.nz]) - 4) * wl.h
         assert np.all(wl.x.min(axis=1) > lo) and np.all(wl.x.max(axis=1) < hi)
