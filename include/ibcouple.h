@@ -1,0 +1,164 @@
+/*
+ * ibcouple.h -- C ABI of libibcouple: the Lagrangian-Eulerian coupling step of the matrix-free
+ * immersed boundary (IB) method of arXiv 2503.22695, hand-written CUDA for NVIDIA B200 (sm_100a).
+ *
+ * One time step's coupling (Eq.(16), Eq.(20)-(22) L191-196) has three parts:
+ *   (1) the hyperelastic finite-element nodal force, Eq.(20) L191 / L249-251, with F, J (L28-32)
+ *       and P = dW/dF (L42-44) per element at 2x2x2 Gauss points, for the neo-Hookean (L441-445)
+ *       and Holzapfel-Ogden (Eq.(12)-(15) L147-155) laws, accumulated to nodes with no assembled
+ *       sparse matrix (abstract, L13);
+ *   (2) spreading of that force to the staggered (MAC, L205) grid with the regularised delta
+ *       delta_h, Eq.(24)-(26) L211-217 / L253-257 (Peskin 4-point kernel, ref. 1 L474);
+ *   (3) interpolation of the MAC velocity to the Lagrangian points, Eq.(27)-(29) L222-229 /
+ *       L243-247, followed by the lumped L2 projection onto the nodes (L233-237, L241).
+ *
+ * Data layout:
+ *   grid arrays u,v,w,fu,fv,fw : nx*ny*nz doubles each, x fastest: idx = (k*ny + j)*nx + i,
+ *       periodic in all three directions; u[i,j,k] lives at (x0+i h, y0+(j+1/2)h, z0+(k+1/2)h),
+ *       v at ((i+1/2)h, j h, (k+1/2)h), w at ((i+1/2)h, (j+1/2)h, k h) (+origin).
+ *       nx, ny, nz must be multiples of 8 (tile edge of the binning key).
+ *   node arrays X_ref, x, B, Un : component-major [3][n_nodes] doubles.
+ *   point arrays xp, Gp, Up     : component-major [3][P] doubles.
+ *   conn [n_elems][8] int32, local node a = ia + 2 ja + 4 ka (Q1 hexahedron);
+ *   fibers [6][n_elems] doubles = (e_f, e_s) per element, unit and orthogonal;
+ *   nsub [n_elems][3] int32 sub-point counts (n1,n2,n3) per element, each in 1..8.
+ *
+ * Ownership: every pointer is owned by the caller. ib_create COPIES the static mesh description
+ * (host pointers) to the device; the context owns those copies and all scratch. Pointers passed
+ * to the per-step calls are DEVICE pointers unless the name ends in _host.
+ * Streams: `stream` is a cudaStream_t passed as void* (NULL = default stream). Per-step calls
+ * only enqueue work and return; they never synchronise. Device-detected errors (inverted
+ * element, non-finite input) are latched in a device status word and reported by ib_check().
+ * Thread safety: one context may be used from one host thread / one stream at a time.
+ */
+#ifndef IBCOUPLE_H
+#define IBCOUPLE_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ib_ctx ib_ctx;
+
+typedef enum {
+    IB_OK = 0,
+    IB_ERR_INVALID_ARG = 1,      /* NULL pointer, negative size, h <= 0, bad mat_id / nsub / dims      */
+    IB_ERR_UNSUPPORTED = 2,      /* periodic == 0; node shared by more than 8 elements                  */
+    IB_ERR_ALLOC = 3,            /* cudaMalloc / malloc failed                                          */
+    IB_ERR_CUDA = 4,             /* a CUDA runtime call failed (no device, launch error)                */
+    IB_ERR_INVERTED_ELEMENT = 5, /* det J0 <= 0 or J <= 0 at a Gauss point (reported by ib_check)       */
+    IB_ERR_NONFINITE = 6,        /* NaN/Inf position (reported by ib_check)                             */
+    IB_ERR_OUT_OF_DOMAIN = 7     /* reserved for bounded (non-periodic) grids                           */
+} ib_status;
+
+/* Uniform MAC grid. periodic must be 1. */
+typedef struct {
+    int32_t nx, ny, nz;
+    double h, x0, y0, z0;
+    int32_t periodic;
+} ib_grid_desc;
+
+typedef enum { IB_LAW_NEOHOOKEAN = 0, IB_LAW_HO = 1 } ib_law;
+
+/* Material row. HO (Eq.(12)-(15)): a,b isotropic; af,bf / as_,bs fibre and sheet; afs,bfs
+ * coupling; kappa = kappa_stab of U(J) = kappa/2 (ln J)^2 (L94). neo-Hookean (L441-445):
+ * a = mu (= 2 alpha), b = 0, fibre constants ignored. */
+typedef struct {
+    int32_t law;
+    double a, b, af, bf, as_, bs, afs, bfs, kappa;
+} ib_material;
+
+/* Static mesh description; all pointers are HOST pointers, copied by ib_create. */
+typedef struct {
+    int64_t n_nodes, n_elems;
+    const int32_t *conn;      /* [n_elems][8]                                            */
+    const double *X_ref;      /* [3][n_nodes] reference coordinates                      */
+    const double *fibers;     /* [6][n_elems] or NULL (then e_f = e_x, e_s = e_y)        */
+    const int32_t *mat_id;    /* [n_elems] or NULL (all 0)                               */
+    const int32_t *nsub;      /* [n_elems][3] or NULL = nodal rule of L241 (points=nodes)*/
+    const ib_material *mats;  /* [n_mats]                                                */
+    int32_t n_mats;
+} ib_mesh_desc;
+
+/* Create a context: validates, copies the mesh, builds the node->element adjacency (at most 8
+ * incident elements per node), and precomputes on the device the sub-point weights W_s =
+ * det J0(xi_s) 8/(n1 n2 n3) and the lumped nodal weights w_a = sum W_s N_a(xi_s) (L235, L241).
+ * `device` is the CUDA device ordinal. Synchronous. */
+ib_status ib_create(ib_ctx **ctx, const ib_grid_desc *grid, const ib_mesh_desc *mesh, int32_t device);
+ib_status ib_destroy(ib_ctx *ctx);
+
+/* Number of Lagrangian force points P (= n_nodes in nodal mode), nodes, elements. */
+int64_t ib_num_points(const ib_ctx *ctx);
+int64_t ib_num_nodes(const ib_ctx *ctx);
+int64_t ib_num_elems(const ib_ctx *ctx);
+
+/* (1) FE nodal force  B_a = - sum_q P(F(X_q)) grad_X phi_a(X_q) w_q   (Eq.(20)).
+ * x [3][n_nodes] current positions (in); B [3][n_nodes] (out, overwritten). Deterministic:
+ * element contributions are gathered per node in fixed order, no atomics. */
+ib_status ib_fe_force(ib_ctx *ctx, const double *x, double *B, void *stream);
+
+/* Lagrangian force points of the sub-point rule at the current configuration:
+ * xp [3][P] = sum_a N_a(xi_s) x_a ; Gp [3][P] = W_s sum_a N_a(xi_s) B_a / w_a (either may be NULL;
+ * B may be NULL iff Gp is NULL). In nodal mode xp = x, Gp = B. */
+ib_status ib_points(ib_ctx *ctx, const double *x, const double *B, double *xp, double *Gp, void *stream);
+
+/* Lumped L2 projection (L233-237) of point values to nodes: Un_a = (1/w_a) sum_s W_s N_a(xi_s) Up_s.
+ * Deterministic (per-node gather). In nodal mode Un = Up. */
+ib_status ib_restrict(ib_ctx *ctx, const double *Up, double *Un, void *stream);
+
+/* Bin points by Eulerian cell and sort (stable): c_d = floor((xp_d - x0_d) * (1.0/h)) mod n_d,
+ * key = ((tz*nty+ty)*ntx+tx)*512 + ((lz*8+ly)*8+lx) with t = c div 8, l = c mod 8;
+ * perm_out[r] = id of the point of rank r (ties keep ascending id); key_out[p] = key of point p.
+ * Bit-exact against the definition. key_out or perm_out may be NULL. P <= 2^31-1. */
+ib_status ib_bin_sort(ib_ctx *ctx, const double *xp, int64_t P, int64_t *key_out, int32_t *perm_out,
+                      void *stream);
+
+/* (2) Spread, Eq.(24)-(26): f_c[face] (+)= sum_s Gp_{s,c} delta_h(x_face - xp_s), delta_h =
+ * h^-3 phi phi phi on component c's own staggered lattice. accumulate == 0 zero-fills fu,fv,fw
+ * first. Generic over arbitrary point clouds. Sums are reordered (atomics): not bit-reproducible. */
+ib_status ib_spread(ib_ctx *ctx, const double *xp, const double *Gp, int64_t P,
+                    double *fu, double *fv, double *fw, int32_t accumulate, void *stream);
+
+/* (3) Interpolate, Eq.(27)-(29): Up_{s,c} = sum_faces u_c[face] delta_h(x_face - xp_s) h^3. */
+ib_status ib_interp(ib_ctx *ctx, const double *xp, int64_t P, const double *u, const double *v,
+                    const double *w, double *Up, void *stream);
+
+/* The whole coupling step at one position array x (BASELINE.json "one coupling step"):
+ *   B = fe_force(x); points; f = spread(xp, Gp) (overwrites fu,fv,fw); Up = interp(xp,u,v,w);
+ *   Un = restrict(Up).   B may be NULL (not returned). */
+ib_status ib_coupling_step(ib_ctx *ctx, const double *x, const double *u, const double *v,
+                           const double *w, double *fu, double *fv, double *fw, double *Un,
+                           double *B, void *stream);
+
+/* Same step with HOST buffers: copies x,u,v,w host->device, runs the step, copies fu,fv,fw,Un
+ * (and B if non-NULL) device->host, all on `stream`, then synchronises it. Buffers should be
+ * pinned for full PCIe rate. */
+ib_status ib_coupling_step_host(ib_ctx *ctx, const double *x_host, const double *u_host,
+                                const double *v_host, const double *w_host, double *fu_host,
+                                double *fv_host, double *fw_host, double *Un_host, double *B_host,
+                                void *stream);
+
+/* Synchronise the last used stream and report the latched device status. first_bad_index (may be
+ * NULL) receives the smallest offending element or node id, or -1. Clears the latch. */
+ib_status ib_check(ib_ctx *ctx, int64_t *first_bad_index);
+
+/* Number of kernel launches enqueued by this context since creation (for bench accounting). */
+int64_t ib_launch_count(const ib_ctx *ctx);
+
+/* Select the kernel variant used by spread/interp/coupling_step: 0 = reference path (one thread
+ * per point, global atomics), 1 = tiled path (points sorted by cell, shared-memory halo tile).
+ * Default 1. Returns IB_ERR_INVALID_ARG for other values. */
+ib_status ib_set_variant(ib_ctx *ctx, int32_t variant);
+
+/* FP64 FMA peak probe: runs a register-only DFMA loop on `device`; returns achieved DFMA/s in
+ * *dfma_per_s and the kernel time in *ms. Used by bench.py for the "alu" roofline denominator. */
+ib_status ib_probe_dfma(int32_t device, double *dfma_per_s, double *ms);
+
+const char *ib_status_string(ib_status s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* IBCOUPLE_H */

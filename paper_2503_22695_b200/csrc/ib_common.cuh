@@ -1,0 +1,160 @@
+// ib_common.cuh -- device helpers and the host-side context of libibcouple (CUDA path only).
+// Shares nothing with oracle/.  Citations are to /root/reference/PAPER.md lines (see include/ibcouple.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/ibcouple.h"
+
+#define IB_TILE 8              // tile edge of the binning key (A21)
+#define IB_TILE_CELLS 512
+
+// ---------------------------------------------------------------------------------------------
+// host-side context
+// ---------------------------------------------------------------------------------------------
+struct ib_ctx {
+    int device;
+    ib_grid_desc grid;
+    double inv_h;
+    int64_t n_nodes, n_elems, n_points, n_cells;
+    int nodal;                 // nsub == NULL
+    int uniform_S;             // all elements share one nsub triple (0 if not)
+    int n_mats;
+    int variant;
+    // static mesh (device copies)
+    int32_t *d_conn;           // [n_elems][8]
+    double *d_X;               // [3][n_nodes]
+    double *d_fib;             // [6][n_elems]
+    int32_t *d_mat_id;         // [n_elems]
+    int32_t *d_nsub;           // [n_elems][3]
+    int64_t *d_pt_off;         // [n_elems+1]
+    ib_material *d_mats;
+    int32_t *d_adj;            // [8][n_nodes] slot = e*8+a or -1 (ELL, ascending element id)
+    double *d_Wp;              // [P] sub-point weights W_s
+    double *d_wa;              // [n_nodes] lumped weights
+    // per-step scratch
+    double *d_Ce;              // [3][n_elems*8] per-element nodal contributions
+    double *d_Fhat;            // [3][n_nodes]
+    double *d_B;               // [3][n_nodes] (when caller passes B == NULL)
+    double *d_xp, *d_Gp, *d_Up;   // [3][P]
+    // sort scratch (grown on demand)
+    int64_t sort_cap;
+    uint32_t *d_key[2];
+    int32_t *d_val[2];
+    uint32_t *d_hist;
+    int64_t hist_cap;
+    int32_t *d_cell_start;     // [n_cells+1] start rank of every cell (tiled path)
+    int32_t *d_tile_list;      // compacted non-empty tiles
+    int32_t *d_tile_count;     // [1] + work counters
+    // host staging for the *_host entry point
+    double *d_hx, *d_hu, *d_hv, *d_hw, *d_hfu, *d_hfv, *d_hfw, *d_hUn, *d_hB;
+    // status latch: [0] code, [1] first bad id
+    long long *d_status;
+    cudaStream_t last_stream;
+    int64_t launches;
+};
+
+#define IB_CUDA_TRY(expr)                                   \
+    do {                                                    \
+        cudaError_t _e = (expr);                            \
+        if (_e != cudaSuccess) return IB_ERR_CUDA;          \
+    } while (0)
+
+static inline unsigned ib_blocks(int64_t n, int per) { return (unsigned)((n + per - 1) / per); }
+
+// ---------------------------------------------------------------------------------------------
+// device helpers
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void ib_latch(long long *status, int code, long long id)
+{
+    // keep the smallest offending id; code of the first writer wins per id class
+    atomicMax((unsigned long long *)&status[0], (unsigned long long)code);
+    atomicMin(&status[1], id);
+}
+
+// Peskin 4-point kernel (PAPER.md L52 -> ref.1): the four weights of the support that starts at
+// i0 = floor(s) - 1, with r = s - floor(s) in [0,1):
+//   phi(1+r) = (3-2r-q)/8, phi(r) = (3-2r+q)/8, phi(1-r) = (1+2r+q)/8, phi(2-r) = (1+2r-q)/8,
+//   q = sqrt(1+4r-4r^2)  (one square root serves all four).
+__device__ __forceinline__ void ib_phi4(double r, double w[4])
+{
+    double q = sqrt(fma(4.0 * r, 1.0 - r, 1.0)) * 0.125;
+    double a = fma(-0.25, r, 0.375);
+    double b = fma(0.25, r, 0.125);
+    w[0] = a - q;
+    w[1] = a + q;
+    w[2] = b + q;
+    w[3] = b - q;
+}
+
+// scaled coordinate s = (x - x0)/h, computed as a product with 1/h plus one residual correction
+// so that it agrees with true division to ~1 ulp.
+__device__ __forceinline__ double ib_scaled(double x, double x0, double h, double inv_h)
+{
+    double d = x - x0;
+    double s = d * inv_h;
+    double res = fma(-s, h, d);
+    return fma(res, inv_h, s);
+}
+
+__device__ __forceinline__ int ib_wrap(int i, int n)
+{
+    i %= n;
+    return i < 0 ? i + n : i;
+}
+
+// Binning cell index of A21: floor((x - x0) * inv_h) mod n, in IEEE double with NO contraction.
+__device__ __forceinline__ int ib_cell(double x, double x0, double inv_h, int n)
+{
+    double sc = __dmul_rn(__dsub_rn(x, x0), inv_h);
+    long long c = (long long)floor(sc);
+    c %= n;
+    if (c < 0) c += n;
+    return (int)c;
+}
+
+// Q1 shape functions at xi (local node a = ia + 2 ja + 4 ka)
+__device__ __forceinline__ void ib_shape(double x0, double x1, double x2, double N[8])
+{
+    double a0 = 0.5 * (1.0 - x0), a1 = 0.5 * (1.0 + x0);
+    double b0 = 0.5 * (1.0 - x1), b1 = 0.5 * (1.0 + x1);
+    double c0 = 0.5 * (1.0 - x2), c1 = 0.5 * (1.0 + x2);
+    double ab00 = a0 * b0, ab10 = a1 * b0, ab01 = a0 * b1, ab11 = a1 * b1;
+    N[0] = ab00 * c0; N[1] = ab10 * c0; N[2] = ab01 * c0; N[3] = ab11 * c0;
+    N[4] = ab00 * c1; N[5] = ab10 * c1; N[6] = ab01 * c1; N[7] = ab11 * c1;
+}
+
+// shape-function gradients wrt xi
+__device__ __forceinline__ void ib_dshape(double x0, double x1, double x2, double dN[8][3])
+{
+#pragma unroll
+    for (int a = 0; a < 8; ++a) {
+        double s0 = (a & 1) ? 1.0 : -1.0, s1 = (a & 2) ? 1.0 : -1.0, s2 = (a & 4) ? 1.0 : -1.0;
+        double f0 = fma(s0, x0, 1.0), f1 = fma(s1, x1, 1.0), f2 = fma(s2, x2, 1.0);
+        dN[a][0] = 0.125 * s0 * f1 * f2;
+        dN[a][1] = 0.125 * f0 * s1 * f2;
+        dN[a][2] = 0.125 * f0 * f1 * s2;
+    }
+}
+
+// sub-point reference coordinate: xi = -1 + (2m+1)/n
+__device__ __forceinline__ double ib_subxi(int m, int n) { return -1.0 + (double)(2 * m + 1) / (double)n; }
+
+__device__ __forceinline__ double ib_det3(const double A[3][3])
+{
+    return A[0][0] * (A[1][1] * A[2][2] - A[1][2] * A[2][1])
+         - A[0][1] * (A[1][0] * A[2][2] - A[1][2] * A[2][0])
+         + A[0][2] * (A[1][0] * A[2][1] - A[1][1] * A[2][0]);
+}
+
+// internal launchers (defined across the .cu files)
+ib_status ibk_fe_force(ib_ctx *c, const double *x, double *B, double *Fhat, cudaStream_t st);
+ib_status ibk_points(ib_ctx *c, const double *x, const double *Fhat, double *xp, double *Gp, cudaStream_t st);
+ib_status ibk_restrict(ib_ctx *c, const double *Up, double *Un, cudaStream_t st);
+ib_status ibk_precompute_weights(ib_ctx *c, cudaStream_t st);
+ib_status ibk_bin_sort(ib_ctx *c, const double *xp, int64_t P, int64_t *key_out, int32_t *perm_out,
+                       int build_cells, cudaStream_t st);
+ib_status ibk_spread_interp(ib_ctx *c, const double *xp, const double *Gp, int64_t P,
+                            const double *u, const double *v, const double *w,
+                            double *fu, double *fv, double *fw, double *Up, int accumulate,
+                            cudaStream_t st);
+ib_status ibk_sort_reserve(ib_ctx *c, int64_t P);

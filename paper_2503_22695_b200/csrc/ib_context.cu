@@ -1,0 +1,397 @@
+// ib_context.cu -- C-ABI entry points of libibcouple (include/ibcouple.h): context lifetime,
+// argument validation, and the per-step calls that enqueue the kernels of the other files.
+#include <climits>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+#include "ib_common.cuh"
+
+#define ST(s) ((cudaStream_t)(s))
+
+static ib_status dev_alloc(void **p, size_t bytes)
+{
+    *p = nullptr;
+    if (bytes == 0) bytes = 16;
+    return cudaMalloc(p, bytes) == cudaSuccess ? IB_OK : IB_ERR_ALLOC;
+}
+
+template <class T>
+static ib_status dev_upload(T **dst, const T *src, size_t n)
+{
+    ib_status s = dev_alloc((void **)dst, n * sizeof(T));
+    if (s != IB_OK) return s;
+    if (n && cudaMemcpy(*dst, src, n * sizeof(T), cudaMemcpyHostToDevice) != cudaSuccess) return IB_ERR_CUDA;
+    return IB_OK;
+}
+
+extern "C" const char *ib_status_string(ib_status s)
+{
+    switch (s) {
+    case IB_OK: return "IB_OK";
+    case IB_ERR_INVALID_ARG: return "IB_ERR_INVALID_ARG";
+    case IB_ERR_UNSUPPORTED: return "IB_ERR_UNSUPPORTED";
+    case IB_ERR_ALLOC: return "IB_ERR_ALLOC";
+    case IB_ERR_CUDA: return "IB_ERR_CUDA";
+    case IB_ERR_INVERTED_ELEMENT: return "IB_ERR_INVERTED_ELEMENT";
+    case IB_ERR_NONFINITE: return "IB_ERR_NONFINITE";
+    case IB_ERR_OUT_OF_DOMAIN: return "IB_ERR_OUT_OF_DOMAIN";
+    }
+    return "IB_ERR_UNKNOWN";
+}
+
+static ib_status reset_status(ib_ctx *c, cudaStream_t st)
+{
+    long long init[2] = {0, LLONG_MAX};
+    IB_CUDA_TRY(cudaMemcpyAsync(c->d_status, init, sizeof(init), cudaMemcpyHostToDevice, st));
+    return IB_OK;
+}
+
+extern "C" ib_status ib_destroy(ib_ctx *c)
+{
+    if (!c) return IB_ERR_INVALID_ARG;
+    cudaSetDevice(c->device);
+    void *ptrs[] = {c->d_conn, c->d_X, c->d_fib, c->d_mat_id, c->d_nsub, c->d_pt_off, c->d_mats, c->d_adj,
+                    c->d_Wp, c->d_wa, c->d_Ce, c->d_Fhat, c->d_B, c->d_xp, c->d_Gp, c->d_Up, c->d_key[0],
+                    c->d_key[1], c->d_val[0], c->d_val[1], c->d_hist, c->d_cell_start, c->d_tile_list,
+                    c->d_tile_count, c->d_hx, c->d_hu, c->d_hv, c->d_hw, c->d_hfu, c->d_hfv, c->d_hfw,
+                    c->d_hUn, c->d_hB, c->d_status};
+    for (void *p : ptrs)
+        if (p) cudaFree(p);
+    delete c;
+    return IB_OK;
+}
+
+extern "C" ib_status ib_create(ib_ctx **out, const ib_grid_desc *g, const ib_mesh_desc *m, int32_t device)
+{
+    if (!out) return IB_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!g || !m) return IB_ERR_INVALID_ARG;
+    if (g->nx <= 0 || g->ny <= 0 || g->nz <= 0 || (g->nx % IB_TILE) || (g->ny % IB_TILE) || (g->nz % IB_TILE))
+        return IB_ERR_INVALID_ARG;
+    if (!(g->h > 0.0) || !std::isfinite(g->h) || !std::isfinite(g->x0) || !std::isfinite(g->y0) || !std::isfinite(g->z0))
+        return IB_ERR_INVALID_ARG;
+    if ((int64_t)g->nx * g->ny * g->nz > (int64_t)INT32_MAX) return IB_ERR_INVALID_ARG;
+    if (!g->periodic) return IB_ERR_UNSUPPORTED;
+    if (m->n_nodes < 0 || m->n_elems < 0 || m->n_nodes > INT32_MAX || m->n_elems > INT32_MAX / 8) return IB_ERR_INVALID_ARG;
+    if (m->n_elems > 0 && (!m->conn || !m->X_ref || !m->mats || m->n_mats <= 0)) return IB_ERR_INVALID_ARG;
+    if (m->n_nodes > 0 && !m->X_ref) return IB_ERR_INVALID_ARG;
+    for (int i = 0; i < m->n_mats; ++i)
+        if (m->mats[i].law != IB_LAW_NEOHOOKEAN && m->mats[i].law != IB_LAW_HO) return IB_ERR_INVALID_ARG;
+
+    // host-side validation and topology
+    const int64_t nn = m->n_nodes, ne = m->n_elems;
+    std::vector<int64_t> off((size_t)ne + 1, 0);
+    int uniform = 0;
+    if (m->nsub) {
+        for (int64_t e = 0; e < ne; ++e) {
+            const int32_t *s = m->nsub + 3 * e;
+            if (s[0] < 1 || s[1] < 1 || s[2] < 1 || s[0] > 8 || s[1] > 8 || s[2] > 8) return IB_ERR_INVALID_ARG;
+            off[e + 1] = off[e] + (int64_t)s[0] * s[1] * s[2];
+        }
+        if (off[ne] > (int64_t)INT32_MAX) return IB_ERR_INVALID_ARG;
+        uniform = ne > 0 ? m->nsub[0] * m->nsub[1] * m->nsub[2] : 0;
+        for (int64_t e = 1; e < ne && uniform; ++e)
+            if (m->nsub[3 * e] != m->nsub[0] || m->nsub[3 * e + 1] != m->nsub[1] || m->nsub[3 * e + 2] != m->nsub[2])
+                uniform = 0;
+    }
+    std::vector<int32_t> adj((size_t)8 * (nn > 0 ? nn : 1), -1);
+    {
+        std::vector<unsigned char> cnt((size_t)(nn > 0 ? nn : 1), 0);
+        for (int64_t e = 0; e < ne; ++e) {
+            if (m->mat_id && (m->mat_id[e] < 0 || m->mat_id[e] >= m->n_mats)) return IB_ERR_INVALID_ARG;
+            for (int a = 0; a < 8; ++a) {
+                int32_t n = m->conn[e * 8 + a];
+                if (n < 0 || n >= nn) return IB_ERR_INVALID_ARG;
+                if (cnt[n] >= 8) return IB_ERR_UNSUPPORTED;
+                adj[(size_t)cnt[n] * nn + n] = (int32_t)(e * 8 + a);      // ascending element id
+                cnt[n]++;
+            }
+        }
+    }
+
+    if (cudaSetDevice(device) != cudaSuccess) return IB_ERR_CUDA;
+    ib_ctx *c = new (std::nothrow) ib_ctx();
+    if (!c) return IB_ERR_ALLOC;
+    memset(c, 0, sizeof(*c));
+    c->device = device;
+    c->grid = *g;
+    c->inv_h = 1.0 / g->h;
+    c->n_nodes = nn;
+    c->n_elems = ne;
+    c->n_cells = (int64_t)g->nx * g->ny * g->nz;
+    c->nodal = m->nsub == nullptr;
+    c->n_points = c->nodal ? nn : off[ne];
+    c->uniform_S = uniform;
+    c->n_mats = m->n_mats;
+    c->variant = 0;
+
+    ib_status s = IB_OK;
+#define TRY(x) do { if (s == IB_OK) s = (x); } while (0)
+    TRY(dev_upload(&c->d_conn, m->conn, (size_t)ne * 8));
+    TRY(dev_upload(&c->d_X, m->X_ref, (size_t)nn * 3));
+    if (m->fibers) TRY(dev_upload(&c->d_fib, m->fibers, (size_t)ne * 6));
+    if (m->mat_id) TRY(dev_upload(&c->d_mat_id, m->mat_id, (size_t)ne));
+    if (m->nsub) TRY(dev_upload(&c->d_nsub, m->nsub, (size_t)ne * 3));
+    TRY(dev_upload(&c->d_pt_off, off.data(), (size_t)ne + 1));
+    TRY(dev_upload(&c->d_mats, m->mats, (size_t)(m->n_mats > 0 ? m->n_mats : 0)));
+    TRY(dev_upload(&c->d_adj, adj.data(), (size_t)8 * (nn > 0 ? nn : 1)));
+    const size_t P = (size_t)c->n_points;
+    TRY(dev_alloc((void **)&c->d_wa, (size_t)nn * sizeof(double)));
+    TRY(dev_alloc((void **)&c->d_Ce, (size_t)ne * 24 * sizeof(double)));
+    TRY(dev_alloc((void **)&c->d_Fhat, (size_t)nn * 3 * sizeof(double)));
+    TRY(dev_alloc((void **)&c->d_B, (size_t)nn * 3 * sizeof(double)));
+    if (!c->nodal) {
+        TRY(dev_alloc((void **)&c->d_Wp, P * sizeof(double)));
+        TRY(dev_alloc((void **)&c->d_xp, P * 3 * sizeof(double)));
+        TRY(dev_alloc((void **)&c->d_Gp, P * 3 * sizeof(double)));
+        TRY(dev_alloc((void **)&c->d_Up, P * 3 * sizeof(double)));
+    }
+    const int n_tiles = (int)(c->n_cells / IB_TILE_CELLS);
+    TRY(dev_alloc((void **)&c->d_cell_start, (size_t)(n_tiles + 1) * sizeof(int32_t)));
+    TRY(dev_alloc((void **)&c->d_tile_list, (size_t)(n_tiles + 1) * sizeof(int32_t)));
+    TRY(dev_alloc((void **)&c->d_tile_count, 64 * sizeof(int32_t)));
+    TRY(dev_alloc((void **)&c->d_status, 2 * sizeof(long long)));
+    if (s == IB_OK) s = reset_status(c, 0);
+    if (s == IB_OK) s = ibk_sort_reserve(c, c->n_points);
+    if (s == IB_OK) s = ibk_precompute_weights(c, 0);
+    if (s == IB_OK && cudaDeviceSynchronize() != cudaSuccess) s = IB_ERR_CUDA;
+#undef TRY
+    if (s == IB_OK) {
+        long long hs[2];
+        if (cudaMemcpy(hs, c->d_status, sizeof(hs), cudaMemcpyDeviceToHost) != cudaSuccess) s = IB_ERR_CUDA;
+        else if (hs[0] != 0) s = (ib_status)hs[0];                  // inverted reference element
+    }
+    if (s != IB_OK) { ib_destroy(c); return s; }
+    *out = c;
+    return IB_OK;
+}
+
+extern "C" int64_t ib_num_points(const ib_ctx *c) { return c ? c->n_points : -1; }
+extern "C" int64_t ib_num_nodes(const ib_ctx *c) { return c ? c->n_nodes : -1; }
+extern "C" int64_t ib_num_elems(const ib_ctx *c) { return c ? c->n_elems : -1; }
+extern "C" int64_t ib_launch_count(const ib_ctx *c) { return c ? c->launches : -1; }
+
+extern "C" ib_status ib_set_variant(ib_ctx *c, int32_t variant)
+{
+    if (!c || (variant != 0 && variant != 1)) return IB_ERR_INVALID_ARG;
+    c->variant = variant;
+    return IB_OK;
+}
+
+static inline ib_status enter(ib_ctx *c, void *stream)
+{
+    if (!c) return IB_ERR_INVALID_ARG;
+    if (cudaSetDevice(c->device) != cudaSuccess) return IB_ERR_CUDA;
+    c->last_stream = ST(stream);
+    return IB_OK;
+}
+
+extern "C" ib_status ib_fe_force(ib_ctx *c, const double *x, double *B, void *stream)
+{
+    ib_status s = enter(c, stream);
+    if (s != IB_OK) return s;
+    if (!x || !B) return IB_ERR_INVALID_ARG;
+    return ibk_fe_force(c, x, B, nullptr, ST(stream));
+}
+
+__global__ void ibk_scale_by_inv(int64_t n_nodes, const double *__restrict__ B, const double *__restrict__ wa,
+                                 double *__restrict__ Fhat)
+{
+    int64_t n = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= n_nodes) return;
+    double r = 1.0 / wa[n];
+    Fhat[n] = B[n] * r; Fhat[n_nodes + n] = B[n_nodes + n] * r; Fhat[2 * n_nodes + n] = B[2 * n_nodes + n] * r;
+}
+
+extern "C" ib_status ib_points(ib_ctx *c, const double *x, const double *B, double *xp, double *Gp, void *stream)
+{
+    ib_status s = enter(c, stream);
+    if (s != IB_OK) return s;
+    if ((xp && !x) || (Gp && !B)) return IB_ERR_INVALID_ARG;
+    cudaStream_t st = ST(stream);
+    const size_t nb = (size_t)c->n_nodes * 3 * sizeof(double);
+    if (c->nodal) {
+        if (xp && nb) IB_CUDA_TRY(cudaMemcpyAsync(xp, x, nb, cudaMemcpyDeviceToDevice, st));
+        if (Gp && nb) IB_CUDA_TRY(cudaMemcpyAsync(Gp, B, nb, cudaMemcpyDeviceToDevice, st));
+        return IB_OK;
+    }
+    if (Gp && c->n_nodes > 0) {
+        ibk_scale_by_inv<<<ib_blocks(c->n_nodes, 256), 256, 0, st>>>(c->n_nodes, B, c->d_wa, c->d_Fhat);
+        c->launches++;
+    }
+    return ibk_points(c, x, c->d_Fhat, xp, Gp, st);
+}
+
+extern "C" ib_status ib_restrict(ib_ctx *c, const double *Up, double *Un, void *stream)
+{
+    ib_status s = enter(c, stream);
+    if (s != IB_OK) return s;
+    if (!Up || !Un) return IB_ERR_INVALID_ARG;
+    if (c->nodal) {
+        const size_t nb = (size_t)c->n_nodes * 3 * sizeof(double);
+        if (nb) IB_CUDA_TRY(cudaMemcpyAsync(Un, Up, nb, cudaMemcpyDeviceToDevice, ST(stream)));
+        return IB_OK;
+    }
+    return ibk_restrict(c, Up, Un, ST(stream));
+}
+
+extern "C" ib_status ib_bin_sort(ib_ctx *c, const double *xp, int64_t P, int64_t *key_out, int32_t *perm_out,
+                                 void *stream)
+{
+    ib_status s = enter(c, stream);
+    if (s != IB_OK) return s;
+    if (P < 0 || P > (int64_t)INT32_MAX || (P > 0 && !xp)) return IB_ERR_INVALID_ARG;
+    return ibk_bin_sort(c, xp, P, key_out, perm_out, 0, ST(stream));
+}
+
+extern "C" ib_status ib_spread(ib_ctx *c, const double *xp, const double *Gp, int64_t P, double *fu, double *fv,
+                               double *fw, int32_t accumulate, void *stream)
+{
+    ib_status s = enter(c, stream);
+    if (s != IB_OK) return s;
+    if (P < 0 || P > (int64_t)INT32_MAX || !fu || !fv || !fw || (P > 0 && (!xp || !Gp))) return IB_ERR_INVALID_ARG;
+    if (P == 0) {
+        if (!accumulate) {
+            size_t nb = (size_t)c->n_cells * sizeof(double);
+            IB_CUDA_TRY(cudaMemsetAsync(fu, 0, nb, ST(stream)));
+            IB_CUDA_TRY(cudaMemsetAsync(fv, 0, nb, ST(stream)));
+            IB_CUDA_TRY(cudaMemsetAsync(fw, 0, nb, ST(stream)));
+        }
+        return IB_OK;
+    }
+    return ibk_spread_interp(c, xp, Gp, P, nullptr, nullptr, nullptr, fu, fv, fw, nullptr, accumulate, ST(stream));
+}
+
+extern "C" ib_status ib_interp(ib_ctx *c, const double *xp, int64_t P, const double *u, const double *v,
+                               const double *w, double *Up, void *stream)
+{
+    ib_status s = enter(c, stream);
+    if (s != IB_OK) return s;
+    if (P < 0 || P > (int64_t)INT32_MAX || !u || !v || !w || (P > 0 && (!xp || !Up))) return IB_ERR_INVALID_ARG;
+    if (P == 0) return IB_OK;
+    return ibk_spread_interp(c, xp, nullptr, P, u, v, w, nullptr, nullptr, nullptr, Up, 0, ST(stream));
+}
+
+extern "C" ib_status ib_coupling_step(ib_ctx *c, const double *x, const double *u, const double *v,
+                                      const double *w, double *fu, double *fv, double *fw, double *Un,
+                                      double *B, void *stream)
+{
+    ib_status s = enter(c, stream);
+    if (s != IB_OK) return s;
+    if (!x || !u || !v || !w || !fu || !fv || !fw || !Un) return IB_ERR_INVALID_ARG;
+    cudaStream_t st = ST(stream);
+    double *Bd = B ? B : c->d_B;
+    if (c->nodal) {
+        // the paper's nodal rule verbatim (L241-257): points = nodes, spread B itself, Un = U^IB
+        s = ibk_fe_force(c, x, Bd, nullptr, st);
+        if (s != IB_OK) return s;
+        return ibk_spread_interp(c, x, Bd, c->n_nodes, u, v, w, fu, fv, fw, Un, 0, st);
+    }
+    s = ibk_fe_force(c, x, Bd, c->d_Fhat, st);
+    if (s != IB_OK) return s;
+    s = ibk_points(c, x, c->d_Fhat, c->d_xp, c->d_Gp, st);
+    if (s != IB_OK) return s;
+    s = ibk_spread_interp(c, c->d_xp, c->d_Gp, c->n_points, u, v, w, fu, fv, fw, c->d_Up, 0, st);
+    if (s != IB_OK) return s;
+    return ibk_restrict(c, c->d_Up, Un, st);
+}
+
+extern "C" ib_status ib_coupling_step_host(ib_ctx *c, const double *x_h, const double *u_h, const double *v_h,
+                                           const double *w_h, double *fu_h, double *fv_h, double *fw_h,
+                                           double *Un_h, double *B_h, void *stream)
+{
+    ib_status s = enter(c, stream);
+    if (s != IB_OK) return s;
+    if (!x_h || !u_h || !v_h || !w_h || !fu_h || !fv_h || !fw_h || !Un_h) return IB_ERR_INVALID_ARG;
+    cudaStream_t st = ST(stream);
+    const size_t nb = (size_t)c->n_nodes * 3 * sizeof(double), gb = (size_t)c->n_cells * sizeof(double);
+    if (!c->d_hx) {
+        ib_status a = IB_OK;
+        double **bufs[] = {&c->d_hx, &c->d_hUn, &c->d_hB};
+        for (auto b : bufs) if (a == IB_OK) a = dev_alloc((void **)b, nb);
+        double **gbufs[] = {&c->d_hu, &c->d_hv, &c->d_hw, &c->d_hfu, &c->d_hfv, &c->d_hfw};
+        for (auto b : gbufs) if (a == IB_OK) a = dev_alloc((void **)b, gb);
+        if (a != IB_OK) return a;
+    }
+    IB_CUDA_TRY(cudaMemcpyAsync(c->d_hx, x_h, nb, cudaMemcpyHostToDevice, st));
+    IB_CUDA_TRY(cudaMemcpyAsync(c->d_hu, u_h, gb, cudaMemcpyHostToDevice, st));
+    IB_CUDA_TRY(cudaMemcpyAsync(c->d_hv, v_h, gb, cudaMemcpyHostToDevice, st));
+    IB_CUDA_TRY(cudaMemcpyAsync(c->d_hw, w_h, gb, cudaMemcpyHostToDevice, st));
+    s = ib_coupling_step(c, c->d_hx, c->d_hu, c->d_hv, c->d_hw, c->d_hfu, c->d_hfv, c->d_hfw, c->d_hUn,
+                         B_h ? c->d_hB : nullptr, stream);
+    if (s != IB_OK) return s;
+    IB_CUDA_TRY(cudaMemcpyAsync(fu_h, c->d_hfu, gb, cudaMemcpyDeviceToHost, st));
+    IB_CUDA_TRY(cudaMemcpyAsync(fv_h, c->d_hfv, gb, cudaMemcpyDeviceToHost, st));
+    IB_CUDA_TRY(cudaMemcpyAsync(fw_h, c->d_hfw, gb, cudaMemcpyDeviceToHost, st));
+    IB_CUDA_TRY(cudaMemcpyAsync(Un_h, c->d_hUn, nb, cudaMemcpyDeviceToHost, st));
+    if (B_h) IB_CUDA_TRY(cudaMemcpyAsync(B_h, c->d_hB, nb, cudaMemcpyDeviceToHost, st));
+    IB_CUDA_TRY(cudaStreamSynchronize(st));
+    return IB_OK;
+}
+
+extern "C" ib_status ib_check(ib_ctx *c, int64_t *first_bad)
+{
+    if (!c) return IB_ERR_INVALID_ARG;
+    if (cudaSetDevice(c->device) != cudaSuccess) return IB_ERR_CUDA;
+    if (first_bad) *first_bad = -1;
+    if (cudaStreamSynchronize(c->last_stream) != cudaSuccess) return IB_ERR_CUDA;
+    long long hs[2];
+    IB_CUDA_TRY(cudaMemcpy(hs, c->d_status, sizeof(hs), cudaMemcpyDeviceToHost));
+    if (cudaGetLastError() != cudaSuccess) return IB_ERR_CUDA;
+    if (hs[0] == 0) return IB_OK;
+    if (first_bad) *first_bad = hs[1] == LLONG_MAX ? -1 : hs[1];
+    ib_status r = reset_status(c, c->last_stream);
+    if (r != IB_OK) return r;
+    cudaStreamSynchronize(c->last_stream);
+    return (ib_status)hs[0];
+}
+
+// ---------------------------------------------------------------------------------------------
+// FP64 FMA peak probe (denominator of the "alu" roofline; MEASURED_PEAKS.json has no fp64 figure)
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+ibk_dfma_probe(double *out, int iters, double a, double b)
+{
+    double r0 = threadIdx.x, r1 = r0 + 1, r2 = r0 + 2, r3 = r0 + 3, r4 = r0 + 4, r5 = r0 + 5, r6 = r0 + 6, r7 = r0 + 7;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            r0 = fma(r0, a, b); r1 = fma(r1, a, b); r2 = fma(r2, a, b); r3 = fma(r3, a, b);
+            r4 = fma(r4, a, b); r5 = fma(r5, a, b); r6 = fma(r6, a, b); r7 = fma(r7, a, b);
+        }
+    }
+    double s = r0 + r1 + r2 + r3 + r4 + r5 + r6 + r7;
+    if (s == 123.456) out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+extern "C" ib_status ib_probe_dfma(int32_t device, double *dfma_per_s, double *ms_out)
+{
+    if (!dfma_per_s) return IB_ERR_INVALID_ARG;
+    if (cudaSetDevice(device) != cudaSuccess) return IB_ERR_CUDA;
+    cudaDeviceProp prop;
+    IB_CUDA_TRY(cudaGetDeviceProperties(&prop, device));
+    double *d = nullptr;
+    int blocks = prop.multiProcessorCount * 8, iters = 4096;
+    IB_CUDA_TRY(cudaMalloc(&d, (size_t)blocks * 256 * sizeof(double)));
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    float best = 1e30f;
+    for (int rep = 0; rep < 5; ++rep) {
+        cudaEventRecord(e0);
+        ibk_dfma_probe<<<blocks, 256>>>(d, iters, 0.999999, 1e-9);
+        cudaEventRecord(e1);
+        if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(d); return IB_ERR_CUDA; }
+        float ms;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (rep > 0 && ms < best) best = ms;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(d);
+    double n = (double)blocks * 256.0 * iters * 64.0;
+    *dfma_per_s = n / (best * 1e-3);
+    if (ms_out) *ms_out = best;
+    return IB_OK;
+}

@@ -1,0 +1,234 @@
+// ib_fe_force.cu -- matrix-free hyperelastic FE nodal force.
+//   B_a = - sum_q P(F(X_q)) grad_X phi_a(X_q) w_q          PAPER.md Eq.(20)
+//   F = d chi / d X, J = det F                              L28-32
+//   P = d Psi / d F for neo-Hookean (L441-445) and Holzapfel-Ogden (Eq.(12)-(15) L147-155)
+// "eliminating sparse matrix storage and operations entirely" (L13): one thread per Gauss point,
+// the 8 Gauss points of an element sit in 8 adjacent lanes and exchange their 8x3 nodal
+// contributions with a transposing shuffle reduction; a second kernel gathers, per node, the
+// <= 8 element contributions through an ELL adjacency in fixed order (deterministic, no atomics,
+// no CSR, no assembled operator).
+#include "ib_common.cuh"
+
+// first Piola-Kirchhoff stress. Readings A2 (F^-T in the isotropic term), A3 (symmetric I8 term),
+// A6 (NH: a = mu, b = 0), A9 (I4* = max(I4,1)). Returns J.
+__device__ __forceinline__ double ib_pk1(const ib_material &m, const double F[3][3], const double ef[3],
+                                         const double es[3], double P[3][3])
+{
+    // cofactor matrix: cof[c][K] = J * F^-T[c][K]
+    double cof[3][3];
+    cof[0][0] = F[1][1] * F[2][2] - F[1][2] * F[2][1];
+    cof[0][1] = F[1][2] * F[2][0] - F[1][0] * F[2][2];
+    cof[0][2] = F[1][0] * F[2][1] - F[1][1] * F[2][0];
+    cof[1][0] = F[0][2] * F[2][1] - F[0][1] * F[2][2];
+    cof[1][1] = F[0][0] * F[2][2] - F[0][2] * F[2][0];
+    cof[1][2] = F[0][1] * F[2][0] - F[0][0] * F[2][1];
+    cof[2][0] = F[0][1] * F[1][2] - F[0][2] * F[1][1];
+    cof[2][1] = F[0][2] * F[1][0] - F[0][0] * F[1][2];
+    cof[2][2] = F[0][0] * F[1][1] - F[0][1] * F[1][0];
+    double J = F[0][0] * cof[0][0] + F[0][1] * cof[0][1] + F[0][2] * cof[0][2];
+    if (!(J > 0.0)) return J;
+    double rJ = 1.0 / J;
+    double I1 = 0.0;
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+#pragma unroll
+        for (int K = 0; K < 3; ++K) I1 = fma(F[c][K], F[c][K], I1);
+    double cb = cbrt(J);
+    double Jm23 = 1.0 / (cb * cb);
+    double lnJ = log(J);
+    double e_iso = (m.b != 0.0) ? exp(m.b * (Jm23 * I1 - 3.0)) : 1.0;
+    double ciso = m.a * e_iso * Jm23;
+    // P = ciso (F - I1/3 F^-T) + kappa lnJ F^-T = ciso F + (kappa lnJ - ciso I1/3)/J cof
+    double cvol = (m.kappa * lnJ - ciso * I1 * (1.0 / 3.0)) * rJ;
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+#pragma unroll
+        for (int K = 0; K < 3; ++K) P[c][K] = fma(ciso, F[c][K], cvol * cof[c][K]);
+    if (m.law == IB_LAW_HO) {
+        double Ff[3], Fs[3];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            Ff[c] = F[c][0] * ef[0] + F[c][1] * ef[1] + F[c][2] * ef[2];
+            Fs[c] = F[c][0] * es[0] + F[c][1] * es[1] + F[c][2] * es[2];
+        }
+        double I4f = Ff[0] * Ff[0] + Ff[1] * Ff[1] + Ff[2] * Ff[2];
+        double I4s = Fs[0] * Fs[0] + Fs[1] * Fs[1] + Fs[2] * Fs[2];
+        double I8 = Ff[0] * Fs[0] + Ff[1] * Fs[1] + Ff[2] * Fs[2];
+        double df = fmax(I4f, 1.0) - 1.0, ds = fmax(I4s, 1.0) - 1.0;
+        double cf = (m.af != 0.0 && df > 0.0) ? 2.0 * m.af * df * exp(m.bf * df * df) : 0.0;
+        double cs = (m.as_ != 0.0 && ds > 0.0) ? 2.0 * m.as_ * ds * exp(m.bs * ds * ds) : 0.0;
+        double cfs = (m.afs != 0.0) ? m.afs * I8 * exp(m.bfs * I8 * I8) : 0.0;
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+#pragma unroll
+            for (int K = 0; K < 3; ++K)
+                P[c][K] += cf * Ff[c] * ef[K] + cs * Fs[c] * es[K] + cfs * (Ff[c] * es[K] + Fs[c] * ef[K]);
+    }
+    return J;
+}
+
+// One thread per Gauss point; lanes 8g..8g+7 of a warp hold the 8 Gauss points of one element.
+__global__ void __launch_bounds__(256)
+ibk_fe_gauss(int64_t n_elems, int64_t n_nodes, const int32_t *__restrict__ conn,
+             const double *__restrict__ X, const double *__restrict__ x,
+             const double *__restrict__ fib, const int32_t *__restrict__ mat_id,
+             const ib_material *__restrict__ mats, double *__restrict__ Ce, long long *status)
+{
+    int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    int64_t e = t >> 3;
+    int q = (int)(t & 7);
+    bool live = e < n_elems;
+    int64_t ee = live ? e : n_elems - 1;          // dead lanes recompute the last element (keeps shuffles uniform)
+    int nd[8];
+    {
+        const int4 *cp = reinterpret_cast<const int4 *>(conn + ee * 8);
+        int4 c0 = __ldg(cp), c1 = __ldg(cp + 1);
+        nd[0] = c0.x; nd[1] = c0.y; nd[2] = c0.z; nd[3] = c0.w;
+        nd[4] = c1.x; nd[5] = c1.y; nd[6] = c1.z; nd[7] = c1.w;
+    }
+    const double g = 0.57735026918962576451;      // 1/sqrt(3): 2x2x2 Gauss rule, weight 1 (L251)
+    double dN[8][3];
+    ib_dshape((q & 1) ? g : -g, (q & 2) ? g : -g, (q & 4) ? g : -g, dN);
+
+    // reference Jacobian J0_{I d} = sum_a X_{a,I} dN_a/dxi_d, and F0_{c d} = sum_a x_{a,c} dN_a/dxi_d
+    double J0[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}}, Fx[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
+    bool finite = true;
+#pragma unroll
+    for (int a = 0; a < 8; ++a) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            double Xa = __ldg(X + c * n_nodes + nd[a]);
+            double xa = __ldg(x + c * n_nodes + nd[a]);
+            finite = finite && isfinite(xa);
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                J0[c][d] = fma(Xa, dN[a][d], J0[c][d]);
+                Fx[c][d] = fma(xa, dN[a][d], Fx[c][d]);
+            }
+        }
+    }
+    // J0^-1 (rows d, cols I): xi-derivative -> X-derivative.  F = Fx * J0^-1.
+    double w = ib_det3(J0);
+    double rw = 1.0 / w;
+    double Ji[3][3];
+    Ji[0][0] = (J0[1][1] * J0[2][2] - J0[1][2] * J0[2][1]) * rw;
+    Ji[0][1] = (J0[0][2] * J0[2][1] - J0[0][1] * J0[2][2]) * rw;
+    Ji[0][2] = (J0[0][1] * J0[1][2] - J0[0][2] * J0[1][1]) * rw;
+    Ji[1][0] = (J0[1][2] * J0[2][0] - J0[1][0] * J0[2][2]) * rw;
+    Ji[1][1] = (J0[0][0] * J0[2][2] - J0[0][2] * J0[2][0]) * rw;
+    Ji[1][2] = (J0[0][2] * J0[1][0] - J0[0][0] * J0[1][2]) * rw;
+    Ji[2][0] = (J0[1][0] * J0[2][1] - J0[1][1] * J0[2][0]) * rw;
+    Ji[2][1] = (J0[0][1] * J0[2][0] - J0[0][0] * J0[2][1]) * rw;
+    Ji[2][2] = (J0[0][0] * J0[1][1] - J0[0][1] * J0[1][0]) * rw;
+    double F[3][3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+#pragma unroll
+        for (int I = 0; I < 3; ++I)
+            F[c][I] = Fx[c][0] * Ji[0][I] + Fx[c][1] * Ji[1][I] + Fx[c][2] * Ji[2][I];
+
+    double ef[3] = {1.0, 0.0, 0.0}, es[3] = {0.0, 1.0, 0.0};
+    if (fib) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            ef[c] = __ldg(fib + c * n_elems + ee);
+            es[c] = __ldg(fib + (3 + c) * n_elems + ee);
+        }
+    }
+    ib_material m = mats[mat_id ? __ldg(mat_id + ee) : 0];
+    double P[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
+    double J = ib_pk1(m, F, ef, es, P);
+    if (live && !finite) ib_latch(status, IB_ERR_NONFINITE, e);
+    else if (live && (!(w > 0.0) || !(J > 0.0))) ib_latch(status, IB_ERR_INVERTED_ELEMENT, e);
+
+    // contribution of this Gauss point to node a:  -(P G_a) w,  G_a = J0^-T dN_a  =>  -(P J0^-T) dN_a w
+    double Q[3][3];                                // Q_{c d} = -w sum_I P_{cI} Ji[d][I]
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+#pragma unroll
+        for (int d = 0; d < 3; ++d)
+            Q[c][d] = -w * (P[c][0] * Ji[d][0] + P[c][1] * Ji[d][1] + P[c][2] * Ji[d][2]);
+    double v[8][3];
+#pragma unroll
+    for (int a = 0; a < 8; ++a)
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+            v[a][c] = Q[c][0] * dN[a][0] + Q[c][1] * dN[a][1] + Q[c][2] * dN[a][2];
+
+    // transposing reduction over the 8 Gauss-point lanes: lane q ends with node q's total
+    const unsigned full = 0xffffffffu;
+    double s4[4][3];
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            double keep = (q & 4) ? v[a + 4][c] : v[a][c];
+            double send = (q & 4) ? v[a][c] : v[a + 4][c];
+            s4[a][c] = keep + __shfl_xor_sync(full, send, 4);
+        }
+    double s2[2][3];
+#pragma unroll
+    for (int a = 0; a < 2; ++a)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            double keep = (q & 2) ? s4[a + 2][c] : s4[a][c];
+            double send = (q & 2) ? s4[a][c] : s4[a + 2][c];
+            s2[a][c] = keep + __shfl_xor_sync(full, send, 2);
+        }
+    double s1[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        double keep = (q & 1) ? s2[1][c] : s2[0][c];
+        double send = (q & 1) ? s2[0][c] : s2[1][c];
+        s1[c] = keep + __shfl_xor_sync(full, send, 1);
+    }
+    if (live) {
+        int64_t ne8 = n_elems * 8;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) Ce[c * ne8 + e * 8 + q] = s1[c];
+    }
+}
+
+// Per node: sum the <= 8 incident element contributions in ascending element order.
+// Optionally also writes Fhat = B / w_a (force density coefficients for the prolongation, A13).
+__global__ void __launch_bounds__(256)
+ibk_node_gather(int64_t n_nodes, int64_t ne8, const int32_t *__restrict__ adj,
+                const double *__restrict__ Ce, const double *__restrict__ wa,
+                double *__restrict__ B, double *__restrict__ Fhat)
+{
+    int64_t n = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= n_nodes) return;
+    double s0 = 0.0, s1 = 0.0, s2 = 0.0;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+        int slot = __ldg(adj + j * n_nodes + n);
+        if (slot >= 0) {
+            s0 += __ldg(Ce + slot);
+            s1 += __ldg(Ce + ne8 + slot);
+            s2 += __ldg(Ce + 2 * ne8 + slot);
+        }
+    }
+    if (B) { B[n] = s0; B[n_nodes + n] = s1; B[2 * n_nodes + n] = s2; }
+    if (Fhat) {
+        double r = 1.0 / __ldg(wa + n);
+        Fhat[n] = s0 * r; Fhat[n_nodes + n] = s1 * r; Fhat[2 * n_nodes + n] = s2 * r;
+    }
+}
+
+ib_status ibk_fe_force(ib_ctx *c, const double *x, double *B, double *Fhat, cudaStream_t st)
+{
+    if (c->n_elems > 0) {
+        int64_t nt = c->n_elems * 8;
+        ibk_fe_gauss<<<ib_blocks(nt, 256), 256, 0, st>>>(c->n_elems, c->n_nodes, c->d_conn, c->d_X, x,
+                                                         c->d_fib, c->d_mat_id, c->d_mats, c->d_Ce,
+                                                         c->d_status);
+        c->launches++;
+    }
+    if (c->n_nodes > 0) {
+        ibk_node_gather<<<ib_blocks(c->n_nodes, 256), 256, 0, st>>>(c->n_nodes, c->n_elems * 8, c->d_adj,
+                                                                    c->d_Ce, c->d_wa, B, Fhat);
+        c->launches++;
+    }
+    IB_CUDA_TRY(cudaGetLastError());
+    return IB_OK;
+}

@@ -1,0 +1,217 @@
+// ib_points.cu -- Lagrangian force points of the sub-point rule, prolongation and restriction
+// (reading A13 of PAPER.md L233-237, L241):
+//   W_s  = det J0(xi_s) 8/(n1 n2 n3)                       (precomputed, reference is static)
+//   w_a  = sum_{e contains a} sum_s W_s N_a(xi_s)          (precomputed, lumped mass)
+//   x_s  = sum_a N_a(xi_s) x_a ;  G_s = W_s sum_a N_a(xi_s) Fhat_a,  Fhat_a = B_a / w_a
+//   Un_a = (1/w_a) sum_{e,s} W_s N_a(xi_s) Up_s            (lumped L2 projection)
+// Node sums use the same deterministic ELL gather as the FE force (no atomics).
+#include "ib_common.cuh"
+
+__device__ __forceinline__ int64_t ib_find_elem(const int64_t *__restrict__ off, int64_t n_elems, int64_t p)
+{
+    int64_t lo = 0, hi = n_elems;                 // off[lo] <= p < off[hi]
+    while (hi - lo > 1) {
+        int64_t mid = (lo + hi) >> 1;
+        if (__ldg(off + mid) <= p) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+
+struct ib_sub {
+    int64_t e;
+    int s, n1, n2, n3;
+};
+
+__device__ __forceinline__ ib_sub ib_locate(int64_t p, int64_t n_elems, int uniform_S,
+                                            const int32_t *__restrict__ nsub,
+                                            const int64_t *__restrict__ off)
+{
+    ib_sub r;
+    if (uniform_S > 0) {
+        r.e = p / uniform_S;
+        r.s = (int)(p - r.e * uniform_S);
+        r.n1 = __ldg(nsub); r.n2 = __ldg(nsub + 1); r.n3 = __ldg(nsub + 2);
+    } else {
+        r.e = ib_find_elem(off, n_elems, p);
+        r.s = (int)(p - __ldg(off + r.e));
+        r.n1 = __ldg(nsub + 3 * r.e); r.n2 = __ldg(nsub + 3 * r.e + 1); r.n3 = __ldg(nsub + 3 * r.e + 2);
+    }
+    return r;
+}
+
+__device__ __forceinline__ void ib_sub_shape(const ib_sub &r, double N[8])
+{
+    int m1 = r.s % r.n1, m2 = (r.s / r.n1) % r.n2, m3 = r.s / (r.n1 * r.n2);
+    ib_shape(ib_subxi(m1, r.n1), ib_subxi(m2, r.n2), ib_subxi(m3, r.n3), N);
+}
+
+// W_s for every sub-point (create time)
+__global__ void __launch_bounds__(256)
+ibk_subpoint_weights(int64_t P, int64_t n_elems, int64_t n_nodes, int uniform_S,
+                     const int32_t *__restrict__ nsub, const int64_t *__restrict__ off,
+                     const int32_t *__restrict__ conn, const double *__restrict__ X,
+                     double *__restrict__ Wp, long long *status)
+{
+    int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= P) return;
+    ib_sub r = ib_locate(p, n_elems, uniform_S, nsub, off);
+    int m1 = r.s % r.n1, m2 = (r.s / r.n1) % r.n2, m3 = r.s / (r.n1 * r.n2);
+    double dN[8][3];
+    ib_dshape(ib_subxi(m1, r.n1), ib_subxi(m2, r.n2), ib_subxi(m3, r.n3), dN);
+    double J0[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
+#pragma unroll
+    for (int a = 0; a < 8; ++a) {
+        int n = __ldg(conn + r.e * 8 + a);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            double Xa = __ldg(X + c * n_nodes + n);
+#pragma unroll
+            for (int d = 0; d < 3; ++d) J0[c][d] = fma(Xa, dN[a][d], J0[c][d]);
+        }
+    }
+    double dj = ib_det3(J0);
+    if (!(dj > 0.0)) ib_latch(status, IB_ERR_INVERTED_ELEMENT, r.e);
+    Wp[p] = dj * 8.0 / (double)(r.n1 * r.n2 * r.n3);
+}
+
+// per element, per local node a: sum_s W_s N_a(xi_s) [* Up_s,c]   (8 lanes per element, lane = node)
+template <int WITH_U>
+__global__ void __launch_bounds__(256)
+ibk_elem_node_sums(int64_t n_elems, int64_t P, const int32_t *__restrict__ nsub,
+                   const int64_t *__restrict__ off, const double *__restrict__ Wp,
+                   const double *__restrict__ Up, double *__restrict__ Ce)
+{
+    int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    int64_t e = t >> 3;
+    int a = (int)(t & 7);
+    if (e >= n_elems) return;
+    int n1 = __ldg(nsub + 3 * e), n2 = __ldg(nsub + 3 * e + 1), n3 = __ldg(nsub + 3 * e + 2);
+    int64_t p0 = __ldg(off + e);
+    double s1 = (a & 1) ? 1.0 : -1.0, s2 = (a & 2) ? 1.0 : -1.0, s3 = (a & 4) ? 1.0 : -1.0;
+    double acc0 = 0.0, acc1 = 0.0, acc2 = 0.0;
+    int s = 0;
+    for (int m3 = 0; m3 < n3; ++m3) {
+        double f3 = 0.5 * fma(s3, ib_subxi(m3, n3), 1.0);
+        for (int m2 = 0; m2 < n2; ++m2) {
+            double f23 = f3 * 0.5 * fma(s2, ib_subxi(m2, n2), 1.0);
+            for (int m1 = 0; m1 < n1; ++m1, ++s) {
+                double Na = f23 * 0.5 * fma(s1, ib_subxi(m1, n1), 1.0);
+                double wn = __ldg(Wp + p0 + s) * Na;
+                if (WITH_U) {
+                    acc0 = fma(wn, __ldg(Up + p0 + s), acc0);
+                    acc1 = fma(wn, __ldg(Up + P + p0 + s), acc1);
+                    acc2 = fma(wn, __ldg(Up + 2 * P + p0 + s), acc2);
+                } else {
+                    acc0 += wn;
+                }
+            }
+        }
+    }
+    int64_t ne8 = n_elems * 8;
+    Ce[e * 8 + a] = acc0;
+    if (WITH_U) { Ce[ne8 + e * 8 + a] = acc1; Ce[2 * ne8 + e * 8 + a] = acc2; }
+}
+
+// per node gather of Ce; mode 0: w_a = sum ; mode 1: Un_c = sum_c / w_a
+template <int WITH_U>
+__global__ void __launch_bounds__(256)
+ibk_node_gather_w(int64_t n_nodes, int64_t ne8, const int32_t *__restrict__ adj,
+                  const double *__restrict__ Ce, double *__restrict__ wa, double *__restrict__ Un)
+{
+    int64_t n = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= n_nodes) return;
+    double s0 = 0.0, s1 = 0.0, s2 = 0.0;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+        int slot = __ldg(adj + j * n_nodes + n);
+        if (slot >= 0) {
+            s0 += __ldg(Ce + slot);
+            if (WITH_U) { s1 += __ldg(Ce + ne8 + slot); s2 += __ldg(Ce + 2 * ne8 + slot); }
+        }
+    }
+    if (WITH_U) {
+        double r = 1.0 / __ldg(wa + n);
+        Un[n] = s0 * r; Un[n_nodes + n] = s1 * r; Un[2 * n_nodes + n] = s2 * r;
+    } else {
+        wa[n] = s0;
+    }
+}
+
+// x_s and G_s for every sub-point
+__global__ void __launch_bounds__(256)
+ibk_points_kernel(int64_t P, int64_t n_elems, int64_t n_nodes, int uniform_S,
+                  const int32_t *__restrict__ nsub, const int64_t *__restrict__ off,
+                  const int32_t *__restrict__ conn, const double *__restrict__ x,
+                  const double *__restrict__ Fhat, const double *__restrict__ Wp,
+                  double *__restrict__ xp, double *__restrict__ Gp)
+{
+    int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= P) return;
+    ib_sub r = ib_locate(p, n_elems, uniform_S, nsub, off);
+    double N[8];
+    ib_sub_shape(r, N);
+    int nd[8];
+    {
+        const int4 *cp = reinterpret_cast<const int4 *>(conn + r.e * 8);
+        int4 c0 = __ldg(cp), c1 = __ldg(cp + 1);
+        nd[0] = c0.x; nd[1] = c0.y; nd[2] = c0.z; nd[3] = c0.w;
+        nd[4] = c1.x; nd[5] = c1.y; nd[6] = c1.z; nd[7] = c1.w;
+    }
+    if (xp) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            double v = 0.0;
+#pragma unroll
+            for (int a = 0; a < 8; ++a) v = fma(N[a], __ldg(x + c * n_nodes + nd[a]), v);
+            xp[c * P + p] = v;
+        }
+    }
+    if (Gp) {
+        double W = __ldg(Wp + p);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            double v = 0.0;
+#pragma unroll
+            for (int a = 0; a < 8; ++a) v = fma(N[a], __ldg(Fhat + c * n_nodes + nd[a]), v);
+            Gp[c * P + p] = W * v;
+        }
+    }
+}
+
+ib_status ibk_precompute_weights(ib_ctx *c, cudaStream_t st)
+{
+    if (c->nodal || c->n_points == 0) return IB_OK;
+    ibk_subpoint_weights<<<ib_blocks(c->n_points, 256), 256, 0, st>>>(
+        c->n_points, c->n_elems, c->n_nodes, c->uniform_S, c->d_nsub, c->d_pt_off, c->d_conn, c->d_X,
+        c->d_Wp, c->d_status);
+    ibk_elem_node_sums<0><<<ib_blocks(c->n_elems * 8, 256), 256, 0, st>>>(
+        c->n_elems, c->n_points, c->d_nsub, c->d_pt_off, c->d_Wp, nullptr, c->d_Ce);
+    ibk_node_gather_w<0><<<ib_blocks(c->n_nodes, 256), 256, 0, st>>>(c->n_nodes, c->n_elems * 8, c->d_adj,
+                                                                      c->d_Ce, c->d_wa, nullptr);
+    c->launches += 3;
+    IB_CUDA_TRY(cudaGetLastError());
+    return IB_OK;
+}
+
+ib_status ibk_points(ib_ctx *c, const double *x, const double *Fhat, double *xp, double *Gp, cudaStream_t st)
+{
+    if (c->n_points == 0) return IB_OK;
+    ibk_points_kernel<<<ib_blocks(c->n_points, 256), 256, 0, st>>>(
+        c->n_points, c->n_elems, c->n_nodes, c->uniform_S, c->d_nsub, c->d_pt_off, c->d_conn, x, Fhat,
+        c->d_Wp, xp, Gp);
+    c->launches++;
+    IB_CUDA_TRY(cudaGetLastError());
+    return IB_OK;
+}
+
+ib_status ibk_restrict(ib_ctx *c, const double *Up, double *Un, cudaStream_t st)
+{
+    if (c->n_elems == 0 || c->n_nodes == 0) return IB_OK;
+    ibk_elem_node_sums<1><<<ib_blocks(c->n_elems * 8, 256), 256, 0, st>>>(
+        c->n_elems, c->n_points, c->d_nsub, c->d_pt_off, c->d_Wp, Up, c->d_Ce);
+    ibk_node_gather_w<1><<<ib_blocks(c->n_nodes, 256), 256, 0, st>>>(c->n_nodes, c->n_elems * 8, c->d_adj,
+                                                                      c->d_Ce, c->d_wa, Un);
+    c->launches += 2;
+    IB_CUDA_TRY(cudaGetLastError());
+    return IB_OK;
+}

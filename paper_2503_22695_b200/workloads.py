@@ -292,11 +292,24 @@ def _leaflet(idx, n1=64, n2=48, n3=2, thick=0.05, x_base=3.3, height=1.4, r_wall
     r, s, q = i.ravel() / n1, j.ravel() / n2, k.ravel() / n3
 
     def mid(r, s):
-        phi = np.deg2rad(120.0 * idx + 6.0 + 108.0 * r)
-        bulge = np.sin(np.pi * r) * s ** 1.5
-        rho = r_wall - 0.02 - (r_wall - 0.02 - 0.15) * bulge
+        # attachment arc on the wall and a free edge that is a quadratic Bezier curve from
+        # commissure to commissure dipping to 0.15 cm from the axis, blended by g(s) = s^1.5;
+        # element sizes stay ~uniform (a polar parametrisation would shrink them near the axis)
+        rw = r_wall - 0.02
+        phi0 = np.deg2rad(120.0 * idx + 6.0)
+        phi1 = phi0 + np.deg2rad(108.0)
+        phim = 0.5 * (phi0 + phi1)
+        A = rw * np.array([np.cos(phi0), np.sin(phi0)])
+        Bp = rw * np.array([np.cos(phi1), np.sin(phi1)])
+        em = np.array([np.cos(phim), np.sin(phim)])
+        Cc = 2.0 * (0.15 * em - 0.25 * (A + Bp))
+        phi = phi0 + (phi1 - phi0) * r
+        att = rw * np.stack([np.cos(phi), np.sin(phi)])
+        free = ((1 - r) ** 2)[None] * A[:, None] + (2 * r * (1 - r))[None] * Cc[:, None] + (r ** 2)[None] * Bp[:, None]
+        gs = s ** 1.5
+        yz = (1 - gs)[None] * att + gs[None] * free
         xx = x_base + height * s * (0.55 + 0.45 * np.sin(np.pi * r))
-        return np.stack([xx, yc + rho * np.cos(phi), zc + rho * np.sin(phi)]), phi
+        return np.stack([xx, yc + yz[0], zc + yz[1]]), phi
 
     P, _ = mid(r, s)
     d = 1e-6

@@ -1,0 +1,215 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle on identical seeded inputs.
+
+Bar (BASELINE.json north_star): fp64 rel-L2 <= 1e-12 and max-abs <= 1e-10 x ||oracle||_inf per output
+array (A20); bit-exact for the integer binning/sort permutation.
+"""
+import numpy as np
+import pytest
+
+from helpers import distorted_block, max_abs_scaled, rel_l2
+from paper_2503_22695_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+REL, MAXABS = 1e-12, 1e-10
+
+
+@pytest.fixture(scope="module")
+def ib():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    from paper_2503_22695_b200 import build, ibcouple
+    build.build()
+    ibcouple.lib()
+    return ibcouple
+
+
+def _t(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _close(got, exp, what):
+    got = got.cpu().numpy() if hasattr(got, "cpu") else got
+    r, m = rel_l2(got, exp), max_abs_scaled(got, exp)
+    assert r <= REL and m <= MAXABS, f"{what}: rel-L2 {r:.3e} max-abs/scale {m:.3e}"
+    return r, m
+
+
+def _grid(orc, wl):
+    return orc.make_grid(wl.nx, wl.ny, wl.nz, wl.h, wl.origin)
+
+
+def _run_step(ib, wl, variant, nodal=False):
+    import torch
+    ctx = ib.Context.from_workload(wl, nodal=nodal)
+    ctx.ib_set_variant(variant)
+    x, u, v, w = _t(wl.x), _t(wl.u), _t(wl.v), _t(wl.w)
+    fu, fv, fw = (torch.full((wl.n_cells,), 7.0, dtype=torch.float64, device="cuda") for _ in range(3))
+    Un = torch.empty((3, wl.n_nodes), dtype=torch.float64, device="cuda")
+    B = torch.empty((3, wl.n_nodes), dtype=torch.float64, device="cuda")
+    ctx.ib_coupling_step(x, u, v, w, fu, fv, fw, Un, B)
+    ctx.check()
+    out = dict(fu=fu.cpu().numpy(), fv=fv.cpu().numpy(), fw=fw.cpu().numpy(), Un=Un.cpu().numpy(), B=B.cpu().numpy())
+    ctx.close()
+    return out
+
+
+CONFIGS = {
+    "C1": lambda: W.config1(),
+    "C1-wrap": lambda: W.config1(shift_cells=(14, 15, 17)),      # block straddles the periodic wrap (A18)
+    "C2": lambda: W.config2(),
+    "LV-small": lambda: W.lv_small(),
+}
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("name", list(CONFIGS))
+def test_coupling_step_matches_oracle(ib, orc, name, variant):
+    wl = CONFIGS[name]()
+    ref = orc.coupling_step(_grid(orc, wl), wl.conn, wl.X, wl.fibers, wl.mat_id, wl.nsub, wl.mats, wl.x, wl.u, wl.v, wl.w)
+    got = _run_step(ib, wl, variant)
+    for k in ("B", "fu", "fv", "fw", "Un"):
+        _close(got[k], ref[k], f"{name} v{variant} {k}")
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_nodal_mode_matches_oracle(ib, orc, variant):
+    wl = W.config1()
+    ref = orc.coupling_step(_grid(orc, wl), wl.conn, wl.X, wl.fibers, wl.mat_id, None, wl.mats, wl.x, wl.u, wl.v, wl.w)
+    got = _run_step(ib, wl, variant, nodal=True)
+    for k in ("B", "fu", "fv", "fw", "Un"):
+        _close(got[k], ref[k], f"nodal v{variant} {k}")
+
+
+def test_fe_force_pieces_and_determinism(ib, orc):
+    import torch
+    conn, X, x, fib = distorted_block(5, 4, 3, seed=8)
+    ne, nn = conn.shape[0], X.shape[1]
+    rng = np.random.default_rng(0)
+    mats = [W.material(W.LAW_NEOHOOKEAN, a=1e4, kappa=1e6), W.material(W.LAW_HO, **W.HO_LV)]
+    mid = rng.integers(0, 2, ne).astype(np.int32)
+    nsub = rng.integers(1, 5, (ne, 3)).astype(np.int32)        # ragged sub-point counts
+    ctx = ib.Context(16, 16, 16, 1 / 16, (0, 0, 0), conn, X, fib, mid, nsub, mats)
+    xd = _t(x)
+    B = torch.empty((3, nn), dtype=torch.float64, device="cuda")
+    ctx.ib_fe_force(xd, B)
+    ctx.check()
+    ref = orc.fe_force(conn, X, x, fib, mid, mats)
+    _close(B, ref["B"], "fe_force B")
+    B2 = torch.empty_like(B)
+    ctx.ib_fe_force(xd, B2)
+    assert torch.equal(B, B2)                                     # node-gathered: bit-reproducible
+    # points / prolongation / restriction
+    P = ctx.n_points
+    xp_r, Wp_r, wa_r = orc.points(conn, X, x, nsub)
+    assert P == xp_r.shape[1]
+    xp = torch.empty((3, P), dtype=torch.float64, device="cuda")
+    Gp = torch.empty((3, P), dtype=torch.float64, device="cuda")
+    ctx.ib_points(xd, B, xp, Gp)
+    _close(xp, xp_r, "xp")
+    _close(Gp, orc.prolong(conn, nsub, wa_r, Wp_r, ref["B"]), "Gp")
+    Up = rng.normal(size=(3, P))
+    Un = torch.empty((3, nn), dtype=torch.float64, device="cuda")
+    ctx.ib_restrict(_t(Up), Un)
+    ctx.check()
+    _close(Un, orc.restrict(conn, nsub, wa_r, Wp_r, Up), "Un")
+    ctx.close()
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_spread_interp_generic_cloud(ib, orc, variant):
+    import torch
+    n, h, org = (24, 16, 32), 0.05, (-0.4, 0.1, 0.3)
+    ctx = ib.Context(*n, h, org, np.zeros((0, 8), np.int32), np.zeros((3, 0)), None, None, None, [])
+    ctx.ib_set_variant(variant)
+    g = orc.make_grid(*n, h, org)
+    rng = np.random.default_rng(3)
+    L = np.array(n) * h
+    P = 20011                                                  # ragged tail
+    xp = np.asarray(org)[:, None] + rng.uniform(-0.5, 1.5, (3, P)) * L[:, None]     # outside the box too
+    xp[:, :64] = np.asarray(org)[:, None] + (rng.integers(0, 24, (3, 64)) * h)      # exactly on cell boundaries
+    G = rng.normal(size=(3, P))
+    ncell = n[0] * n[1] * n[2]
+    uvw = rng.normal(size=(3, ncell))
+    f = [torch.full((ncell,), 3.0, dtype=torch.float64, device="cuda") for _ in range(3)]
+    ctx.ib_spread(_t(xp), _t(G), P, *f, accumulate=0)
+    Up = torch.empty((3, P), dtype=torch.float64, device="cuda")
+    ctx.ib_interp(_t(xp), P, _t(uvw[0]), _t(uvw[1]), _t(uvw[2]), Up)
+    ctx.check()
+    fr = orc.spread(g, xp, G)
+    for c in range(3):
+        _close(f[c], fr[c], f"spread c{c}")
+    _close(Up, orc.interp(g, xp, *uvw), "interp")
+    # accumulate=1 adds to what is there
+    ctx.ib_spread(_t(xp), _t(G), P, *f, accumulate=1)
+    for c in range(3):
+        _close(f[c], 2 * fr[c], f"spread accumulate c{c}")
+    # empty cloud: zero-fill only
+    ctx.ib_spread(None, None, 0, *f, accumulate=0)
+    assert all(float(t.abs().max()) == 0.0 for t in f)
+    # GPU-vs-GPU adjointness
+    ctx.ib_spread(_t(xp), _t(G), P, *f, accumulate=0)
+    lhs = h ** 3 * sum(float(torch.dot(f[c], _t(uvw[c]))) for c in range(3))
+    rhs = float((Up * _t(G)).sum())
+    assert abs(lhs - rhs) < 1e-11 * abs(rhs)
+    ctx.close()
+
+
+def test_bin_sort_bit_exact(ib, orc):
+    import torch
+    for n, P in (((16, 8, 24), 0), ((16, 8, 24), 1), ((16, 8, 24), 5000), ((64, 64, 64), 300007)):
+        h, org = 0.25, (-1.0, 0.5, 2.0)
+        ctx = ib.Context(*n, h, org, np.zeros((0, 8), np.int32), np.zeros((3, 0)), None, None, None, [])
+        rng = np.random.default_rng(P)
+        xp = np.asarray(org)[:, None] + rng.uniform(-0.2, 1.2, (3, P)) * (np.array(n) * h)[:, None]
+        if P > 100:
+            xp[:, :50] = np.asarray(org)[:, None] + rng.integers(0, 8, (3, 50)) * h     # exact boundaries
+            xp[:, 50:100] = xp[:, 100:101]                                              # many ties
+        key = torch.empty(P, dtype=torch.int64, device="cuda")
+        perm = torch.empty(P, dtype=torch.int32, device="cuda")
+        ctx.ib_bin_sort(_t(xp) if P else None, P, key, perm)
+        ctx.check()
+        k_ref, p_ref = orc.bin_sort(orc.make_grid(*n, h, org), xp)
+        assert np.array_equal(key.cpu().numpy(), k_ref)
+        assert np.array_equal(perm.cpu().numpy(), p_ref)
+        ctx.close()
+
+
+def test_error_latch_inverted_element_and_nan(ib):
+    import torch
+    conn, X, x, fib = distorted_block(3, 3, 2, seed=9)
+    nn = X.shape[1]
+    ctx = ib.Context(16, 16, 16, 1 / 16, (0, 0, 0), conn, X, fib, None, None, [W.material(0, a=1.0, kappa=10.0)])
+    B = torch.empty((3, nn), dtype=torch.float64, device="cuda")
+    xi = x.copy()
+    n0, n7 = conn[7, 0], conn[7, 7]
+    xi[:, n0] = x[:, n7] + (x[:, n7] - x[:, n0])
+    ctx.ib_fe_force(_t(xi), B)
+    code, bad = ctx.ib_check()
+    assert code == 5 and bad >= 0
+    xn = x.copy()
+    xn[1, 3] = np.nan
+    ctx.ib_fe_force(_t(xn), B)
+    code, bad = ctx.ib_check()
+    assert code == 6
+    ctx.ib_fe_force(_t(x), B)                                    # latch was cleared
+    assert ctx.ib_check()[0] == 0
+    ctx.close()
+
+
+def test_host_entry_point_matches_device_path(ib):
+    import torch
+    wl = W.config1()
+    ctx = ib.Context.from_workload(wl)
+    dev = _run_step(ib, wl, 0)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    outs = [torch.empty(wl.n_cells, dtype=torch.float64).pin_memory() for _ in range(3)]
+    Un = torch.empty((3, wl.n_nodes), dtype=torch.float64).pin_memory()
+    B = torch.empty((3, wl.n_nodes), dtype=torch.float64).pin_memory()
+    ctx.ib_set_variant(0)
+    ctx.ib_coupling_step_host(pin(wl.x), pin(wl.u), pin(wl.v), pin(wl.w), *outs, Un, B)
+    assert np.array_equal(B.numpy(), dev["B"])
+    _close(outs[0].numpy(), dev["fu"], "host fu")
+    _close(Un.numpy(), dev["Un"], "host Un")
+    ctx.close()
