@@ -152,6 +152,15 @@ int64_t ib_launch_count(const ib_ctx *ctx);
  * Default 1. Returns IB_ERR_INVALID_ARG for other values. */
 ib_status ib_set_variant(ib_ctx *ctx, int32_t variant);
 
+/* Per-phase device timing with CUDA events recorded on the launching stream (used by bench.py for
+ * the roofline of the dominant kernel). Phases of ib_coupling_step / ib_spread / ib_interp: */
+enum { IB_PHASE_FE_FORCE = 0, IB_PHASE_POINTS = 1, IB_PHASE_SORT = 2, IB_PHASE_SPREAD_INTERP = 3,
+       IB_PHASE_RESTRICT = 4, IB_PHASE_ZERO = 5, IB_PHASE_COUNT = 6 };
+ib_status ib_profile_enable(ib_ctx *ctx, int32_t on);
+/* Synchronises the recorded events, adds up milliseconds and call counts per phase since the last
+ * read into ms_sum[IB_PHASE_COUNT] / calls[IB_PHASE_COUNT], and resets the accumulators. */
+ib_status ib_profile_read(ib_ctx *ctx, double *ms_sum, int64_t *calls);
+
 /* FP64 FMA peak probe: runs a register-only DFMA loop on `device`; returns achieved DFMA/s in
  * *dfma_per_s and the kernel time in *ms. Used by bench.py for the "alu" roofline denominator. */
 ib_status ib_probe_dfma(int32_t device, double *dfma_per_s, double *ms);

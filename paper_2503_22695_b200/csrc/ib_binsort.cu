@@ -190,14 +190,15 @@ ibk_radix_scatter(const uint32_t *__restrict__ keys_in, const int32_t *__restric
     }
 }
 
-// start rank of every tile (n_tiles+1 entries) from the sorted keys
+// start rank of every tile (n_tiles+1 entries) from the sorted keys; tile = key >> shift
 __global__ void __launch_bounds__(256)
-ibk_tile_starts(const uint32_t *__restrict__ skeys, int64_t P, int n_tiles, int32_t *__restrict__ tile_start)
+ibk_tile_starts_shift(const uint32_t *__restrict__ skeys, int64_t P, int n_tiles, int shift,
+                      int32_t *__restrict__ tile_start)
 {
     int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (r > P) return;
-    int t = (r < P) ? (int)(skeys[r] >> 9) : n_tiles;
-    int tp = (r > 0) ? (int)(skeys[r - 1] >> 9) : -1;
+    int t = (r < P) ? (int)(skeys[r] >> shift) : n_tiles;
+    int tp = (r > 0) ? (int)(skeys[r - 1] >> shift) : -1;
     for (int tt = tp + 1; tt <= t; ++tt) tile_start[tt] = (int32_t)r;
 }
 
@@ -232,49 +233,55 @@ ib_status ibk_sort_reserve(ib_ctx *c, int64_t P)
     return IB_OK;
 }
 
-// Sort. On return d_key[0]/d_val[0] hold the sorted keys / permutation (result is copied back to
-// buffer 0 when the pass count is odd); d_cell_start holds tile starts when build_cells != 0.
+// LSD radix sort of the `bits` low bits of the keys in d_key[0] (values = point ids, implicit
+// iota on the first pass). On return the sorted keys / permutation are in d_key[0] / d_val[0]
+// (copied back when the pass count is odd).
+ib_status ibk_sort_keys_inplace(ib_ctx *c, int64_t P, int bits, cudaStream_t st)
+{
+    if (P <= 0) return IB_OK;
+    int passes = (bits + 7) / 8;
+    int nb = (int)((P + RS_TILE - 1) / RS_TILE);
+    int64_t hl = 256ll * nb;
+    int nsum = (int)((hl + SC_TILE - 1) / SC_TILE);
+    uint32_t *sums = c->d_hist + hl;
+    int cur = 0;
+    for (int ps = 0; ps < passes; ++ps) {
+        int shift = 8 * ps;
+        ibk_radix_hist<<<nb, RS_THREADS, 0, st>>>(c->d_key[cur], P, shift, c->d_hist, nb);
+        ibk_scan_reduce<<<nsum, SC_THREADS, 0, st>>>(c->d_hist, hl, sums);
+        ibk_scan_sums<<<1, 1024, 0, st>>>(sums, nsum);
+        ibk_scan_apply<<<nsum, SC_THREADS, 0, st>>>(c->d_hist, hl, sums);
+        ibk_radix_scatter<<<nb, RS_THREADS, 0, st>>>(c->d_key[cur], ps == 0 ? nullptr : c->d_val[cur],
+                                                     c->d_key[cur ^ 1], c->d_val[cur ^ 1], P, shift,
+                                                     c->d_hist, nb);
+        c->launches += 5;
+        cur ^= 1;
+    }
+    if (cur != 0) {
+        IB_CUDA_TRY(cudaMemcpyAsync(c->d_key[0], c->d_key[1], P * sizeof(uint32_t), cudaMemcpyDeviceToDevice, st));
+        IB_CUDA_TRY(cudaMemcpyAsync(c->d_val[0], c->d_val[1], P * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+    }
+    IB_CUDA_TRY(cudaGetLastError());
+    return IB_OK;
+}
+
 ib_status ibk_bin_sort(ib_ctx *c, const double *xp, int64_t P, int64_t *key_out, int32_t *perm_out,
                        int build_cells, cudaStream_t st)
 {
     ib_status rs = ibk_sort_reserve(c, P);
     if (rs != IB_OK) return rs;
-    int n_tiles = (int)(c->n_cells / IB_TILE_CELLS);
+    (void)build_cells;
     if (P > 0) {
         ibk_keys<<<ib_blocks(P, 256), 256, 0, st>>>(P, xp, c->grid, c->inv_h, c->d_key[0], key_out, c->d_status);
         c->launches++;
         int bits = 1;
         while ((1ll << bits) < c->n_cells) ++bits;
-        int passes = (bits + 7) / 8;
-        int nb = (int)((P + RS_TILE - 1) / RS_TILE);
-        int64_t hl = 256ll * nb;
-        int nsum = (int)((hl + SC_TILE - 1) / SC_TILE);
-        uint32_t *sums = c->d_hist + hl;
-        int cur = 0;
-        for (int ps = 0; ps < passes; ++ps) {
-            int shift = 8 * ps;
-            ibk_radix_hist<<<nb, RS_THREADS, 0, st>>>(c->d_key[cur], P, shift, c->d_hist, nb);
-            ibk_scan_reduce<<<nsum, SC_THREADS, 0, st>>>(c->d_hist, hl, sums);
-            ibk_scan_sums<<<1, 1024, 0, st>>>(sums, nsum);
-            ibk_scan_apply<<<nsum, SC_THREADS, 0, st>>>(c->d_hist, hl, sums);
-            ibk_radix_scatter<<<nb, RS_THREADS, 0, st>>>(c->d_key[cur], ps == 0 ? nullptr : c->d_val[cur],
-                                                         c->d_key[cur ^ 1], c->d_val[cur ^ 1], P, shift,
-                                                         c->d_hist, nb);
-            c->launches += 5;
-            cur ^= 1;
-        }
-        if (cur != 0) {
-            IB_CUDA_TRY(cudaMemcpyAsync(c->d_key[0], c->d_key[1], P * sizeof(uint32_t), cudaMemcpyDeviceToDevice, st));
-            IB_CUDA_TRY(cudaMemcpyAsync(c->d_val[0], c->d_val[1], P * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
-        }
+        rs = ibk_sort_keys_inplace(c, P, bits, st);
+        if (rs != IB_OK) return rs;
         if (perm_out) {
             ibk_copy_perm<<<ib_blocks(P, 256), 256, 0, st>>>(c->d_val[0], perm_out, P);
             c->launches++;
         }
-    }
-    if (build_cells) {
-        ibk_tile_starts<<<ib_blocks(P + 1, 256), 256, 0, st>>>(c->d_key[0], P, n_tiles, c->d_cell_start);
-        c->launches++;
     }
     IB_CUDA_TRY(cudaGetLastError());
     return IB_OK;

@@ -51,7 +51,13 @@ struct ib_ctx {
     long long *d_status;
     cudaStream_t last_stream;
     int64_t launches;
+    // optional per-phase event timing
+    int profile;
+    void *prof;                // std::vector<ib_prof_rec>* (ib_context.cu)
 };
+
+void ib_prof_begin(ib_ctx *c, int phase, cudaStream_t st);
+void ib_prof_end(ib_ctx *c, int phase, cudaStream_t st);
 
 #define IB_CUDA_TRY(expr)                                   \
     do {                                                    \

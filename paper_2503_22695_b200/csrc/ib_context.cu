@@ -25,6 +25,56 @@ static ib_status dev_upload(T **dst, const T *src, size_t n)
     return IB_OK;
 }
 
+struct ib_prof_rec { int phase; cudaEvent_t e0, e1; };
+typedef std::vector<ib_prof_rec> ib_prof_vec;
+
+void ib_prof_begin(ib_ctx *c, int phase, cudaStream_t st)
+{
+    if (!c->profile) return;
+    ib_prof_vec *v = (ib_prof_vec *)c->prof;
+    ib_prof_rec r;
+    r.phase = phase;
+    cudaEventCreate(&r.e0);
+    cudaEventCreate(&r.e1);
+    cudaEventRecord(r.e0, st);
+    v->push_back(r);
+}
+
+void ib_prof_end(ib_ctx *c, int phase, cudaStream_t st)
+{
+    if (!c->profile) return;
+    ib_prof_vec *v = (ib_prof_vec *)c->prof;
+    for (size_t i = v->size(); i-- > 0;)
+        if ((*v)[i].phase == phase) { cudaEventRecord((*v)[i].e1, st); return; }
+}
+
+extern "C" ib_status ib_profile_enable(ib_ctx *c, int32_t on)
+{
+    if (!c) return IB_ERR_INVALID_ARG;
+    if (!c->prof) c->prof = new ib_prof_vec();
+    c->profile = on ? 1 : 0;
+    return IB_OK;
+}
+
+extern "C" ib_status ib_profile_read(ib_ctx *c, double *ms_sum, int64_t *calls)
+{
+    if (!c || !ms_sum || !calls) return IB_ERR_INVALID_ARG;
+    for (int i = 0; i < IB_PHASE_COUNT; ++i) { ms_sum[i] = 0.0; calls[i] = 0; }
+    if (!c->prof) return IB_OK;
+    ib_prof_vec *v = (ib_prof_vec *)c->prof;
+    for (auto &r : *v) {
+        float ms = 0.f;
+        if (cudaEventSynchronize(r.e1) == cudaSuccess && cudaEventElapsedTime(&ms, r.e0, r.e1) == cudaSuccess) {
+            ms_sum[r.phase] += ms;
+            calls[r.phase]++;
+        }
+        cudaEventDestroy(r.e0);
+        cudaEventDestroy(r.e1);
+    }
+    v->clear();
+    return IB_OK;
+}
+
 extern "C" const char *ib_status_string(ib_status s)
 {
     switch (s) {
@@ -58,6 +108,12 @@ extern "C" ib_status ib_destroy(ib_ctx *c)
                     c->d_hUn, c->d_hB, c->d_status};
     for (void *p : ptrs)
         if (p) cudaFree(p);
+    if (c->prof) {
+        double ms[IB_PHASE_COUNT];
+        int64_t n[IB_PHASE_COUNT];
+        ib_profile_read(c, ms, n);
+        delete (ib_prof_vec *)c->prof;
+    }
     delete c;
     return IB_OK;
 }
@@ -124,7 +180,7 @@ extern "C" ib_status ib_create(ib_ctx **out, const ib_grid_desc *g, const ib_mes
     c->n_points = c->nodal ? nn : off[ne];
     c->uniform_S = uniform;
     c->n_mats = m->n_mats;
-    c->variant = 0;
+    c->variant = 1;
 
     ib_status s = IB_OK;
 #define TRY(x) do { if (s == IB_OK) s = (x); } while (0)
@@ -147,7 +203,7 @@ extern "C" ib_status ib_create(ib_ctx **out, const ib_grid_desc *g, const ib_mes
         TRY(dev_alloc((void **)&c->d_Gp, P * 3 * sizeof(double)));
         TRY(dev_alloc((void **)&c->d_Up, P * 3 * sizeof(double)));
     }
-    const int n_tiles = (int)(c->n_cells / IB_TILE_CELLS);
+    const int n_tiles = (int)(c->n_cells / 64);          // 4x4x4-cell tiles of the tiled path
     TRY(dev_alloc((void **)&c->d_cell_start, (size_t)(n_tiles + 1) * sizeof(int32_t)));
     TRY(dev_alloc((void **)&c->d_tile_list, (size_t)(n_tiles + 1) * sizeof(int32_t)));
     TRY(dev_alloc((void **)&c->d_tile_count, 64 * sizeof(int32_t)));
@@ -284,17 +340,26 @@ extern "C" ib_status ib_coupling_step(ib_ctx *c, const double *x, const double *
     double *Bd = B ? B : c->d_B;
     if (c->nodal) {
         // the paper's nodal rule verbatim (L241-257): points = nodes, spread B itself, Un = U^IB
+        ib_prof_begin(c, IB_PHASE_FE_FORCE, st);
         s = ibk_fe_force(c, x, Bd, nullptr, st);
+        ib_prof_end(c, IB_PHASE_FE_FORCE, st);
         if (s != IB_OK) return s;
         return ibk_spread_interp(c, x, Bd, c->n_nodes, u, v, w, fu, fv, fw, Un, 0, st);
     }
+    ib_prof_begin(c, IB_PHASE_FE_FORCE, st);
     s = ibk_fe_force(c, x, Bd, c->d_Fhat, st);
+    ib_prof_end(c, IB_PHASE_FE_FORCE, st);
     if (s != IB_OK) return s;
+    ib_prof_begin(c, IB_PHASE_POINTS, st);
     s = ibk_points(c, x, c->d_Fhat, c->d_xp, c->d_Gp, st);
+    ib_prof_end(c, IB_PHASE_POINTS, st);
     if (s != IB_OK) return s;
     s = ibk_spread_interp(c, c->d_xp, c->d_Gp, c->n_points, u, v, w, fu, fv, fw, c->d_Up, 0, st);
     if (s != IB_OK) return s;
-    return ibk_restrict(c, c->d_Up, Un, st);
+    ib_prof_begin(c, IB_PHASE_RESTRICT, st);
+    s = ibk_restrict(c, c->d_Up, Un, st);
+    ib_prof_end(c, IB_PHASE_RESTRICT, st);
+    return s;
 }
 
 extern "C" ib_status ib_coupling_step_host(ib_ctx *c, const double *x_h, const double *u_h, const double *v_h,

@@ -95,19 +95,23 @@ ib_status ibk_spread_interp(ib_ctx *c, const double *xp, const double *Gp, int64
     const bool sp = Gp != nullptr, in = Up != nullptr;
     if (sp && !accumulate) {
         size_t nb = (size_t)c->n_cells * sizeof(double);
+        ib_prof_begin(c, IB_PHASE_ZERO, st);
         IB_CUDA_TRY(cudaMemsetAsync(fu, 0, nb, st));
         IB_CUDA_TRY(cudaMemsetAsync(fv, 0, nb, st));
         IB_CUDA_TRY(cudaMemsetAsync(fw, 0, nb, st));
+        ib_prof_end(c, IB_PHASE_ZERO, st);
     }
     if (P == 0) return IB_OK;
     if (c->variant == 1) return ibk_tiled_spread_interp(c, xp, Gp, P, u, v, w, fu, fv, fw, Up, st);
     unsigned nb = ib_blocks(P, 128);
+    ib_prof_begin(c, IB_PHASE_SPREAD_INTERP, st);
     if (sp && in)
         ibk_point_kernel<1, 1><<<nb, 128, 0, st>>>(P, xp, Gp, u, v, w, fu, fv, fw, Up, c->grid, c->inv_h, c->d_status);
     else if (sp)
         ibk_point_kernel<1, 0><<<nb, 128, 0, st>>>(P, xp, Gp, u, v, w, fu, fv, fw, Up, c->grid, c->inv_h, c->d_status);
     else if (in)
         ibk_point_kernel<0, 1><<<nb, 128, 0, st>>>(P, xp, Gp, u, v, w, fu, fv, fw, Up, c->grid, c->inv_h, c->d_status);
+    ib_prof_end(c, IB_PHASE_SPREAD_INTERP, st);
     c->launches++;
     IB_CUDA_TRY(cudaGetLastError());
     return IB_OK;

@@ -21,6 +21,7 @@ STATUS = {0: "IB_OK", 1: "IB_ERR_INVALID_ARG", 2: "IB_ERR_UNSUPPORTED", 3: "IB_E
 EXPORTS = ["ib_create", "ib_destroy", "ib_num_points", "ib_num_nodes", "ib_num_elems", "ib_fe_force",
            "ib_points", "ib_restrict", "ib_bin_sort", "ib_spread", "ib_interp", "ib_coupling_step",
            "ib_coupling_step_host", "ib_check", "ib_launch_count", "ib_set_variant", "ib_probe_dfma",
+           "ib_profile_enable", "ib_profile_read",
            "ib_status_string"]
 
 
@@ -70,6 +71,8 @@ def lib():
         L.ib_coupling_step_host.argtypes = [vp] * 11
         L.ib_check.argtypes = [vp, C.POINTER(i64)]
         L.ib_set_variant.argtypes = [vp, i32]
+        L.ib_profile_enable.argtypes = [vp, i32]
+        L.ib_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(i64)]
         L.ib_probe_dfma.argtypes = [i32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.ib_status_string.argtypes = [i32]
         L.ib_status_string.restype = C.c_char_p
@@ -154,6 +157,18 @@ class Context:
     # ---- the C ABI, same names ---------------------------------------------------------------
     def ib_set_variant(self, variant):
         _chk(lib().ib_set_variant(self._h, int(variant)), "ib_set_variant")
+
+    PHASES = ("fe_force", "points", "sort", "spread_interp", "restrict", "zero")
+
+    def ib_profile_enable(self, on=True):
+        _chk(lib().ib_profile_enable(self._h, int(bool(on))), "ib_profile_enable")
+
+    def ib_profile_read(self):
+        """{phase: (ms_sum, calls)} since the last read."""
+        ms = (C.c_double * len(self.PHASES))()
+        n = (C.c_int64 * len(self.PHASES))()
+        _chk(lib().ib_profile_read(self._h, ms, n), "ib_profile_read")
+        return {k: (ms[i], int(n[i])) for i, k in enumerate(self.PHASES)}
 
     def ib_launch_count(self):
         return int(lib().ib_launch_count(self._h))
