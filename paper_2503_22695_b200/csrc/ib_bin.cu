@@ -1,0 +1,279 @@
+// ib_bin.cu -- tile-level counting sort of the Lagrangian force points (SURVEY.md §8(a) a4+a5 fused).
+// Not in the paper (north_star: "points binned and sorted by Eulerian cell").
+//
+// Points are grouped by 4x4x4-cell tile with a counting sort: count pass -> single-CTA scan ->
+// scatter pass that writes the point records (x_s, G_s, id) contiguously per tile.  The order of
+// points inside a tile is whatever the atomics give; the tile kernel (ib_tiled.cu) sorts them by
+// half-cell in shared memory.  Two point sources:
+//   cloud : xp/Gp arrays given by the caller (ib_spread / ib_interp, nodal rule of L241)
+//   mesh  : sub-points generated on the fly from the element nodes -- x_s = sum_a N_a(xi_s) x_a,
+//           G_s = W_s sum_a N_a(xi_s) Fhat_a (reading A13) -- one thread per row of n1 sub-points,
+//           so the element-ordered xp/Gp arrays never touch HBM in ib_coupling_step.
+// The cell of a point is the binning formula of A21 (IEEE double, no contraction); positions are
+// computed with explicit __fma_rn/__dmul_rn so that the count and scatter passes agree bit for bit.
+#include "ib_common.cuh"
+
+#define BT 4                       // tile edge in cells
+
+struct ib_bin_params {
+    // cloud source
+    int64_t P;
+    const double *xp, *Gp;
+    // mesh source
+    int64_t n_rows, n_elems, n_nodes;
+    int un1, un2, un3;             // uniform nsub (un1 == 0: per-element nsub / row_off / pt_off)
+    const int32_t *nsub;
+    const int64_t *pt_off, *row_off;
+    const int32_t *conn;
+    const double *x, *Fhat, *Wp;
+    // grid
+    ib_grid_desc g;
+    double inv_h;
+    // bins
+    int32_t *tile_cur;             // count pass: counts; scatter pass: running cursors
+    double *sx, *sG;               // [3][P] sorted records
+    int32_t *sid;                  // [P] original point id
+    double *Up;                    // non-finite points get Up = 0 (scatter pass), may be NULL
+    long long *status;
+};
+
+__device__ __forceinline__ int ib_tile_of(double x, double y, double z, const ib_grid_desc &g, double inv_h)
+{
+    int cx = ib_cell(x, g.x0, inv_h, g.nx), cy = ib_cell(y, g.y0, inv_h, g.ny), cz = ib_cell(z, g.z0, inv_h, g.nz);
+    return ((cz >> 2) * (g.ny / BT) + (cy >> 2)) * (g.nx / BT) + (cx >> 2);
+}
+
+// warp-aggregated count / slot allocation; every lane of the warp must call (valid may differ)
+template <int SCATTER>
+__device__ __forceinline__ int ib_bin_slot(bool valid, int tile, int32_t *tile_cur)
+{
+    const unsigned full = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    unsigned act = __ballot_sync(full, valid);
+    int pos = -1;
+    if (valid) {
+        unsigned peers = __match_any_sync(act, tile);
+        int leader = __ffs(peers) - 1;
+        int base = 0;
+        if (lane == leader) base = atomicAdd(&tile_cur[tile], __popc(peers));
+        if (SCATTER) {
+            base = __shfl_sync(peers, base, leader);
+            pos = base + __popc(peers & ((1u << lane) - 1u));
+        }
+    }
+    return pos;
+}
+
+// ---- cloud source ------------------------------------------------------------------------------
+template <int SCATTER>
+__global__ void __launch_bounds__(256)
+ibk_bin_cloud(ib_bin_params pr)
+{
+    const int64_t P = pr.P;
+    int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    bool valid = p < P;
+    double x = 0, y = 0, z = 0;
+    if (valid) {
+        x = __ldg(pr.xp + p); y = __ldg(pr.xp + P + p); z = __ldg(pr.xp + 2 * P + p);
+        if (!(isfinite(x) && isfinite(y) && isfinite(z))) {
+            if (SCATTER) {
+                ib_latch(pr.status, IB_ERR_NONFINITE, p);
+                if (pr.Up) { pr.Up[p] = 0.0; pr.Up[P + p] = 0.0; pr.Up[2 * P + p] = 0.0; }
+            }
+            valid = false;
+        }
+    }
+    int tile = valid ? ib_tile_of(x, y, z, pr.g, pr.inv_h) : 0;
+    int pos = ib_bin_slot<SCATTER>(valid, tile, pr.tile_cur);
+    if (SCATTER && valid) {
+        pr.sx[pos] = x; pr.sx[P + pos] = y; pr.sx[2 * P + pos] = z;
+        pr.sid[pos] = (int32_t)p;
+        if (pr.Gp) {
+            pr.sG[pos] = __ldg(pr.Gp + p); pr.sG[P + pos] = __ldg(pr.Gp + P + p); pr.sG[2 * P + pos] = __ldg(pr.Gp + 2 * P + p);
+        }
+    }
+}
+
+// ---- mesh source: one thread per row (e, m2, m3) of n1 sub-points ----------------------------------
+__device__ __forceinline__ int64_t ib_find_row_elem(const int64_t *__restrict__ off, int64_t n_elems, int64_t r)
+{
+    int64_t lo = 0, hi = n_elems;                 // off[lo] <= r < off[hi]
+    while (hi - lo > 1) {
+        int64_t mid = (lo + hi) >> 1;
+        if (__ldg(off + mid) <= r) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+
+// bilinear combination of the 4 nodes (ja,ka) of one x-face of the element, no contraction freedom
+__device__ __forceinline__ double ib_face_lerp(double w00, double w10, double w01, double w11,
+                                               double v0, double v2, double v4, double v6)
+{
+    return __fma_rn(w11, v6, __fma_rn(w01, v4, __fma_rn(w10, v2, __dmul_rn(w00, v0))));
+}
+
+template <int SCATTER>
+__global__ void __launch_bounds__(256)
+ibk_bin_mesh(ib_bin_params pr)
+{
+    const unsigned full = 0xffffffffu;
+    int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    bool live = row < pr.n_rows;
+    int64_t e = 0, p0 = 0;
+    int n1 = 0, n2 = 1, n3 = 1, m2 = 0, m3 = 0;
+    if (live) {
+        int r;
+        if (pr.un1 > 0) {
+            n1 = pr.un1; n2 = pr.un2; n3 = pr.un3;
+            int rpe = n2 * n3;
+            e = row / rpe;
+            r = (int)(row - e * rpe);
+            p0 = e * (int64_t)(n1 * rpe) + (int64_t)r * n1;
+        } else {
+            e = ib_find_row_elem(pr.row_off, pr.n_elems, row);
+            n1 = __ldg(pr.nsub + 3 * e); n2 = __ldg(pr.nsub + 3 * e + 1); n3 = __ldg(pr.nsub + 3 * e + 2);
+            r = (int)(row - __ldg(pr.row_off + e));
+            p0 = __ldg(pr.pt_off + e) + (int64_t)r * n1;
+        }
+        m2 = r % n2; m3 = r / n2;
+    }
+    double L[3] = {0, 0, 0}, D[3] = {0, 0, 0}, LF[3] = {0, 0, 0}, DF[3] = {0, 0, 0};
+    bool finite = true;
+    if (live) {
+        int nd[8];
+        const int4 *cp = reinterpret_cast<const int4 *>(pr.conn + e * 8);
+        int4 c0 = __ldg(cp), c1 = __ldg(cp + 1);
+        nd[0] = c0.x; nd[1] = c0.y; nd[2] = c0.z; nd[3] = c0.w;
+        nd[4] = c1.x; nd[5] = c1.y; nd[6] = c1.z; nd[7] = c1.w;
+        double x2 = ib_subxi(m2, n2), x3 = ib_subxi(m3, n3);
+        double b0 = 0.5 * (1.0 - x2), b1 = 0.5 * (1.0 + x2), g0 = 0.5 * (1.0 - x3), g1 = 0.5 * (1.0 + x3);
+        double w00 = __dmul_rn(b0, g0), w10 = __dmul_rn(b1, g0), w01 = __dmul_rn(b0, g1), w11 = __dmul_rn(b1, g1);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const double *xc = pr.x + (int64_t)c * pr.n_nodes;
+            double v[8];
+#pragma unroll
+            for (int a = 0; a < 8; ++a) { v[a] = __ldg(xc + nd[a]); finite = finite && isfinite(v[a]); }
+            L[c] = ib_face_lerp(w00, w10, w01, w11, v[0], v[2], v[4], v[6]);
+            double R = ib_face_lerp(w00, w10, w01, w11, v[1], v[3], v[5], v[7]);
+            D[c] = __dsub_rn(R, L[c]);
+            if (SCATTER && pr.Fhat) {
+                const double *fc = pr.Fhat + (int64_t)c * pr.n_nodes;
+#pragma unroll
+                for (int a = 0; a < 8; ++a) v[a] = __ldg(fc + nd[a]);
+                LF[c] = ib_face_lerp(w00, w10, w01, w11, v[0], v[2], v[4], v[6]);
+                DF[c] = ib_face_lerp(w00, w10, w01, w11, v[1], v[3], v[5], v[7]) - LF[c];
+            }
+        }
+        if (!finite) {
+            if (SCATTER) {
+                ib_latch(pr.status, IB_ERR_NONFINITE, e);
+                if (pr.Up)
+                    for (int j = 0; j < n1; ++j) { pr.Up[p0 + j] = 0.0; pr.Up[pr.P + p0 + j] = 0.0; pr.Up[2 * pr.P + p0 + j] = 0.0; }
+            }
+            live = false;
+        }
+    }
+    int nmax = __reduce_max_sync(full, live ? n1 : 0);
+    for (int j = 0; j < nmax; ++j) {
+        bool valid = live && j < n1;
+        double t = 0.5 * (1.0 + ib_subxi(j, n1 > 0 ? n1 : 1));
+        double x = __fma_rn(t, D[0], L[0]), y = __fma_rn(t, D[1], L[1]), z = __fma_rn(t, D[2], L[2]);
+        int tile = valid ? ib_tile_of(x, y, z, pr.g, pr.inv_h) : 0;
+        int pos = ib_bin_slot<SCATTER>(valid, tile, pr.tile_cur);
+        if (SCATTER && valid) {
+            const int64_t P = pr.P;
+            pr.sx[pos] = x; pr.sx[P + pos] = y; pr.sx[2 * P + pos] = z;
+            pr.sid[pos] = (int32_t)(p0 + j);
+            if (pr.Fhat) {
+                double W = __ldg(pr.Wp + p0 + j);
+                pr.sG[pos] = W * fma(t, DF[0], LF[0]);
+                pr.sG[P + pos] = W * fma(t, DF[1], LF[1]);
+                pr.sG[2 * P + pos] = W * fma(t, DF[2], LF[2]);
+            }
+        }
+    }
+}
+
+// ---- single-CTA scan over the tiles: start offsets, cursors, compacted list of non-empty tiles ----
+__global__ void __launch_bounds__(1024)
+ibk_tile_scan(int32_t *__restrict__ tile_cur, int n_tiles, int32_t *__restrict__ tile_start,
+              int32_t *__restrict__ tile_list, int32_t *__restrict__ counters)
+{
+    __shared__ int ws[32], wl[32];
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int per = (n_tiles + 1023) / 1024;
+    const int t0 = min(tid * per, n_tiles), t1 = min(t0 + per, n_tiles);
+    int s = 0, l = 0;
+    for (int t = t0; t < t1; ++t) { int c = tile_cur[t]; s += c; l += c > 0; }
+    int is = s, il = l;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        int a = __shfl_up_sync(0xffffffffu, is, o), b = __shfl_up_sync(0xffffffffu, il, o);
+        if (lane >= o) { is += a; il += b; }
+    }
+    if (lane == 31) { ws[wid] = is; wl[wid] = il; }
+    __syncthreads();
+    if (wid == 0) {
+        int a = ws[lane], b = wl[lane], ia = a, ib = b;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            int x = __shfl_up_sync(0xffffffffu, ia, o), y = __shfl_up_sync(0xffffffffu, ib, o);
+            if (lane >= o) { ia += x; ib += y; }
+        }
+        ws[lane] = ia - a; wl[lane] = ib - b;
+        if (lane == 31) { tile_start[n_tiles] = ia; counters[0] = ib; counters[1] = 0; }
+    }
+    __syncthreads();
+    int es = ws[wid] + is - s, el = wl[wid] + il - l;
+    for (int t = t0; t < t1; ++t) {
+        int c = tile_cur[t];
+        tile_start[t] = es;
+        tile_cur[t] = es;
+        if (c > 0) tile_list[el++] = t;
+        es += c;
+    }
+}
+
+// ---- host side ------------------------------------------------------------------------------------
+ib_status ibk_bin_points(ib_ctx *c, int mesh, const double *xp, const double *Gp, int64_t P,
+                         const double *x, const double *Fhat, double *Up, cudaStream_t st)
+{
+    const int n_tiles = (int)(c->n_cells / (BT * BT * BT));
+    ib_bin_params pr;
+    memset(&pr, 0, sizeof(pr));
+    pr.P = P; pr.xp = xp; pr.Gp = Gp;
+    pr.n_rows = c->n_rows; pr.n_elems = c->n_elems; pr.n_nodes = c->n_nodes;
+    pr.un1 = c->un[0]; pr.un2 = c->un[1]; pr.un3 = c->un[2];
+    pr.nsub = c->d_nsub; pr.pt_off = c->d_pt_off; pr.row_off = c->d_row_off; pr.conn = c->d_conn;
+    pr.x = x; pr.Fhat = Fhat; pr.Wp = c->d_Wp;
+    pr.g = c->grid; pr.inv_h = c->inv_h;
+    pr.tile_cur = c->d_tile_cur; pr.sx = c->d_sx; pr.sG = c->d_sG; pr.sid = c->d_sid;
+    pr.Up = Up; pr.status = c->d_status;
+    IB_CUDA_TRY(cudaMemsetAsync(c->d_tile_cur, 0, (size_t)n_tiles * sizeof(int32_t), st));
+    const int64_t nthr = mesh ? c->n_rows : P;
+    if (mesh) ibk_bin_mesh<0><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
+    else ibk_bin_cloud<0><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
+    ibk_tile_scan<<<1, 1024, 0, st>>>(c->d_tile_cur, n_tiles, c->d_tile_start, c->d_tile_list, c->d_tile_count);
+    if (mesh) ibk_bin_mesh<1><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
+    else ibk_bin_cloud<1><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
+    c->launches += 3;
+    IB_CUDA_TRY(cudaGetLastError());
+    return IB_OK;
+}
+
+ib_status ibk_bin_reserve(ib_ctx *c, int64_t P)
+{
+    if (P <= c->bin_cap) return IB_OK;
+    if (c->d_sx) cudaFree(c->d_sx);
+    if (c->d_sG) cudaFree(c->d_sG);
+    if (c->d_sid) cudaFree(c->d_sid);
+    c->d_sx = c->d_sG = nullptr; c->d_sid = nullptr;
+    c->bin_cap = 0;
+    int64_t cap = P + P / 8 + 1024;
+    if (cudaMalloc(&c->d_sx, (size_t)cap * 3 * sizeof(double)) != cudaSuccess) return IB_ERR_ALLOC;
+    if (cudaMalloc(&c->d_sG, (size_t)cap * 3 * sizeof(double)) != cudaSuccess) return IB_ERR_ALLOC;
+    if (cudaMalloc(&c->d_sid, (size_t)cap * sizeof(int32_t)) != cudaSuccess) return IB_ERR_ALLOC;
+    c->bin_cap = cap;
+    return IB_OK;
+}

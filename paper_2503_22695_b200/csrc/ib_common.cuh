@@ -42,9 +42,17 @@ struct ib_ctx {
     int32_t *d_val[2];
     uint32_t *d_hist;
     int64_t hist_cap;
-    int32_t *d_cell_start;     // [n_cells+1] start rank of every cell (tiled path)
+    // tile-level counting sort of the points (ib_bin.cu), tiles of 4x4x4 cells
+    int64_t n_rows;            // rows (e,m2,m3) of sub-points of the mesh source
+    int un[3];                 // uniform nsub triple, un[0] == 0 if elements differ
+    int64_t *d_row_off;        // [n_elems+1]
+    int32_t *d_tile_cur;       // [n_tiles] counts, then running cursors
+    int32_t *d_tile_start;     // [n_tiles+1]
     int32_t *d_tile_list;      // compacted non-empty tiles
-    int32_t *d_tile_count;     // [1] + work counters
+    int32_t *d_tile_count;     // [0] number of non-empty tiles, [1] work counter
+    int64_t bin_cap;
+    double *d_sx, *d_sG;       // [3][P] point records grouped by tile
+    int32_t *d_sid;            // [P] original point id of each record
     // host staging for the *_host entry point
     double *d_hx, *d_hu, *d_hv, *d_hw, *d_hfu, *d_hfv, *d_hfw, *d_hUn, *d_hB;
     // status latch: [0] code, [1] first bad id
@@ -164,3 +172,8 @@ ib_status ibk_spread_interp(ib_ctx *c, const double *xp, const double *Gp, int64
                             double *fu, double *fv, double *fw, double *Up, int accumulate,
                             cudaStream_t st);
 ib_status ibk_sort_reserve(ib_ctx *c, int64_t P);
+ib_status ibk_bin_reserve(ib_ctx *c, int64_t P);
+ib_status ibk_tiled_spread_interp(ib_ctx *c, int mesh, const double *xp, const double *Gp, int64_t P,
+                                  const double *x, const double *Fhat,
+                                  const double *u, const double *v, const double *w,
+                                  double *fu, double *fv, double *fw, double *Up, cudaStream_t st);

@@ -103,7 +103,8 @@ extern "C" ib_status ib_destroy(ib_ctx *c)
     cudaSetDevice(c->device);
     void *ptrs[] = {c->d_conn, c->d_X, c->d_fib, c->d_mat_id, c->d_nsub, c->d_pt_off, c->d_mats, c->d_adj,
                     c->d_Wp, c->d_wa, c->d_Ce, c->d_Fhat, c->d_B, c->d_xp, c->d_Gp, c->d_Up, c->d_key[0],
-                    c->d_key[1], c->d_val[0], c->d_val[1], c->d_hist, c->d_cell_start, c->d_tile_list,
+                    c->d_key[1], c->d_val[0], c->d_val[1], c->d_hist, c->d_tile_cur, c->d_tile_start, c->d_tile_list,
+                    c->d_row_off, c->d_sx, c->d_sG, c->d_sid,
                     c->d_tile_count, c->d_hx, c->d_hu, c->d_hv, c->d_hw, c->d_hfu, c->d_hfv, c->d_hfw,
                     c->d_hUn, c->d_hB, c->d_status};
     for (void *p : ptrs)
@@ -137,13 +138,14 @@ extern "C" ib_status ib_create(ib_ctx **out, const ib_grid_desc *g, const ib_mes
 
     // host-side validation and topology
     const int64_t nn = m->n_nodes, ne = m->n_elems;
-    std::vector<int64_t> off((size_t)ne + 1, 0);
+    std::vector<int64_t> off((size_t)ne + 1, 0), roff((size_t)ne + 1, 0);
     int uniform = 0;
     if (m->nsub) {
         for (int64_t e = 0; e < ne; ++e) {
             const int32_t *s = m->nsub + 3 * e;
             if (s[0] < 1 || s[1] < 1 || s[2] < 1 || s[0] > 8 || s[1] > 8 || s[2] > 8) return IB_ERR_INVALID_ARG;
             off[e + 1] = off[e] + (int64_t)s[0] * s[1] * s[2];
+            roff[e + 1] = roff[e] + (int64_t)s[1] * s[2];
         }
         if (off[ne] > (int64_t)INT32_MAX) return IB_ERR_INVALID_ARG;
         uniform = ne > 0 ? m->nsub[0] * m->nsub[1] * m->nsub[2] : 0;
@@ -179,6 +181,8 @@ extern "C" ib_status ib_create(ib_ctx **out, const ib_grid_desc *g, const ib_mes
     c->nodal = m->nsub == nullptr;
     c->n_points = c->nodal ? nn : off[ne];
     c->uniform_S = uniform;
+    c->n_rows = roff[ne];
+    if (uniform) { c->un[0] = m->nsub[0]; c->un[1] = m->nsub[1]; c->un[2] = m->nsub[2]; }
     c->n_mats = m->n_mats;
     c->variant = 1;
 
@@ -204,12 +208,15 @@ extern "C" ib_status ib_create(ib_ctx **out, const ib_grid_desc *g, const ib_mes
         TRY(dev_alloc((void **)&c->d_Up, P * 3 * sizeof(double)));
     }
     const int n_tiles = (int)(c->n_cells / 64);          // 4x4x4-cell tiles of the tiled path
-    TRY(dev_alloc((void **)&c->d_cell_start, (size_t)(n_tiles + 1) * sizeof(int32_t)));
+    TRY(dev_alloc((void **)&c->d_tile_cur, (size_t)(n_tiles + 1) * sizeof(int32_t)));
+    TRY(dev_alloc((void **)&c->d_tile_start, (size_t)(n_tiles + 1) * sizeof(int32_t)));
+    TRY(dev_upload(&c->d_row_off, roff.data(), (size_t)ne + 1));
     TRY(dev_alloc((void **)&c->d_tile_list, (size_t)(n_tiles + 1) * sizeof(int32_t)));
     TRY(dev_alloc((void **)&c->d_tile_count, 64 * sizeof(int32_t)));
     TRY(dev_alloc((void **)&c->d_status, 2 * sizeof(long long)));
     if (s == IB_OK) s = reset_status(c, 0);
     if (s == IB_OK) s = ibk_sort_reserve(c, c->n_points);
+    if (s == IB_OK) s = ibk_bin_reserve(c, c->n_points);
     if (s == IB_OK) s = ibk_precompute_weights(c, 0);
     if (s == IB_OK && cudaDeviceSynchronize() != cudaSuccess) s = IB_ERR_CUDA;
 #undef TRY
@@ -350,11 +357,24 @@ extern "C" ib_status ib_coupling_step(ib_ctx *c, const double *x, const double *
     s = ibk_fe_force(c, x, Bd, c->d_Fhat, st);
     ib_prof_end(c, IB_PHASE_FE_FORCE, st);
     if (s != IB_OK) return s;
-    ib_prof_begin(c, IB_PHASE_POINTS, st);
-    s = ibk_points(c, x, c->d_Fhat, c->d_xp, c->d_Gp, st);
-    ib_prof_end(c, IB_PHASE_POINTS, st);
-    if (s != IB_OK) return s;
-    s = ibk_spread_interp(c, c->d_xp, c->d_Gp, c->n_points, u, v, w, fu, fv, fw, c->d_Up, 0, st);
+    if (c->variant == 1) {
+        // points generated on the fly inside the tile-level counting sort (ib_bin.cu)
+        const size_t gb = (size_t)c->n_cells * sizeof(double);
+        ib_prof_begin(c, IB_PHASE_ZERO, st);
+        IB_CUDA_TRY(cudaMemsetAsync(fu, 0, gb, st));
+        IB_CUDA_TRY(cudaMemsetAsync(fv, 0, gb, st));
+        IB_CUDA_TRY(cudaMemsetAsync(fw, 0, gb, st));
+        ib_prof_end(c, IB_PHASE_ZERO, st);
+        if (c->n_points > 0)
+            s = ibk_tiled_spread_interp(c, 1, nullptr, nullptr, c->n_points, x, c->d_Fhat, u, v, w, fu, fv, fw,
+                                        c->d_Up, st);
+    } else {
+        ib_prof_begin(c, IB_PHASE_POINTS, st);
+        s = ibk_points(c, x, c->d_Fhat, c->d_xp, c->d_Gp, st);
+        ib_prof_end(c, IB_PHASE_POINTS, st);
+        if (s != IB_OK) return s;
+        s = ibk_spread_interp(c, c->d_xp, c->d_Gp, c->n_points, u, v, w, fu, fv, fw, c->d_Up, 0, st);
+    }
     if (s != IB_OK) return s;
     ib_prof_begin(c, IB_PHASE_RESTRICT, st);
     s = ibk_restrict(c, c->d_Up, Un, st);

@@ -8,10 +8,6 @@
 // variant 1 (ib_tiled.cu): points sorted by Eulerian cell, shared-memory halo tile per 8^3 tile.
 #include "ib_common.cuh"
 
-ib_status ibk_tiled_spread_interp(ib_ctx *c, const double *xp, const double *Gp, int64_t P,
-                                  const double *u, const double *v, const double *w,
-                                  double *fu, double *fv, double *fw, double *Up, cudaStream_t st);
-
 struct ib_stencil {
     int ix[2][4], iy[2][4], iz[2][4];      // wrapped indices, [0] face-aligned, [1] centre-aligned
     double wx[2][4], wy[2][4], wz[2][4];
@@ -102,7 +98,7 @@ ib_status ibk_spread_interp(ib_ctx *c, const double *xp, const double *Gp, int64
         ib_prof_end(c, IB_PHASE_ZERO, st);
     }
     if (P == 0) return IB_OK;
-    if (c->variant == 1) return ibk_tiled_spread_interp(c, xp, Gp, P, u, v, w, fu, fv, fw, Up, st);
+    if (c->variant == 1) return ibk_tiled_spread_interp(c, 0, xp, Gp, P, nullptr, nullptr, u, v, w, fu, fv, fw, Up, st);
     unsigned nb = ib_blocks(P, 128);
     ib_prof_begin(c, IB_PHASE_SPREAD_INTERP, st);
     if (sp && in)
