@@ -195,43 +195,87 @@ ibk_bin_mesh(ib_bin_params pr)
     }
 }
 
-// ---- single-CTA scan over the tiles: start offsets, cursors, compacted list of non-empty tiles ----
-__global__ void __launch_bounds__(1024)
-ibk_tile_scan(int32_t *__restrict__ tile_cur, int n_tiles, int32_t *__restrict__ tile_start,
-              int32_t *__restrict__ tile_list, int32_t *__restrict__ counters)
+// ---- scan over the tiles (two small kernels, 4096 tiles per CTA): start offsets, cursors, compacted
+// list of non-empty tiles -----------------------------------------------------------------------------
+#define SCT 1024
+#define SCI 4
+
+__device__ __forceinline__ void ib_block_scan2(int &a, int &b, int *ws, int *wl, int &ta, int &tb)
 {
-    __shared__ int ws[32], wl[32];
-    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-    const int per = (n_tiles + 1023) / 1024;
-    const int t0 = min(tid * per, n_tiles), t1 = min(t0 + per, n_tiles);
-    int s = 0, l = 0;
-    for (int t = t0; t < t1; ++t) { int c = tile_cur[t]; s += c; l += c > 0; }
-    int is = s, il = l;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    int ia = a, ib = b;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
-        int a = __shfl_up_sync(0xffffffffu, is, o), b = __shfl_up_sync(0xffffffffu, il, o);
-        if (lane >= o) { is += a; il += b; }
+        int x = __shfl_up_sync(0xffffffffu, ia, o), y = __shfl_up_sync(0xffffffffu, ib, o);
+        if (lane >= o) { ia += x; ib += y; }
     }
-    if (lane == 31) { ws[wid] = is; wl[wid] = il; }
+    if (lane == 31) { ws[wid] = ia; wl[wid] = ib; }
     __syncthreads();
     if (wid == 0) {
-        int a = ws[lane], b = wl[lane], ia = a, ib = b;
+        int x = ws[lane], y = wl[lane], ix = x, iy = y;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
-            int x = __shfl_up_sync(0xffffffffu, ia, o), y = __shfl_up_sync(0xffffffffu, ib, o);
-            if (lane >= o) { ia += x; ib += y; }
+            int p = __shfl_up_sync(0xffffffffu, ix, o), r = __shfl_up_sync(0xffffffffu, iy, o);
+            if (lane >= o) { ix += p; iy += r; }
         }
-        ws[lane] = ia - a; wl[lane] = ib - b;
-        if (lane == 31) { tile_start[n_tiles] = ia; counters[0] = ib; counters[1] = 0; }
+        ws[lane] = ix - x; wl[lane] = iy - y;
+        if (lane == 31) { ws[32] = ix; wl[32] = iy; }
     }
     __syncthreads();
-    int es = ws[wid] + is - s, el = wl[wid] + il - l;
-    for (int t = t0; t < t1; ++t) {
-        int c = tile_cur[t];
-        tile_start[t] = es;
-        tile_cur[t] = es;
-        if (c > 0) tile_list[el++] = t;
-        es += c;
+    ta = ws[32]; tb = wl[32];
+    a = ws[wid] + ia - a;                          // exclusive prefixes
+    b = wl[wid] + ib - b;
+}
+
+__global__ void __launch_bounds__(SCT)
+ibk_tile_partials(const int32_t *__restrict__ tile_cur, int n_tiles, int2 *__restrict__ partial)
+{
+    __shared__ int ws[33], wl[33];
+    const int t0 = (blockIdx.x * SCT + threadIdx.x) * SCI;
+    int s = 0, l = 0;
+    if (t0 < n_tiles) {
+        int4 c = *reinterpret_cast<const int4 *>(tile_cur + t0);
+        s = c.x + c.y + c.z + c.w;
+        l = (c.x > 0) + (c.y > 0) + (c.z > 0) + (c.w > 0);
+    }
+    int ts, tl;
+    ib_block_scan2(s, l, ws, wl, ts, tl);
+    if (threadIdx.x == 0) partial[blockIdx.x] = make_int2(ts, tl);
+}
+
+__global__ void __launch_bounds__(SCT)
+ibk_tile_scan(int32_t *__restrict__ tile_cur, int n_tiles, const int2 *__restrict__ partial,
+              int32_t *__restrict__ tile_start, int32_t *__restrict__ tile_list, int32_t *__restrict__ counters)
+{
+    __shared__ int ws[33], wl[33];
+    __shared__ int base_s, base_l;
+    if (threadIdx.x < 32) {
+        int s = 0, l = 0;
+        for (int b = threadIdx.x; b < (int)blockIdx.x; b += 32) { int2 p = partial[b]; s += p.x; l += p.y; }
+#pragma unroll
+        for (int o = 16; o >= 1; o >>= 1) { s += __shfl_xor_sync(0xffffffffu, s, o); l += __shfl_xor_sync(0xffffffffu, l, o); }
+        if (threadIdx.x == 0) { base_s = s; base_l = l; }
+    }
+    const int t0 = (blockIdx.x * SCT + threadIdx.x) * SCI;
+    int4 c = make_int4(0, 0, 0, 0);
+    if (t0 < n_tiles) c = *reinterpret_cast<const int4 *>(tile_cur + t0);
+    int s = c.x + c.y + c.z + c.w, l = (c.x > 0) + (c.y > 0) + (c.z > 0) + (c.w > 0);
+    int ts, tl;
+    ib_block_scan2(s, l, ws, wl, ts, tl);          // includes the barrier that publishes base_s/base_l
+    s += base_s; l += base_l;
+    if (t0 < n_tiles) {
+        int4 st = make_int4(s, s + c.x, s + c.x + c.y, s + c.x + c.y + c.z);
+        *reinterpret_cast<int4 *>(tile_start + t0) = st;
+        *reinterpret_cast<int4 *>(tile_cur + t0) = st;
+        if (c.x > 0) tile_list[l++] = t0;
+        if (c.y > 0) tile_list[l++] = t0 + 1;
+        if (c.z > 0) tile_list[l++] = t0 + 2;
+        if (c.w > 0) tile_list[l++] = t0 + 3;
+    }
+    if (blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) {
+        tile_start[n_tiles] = base_s + ts;
+        counters[0] = base_l + tl;
+        counters[1] = 0;
     }
 }
 
@@ -254,10 +298,13 @@ ib_status ibk_bin_points(ib_ctx *c, int mesh, const double *xp, const double *Gp
     const int64_t nthr = mesh ? c->n_rows : P;
     if (mesh) ibk_bin_mesh<0><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
     else ibk_bin_cloud<0><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
-    ibk_tile_scan<<<1, 1024, 0, st>>>(c->d_tile_cur, n_tiles, c->d_tile_start, c->d_tile_list, c->d_tile_count);
+    const int nsb = (n_tiles + SCT * SCI - 1) / (SCT * SCI);
+    int2 *partial = reinterpret_cast<int2 *>(c->d_tile_count + 16);
+    ibk_tile_partials<<<nsb, SCT, 0, st>>>(c->d_tile_cur, n_tiles, partial);
+    ibk_tile_scan<<<nsb, SCT, 0, st>>>(c->d_tile_cur, n_tiles, partial, c->d_tile_start, c->d_tile_list, c->d_tile_count);
     if (mesh) ibk_bin_mesh<1><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
     else ibk_bin_cloud<1><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
-    c->launches += 3;
+    c->launches += 4;
     IB_CUDA_TRY(cudaGetLastError());
     return IB_OK;
 }

@@ -89,9 +89,24 @@ __device__ __forceinline__ void ib_latch(long long *status, int code, long long 
 // i0 = floor(s) - 1, with r = s - floor(s) in [0,1):
 //   phi(1+r) = (3-2r-q)/8, phi(r) = (3-2r+q)/8, phi(1-r) = (1+2r+q)/8, phi(2-r) = (1+2r-q)/8,
 //   q = sqrt(1+4r-4r^2)  (one square root serves all four).
+// sqrt(a) for a in [1,2] (the argument 1+4r-4r^2 of the kernel): float rsqrt seed, two Goldschmidt
+// steps and a final residual correction -- no special cases, no branches; error <= 1 ulp.
+__device__ __forceinline__ double ib_sqrt12(double a)
+{
+    double y = (double)rsqrtf((float)a);
+    double g = a * y, h = 0.5 * y;
+    double r = fma(-g, h, 0.5);
+    g = fma(g, r, g);
+    h = fma(h, r, h);
+    r = fma(-g, h, 0.5);
+    g = fma(g, r, g);
+    h = fma(h, r, h);
+    return fma(fma(-g, g, a), h, g);
+}
+
 __device__ __forceinline__ void ib_phi4(double r, double w[4])
 {
-    double q = sqrt(fma(4.0 * r, 1.0 - r, 1.0)) * 0.125;
+    double q = ib_sqrt12(fma(4.0 * r, 1.0 - r, 1.0)) * 0.125;
     double a = fma(-0.25, r, 0.375);
     double b = fma(0.25, r, 0.125);
     w[0] = a - q;

@@ -208,11 +208,11 @@ extern "C" ib_status ib_create(ib_ctx **out, const ib_grid_desc *g, const ib_mes
         TRY(dev_alloc((void **)&c->d_Up, P * 3 * sizeof(double)));
     }
     const int n_tiles = (int)(c->n_cells / 64);          // 4x4x4-cell tiles of the tiled path
-    TRY(dev_alloc((void **)&c->d_tile_cur, (size_t)(n_tiles + 1) * sizeof(int32_t)));
-    TRY(dev_alloc((void **)&c->d_tile_start, (size_t)(n_tiles + 1) * sizeof(int32_t)));
+    TRY(dev_alloc((void **)&c->d_tile_cur, (size_t)(n_tiles + 4) * sizeof(int32_t)));
+    TRY(dev_alloc((void **)&c->d_tile_start, (size_t)(n_tiles + 4) * sizeof(int32_t)));
     TRY(dev_upload(&c->d_row_off, roff.data(), (size_t)ne + 1));
     TRY(dev_alloc((void **)&c->d_tile_list, (size_t)(n_tiles + 1) * sizeof(int32_t)));
-    TRY(dev_alloc((void **)&c->d_tile_count, 64 * sizeof(int32_t)));
+    TRY(dev_alloc((void **)&c->d_tile_count, (size_t)(16 + 2 * (n_tiles / 4096 + 2)) * sizeof(int32_t)));
     TRY(dev_alloc((void **)&c->d_status, 2 * sizeof(long long)));
     if (s == IB_OK) s = reset_status(c, 0);
     if (s == IB_OK) s = ibk_sort_reserve(c, c->n_points);

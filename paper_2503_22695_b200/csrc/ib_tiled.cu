@@ -28,7 +28,9 @@
 #define NWARP (TB / 32)
 #define CH 2048                 // points staged per chunk
 #define REC 14                  // staging record: wx[4] wy[4] wz[4] G pad (doubles)
-#define GSTRIDE 58              // doubles per group staging block (4 records = 56, +2: bank spread, 16B aligned)
+#define GSTRIDE 56              // doubles per group staging block (4 records; 28 16-byte units = 4 mod 8: conflict-free STS.128)
+#define SZ 68                   // z-plane stride of the halo in doubles (64 + 4: the 4 lanes of a group hit distinct banks)
+#define SU3 (TH * SZ)           // one component of the halo
 #define NBIN 66
 
 struct ib_tiled_params {
@@ -88,9 +90,8 @@ __global__ void __launch_bounds__(TB, 2)
 ibk_tiled_kernel(ib_tiled_params pr)
 {
     extern __shared__ __align__(16) double smem[];
-    double *su = smem;                                   // [3][512]
-    double *sf = su + 3 * TH3;                           // [3][512]
-    double *sxi = sf + 3 * TH3;                          // [3][CH] tile-relative scaled coordinates
+    double *su = smem;                                   // [3][8][SZ] halo of u,v,w
+    double *sxi = su + 3 * SU3;                          // [3][CH] tile-relative scaled coordinates
     double *stg = sxi + 3 * CH;                          // [NWARP*8][GSTRIDE]
     int *oc_start = (int *)(stg + NWARP * 8 * GSTRIDE);  // [516]
     int *oc_cur = oc_start + 516;                        // [512]
@@ -121,13 +122,12 @@ ibk_tiled_kernel(ib_tiled_params pr)
         for (int d = 0; d < 3; ++d) h0[d] = ib_wrap(TT * t3[d] - 2, n[d]);
 
         // ---- halo load, zero the accumulators ---------------------------------------------------
-        for (int idx = tid; idx < 3 * TH3; idx += TB) {
-            if (DO_SPREAD) sf[idx] = 0.0;
-            if (DO_INTERP) {
+        if (DO_INTERP) {
+            for (int idx = tid; idx < 3 * TH3; idx += TB) {
                 int c = idx >> 9, r = idx & 511;
                 int i = h0[0] + (r & 7), j = h0[1] + ((r >> 3) & 7), k = h0[2] + (r >> 6);
                 i -= (i >= n[0]) ? n[0] : 0; j -= (j >= n[1]) ? n[1] : 0; k -= (k >= n[2]) ? n[2] : 0;
-                su[idx] = __ldg(pr.fld[c] + ((int64_t)k * n[1] + j) * n[0] + i);
+                su[c * SU3 + (r >> 6) * SZ + (r & 63)] = __ldg(pr.fld[c] + ((int64_t)k * n[1] + j) * n[0] + i);
             }
         }
 
@@ -244,8 +244,7 @@ ibk_tiled_kernel(ib_tiled_params pr)
                     o3[d] = l[d] + ((d == c) ? 1 : 0);
                     base3[d] = (d == c) ? (double)l[d] : (double)l[d] - 0.5;
                 }
-                const double *suc = su + c * TH3 + ((o3[2] + q) * TH + o3[1]) * TH + o3[0];
-                double *sfc = sf + c * TH3 + ((o3[2] + q) * TH + o3[1]) * TH + o3[0];
+                const double *suc = su + c * SU3 + (o3[2] + q) * SZ + o3[1] * TH + o3[0];
                 double uu[4][4], ff[4][4];
 #pragma unroll
                 for (int j = 0; j < 4; ++j)
@@ -321,25 +320,21 @@ ibk_tiled_kernel(ib_tiled_params pr)
                     __syncwarp();
                 }
                 if (DO_SPREAD && have) {
+                    int gi[4], gj[4];
+                    int gk = h0[2] + o3[2] + q; gk -= (gk >= n[2]) ? n[2] : 0;
+#pragma unroll
+                    for (int m = 0; m < 4; ++m) {
+                        gi[m] = h0[0] + o3[0] + m; gi[m] -= (gi[m] >= n[0]) ? n[0] : 0;
+                        gj[m] = h0[1] + o3[1] + m; gj[m] -= (gj[m] >= n[1]) ? n[1] : 0;
+                    }
+                    double *fp = pr.frc[c] + (int64_t)gk * n[1] * n[0];
 #pragma unroll
                     for (int j = 0; j < 4; ++j)
 #pragma unroll
-                        for (int i = 0; i < 4; ++i) atomicAdd(sfc + j * TH + i, ff[j][i]);
+                        for (int i = 0; i < 4; ++i) atomicAdd(fp + (int64_t)gj[j] * n[0] + gi[i], ff[j][i]);
                 }
             }
             __syncthreads();                          // chunk buffers are reused by the next chunk
-        }
-        // ---- one global reduction per touched face of the halo ---------------------------------------
-        if (DO_SPREAD) {
-            for (int idx = tid; idx < 3 * TH3; idx += TB) {
-                double val = sf[idx];
-                if (val != 0.0) {
-                    int c = idx >> 9, r = idx & 511;
-                    int i = h0[0] + (r & 7), j = h0[1] + ((r >> 3) & 7), k = h0[2] + (r >> 6);
-                    i -= (i >= n[0]) ? n[0] : 0; j -= (j >= n[1]) ? n[1] : 0; k -= (k >= n[2]) ? n[2] : 0;
-                    atomicAdd(pr.frc[c] + ((int64_t)k * n[1] + j) * n[0] + i, val);
-                }
-            }
         }
         __syncthreads();
     }
@@ -353,7 +348,7 @@ template <int S, int I>
 static ib_status launch_tiled(ib_ctx *c, const ib_tiled_params &pr, cudaStream_t st)
 {
     static int configured = 0;
-    const size_t smem = (size_t)(6 * TH3 + 3 * CH + NWARP * 8 * GSTRIDE) * sizeof(double) +
+    const size_t smem = (size_t)(3 * SU3 + 3 * CH + NWARP * 8 * GSTRIDE) * sizeof(double) +
                         (516 + NOC + 2 * NITEM + 68) * sizeof(int) + CH * sizeof(unsigned short);
     if (!configured) {
         IB_CUDA_TRY(cudaFuncSetAttribute(ibk_tiled_kernel<S, I>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
