@@ -68,14 +68,13 @@ __device__ __forceinline__ void ib_half_range(int c, int d, int l, int &lo, int 
 // scaled coordinate of a point relative to the origin of its tile, xi in [0,4) up to rounding:
 // s = (x-x0)/h to ~1 ulp; the tile is the one the binning formula (A21) assigned, so the integer
 // part comes from that formula and only the fraction from s.
-__device__ __forceinline__ double ib_tile_coord(double x, double x0, double h, double inv_h, int n)
+__device__ __forceinline__ double ib_tile_coord(double x, double x0, double h, double inv_h)
 {
     double sc = __dmul_rn(__dsub_rn(x, x0), inv_h);
     double fl = floor(sc);
-    long long c = (long long)fl;
-    int cw = (int)(c % n);
-    if (cw < 0) cw += n;
-    return (ib_scaled(x, x0, h, inv_h) - fl) + (double)(cw & (TT - 1));
+    // grid dims are multiples of 8, so the periodically wrapped cell index is congruent to the
+    // unwrapped one modulo the tile edge 4
+    return (ib_scaled(x, x0, h, inv_h) - fl) + (double)((long long)fl & (TT - 1));
 }
 
 __device__ __forceinline__ int ib_octant_key(double a, double b, double c)
@@ -99,7 +98,7 @@ ibk_tiled_kernel(ib_tiled_params pr)
     int *order = item_cnt + NITEM;                       // [NITEM]
     int *bins = order + NITEM;                           // [68]
     unsigned short *sidx = (unsigned short *)(bins + 68);// [CH]
-    __shared__ int s_tile, s_nitems;
+    __shared__ int s_tile, s_nitems, s_next;
     __shared__ int wsum[NWARP];
 
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -136,15 +135,30 @@ ibk_tiled_kernel(ib_tiled_params pr)
             // ---- stage the chunk, count points per half-cell -----------------------------------
             for (int i = tid; i < NOC; i += TB) oc_cur[i] = 0;
             for (int i = tid; i < 68; i += TB) bins[i] = 0;
+            if (tid == 0) s_next = 0;
             __syncthreads();
-            for (int i = tid; i < cn; i += TB) {
-                double xi[3];
+            {
+                double xr[CH / TB][3];                   // all loads of the chunk in flight at once
 #pragma unroll
-                for (int d = 0; d < 3; ++d) {
-                    xi[d] = ib_tile_coord(__ldg(pr.sx + (int64_t)d * P + cb + i), org[d], pr.g.h, pr.inv_h, n[d]);
-                    sxi[d * CH + i] = xi[d];
+                for (int k = 0; k < CH / TB; ++k) {
+                    const int i = tid + k * TB;
+#pragma unroll
+                    for (int d = 0; d < 3; ++d)
+                        xr[k][d] = (i < cn) ? __ldg(pr.sx + (int64_t)d * P + cb + i) : 0.0;
                 }
-                atomicAdd(&oc_cur[ib_octant_key(xi[0], xi[1], xi[2])], 1);
+#pragma unroll
+                for (int k = 0; k < CH / TB; ++k) {
+                    const int i = tid + k * TB;
+                    if (i < cn) {
+                        double xi[3];
+#pragma unroll
+                        for (int d = 0; d < 3; ++d) {
+                            xi[d] = ib_tile_coord(xr[k][d], org[d], pr.g.h, pr.inv_h);
+                            sxi[d * CH + i] = xi[d];
+                        }
+                        atomicAdd(&oc_cur[ib_octant_key(xi[0], xi[1], xi[2])], 1);
+                    }
+                }
             }
             __syncthreads();
             {                                            // exclusive scan of 512 counts, 2 per thread
@@ -210,7 +224,11 @@ ibk_tiled_kernel(ib_tiled_params pr)
 
             // ---- the items --------------------------------------------------------------------------
             double *mystg = stg + (wid * 8 + grp) * GSTRIDE;
-            for (int base = wid * 8; base < nitems; base += NWARP * 8) {
+            for (;;) {
+                int base = 0;
+                if (lane == 0) base = atomicAdd(&s_next, 8);     // warps pull 8 items at a time (largest first)
+                base = __shfl_sync(0xffffffffu, base, 0);
+                if (base >= nitems) break;
                 const int wi = base + grp;
                 const bool have = wi < nitems;
                 int c = 0, l[3] = {0, 0, 0};
@@ -256,12 +274,24 @@ ibk_tiled_kernel(ib_tiled_params pr)
                 const double *Gc = DO_SPREAD ? pr.sG + (int64_t)c * P + cb : nullptr;
                 double *Uc = DO_INTERP ? pr.Up + (int64_t)c * P : nullptr;
 
+                // point of lane q in the first quad (index, force, id are fetched one quad ahead)
+                int si, id = 0;
+                bool valid;
+                double Gv = 0.0;
+#define IB_FETCH(R0)                                                                                         \
+    {                                                                                                        \
+        const int vi = (R0) + q;                                                                             \
+        valid = vi < npts;                                                                                   \
+        int rank = vi + ((vi < rend[0]) ? rstart[0] : (vi < rend[1]) ? rstart[1] : (vi < rend[2]) ? rstart[2] : rstart[3]); \
+        si = valid ? (int)sidx[rank] : 0;                                                                    \
+        Gv = (DO_SPREAD && valid) ? __ldg(Gc + si) * pr.ih3 : 0.0;                                            \
+        if (DO_INTERP && valid) id = __ldg(pr.sid + cb + si);                                                \
+    }
+                IB_FETCH(0)
                 for (int r0 = 0; r0 < nmax; r0 += 4) {
                     // -- lane q prepares point r0+q: delta weights of the 3 directions on comp c's lattice
-                    const int vi = r0 + q;
-                    const bool valid = vi < npts;
-                    int rank = vi + ((vi < rend[0]) ? rstart[0] : (vi < rend[1]) ? rstart[1] : (vi < rend[2]) ? rstart[2] : rstart[3]);
-                    const int si = valid ? (int)sidx[rank] : 0;
+                    const bool cur_valid = valid;
+                    const int cur_id = id;
                     double wgt[3][4];
 #pragma unroll
                     for (int d = 0; d < 3; ++d) {
@@ -269,7 +299,6 @@ ibk_tiled_kernel(ib_tiled_params pr)
                         r = fmin(fmax(r, 0.0), 1.0);     // rounding at cell boundaries; phi is continuous (A19)
                         ib_phi4(r, wgt[d]);
                     }
-                    double Gv = (DO_SPREAD && valid) ? __ldg(Gc + si) * pr.ih3 : 0.0;
                     if (!valid) {
 #pragma unroll
                         for (int m = 0; m < 4; ++m) wgt[2][m] = 0.0;
@@ -283,6 +312,7 @@ ibk_tiled_kernel(ib_tiled_params pr)
                     *reinterpret_cast<double2 *>(rec + 10) = make_double2(wgt[2][2], wgt[2][3]);
                     rec[12] = Gv;
                     __syncwarp();
+                    IB_FETCH(r0 + 4)
                     double mine = 0.0;
 #pragma unroll
                     for (int jp = 0; jp < 4; ++jp) {
@@ -316,7 +346,7 @@ ibk_tiled_kernel(ib_tiled_params pr)
                             }
                         }
                     }
-                    if (DO_INTERP && valid) Uc[__ldg(pr.sid + cb + si)] = mine;
+                    if (DO_INTERP && cur_valid) Uc[cur_id] = mine;
                     __syncwarp();
                 }
                 if (DO_SPREAD && have) {
