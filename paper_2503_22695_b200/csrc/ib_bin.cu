@@ -145,8 +145,9 @@ ibk_bin_mesh(ib_bin_params pr)
         int4 c0 = __ldg(cp), c1 = __ldg(cp + 1);
         nd[0] = c0.x; nd[1] = c0.y; nd[2] = c0.z; nd[3] = c0.w;
         nd[4] = c1.x; nd[5] = c1.y; nd[6] = c1.z; nd[7] = c1.w;
-        double x2 = ib_subxi(m2, n2), x3 = ib_subxi(m3, n3);
-        double b0 = 0.5 * (1.0 - x2), b1 = 0.5 * (1.0 + x2), g0 = 0.5 * (1.0 - x3), g1 = 0.5 * (1.0 + x3);
+        // N-weights of the row: 1/2 (1 +- xi) with xi = -1 + (2m+1)/n  ->  (m + 1/2)/n and its complement
+        double b1 = ((double)m2 + 0.5) * (1.0 / (double)n2), g1 = ((double)m3 + 0.5) * (1.0 / (double)n3);
+        double b0 = 1.0 - b1, g0 = 1.0 - g1;
         double w00 = __dmul_rn(b0, g0), w10 = __dmul_rn(b1, g0), w01 = __dmul_rn(b0, g1), w11 = __dmul_rn(b1, g1);
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
@@ -174,13 +175,47 @@ ibk_bin_mesh(ib_bin_params pr)
             live = false;
         }
     }
-    int nmax = __reduce_max_sync(full, live ? n1 : 0);
+    const int nmax = __reduce_max_sync(full, live ? n1 : 0);
+    const double rn1 = 1.0 / (double)(n1 > 0 ? n1 : 1);
+    // fast path: every live row of the warp lies inside one tile (a row of sub-points spans a
+    // fraction of a cell) -> one aggregated atomic per distinct tile for the whole row
+    int tile0 = 0;
+    bool same = true;
+    if (live) {
+        for (int j = 0; j < n1; ++j) {
+            double t = ((double)j + 0.5) * rn1;
+            int tl = ib_tile_of(__fma_rn(t, D[0], L[0]), __fma_rn(t, D[1], L[1]), __fma_rn(t, D[2], L[2]), pr.g, pr.inv_h);
+            if (j == 0) tile0 = tl;
+            same = same && (tl == tile0);
+        }
+    }
+    const bool warp_same = __all_sync(full, same) && __all_sync(full, !live || n1 == nmax);
+    int base = -1, pstride = 0;
+    if (warp_same) {
+        unsigned act = __ballot_sync(full, live);
+        if (live) {
+            unsigned peers = __match_any_sync(act, tile0);
+            int leader = __ffs(peers) - 1;
+            const int lane = threadIdx.x & 31;
+            int b0 = 0;
+            if (lane == leader) b0 = atomicAdd(&pr.tile_cur[tile0], __popc(peers) * n1);
+            if (SCATTER) {
+                b0 = __shfl_sync(peers, b0, leader);
+                base = b0 + __popc(peers & ((1u << lane) - 1u));      // slot j of the row: base + j*pstride
+                pstride = __popc(peers);
+            }
+        }
+    }
     for (int j = 0; j < nmax; ++j) {
         bool valid = live && j < n1;
-        double t = 0.5 * (1.0 + ib_subxi(j, n1 > 0 ? n1 : 1));
+        double t = ((double)j + 0.5) * rn1;
         double x = __fma_rn(t, D[0], L[0]), y = __fma_rn(t, D[1], L[1]), z = __fma_rn(t, D[2], L[2]);
-        int tile = valid ? ib_tile_of(x, y, z, pr.g, pr.inv_h) : 0;
-        int pos = ib_bin_slot<SCATTER>(valid, tile, pr.tile_cur);
+        int pos;
+        if (warp_same) pos = base + j * pstride;
+        else {
+            int tile = valid ? ib_tile_of(x, y, z, pr.g, pr.inv_h) : 0;
+            pos = ib_bin_slot<SCATTER>(valid, tile, pr.tile_cur);
+        }
         if (SCATTER && valid) {
             const int64_t P = pr.P;
             pr.sx[pos] = x; pr.sx[P + pos] = y; pr.sx[2 * P + pos] = z;

@@ -134,8 +134,9 @@ __device__ __forceinline__ int ib_wrap(int i, int n)
 // Binning cell index of A21: floor((x - x0) * inv_h) mod n, in IEEE double with NO contraction.
 __device__ __forceinline__ int ib_cell(double x, double x0, double inv_h, int n)
 {
-    double sc = __dmul_rn(__dsub_rn(x, x0), inv_h);
-    long long c = (long long)floor(sc);
+    double fl = floor(__dmul_rn(__dsub_rn(x, x0), inv_h));
+    if (fl >= 0.0 && fl < (double)n) return (int)fl;      // inside the box: no wrap, no 64-bit modulo
+    long long c = (long long)fl;
     c %= n;
     if (c < 0) c += n;
     return (int)c;

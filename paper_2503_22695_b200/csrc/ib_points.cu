@@ -112,6 +112,62 @@ ibk_elem_node_sums(int64_t n_elems, int64_t P, const int32_t *__restrict__ nsub,
     if (WITH_U) { Ce[ne8 + e * 8 + a] = acc1; Ce[2 * ne8 + e * 8 + a] = acc2; }
 }
 
+
+// Fast path of the restriction for a uniform nsub whose rows-per-element n2*n3 is a power of two <= 32:
+// one thread per row (e, m2, m3) of n1 sub-points (coalesced reads of W_s and Up), sum-factorised
+// over m1 in the thread, then a butterfly over the rows of the element.
+template <int N1>
+__global__ void __launch_bounds__(256)
+ibk_restrict_rows(int64_t n_rows, int64_t P, int n1r, int n2, int n3, const double *__restrict__ Wp,
+                  const double *__restrict__ Up, double *__restrict__ Ce, int64_t ne8)
+{
+    const int rpe = n2 * n3;
+    int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool live = row < n_rows;
+    if (!live) row = n_rows - 1;
+    const int64_t e = row / rpe;
+    const int r = (int)(row - e * rpe);
+    const int m2 = r % n2, m3 = r / n2;
+    const int n1 = N1 > 0 ? N1 : n1r;
+    const int64_t p0 = row * n1;
+    double A0[3] = {0, 0, 0}, A1[3] = {0, 0, 0};
+#pragma unroll
+    for (int j = 0; j < (N1 > 0 ? N1 : 8); ++j) {
+        if (N1 == 0 && j >= n1) break;
+        double t = 0.5 * (1.0 + ib_subxi(j, n1));
+        double W = __ldcs(Wp + p0 + j);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            double wu = W * __ldcs(Up + (int64_t)c * P + p0 + j);
+            A1[c] = fma(wu, t, A1[c]);
+            A0[c] = fma(wu, 1.0 - t, A0[c]);
+        }
+    }
+    const double x2 = ib_subxi(m2, n2), x3 = ib_subxi(m3, n3);
+    const double b[2] = {0.5 * (1.0 - x2), 0.5 * (1.0 + x2)}, g[2] = {0.5 * (1.0 - x3), 0.5 * (1.0 + x3)};
+    double v[8][3];
+#pragma unroll
+    for (int a = 0; a < 8; ++a) {
+        double w = b[(a >> 1) & 1] * g[a >> 2];
+        if (!live) w = 0.0;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) v[a][c] = w * ((a & 1) ? A1[c] : A0[c]);
+    }
+    for (int o = 1; o < rpe; o <<= 1) {
+#pragma unroll
+        for (int a = 0; a < 8; ++a)
+#pragma unroll
+            for (int c = 0; c < 3; ++c) v[a][c] += __shfl_xor_sync(0xffffffffu, v[a][c], o);
+    }
+    if (live) {
+#pragma unroll
+        for (int a = 0; a < 8; ++a)
+#pragma unroll
+            for (int c = 0; c < 3; ++c)
+                if ((a * 3 + c) % rpe == r) Ce[c * ne8 + e * 8 + a] = v[a][c];
+    }
+}
+
 // per node gather of Ce; mode 0: w_a = sum ; mode 1: Un_c = sum_c / w_a
 template <int WITH_U>
 __global__ void __launch_bounds__(256)
@@ -207,8 +263,19 @@ ib_status ibk_points(ib_ctx *c, const double *x, const double *Fhat, double *xp,
 ib_status ibk_restrict(ib_ctx *c, const double *Up, double *Un, cudaStream_t st)
 {
     if (c->n_elems == 0 || c->n_nodes == 0) return IB_OK;
-    ibk_elem_node_sums<1><<<ib_blocks(c->n_elems * 8, 256), 256, 0, st>>>(
-        c->n_elems, c->n_points, c->d_nsub, c->d_pt_off, c->d_Wp, Up, c->d_Ce);
+    const int rpe = c->un[1] * c->un[2];
+    if (c->un[0] > 0 && rpe <= 32 && (rpe & (rpe - 1)) == 0)
+    {
+        if (c->un[0] == 4)
+            ibk_restrict_rows<4><<<ib_blocks(c->n_rows, 256), 256, 0, st>>>(c->n_rows, c->n_points, 4, c->un[1], c->un[2],
+                                                                          c->d_Wp, Up, c->d_Ce, c->n_elems * 8);
+        else
+            ibk_restrict_rows<0><<<ib_blocks(c->n_rows, 256), 256, 0, st>>>(c->n_rows, c->n_points, c->un[0], c->un[1],
+                                                                          c->un[2], c->d_Wp, Up, c->d_Ce, c->n_elems * 8);
+    }
+    else
+        ibk_elem_node_sums<1><<<ib_blocks(c->n_elems * 8, 256), 256, 0, st>>>(
+            c->n_elems, c->n_points, c->d_nsub, c->d_pt_off, c->d_Wp, Up, c->d_Ce);
     ibk_node_gather_w<1><<<ib_blocks(c->n_nodes, 256), 256, 0, st>>>(c->n_nodes, c->n_elems * 8, c->d_adj,
                                                                       c->d_Ce, c->d_wa, Un);
     c->launches += 2;

@@ -144,7 +144,7 @@ ibk_tiled_kernel(ib_tiled_params pr)
                     const int i = tid + k * TB;
 #pragma unroll
                     for (int d = 0; d < 3; ++d)
-                        xr[k][d] = (i < cn) ? __ldg(pr.sx + (int64_t)d * P + cb + i) : 0.0;
+                        xr[k][d] = (i < cn) ? __ldcs(pr.sx + (int64_t)d * P + cb + i) : 0.0;
                 }
 #pragma unroll
                 for (int k = 0; k < CH / TB; ++k) {
@@ -284,8 +284,8 @@ ibk_tiled_kernel(ib_tiled_params pr)
         valid = vi < npts;                                                                                   \
         int rank = vi + ((vi < rend[0]) ? rstart[0] : (vi < rend[1]) ? rstart[1] : (vi < rend[2]) ? rstart[2] : rstart[3]); \
         si = valid ? (int)sidx[rank] : 0;                                                                    \
-        Gv = (DO_SPREAD && valid) ? __ldg(Gc + si) * pr.ih3 : 0.0;                                            \
-        if (DO_INTERP && valid) id = __ldg(pr.sid + cb + si);                                                \
+        Gv = (DO_SPREAD && valid) ? __ldcs(Gc + si) : 0.0;                                                    \
+        if (DO_INTERP && valid) id = __ldcs(pr.sid + cb + si);                                               \
     }
                 IB_FETCH(0)
                 for (int r0 = 0; r0 < nmax; r0 += 4) {
@@ -310,7 +310,7 @@ ibk_tiled_kernel(ib_tiled_params pr)
                     *reinterpret_cast<double2 *>(rec + 6) = make_double2(wgt[1][2], wgt[1][3]);
                     *reinterpret_cast<double2 *>(rec + 8) = make_double2(wgt[2][0], wgt[2][1]);
                     *reinterpret_cast<double2 *>(rec + 10) = make_double2(wgt[2][2], wgt[2][3]);
-                    rec[12] = Gv;
+                    rec[12] = Gv * pr.ih3;
                     __syncwarp();
                     IB_FETCH(r0 + 4)
                     double mine = 0.0;
@@ -346,7 +346,7 @@ ibk_tiled_kernel(ib_tiled_params pr)
                             }
                         }
                     }
-                    if (DO_INTERP && cur_valid) Uc[cur_id] = mine;
+                    if (DO_INTERP && cur_valid) __stcs(Uc + cur_id, mine);
                     __syncwarp();
                 }
                 if (DO_SPREAD && have) {
