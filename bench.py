@@ -114,6 +114,38 @@ class ClockSampler(threading.Thread):
                 "samples": len(self.samples)}
 
 
+def max_over_ranks(value, world, device=None):
+    """Max of a per-rank scalar over all ranks (torch.distributed must be initialised when
+    world > 1; works on nccl with a CUDA device and on gloo with device=None)."""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(units_per_rank_per_step, steps, t_rank_s, world, device=None):
+    """Replicas only: every rank processes the same number of units; the job's time
+    is the slowest rank's; value = units of all ranks / that time."""
+    t = max_over_ranks(t_rank_s, world, device)
+    return world * units_per_rank_per_step * steps / t, t
+
+
+def ncu_traffic_bytes(workload_name):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu capture
+    (profiles/r01_traffic.txt: '<workload> <bytes>' lines), or None."""
+    path = os.path.join(ROOT, "profiles", "r01_traffic.txt")
+    if not os.path.exists(path):
+        return None
+    for line in open(path):
+        parts = line.split()
+        if len(parts) >= 2 and parts[0] == workload_name:
+            return int(parts[1])
+    return None
+
+
 # ----------------------------------------------------------------------------------------------
 def cpu_sample(wl, frac):
     """Bounded sample of the workload for the oracle: the first `frac` of the elements (a
@@ -237,12 +269,7 @@ def run_ours(args):
     ctx.ib_profile_enable(False)
     launches = ctx.ib_launch_count() - l0
     ctx.check()
-    t_dev = float(np.sum(ms)) * 1e-3
-    tt = torch.tensor([t_dev], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-    t_dev = float(tt.item())
-    value = world * wl.n_points * args.steps / t_dev
+    value, t_dev = whole_job_value(wl.n_points, args.steps, float(np.sum(ms)) * 1e-3, world, dev)
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
@@ -258,10 +285,7 @@ def run_ours(args):
         ctx.ib_coupling_step_host(hx, hu, hv, hw, hfu, hfv, hfw, hUn, None, stream)
     barrier()
     t_e2e = time.perf_counter() - t0
-    te = torch.tensor([t_e2e], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_val = world * wl.n_points * e2e_steps / float(te.item())
+    e2e_val, _ = whole_job_value(wl.n_points, e2e_steps, t_e2e, world, dev)
     h2d = 8 * (3 * wl.n_nodes + 3 * wl.n_cells)
     d2h = 8 * (3 * wl.n_cells + 3 * wl.n_nodes)
 
@@ -281,7 +305,7 @@ def run_ours(args):
         dom_bytes = 72 * wl.n_points + 48 * wl.n_cells
         roofline = {"bound": "hbm", "kernel": "spread+interp (" + ("tiled" if args.variant else "per-point") + ")",
                     "achieved": dom_bytes / (dom_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
-                    "frac": dom_bytes / (dom_ms * 1e-3) / 1e9 / hbm_peak, "traffic": None,
+                    "frac": dom_bytes / (dom_ms * 1e-3) / 1e9 / hbm_peak, "traffic": ncu_traffic_bytes(wl.name),
                     "peak_source": hbm_src, "kernel_ms": dom_ms,
                     "algorithmic_bytes_per_launch": dom_bytes,
                     "step": {"algorithmic_bytes": abytes, "achieved_GBps": abytes / (step_ms * 1e-3) / 1e9,
