@@ -27,9 +27,10 @@ def needs_build():
 
 
 def build(force=False, verbose=False):
-    if not force and not needs_build():
+    extra = os.environ.get("IB_NVCC_EXTRA", "").split()          # e.g. -D switches for kernel experiments
+    if not force and not extra and not needs_build():
         return SO
-    cmd = [NVCC] + FLAGS + ["-o", SO] + sources()
+    cmd = [NVCC] + FLAGS + extra + ["-o", SO] + sources()
     r = subprocess.run(cmd, capture_output=True, text=True)
     log = r.stdout + r.stderr
     with open(os.path.join(HERE, "build.log"), "w") as f:

@@ -24,11 +24,12 @@
 #define TH3 512
 #define NOC 512                 // half-cells per tile (8^3)
 #define NITEM 300               // 3 components x (4*5*5) shifted cells
-#define TB 256                  // threads per CTA
+#define TB 192                  // threads per CTA (2 CTAs/SM at <= 168 registers)
 #define NWARP (TB / 32)
-#define CH 2048                 // points staged per chunk
+#define CH 1728                 // points staged per chunk (9 per thread)
 #define REC 14                  // staging record: wx[4] wy[4] wz[4] G pad (doubles)
-#define GSTRIDE 56              // doubles per group staging block (4 records; 28 16-byte units = 4 mod 8: conflict-free STS.128)
+#define GBUF 56                 // doubles per staging buffer of a group (4 records)
+#define GSTRIDE 120             // doubles per group: two buffers + pad (60 16-byte units = 4 mod 8: conflict-free STS.128)
 #define SZ 68                   // z-plane stride of the halo in doubles (64 + 4: the 4 lanes of a group hit distinct banks)
 #define SU3 (TH * SZ)           // one component of the halo
 #define NBIN 66
@@ -161,9 +162,15 @@ ibk_tiled_kernel(ib_tiled_params pr)
                 }
             }
             __syncthreads();
-            {                                            // exclusive scan of 512 counts, 2 per thread
-                int v0 = oc_cur[2 * tid], v1 = oc_cur[2 * tid + 1];
-                int s = v0 + v1, inc = s;
+            {                                            // exclusive scan of the 512 counts, SCK per thread
+                constexpr int SCK = (NOC + TB - 1) / TB;
+                int v[SCK], s = 0;
+#pragma unroll
+                for (int k = 0; k < SCK; ++k) {
+                    v[k] = (SCK * tid + k < NOC) ? oc_cur[SCK * tid + k] : 0;
+                    s += v[k];
+                }
+                int inc = s;
 #pragma unroll
                 for (int o = 1; o < 32; o <<= 1) {
                     int t = __shfl_up_sync(0xffffffffu, inc, o);
@@ -171,12 +178,14 @@ ibk_tiled_kernel(ib_tiled_params pr)
                 }
                 if (lane == 31) wsum[wid] = inc;
                 __syncthreads();
-                int off = 0;
-                for (int w = 0; w < wid; ++w) off += wsum[w];
-                int ex = off + inc - s;
-                oc_start[2 * tid] = ex; oc_start[2 * tid + 1] = ex + v0;
-                oc_cur[2 * tid] = ex; oc_cur[2 * tid + 1] = ex + v0;
-                if (tid == TB - 1) oc_start[NOC] = ex + s;
+                int ex = inc - s;
+                for (int w = 0; w < wid; ++w) ex += wsum[w];
+#pragma unroll
+                for (int k = 0; k < SCK; ++k) {
+                    if (SCK * tid + k < NOC) { oc_start[SCK * tid + k] = ex; oc_cur[SCK * tid + k] = ex; }
+                    ex += v[k];
+                }
+                if (tid == TB - 1) oc_start[NOC] = ex;
             }
             __syncthreads();
             for (int i = tid; i < cn; i += TB) {
@@ -262,106 +271,132 @@ ibk_tiled_kernel(ib_tiled_params pr)
                     o3[d] = l[d] + ((d == c) ? 1 : 0);
                     base3[d] = (d == c) ? (double)l[d] : (double)l[d] - 0.5;
                 }
-                const double *suc = su + c * SU3 + (o3[2] + q) * SZ + o3[1] * TH + o3[0];
+                const double *suc = su + c * SU3 + o3[2] * SZ + o3[1] * TH + o3[0] + q;   // lane q owns x-column q
                 double uu[4][4], ff[4][4];
 #pragma unroll
                 for (int j = 0; j < 4; ++j)
 #pragma unroll
                     for (int i = 0; i < 4; ++i) {
-                        uu[j][i] = DO_INTERP ? suc[j * TH + i] : 0.0;
+                        uu[j][i] = DO_INTERP ? suc[i * SZ + j * TH] : 0.0;            // [y j][z i]
                         ff[j][i] = 0.0;
                     }
                 const double *Gc = DO_SPREAD ? pr.sG + (int64_t)c * P + cb : nullptr;
                 double *Uc = DO_INTERP ? pr.Up + (int64_t)c * P : nullptr;
 
-                // point of lane q in the first quad (index, force, id are fetched one quad ahead)
-                int si, id = 0;
-                bool valid;
-                double Gv = 0.0;
-#define IB_FETCH(R0)                                                                                         \
+                // Software pipeline over quads of 4 points: while the group consumes quad k from one staging
+                // buffer, lane q computes the delta weights of its point of quad k+1 into the other buffer and
+                // the index / force / id of its point of quad k+2 are in flight.  One __syncwarp per quad.
+                int si1, id0 = 0, id1 = 0;
+                bool valid0, valid1;
+                double G1 = 0.0;
+#define IB_FETCH(R0, SI, GV, ID, VALID)                                                                      \
     {                                                                                                        \
         const int vi = (R0) + q;                                                                             \
-        valid = vi < npts;                                                                                   \
+        VALID = vi < npts;                                                                                   \
         int rank = vi + ((vi < rend[0]) ? rstart[0] : (vi < rend[1]) ? rstart[1] : (vi < rend[2]) ? rstart[2] : rstart[3]); \
-        si = valid ? (int)sidx[rank] : 0;                                                                    \
-        Gv = (DO_SPREAD && valid) ? __ldcs(Gc + si) : 0.0;                                                    \
-        if (DO_INTERP && valid) id = __ldcs(pr.sid + cb + si);                                               \
+        SI = VALID ? (int)sidx[rank] : 0;                                                                    \
+        GV = (DO_SPREAD && VALID) ? __ldcs(Gc + SI) : 0.0;                                                   \
+        if (DO_INTERP && VALID) ID = __ldcs(pr.sid + cb + SI);                                               \
     }
-                IB_FETCH(0)
-                for (int r0 = 0; r0 < nmax; r0 += 4) {
-                    // -- lane q prepares point r0+q: delta weights of the 3 directions on comp c's lattice
-                    const bool cur_valid = valid;
-                    const int cur_id = id;
-                    double wgt[3][4];
-#pragma unroll
-                    for (int d = 0; d < 3; ++d) {
-                        double r = sxi[d * CH + si] - base3[d];
-                        r = fmin(fmax(r, 0.0), 1.0);     // rounding at cell boundaries; phi is continuous (A19)
-                        ib_phi4(r, wgt[d]);
+#define IB_WEIGHTS(BUF, SI, GV, VALID)                                                                       \
+    {                                                                                                        \
+        double wgt[3][4];                                                                                    \
+        _Pragma("unroll") for (int d = 0; d < 3; ++d) {                                                      \
+            double r = sxi[d * CH + SI] - base3[d];                                                          \
+            r = fmin(fmax(r, 0.0), 1.0); /* rounding at cell boundaries; phi is continuous (A19) */          \
+            ib_phi4(r, wgt[d]);                                                                              \
+        }                                                                                                    \
+        if (!(VALID)) { _Pragma("unroll") for (int m = 0; m < 4; ++m) wgt[2][m] = 0.0; }                     \
+        double *rec = mystg + (BUF) * GBUF + q * REC;                                                        \
+        *reinterpret_cast<double2 *>(rec + 0) = make_double2(wgt[0][0], wgt[0][1]);                          \
+        *reinterpret_cast<double2 *>(rec + 2) = make_double2(wgt[0][2], wgt[0][3]);                          \
+        *reinterpret_cast<double2 *>(rec + 4) = make_double2(wgt[1][0], wgt[1][1]);                          \
+        *reinterpret_cast<double2 *>(rec + 6) = make_double2(wgt[1][2], wgt[1][3]);                          \
+        *reinterpret_cast<double2 *>(rec + 8) = make_double2(wgt[2][0], wgt[2][1]);                          \
+        *reinterpret_cast<double2 *>(rec + 10) = make_double2(wgt[2][2], wgt[2][3]);                         \
+        rec[12] = (GV) * pr.ih3;                                                                             \
+    }
+                {
+                    int si0;
+                    double G0 = 0.0;
+                    IB_FETCH(0, si0, G0, id0, valid0)
+                    IB_WEIGHTS(0, si0, G0, valid0)
+                }
+                IB_FETCH(4, si1, G1, id1, valid1)
+                __syncwarp();
+                int buf = 0;
+#ifdef IB_NO_MAIN
+                nmax = 0;
+#endif
+                for (int r0 = 0; r0 < nmax; r0 += 4, buf ^= 1) {
+                    // -- weights of quad r0+4 into the other buffer, fetch quad r0+8
+                    int si2 = 0, id2 = 0;
+                    bool valid2 = false;
+                    double G2 = 0.0;
+                    if (r0 + 4 < nmax) {
+                        IB_WEIGHTS(buf ^ 1, si1, G1, valid1)
+                        IB_FETCH(r0 + 8, si2, G2, id2, valid2)
                     }
-                    if (!valid) {
-#pragma unroll
-                        for (int m = 0; m < 4; ++m) wgt[2][m] = 0.0;
-                    }
-                    double *rec = mystg + q * REC;
-                    *reinterpret_cast<double2 *>(rec + 0) = make_double2(wgt[0][0], wgt[0][1]);
-                    *reinterpret_cast<double2 *>(rec + 2) = make_double2(wgt[0][2], wgt[0][3]);
-                    *reinterpret_cast<double2 *>(rec + 4) = make_double2(wgt[1][0], wgt[1][1]);
-                    *reinterpret_cast<double2 *>(rec + 6) = make_double2(wgt[1][2], wgt[1][3]);
-                    *reinterpret_cast<double2 *>(rec + 8) = make_double2(wgt[2][0], wgt[2][1]);
-                    *reinterpret_cast<double2 *>(rec + 10) = make_double2(wgt[2][2], wgt[2][3]);
-                    rec[12] = Gv * pr.ih3;
-                    __syncwarp();
-                    IB_FETCH(r0 + 4)
+                    // -- consume quad r0
+                    const double *cur = mystg + buf * GBUF;
                     double mine = 0.0;
 #pragma unroll
                     for (int jp = 0; jp < 4; ++jp) {
-                        const double *rj = mystg + jp * REC;
-                        double2 a0 = *reinterpret_cast<const double2 *>(rj + 0), a1 = *reinterpret_cast<const double2 *>(rj + 2);
-                        double2 b0 = *reinterpret_cast<const double2 *>(rj + 4), b1 = *reinterpret_cast<const double2 *>(rj + 6);
-                        const double wx[4] = {a0.x, a0.y, a1.x, a1.y}, wy[4] = {b0.x, b0.y, b1.x, b1.y};
-                        const double wz = rj[8 + q];
+                        const double *rj = cur + jp * REC;
+                        double2 a0 = *reinterpret_cast<const double2 *>(rj + 4), a1 = *reinterpret_cast<const double2 *>(rj + 6);
+                        double2 b0 = *reinterpret_cast<const double2 *>(rj + 8), b1 = *reinterpret_cast<const double2 *>(rj + 10);
+                        const double wy[4] = {a0.x, a0.y, a1.x, a1.y}, wz[4] = {b0.x, b0.y, b1.x, b1.y};
+                        const double wx = rj[q];
                         if (DO_INTERP) {
-                            double acc = 0.0;
+                            double rr[4];
 #pragma unroll
                             for (int j = 0; j < 4; ++j) {
-                                double rr = uu[j][0] * wx[0];
-                                rr = fma(uu[j][1], wx[1], rr);
-                                rr = fma(uu[j][2], wx[2], rr);
-                                rr = fma(uu[j][3], wx[3], rr);
-                                acc = fma(rr, wy[j], acc);
+                                rr[j] = uu[j][0] * wz[0];
+                                rr[j] = fma(uu[j][1], wz[1], rr[j]);
+                                rr[j] = fma(uu[j][2], wz[2], rr[j]);
+                                rr[j] = fma(uu[j][3], wz[3], rr[j]);
                             }
-                            double pv = acc * wz;
+                            double pv = fma(rr[0], wy[0], rr[1] * wy[1]) + fma(rr[2], wy[2], rr[3] * wy[3]);
+                            pv *= wx;
                             pv += __shfl_xor_sync(0xffffffffu, pv, 1);
                             pv += __shfl_xor_sync(0xffffffffu, pv, 2);
                             if (q == jp) mine = pv;
                         }
                         if (DO_SPREAD) {
-                            double gz = rj[12] * wz;
+                            double gx = rj[12] * wx;
 #pragma unroll
                             for (int j = 0; j < 4; ++j) {
-                                double gj = gz * wy[j];
+                                double gj = gx * wy[j];
 #pragma unroll
-                                for (int i = 0; i < 4; ++i) ff[j][i] = fma(gj, wx[i], ff[j][i]);
+                                for (int i = 0; i < 4; ++i) ff[j][i] = fma(gj, wz[i], ff[j][i]);
                             }
                         }
                     }
-                    if (DO_INTERP && cur_valid) __stcs(Uc + cur_id, mine);
+                    if (DO_INTERP && valid0) __stcs(Uc + id0, mine);
+                    valid0 = valid1; id0 = id1;
+                    si1 = si2; G1 = G2; id1 = id2; valid1 = valid2;
                     __syncwarp();
                 }
+#undef IB_FETCH
+#undef IB_WEIGHTS
+#ifdef IB_NO_FLUSH
+                if (DO_SPREAD && have && ff[0][0] == 123.456) {
+#else
                 if (DO_SPREAD && have) {
-                    int gi[4], gj[4];
-                    int gk = h0[2] + o3[2] + q; gk -= (gk >= n[2]) ? n[2] : 0;
+#endif
+                    // lane q flushes x-column q: for every (y,z) the 4 lanes of the group hit 4 consecutive faces
+                    int gi = h0[0] + o3[0] + q; gi -= (gi >= n[0]) ? n[0] : 0;
+                    int gj[4], gk[4];
 #pragma unroll
                     for (int m = 0; m < 4; ++m) {
-                        gi[m] = h0[0] + o3[0] + m; gi[m] -= (gi[m] >= n[0]) ? n[0] : 0;
                         gj[m] = h0[1] + o3[1] + m; gj[m] -= (gj[m] >= n[1]) ? n[1] : 0;
+                        gk[m] = h0[2] + o3[2] + m; gk[m] -= (gk[m] >= n[2]) ? n[2] : 0;
                     }
-                    double *fp = pr.frc[c] + (int64_t)gk * n[1] * n[0];
+                    double *fp = pr.frc[c] + gi;
 #pragma unroll
-                    for (int j = 0; j < 4; ++j)
+                    for (int i = 0; i < 4; ++i)
 #pragma unroll
-                        for (int i = 0; i < 4; ++i) atomicAdd(fp + (int64_t)gj[j] * n[0] + gi[i], ff[j][i]);
+                        for (int j = 0; j < 4; ++j) atomicAdd(fp + ((int64_t)gk[i] * n[1] + gj[j]) * n[0], ff[j][i]);
                 }
             }
             __syncthreads();                          // chunk buffers are reused by the next chunk
@@ -380,6 +415,7 @@ static ib_status launch_tiled(ib_ctx *c, const ib_tiled_params &pr, cudaStream_t
     static int configured = 0;
     const size_t smem = (size_t)(3 * SU3 + 3 * CH + NWARP * 8 * GSTRIDE) * sizeof(double) +
                         (516 + NOC + 2 * NITEM + 68) * sizeof(int) + CH * sizeof(unsigned short);
+    static_assert(CH % TB == 0, "chunk must be a whole number of points per thread");
     if (!configured) {
         IB_CUDA_TRY(cudaFuncSetAttribute(ibk_tiled_kernel<S, I>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         configured = 1;
