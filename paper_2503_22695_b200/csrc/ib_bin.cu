@@ -315,8 +315,9 @@ ibk_tile_scan(int32_t *__restrict__ tile_cur, int n_tiles, const int2 *__restric
 }
 
 // ---- host side ------------------------------------------------------------------------------------
+// phases: 1 = count pass + scan (needs only the positions), 2 = scatter pass (needs the forces too)
 ib_status ibk_bin_points(ib_ctx *c, int mesh, const double *xp, const double *Gp, int64_t P,
-                         const double *x, const double *Fhat, double *Up, cudaStream_t st)
+                         const double *x, const double *Fhat, double *Up, int phases, cudaStream_t st)
 {
     const int n_tiles = (int)(c->n_cells / (BT * BT * BT));
     ib_bin_params pr;
@@ -329,17 +330,22 @@ ib_status ibk_bin_points(ib_ctx *c, int mesh, const double *xp, const double *Gp
     pr.g = c->grid; pr.inv_h = c->inv_h;
     pr.tile_cur = c->d_tile_cur; pr.sx = c->d_sx; pr.sG = c->d_sG; pr.sid = c->d_sid;
     pr.Up = Up; pr.status = c->d_status;
-    IB_CUDA_TRY(cudaMemsetAsync(c->d_tile_cur, 0, (size_t)n_tiles * sizeof(int32_t), st));
     const int64_t nthr = mesh ? c->n_rows : P;
-    if (mesh) ibk_bin_mesh<0><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
-    else ibk_bin_cloud<0><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
-    const int nsb = (n_tiles + SCT * SCI - 1) / (SCT * SCI);
-    int2 *partial = reinterpret_cast<int2 *>(c->d_tile_count + 16);
-    ibk_tile_partials<<<nsb, SCT, 0, st>>>(c->d_tile_cur, n_tiles, partial);
-    ibk_tile_scan<<<nsb, SCT, 0, st>>>(c->d_tile_cur, n_tiles, partial, c->d_tile_start, c->d_tile_list, c->d_tile_count);
-    if (mesh) ibk_bin_mesh<1><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
-    else ibk_bin_cloud<1><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
-    c->launches += 4;
+    if (phases & 1) {
+        IB_CUDA_TRY(cudaMemsetAsync(c->d_tile_cur, 0, (size_t)n_tiles * sizeof(int32_t), st));
+        if (mesh) ibk_bin_mesh<0><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
+        else ibk_bin_cloud<0><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
+        const int nsb = (n_tiles + SCT * SCI - 1) / (SCT * SCI);
+        int2 *partial = reinterpret_cast<int2 *>(c->d_tile_count + 16);
+        ibk_tile_partials<<<nsb, SCT, 0, st>>>(c->d_tile_cur, n_tiles, partial);
+        ibk_tile_scan<<<nsb, SCT, 0, st>>>(c->d_tile_cur, n_tiles, partial, c->d_tile_start, c->d_tile_list, c->d_tile_count);
+        c->launches += 3;
+    }
+    if (phases & 2) {
+        if (mesh) ibk_bin_mesh<1><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
+        else ibk_bin_cloud<1><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
+        c->launches += 1;
+    }
     IB_CUDA_TRY(cudaGetLastError());
     return IB_OK;
 }

@@ -58,6 +58,8 @@ struct ib_ctx {
     // status latch: [0] code, [1] first bad id
     long long *d_status;
     cudaStream_t last_stream;
+    cudaStream_t side;         // internal stream: work that needs only the positions overlaps the FE force
+    cudaEvent_t ev_fork, ev_join;
     int64_t launches;
     // optional per-phase event timing
     int profile;
@@ -192,4 +194,6 @@ ib_status ibk_bin_reserve(ib_ctx *c, int64_t P);
 ib_status ibk_tiled_spread_interp(ib_ctx *c, int mesh, const double *xp, const double *Gp, int64_t P,
                                   const double *x, const double *Fhat,
                                   const double *u, const double *v, const double *w,
-                                  double *fu, double *fv, double *fw, double *Up, cudaStream_t st);
+                                  double *fu, double *fv, double *fw, double *Up, int counted, cudaStream_t st);
+ib_status ibk_bin_points(ib_ctx *c, int mesh, const double *xp, const double *Gp, int64_t P,
+                         const double *x, const double *Fhat, double *Up, int phases, cudaStream_t st);

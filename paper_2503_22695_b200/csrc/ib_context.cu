@@ -109,6 +109,9 @@ extern "C" ib_status ib_destroy(ib_ctx *c)
                     c->d_hUn, c->d_hB, c->d_status};
     for (void *p : ptrs)
         if (p) cudaFree(p);
+    if (c->side) cudaStreamDestroy(c->side);
+    if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+    if (c->ev_join) cudaEventDestroy(c->ev_join);
     if (c->prof) {
         double ms[IB_PHASE_COUNT];
         int64_t n[IB_PHASE_COUNT];
@@ -214,6 +217,10 @@ extern "C" ib_status ib_create(ib_ctx **out, const ib_grid_desc *g, const ib_mes
     TRY(dev_alloc((void **)&c->d_tile_list, (size_t)(n_tiles + 1) * sizeof(int32_t)));
     TRY(dev_alloc((void **)&c->d_tile_count, (size_t)(16 + 2 * (n_tiles / 4096 + 2)) * sizeof(int32_t)));
     TRY(dev_alloc((void **)&c->d_status, 2 * sizeof(long long)));
+    if (s == IB_OK && (cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) != cudaSuccess ||
+                       cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+                       cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess))
+        s = IB_ERR_CUDA;
     if (s == IB_OK) s = reset_status(c, 0);
     if (s == IB_OK) s = ibk_sort_reserve(c, c->n_points);
     if (s == IB_OK) s = ibk_bin_reserve(c, c->n_points);
@@ -353,22 +360,43 @@ extern "C" ib_status ib_coupling_step(ib_ctx *c, const double *x, const double *
         if (s != IB_OK) return s;
         return ibk_spread_interp(c, x, Bd, c->n_nodes, u, v, w, fu, fv, fw, Un, 0, st);
     }
-    ib_prof_begin(c, IB_PHASE_FE_FORCE, st);
-    s = ibk_fe_force(c, x, Bd, c->d_Fhat, st);
-    ib_prof_end(c, IB_PHASE_FE_FORCE, st);
-    if (s != IB_OK) return s;
     if (c->variant == 1) {
-        // points generated on the fly inside the tile-level counting sort (ib_bin.cu)
+        // Fork: zero-fill of f and the count pass + scan of the point binning need only the positions,
+        // so they run on the context's side stream while the FE force runs on the caller's stream.
         const size_t gb = (size_t)c->n_cells * sizeof(double);
+        const bool overlap = !c->profile && c->n_points > 0;      // per-phase timing wants the phases in sequence
+        cudaStream_t s2 = overlap ? c->side : st;
+        if (overlap) {
+            IB_CUDA_TRY(cudaEventRecord(c->ev_fork, st));
+            IB_CUDA_TRY(cudaStreamWaitEvent(s2, c->ev_fork, 0));
+        }
         ib_prof_begin(c, IB_PHASE_ZERO, st);
-        IB_CUDA_TRY(cudaMemsetAsync(fu, 0, gb, st));
-        IB_CUDA_TRY(cudaMemsetAsync(fv, 0, gb, st));
-        IB_CUDA_TRY(cudaMemsetAsync(fw, 0, gb, st));
+        IB_CUDA_TRY(cudaMemsetAsync(fu, 0, gb, s2));
+        IB_CUDA_TRY(cudaMemsetAsync(fv, 0, gb, s2));
+        IB_CUDA_TRY(cudaMemsetAsync(fw, 0, gb, s2));
         ib_prof_end(c, IB_PHASE_ZERO, st);
+        if (c->n_points > 0) {
+            s = ibk_bin_reserve(c, c->n_points);
+            if (s != IB_OK) return s;
+            ib_prof_begin(c, IB_PHASE_POINTS, st);
+            s = ibk_bin_points(c, 1, nullptr, nullptr, c->n_points, x, nullptr, nullptr, 1, s2);
+            ib_prof_end(c, IB_PHASE_POINTS, st);
+            if (s != IB_OK) return s;
+        }
+        if (overlap) IB_CUDA_TRY(cudaEventRecord(c->ev_join, s2));
+        ib_prof_begin(c, IB_PHASE_FE_FORCE, st);
+        s = ibk_fe_force(c, x, Bd, c->d_Fhat, st);
+        ib_prof_end(c, IB_PHASE_FE_FORCE, st);
+        if (s != IB_OK) return s;
+        if (overlap) IB_CUDA_TRY(cudaStreamWaitEvent(st, c->ev_join, 0));
         if (c->n_points > 0)
             s = ibk_tiled_spread_interp(c, 1, nullptr, nullptr, c->n_points, x, c->d_Fhat, u, v, w, fu, fv, fw,
-                                        c->d_Up, st);
+                                        c->d_Up, 1, st);
     } else {
+        ib_prof_begin(c, IB_PHASE_FE_FORCE, st);
+        s = ibk_fe_force(c, x, Bd, c->d_Fhat, st);
+        ib_prof_end(c, IB_PHASE_FE_FORCE, st);
+        if (s != IB_OK) return s;
         ib_prof_begin(c, IB_PHASE_POINTS, st);
         s = ibk_points(c, x, c->d_Fhat, c->d_xp, c->d_Gp, st);
         ib_prof_end(c, IB_PHASE_POINTS, st);

@@ -98,7 +98,7 @@ ib_status ibk_spread_interp(ib_ctx *c, const double *xp, const double *Gp, int64
         ib_prof_end(c, IB_PHASE_ZERO, st);
     }
     if (P == 0) return IB_OK;
-    if (c->variant == 1) return ibk_tiled_spread_interp(c, 0, xp, Gp, P, nullptr, nullptr, u, v, w, fu, fv, fw, Up, st);
+    if (c->variant == 1) return ibk_tiled_spread_interp(c, 0, xp, Gp, P, nullptr, nullptr, u, v, w, fu, fv, fw, Up, 0, st);
     unsigned nb = ib_blocks(P, 128);
     ib_prof_begin(c, IB_PHASE_SPREAD_INTERP, st);
     if (sp && in)

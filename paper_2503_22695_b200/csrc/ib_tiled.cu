@@ -238,6 +238,9 @@ ibk_tiled_kernel(ib_tiled_params pr)
                 if (lane == 0) base = atomicAdd(&s_next, 8);     // warps pull 8 items at a time (largest first)
                 base = __shfl_sync(0xffffffffu, base, 0);
                 if (base >= nitems) break;
+#ifdef IB_NO_ITEMS
+                if (base >= 0) break;
+#endif
                 const int wi = base + grp;
                 const bool have = wi < nitems;
                 int c = 0, l[3] = {0, 0, 0};
@@ -405,9 +408,6 @@ ibk_tiled_kernel(ib_tiled_params pr)
     }
 }
 
-ib_status ibk_bin_points(ib_ctx *c, int mesh, const double *xp, const double *Gp, int64_t P,
-                         const double *x, const double *Fhat, double *Up, cudaStream_t st);
-ib_status ibk_bin_reserve(ib_ctx *c, int64_t P);
 
 template <int S, int I>
 static ib_status launch_tiled(ib_ctx *c, const ib_tiled_params &pr, cudaStream_t st)
@@ -436,13 +436,13 @@ static ib_status launch_tiled(ib_ctx *c, const ib_tiled_params &pr, cudaStream_t
 ib_status ibk_tiled_spread_interp(ib_ctx *c, int mesh, const double *xp, const double *Gp, int64_t P,
                                   const double *x, const double *Fhat,
                                   const double *u, const double *v, const double *w,
-                                  double *fu, double *fv, double *fw, double *Up, cudaStream_t st)
+                                  double *fu, double *fv, double *fw, double *Up, int counted, cudaStream_t st)
 {
     ib_status rs = ibk_bin_reserve(c, P);
     if (rs != IB_OK) return rs;
     const bool spread = mesh ? (Fhat != nullptr) : (Gp != nullptr);
     ib_prof_begin(c, IB_PHASE_SORT, st);
-    rs = ibk_bin_points(c, mesh, xp, Gp, P, x, Fhat, Up, st);
+    rs = ibk_bin_points(c, mesh, xp, Gp, P, x, Fhat, Up, counted ? 2 : 3, st);   // counted: phase 1 already enqueued
     ib_prof_end(c, IB_PHASE_SORT, st);
     if (rs != IB_OK) return rs;
 
