@@ -262,6 +262,8 @@ __device__ __forceinline__ void ib_block_scan2(int &a, int &b, int *ws, int *wl,
     b = wl[wid] + ib - b;
 }
 
+__device__ __forceinline__ int ib_chunks(int c) { return (c + IB_CHUNK - 1) / IB_CHUNK; }
+
 __global__ void __launch_bounds__(SCT)
 ibk_tile_partials(const int32_t *__restrict__ tile_cur, int n_tiles, int2 *__restrict__ partial)
 {
@@ -271,16 +273,17 @@ ibk_tile_partials(const int32_t *__restrict__ tile_cur, int n_tiles, int2 *__res
     if (t0 < n_tiles) {
         int4 c = *reinterpret_cast<const int4 *>(tile_cur + t0);
         s = c.x + c.y + c.z + c.w;
-        l = (c.x > 0) + (c.y > 0) + (c.z > 0) + (c.w > 0);
+        l = ib_chunks(c.x) + ib_chunks(c.y) + ib_chunks(c.z) + ib_chunks(c.w);
     }
     int ts, tl;
     ib_block_scan2(s, l, ws, wl, ts, tl);
     if (threadIdx.x == 0) partial[blockIdx.x] = make_int2(ts, tl);
 }
 
+// start offsets and cursors of the tiles, and the work list: one entry per chunk of <= IB_CHUNK records
 __global__ void __launch_bounds__(SCT)
 ibk_tile_scan(int32_t *__restrict__ tile_cur, int n_tiles, const int2 *__restrict__ partial,
-              int32_t *__restrict__ tile_start, int32_t *__restrict__ tile_list, int32_t *__restrict__ counters)
+              int32_t *__restrict__ tile_start, int4 *__restrict__ work, int32_t *__restrict__ counters)
 {
     __shared__ int ws[33], wl[33];
     __shared__ int base_s, base_l;
@@ -294,7 +297,7 @@ ibk_tile_scan(int32_t *__restrict__ tile_cur, int n_tiles, const int2 *__restric
     const int t0 = (blockIdx.x * SCT + threadIdx.x) * SCI;
     int4 c = make_int4(0, 0, 0, 0);
     if (t0 < n_tiles) c = *reinterpret_cast<const int4 *>(tile_cur + t0);
-    int s = c.x + c.y + c.z + c.w, l = (c.x > 0) + (c.y > 0) + (c.z > 0) + (c.w > 0);
+    int s = c.x + c.y + c.z + c.w, l = ib_chunks(c.x) + ib_chunks(c.y) + ib_chunks(c.z) + ib_chunks(c.w);
     int ts, tl;
     ib_block_scan2(s, l, ws, wl, ts, tl);          // includes the barrier that publishes base_s/base_l
     s += base_s; l += base_l;
@@ -302,10 +305,10 @@ ibk_tile_scan(int32_t *__restrict__ tile_cur, int n_tiles, const int2 *__restric
         int4 st = make_int4(s, s + c.x, s + c.x + c.y, s + c.x + c.y + c.z);
         *reinterpret_cast<int4 *>(tile_start + t0) = st;
         *reinterpret_cast<int4 *>(tile_cur + t0) = st;
-        if (c.x > 0) tile_list[l++] = t0;
-        if (c.y > 0) tile_list[l++] = t0 + 1;
-        if (c.z > 0) tile_list[l++] = t0 + 2;
-        if (c.w > 0) tile_list[l++] = t0 + 3;
+        const int cnt[4] = {c.x, c.y, c.z, c.w}, beg[4] = {st.x, st.y, st.z, st.w};
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+            for (int o = 0; o < cnt[k]; o += IB_CHUNK) work[l++] = make_int4(t0 + k, beg[k] + o, min(IB_CHUNK, cnt[k] - o), 0);
     }
     if (blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) {
         tile_start[n_tiles] = base_s + ts;
@@ -314,7 +317,6 @@ ibk_tile_scan(int32_t *__restrict__ tile_cur, int n_tiles, const int2 *__restric
     }
 }
 
-// ---- host side ------------------------------------------------------------------------------------
 // phases: 1 = count pass + scan (needs only the positions), 2 = scatter pass (needs the forces too)
 ib_status ibk_bin_points(ib_ctx *c, int mesh, const double *xp, const double *Gp, int64_t P,
                          const double *x, const double *Fhat, double *Up, int phases, cudaStream_t st)
@@ -338,7 +340,7 @@ ib_status ibk_bin_points(ib_ctx *c, int mesh, const double *xp, const double *Gp
         const int nsb = (n_tiles + SCT * SCI - 1) / (SCT * SCI);
         int2 *partial = reinterpret_cast<int2 *>(c->d_tile_count + 16);
         ibk_tile_partials<<<nsb, SCT, 0, st>>>(c->d_tile_cur, n_tiles, partial);
-        ibk_tile_scan<<<nsb, SCT, 0, st>>>(c->d_tile_cur, n_tiles, partial, c->d_tile_start, c->d_tile_list, c->d_tile_count);
+        ibk_tile_scan<<<nsb, SCT, 0, st>>>(c->d_tile_cur, n_tiles, partial, c->d_tile_start, c->d_work, c->d_tile_count);
         c->launches += 3;
     }
     if (phases & 2) {
@@ -356,12 +358,15 @@ ib_status ibk_bin_reserve(ib_ctx *c, int64_t P)
     if (c->d_sx) cudaFree(c->d_sx);
     if (c->d_sG) cudaFree(c->d_sG);
     if (c->d_sid) cudaFree(c->d_sid);
-    c->d_sx = c->d_sG = nullptr; c->d_sid = nullptr;
+    if (c->d_work) cudaFree(c->d_work);
+    c->d_sx = c->d_sG = nullptr; c->d_sid = nullptr; c->d_work = nullptr;
     c->bin_cap = 0;
     int64_t cap = P + P / 8 + 1024;
     if (cudaMalloc(&c->d_sx, (size_t)cap * 3 * sizeof(double)) != cudaSuccess) return IB_ERR_ALLOC;
     if (cudaMalloc(&c->d_sG, (size_t)cap * 3 * sizeof(double)) != cudaSuccess) return IB_ERR_ALLOC;
     if (cudaMalloc(&c->d_sid, (size_t)cap * sizeof(int32_t)) != cudaSuccess) return IB_ERR_ALLOC;
+    c->work_cap = c->n_cells / (BT * BT * BT) + cap / IB_CHUNK + 8;
+    if (cudaMalloc(&c->d_work, (size_t)c->work_cap * sizeof(int4)) != cudaSuccess) return IB_ERR_ALLOC;
     c->bin_cap = cap;
     return IB_OK;
 }

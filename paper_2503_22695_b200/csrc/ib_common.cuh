@@ -7,6 +7,7 @@
 
 #define IB_TILE 8              // tile edge of the binning key (A21)
 #define IB_TILE_CELLS 512
+#define IB_CHUNK 1728            // points per work item of the tile kernel (ib_bin.cu emits the work list)
 
 // ---------------------------------------------------------------------------------------------
 // host-side context
@@ -48,7 +49,8 @@ struct ib_ctx {
     int64_t *d_row_off;        // [n_elems+1]
     int32_t *d_tile_cur;       // [n_tiles] counts, then running cursors
     int32_t *d_tile_start;     // [n_tiles+1]
-    int32_t *d_tile_list;      // compacted non-empty tiles
+    int4 *d_work;              // work list of the tile kernel: {tile, first record, points, 0} per chunk
+    int64_t work_cap;
     int32_t *d_tile_count;     // [0] number of non-empty tiles, [1] work counter
     int64_t bin_cap;
     double *d_sx, *d_sG;       // [3][P] point records grouped by tile

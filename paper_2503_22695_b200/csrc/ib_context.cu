@@ -103,7 +103,7 @@ extern "C" ib_status ib_destroy(ib_ctx *c)
     cudaSetDevice(c->device);
     void *ptrs[] = {c->d_conn, c->d_X, c->d_fib, c->d_mat_id, c->d_nsub, c->d_pt_off, c->d_mats, c->d_adj,
                     c->d_Wp, c->d_wa, c->d_Ce, c->d_Fhat, c->d_B, c->d_xp, c->d_Gp, c->d_Up, c->d_key[0],
-                    c->d_key[1], c->d_val[0], c->d_val[1], c->d_hist, c->d_tile_cur, c->d_tile_start, c->d_tile_list,
+                    c->d_key[1], c->d_val[0], c->d_val[1], c->d_hist, c->d_tile_cur, c->d_tile_start, c->d_work,
                     c->d_row_off, c->d_sx, c->d_sG, c->d_sid,
                     c->d_tile_count, c->d_hx, c->d_hu, c->d_hv, c->d_hw, c->d_hfu, c->d_hfv, c->d_hfw,
                     c->d_hUn, c->d_hB, c->d_status};
@@ -214,7 +214,6 @@ extern "C" ib_status ib_create(ib_ctx **out, const ib_grid_desc *g, const ib_mes
     TRY(dev_alloc((void **)&c->d_tile_cur, (size_t)(n_tiles + 4) * sizeof(int32_t)));
     TRY(dev_alloc((void **)&c->d_tile_start, (size_t)(n_tiles + 4) * sizeof(int32_t)));
     TRY(dev_upload(&c->d_row_off, roff.data(), (size_t)ne + 1));
-    TRY(dev_alloc((void **)&c->d_tile_list, (size_t)(n_tiles + 1) * sizeof(int32_t)));
     TRY(dev_alloc((void **)&c->d_tile_count, (size_t)(16 + 2 * (n_tiles / 4096 + 2)) * sizeof(int32_t)));
     TRY(dev_alloc((void **)&c->d_status, 2 * sizeof(long long)));
     if (s == IB_OK && (cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) != cudaSuccess ||

@@ -26,7 +26,7 @@
 #define NITEM 300               // 3 components x (4*5*5) shifted cells
 #define TB 192                  // threads per CTA (2 CTAs/SM at <= 168 registers)
 #define NWARP (TB / 32)
-#define CH 1728                 // points staged per chunk (9 per thread)
+#define CH IB_CHUNK             // points staged per work item (9 per thread)
 #define REC 14                  // staging record: wx[4] wy[4] wz[4] G pad (doubles)
 #define GBUF 56                 // doubles per staging buffer of a group (4 records)
 #define GSTRIDE 120             // doubles per group: two buffers + pad (60 16-byte units = 4 mod 8: conflict-free STS.128)
@@ -41,9 +41,8 @@ struct ib_tiled_params {
     const double *fld[3];
     double *frc[3];
     double *Up;
-    const int32_t *tile_start;
-    const int32_t *tile_list;
-    int32_t *counters;          // [0] number of non-empty tiles, [1] work counter
+    const int4 *work;           // {tile, first record, points, 0} per chunk
+    int32_t *counters;          // [0] number of work items, [1] work counter
     ib_grid_desc g;
     double inv_h, ih3;
 };
@@ -99,7 +98,8 @@ ibk_tiled_kernel(ib_tiled_params pr)
     int *order = item_cnt + NITEM;                       // [NITEM]
     int *bins = order + NITEM;                           // [68]
     unsigned short *sidx = (unsigned short *)(bins + 68);// [CH]
-    __shared__ int s_tile, s_nitems, s_next;
+    __shared__ int s_nitems, s_next;
+    __shared__ int4 s_work;
     __shared__ int wsum[NWARP];
 
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -109,13 +109,22 @@ ibk_tiled_kernel(ib_tiled_params pr)
     const int ntx = n[0] / TT, nty = n[1] / TT;
     const int64_t P = pr.P;
 
+    if (tid == 0) {
+        const int w = atomicAdd(&pr.counters[1], 1);
+        s_work = (w < pr.counters[0]) ? __ldg(pr.work + w) : make_int4(-1, 0, 0, 0);
+    }
+    __syncthreads();
     for (;;) {
-        if (tid == 0) s_tile = atomicAdd(&pr.counters[1], 1);
+        const int4 wk = s_work;
         __syncthreads();
-        const int ti = s_tile;
-        if (ti >= pr.counters[0]) break;
-        const int tile = __ldg(pr.tile_list + ti);
-        const int beg = __ldg(pr.tile_start + tile), end = __ldg(pr.tile_start + tile + 1);
+        if (wk.x < 0) break;
+        // the next work item is claimed and read now; its latency hides behind this item's processing
+        int4 nwk = make_int4(-1, 0, 0, 0);
+        if (tid == 0) {
+            const int w = atomicAdd(&pr.counters[1], 1);
+            if (w < pr.counters[0]) nwk = __ldg(pr.work + w);
+        }
+        const int tile = wk.x, cb = wk.y, cn = wk.z;
         const int t3[3] = {tile % ntx, (tile / ntx) % nty, tile / (ntx * nty)};
         int h0[3];                                       // halo origin (global index of halo entry 0), wrapped
 #pragma unroll
@@ -131,8 +140,7 @@ ibk_tiled_kernel(ib_tiled_params pr)
             }
         }
 
-        for (int cb = beg; cb < end; cb += CH) {
-            const int cn = min(CH, end - cb);
+        {
             // ---- stage the chunk, count points per half-cell -----------------------------------
             for (int i = tid; i < NOC; i += TB) oc_cur[i] = 0;
             for (int i = tid; i < 68; i += TB) bins[i] = 0;
@@ -402,9 +410,9 @@ ibk_tiled_kernel(ib_tiled_params pr)
                         for (int j = 0; j < 4; ++j) atomicAdd(fp + ((int64_t)gk[i] * n[1] + gj[j]) * n[0], ff[j][i]);
                 }
             }
-            __syncthreads();                          // chunk buffers are reused by the next chunk
         }
-        __syncthreads();
+        if (tid == 0) s_work = nwk;
+        __syncthreads();                              // buffers are reused by the next work item
     }
 }
 
@@ -451,7 +459,7 @@ ib_status ibk_tiled_spread_interp(ib_ctx *c, int mesh, const double *xp, const d
     pr.fld[0] = u; pr.fld[1] = v; pr.fld[2] = w;
     pr.frc[0] = fu; pr.frc[1] = fv; pr.frc[2] = fw;
     pr.Up = Up;
-    pr.tile_start = c->d_tile_start; pr.tile_list = c->d_tile_list; pr.counters = c->d_tile_count;
+    pr.work = c->d_work; pr.counters = c->d_tile_count;
     pr.g = c->grid; pr.inv_h = c->inv_h; pr.ih3 = c->inv_h * c->inv_h * c->inv_h;
     ib_prof_begin(c, IB_PHASE_SPREAD_INTERP, st);
     if (spread && Up) rs = launch_tiled<1, 1>(c, pr, st);
