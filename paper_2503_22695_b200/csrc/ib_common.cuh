@@ -97,7 +97,9 @@ __device__ __forceinline__ void ib_latch(long long *status, int code, long long 
 // steps and a final residual correction -- no special cases, no branches; error <= 1 ulp.
 __device__ __forceinline__ double ib_sqrt12(double a)
 {
-    double y = (double)rsqrtf((float)a);
+    float yf;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(yf) : "f"((float)a));       // one MUFU.RSQ, ~22 good bits
+    double y = (double)yf;
     double g = a * y, h = 0.5 * y;
     double r = fma(-g, h, 0.5);
     g = fma(g, r, g);

@@ -47,15 +47,15 @@ struct ib_tiled_params {
     double inv_h, ih3;
 };
 
-// decode a work item: component c, shifted-cell coordinates l[3]
+// decode a work item: component c, shifted-cell coordinates l[3]  (c*100 + (l2*ny + l1)*nx + l0 with
+// nx = 4 if c == 0 else 5, ny = 4 if c == 1 else 5; compile-time constant divisors only)
 __device__ __forceinline__ void ib_item_decode(int it, int &c, int l[3])
 {
     c = it / 100;
     int r = it - c * 100;
-    int nx = (c == 0) ? 4 : 5, ny = (c == 1) ? 4 : 5;
-    l[0] = r % nx;
-    l[1] = (r / nx) % ny;
-    l[2] = r / (nx * ny);
+    if (c == 0) { l[0] = r % 4; l[1] = (r / 4) % 5; l[2] = r / 20; }
+    else if (c == 1) { l[0] = r % 5; l[1] = (r / 5) % 4; l[2] = r / 20; }
+    else { l[0] = r % 5; l[1] = (r / 5) % 5; l[2] = r / 25; }
 }
 
 // half-cell range [lo,hi] (clipped to the tile) covered by shifted cell l in direction d of comp c
@@ -313,9 +313,8 @@ ibk_tiled_kernel(ib_tiled_params pr)
     {                                                                                                        \
         double wgt[3][4];                                                                                    \
         _Pragma("unroll") for (int d = 0; d < 3; ++d) {                                                      \
-            double r = sxi[d * CH + SI] - base3[d];                                                          \
-            r = fmin(fmax(r, 0.0), 1.0); /* rounding at cell boundaries; phi is continuous (A19) */          \
-            ib_phi4(r, wgt[d]);                                                                              \
+            /* r in [0,1] up to rounding at cell boundaries, where the formula continues phi smoothly (A19) */ \
+            ib_phi4((VALID) ? sxi[d * CH + SI] - base3[d] : 0.0, wgt[d]); /* padding lanes: any r in range */ \
         }                                                                                                    \
         if (!(VALID)) { _Pragma("unroll") for (int m = 0; m < 4; ++m) wgt[2][m] = 0.0; }                     \
         double *rec = mystg + (BUF) * GBUF + q * REC;                                                        \
@@ -404,10 +403,13 @@ ibk_tiled_kernel(ib_tiled_params pr)
                         gk[m] = h0[2] + o3[2] + m; gk[m] -= (gk[m] >= n[2]) ? n[2] : 0;
                     }
                     double *fp = pr.frc[c] + gi;
+                    int ok[4], oj[4];                                  // 32-bit face offsets (n_cells < 2^31)
+#pragma unroll
+                    for (int m = 0; m < 4; ++m) { ok[m] = gk[m] * n[1] * n[0]; oj[m] = gj[m] * n[0]; }
 #pragma unroll
                     for (int i = 0; i < 4; ++i)
 #pragma unroll
-                        for (int j = 0; j < 4; ++j) atomicAdd(fp + ((int64_t)gk[i] * n[1] + gj[j]) * n[0], ff[j][i]);
+                        for (int j = 0; j < 4; ++j) atomicAdd(fp + (ok[i] + oj[j]), ff[j][i]);
                 }
             }
         }
