@@ -32,6 +32,7 @@ struct ib_ctx {
     int32_t *d_adj;            // [8][n_nodes] slot = e*8+a or -1 (ELL, ascending element id)
     double *d_Wp;              // [P] sub-point weights W_s
     double *d_wa;              // [n_nodes] lumped weights
+    double *d_geo;             // [10][8 n_elems] reference J0^-1 and det J0 per Gauss point
     // per-step scratch
     double *d_Ce;              // [3][n_elems*8] per-element nodal contributions
     double *d_Fhat;            // [3][n_nodes]
@@ -187,6 +188,7 @@ ib_status ibk_fe_force(ib_ctx *c, const double *x, double *B, double *Fhat, cuda
 ib_status ibk_points(ib_ctx *c, const double *x, const double *Fhat, double *xp, double *Gp, cudaStream_t st);
 ib_status ibk_restrict(ib_ctx *c, const double *Up, double *Un, cudaStream_t st);
 ib_status ibk_precompute_weights(ib_ctx *c, cudaStream_t st);
+ib_status ibk_fe_precompute(ib_ctx *c, cudaStream_t st);
 ib_status ibk_bin_sort(ib_ctx *c, const double *xp, int64_t P, int64_t *key_out, int32_t *perm_out,
                        int build_cells, cudaStream_t st);
 ib_status ibk_spread_interp(ib_ctx *c, const double *xp, const double *Gp, int64_t P,

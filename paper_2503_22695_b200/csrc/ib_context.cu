@@ -102,7 +102,7 @@ extern "C" ib_status ib_destroy(ib_ctx *c)
     if (!c) return IB_ERR_INVALID_ARG;
     cudaSetDevice(c->device);
     void *ptrs[] = {c->d_conn, c->d_X, c->d_fib, c->d_mat_id, c->d_nsub, c->d_pt_off, c->d_mats, c->d_adj,
-                    c->d_Wp, c->d_wa, c->d_Ce, c->d_Fhat, c->d_B, c->d_xp, c->d_Gp, c->d_Up, c->d_key[0],
+                    c->d_Wp, c->d_wa, c->d_geo, c->d_Ce, c->d_Fhat, c->d_B, c->d_xp, c->d_Gp, c->d_Up, c->d_key[0],
                     c->d_key[1], c->d_val[0], c->d_val[1], c->d_hist, c->d_tile_cur, c->d_tile_start, c->d_work,
                     c->d_row_off, c->d_sx, c->d_sG, c->d_sid,
                     c->d_tile_count, c->d_hx, c->d_hu, c->d_hv, c->d_hw, c->d_hfu, c->d_hfv, c->d_hfw,
@@ -202,6 +202,7 @@ extern "C" ib_status ib_create(ib_ctx **out, const ib_grid_desc *g, const ib_mes
     const size_t P = (size_t)c->n_points;
     TRY(dev_alloc((void **)&c->d_wa, (size_t)nn * sizeof(double)));
     TRY(dev_alloc((void **)&c->d_Ce, (size_t)ne * 24 * sizeof(double)));
+    TRY(dev_alloc((void **)&c->d_geo, (size_t)ne * 80 * sizeof(double)));
     TRY(dev_alloc((void **)&c->d_Fhat, (size_t)nn * 3 * sizeof(double)));
     TRY(dev_alloc((void **)&c->d_B, (size_t)nn * 3 * sizeof(double)));
     if (!c->nodal) {
@@ -224,6 +225,7 @@ extern "C" ib_status ib_create(ib_ctx **out, const ib_grid_desc *g, const ib_mes
     if (s == IB_OK) s = ibk_sort_reserve(c, c->n_points);
     if (s == IB_OK) s = ibk_bin_reserve(c, c->n_points);
     if (s == IB_OK) s = ibk_precompute_weights(c, 0);
+    if (s == IB_OK) s = ibk_fe_precompute(c, 0);
     if (s == IB_OK && cudaDeviceSynchronize() != cudaSuccess) s = IB_ERR_CUDA;
 #undef TRY
     if (s == IB_OK) {

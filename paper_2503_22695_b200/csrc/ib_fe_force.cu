@@ -67,10 +67,50 @@ __device__ __forceinline__ double ib_pk1(const ib_material &m, const double F[3]
     return J;
 }
 
-// One thread per Gauss point; lanes 8g..8g+7 of a warp hold the 8 Gauss points of one element.
+// Reference geometry of every Gauss point (the reference configuration is static):
+// geo[0..8][t] = J0^-1 (rows d, cols I), geo[9][t] = det J0 = quadrature weight w (Gauss weight 1, L251).
 __global__ void __launch_bounds__(256)
+ibk_fe_geometry(int64_t n_elems, int64_t n_nodes, const int32_t *__restrict__ conn,
+                const double *__restrict__ X, double *__restrict__ geo, long long *status)
+{
+    int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    int64_t e = t >> 3;
+    int q = (int)(t & 7);
+    if (e >= n_elems) return;
+    const double g = 0.57735026918962576451;
+    double dN[8][3];
+    ib_dshape((q & 1) ? g : -g, (q & 2) ? g : -g, (q & 4) ? g : -g, dN);
+    double J0[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
+#pragma unroll
+    for (int a = 0; a < 8; ++a) {
+        int nd = __ldg(conn + e * 8 + a);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            double Xa = __ldg(X + c * n_nodes + nd);
+#pragma unroll
+            for (int d = 0; d < 3; ++d) J0[c][d] = fma(Xa, dN[a][d], J0[c][d]);
+        }
+    }
+    double w = ib_det3(J0);
+    if (!(w > 0.0)) ib_latch(status, IB_ERR_INVERTED_ELEMENT, e);
+    double rw = 1.0 / w;
+    const int64_t ng = n_elems * 8;
+    geo[0 * ng + t] = (J0[1][1] * J0[2][2] - J0[1][2] * J0[2][1]) * rw;
+    geo[1 * ng + t] = (J0[0][2] * J0[2][1] - J0[0][1] * J0[2][2]) * rw;
+    geo[2 * ng + t] = (J0[0][1] * J0[1][2] - J0[0][2] * J0[1][1]) * rw;
+    geo[3 * ng + t] = (J0[1][2] * J0[2][0] - J0[1][0] * J0[2][2]) * rw;
+    geo[4 * ng + t] = (J0[0][0] * J0[2][2] - J0[0][2] * J0[2][0]) * rw;
+    geo[5 * ng + t] = (J0[0][2] * J0[1][0] - J0[0][0] * J0[1][2]) * rw;
+    geo[6 * ng + t] = (J0[1][0] * J0[2][1] - J0[1][1] * J0[2][0]) * rw;
+    geo[7 * ng + t] = (J0[0][1] * J0[2][0] - J0[0][0] * J0[2][1]) * rw;
+    geo[8 * ng + t] = (J0[0][0] * J0[1][1] - J0[0][1] * J0[1][0]) * rw;
+    geo[9 * ng + t] = w;
+}
+
+// One thread per Gauss point; lanes 8g..8g+7 of a warp hold the 8 Gauss points of one element.
+__global__ void __launch_bounds__(256, 2)
 ibk_fe_gauss(int64_t n_elems, int64_t n_nodes, const int32_t *__restrict__ conn,
-             const double *__restrict__ X, const double *__restrict__ x,
+             const double *__restrict__ geo, const double *__restrict__ x,
              const double *__restrict__ fib, const int32_t *__restrict__ mat_id,
              const ib_material *__restrict__ mats, double *__restrict__ Ce, long long *status)
 {
@@ -79,6 +119,7 @@ ibk_fe_gauss(int64_t n_elems, int64_t n_nodes, const int32_t *__restrict__ conn,
     int q = (int)(t & 7);
     bool live = e < n_elems;
     int64_t ee = live ? e : n_elems - 1;          // dead lanes recompute the last element (keeps shuffles uniform)
+    const int64_t tt = ee * 8 + q, ng = n_elems * 8;
     int nd[8];
     {
         const int4 *cp = reinterpret_cast<const int4 *>(conn + ee * 8);
@@ -90,36 +131,25 @@ ibk_fe_gauss(int64_t n_elems, int64_t n_nodes, const int32_t *__restrict__ conn,
     double dN[8][3];
     ib_dshape((q & 1) ? g : -g, (q & 2) ? g : -g, (q & 4) ? g : -g, dN);
 
-    // reference Jacobian J0_{I d} = sum_a X_{a,I} dN_a/dxi_d, and F0_{c d} = sum_a x_{a,c} dN_a/dxi_d
-    double J0[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}}, Fx[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
+    // F0_{c d} = sum_a x_{a,c} dN_a/dxi_d ;  F = F0 * J0^-1 with the precomputed reference inverse
+    double Fx[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
     bool finite = true;
 #pragma unroll
     for (int a = 0; a < 8; ++a) {
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
-            double Xa = __ldg(X + c * n_nodes + nd[a]);
             double xa = __ldg(x + c * n_nodes + nd[a]);
             finite = finite && isfinite(xa);
 #pragma unroll
-            for (int d = 0; d < 3; ++d) {
-                J0[c][d] = fma(Xa, dN[a][d], J0[c][d]);
-                Fx[c][d] = fma(xa, dN[a][d], Fx[c][d]);
-            }
+            for (int d = 0; d < 3; ++d) Fx[c][d] = fma(xa, dN[a][d], Fx[c][d]);
         }
     }
-    // J0^-1 (rows d, cols I): xi-derivative -> X-derivative.  F = Fx * J0^-1.
-    double w = ib_det3(J0);
-    double rw = 1.0 / w;
     double Ji[3][3];
-    Ji[0][0] = (J0[1][1] * J0[2][2] - J0[1][2] * J0[2][1]) * rw;
-    Ji[0][1] = (J0[0][2] * J0[2][1] - J0[0][1] * J0[2][2]) * rw;
-    Ji[0][2] = (J0[0][1] * J0[1][2] - J0[0][2] * J0[1][1]) * rw;
-    Ji[1][0] = (J0[1][2] * J0[2][0] - J0[1][0] * J0[2][2]) * rw;
-    Ji[1][1] = (J0[0][0] * J0[2][2] - J0[0][2] * J0[2][0]) * rw;
-    Ji[1][2] = (J0[0][2] * J0[1][0] - J0[0][0] * J0[1][2]) * rw;
-    Ji[2][0] = (J0[1][0] * J0[2][1] - J0[1][1] * J0[2][0]) * rw;
-    Ji[2][1] = (J0[0][1] * J0[2][0] - J0[0][0] * J0[2][1]) * rw;
-    Ji[2][2] = (J0[0][0] * J0[1][1] - J0[0][1] * J0[1][0]) * rw;
+#pragma unroll
+    for (int d = 0; d < 3; ++d)
+#pragma unroll
+        for (int I = 0; I < 3; ++I) Ji[d][I] = __ldg(geo + (int64_t)(3 * d + I) * ng + tt);
+    const double w = __ldg(geo + 9 * ng + tt);
     double F[3][3];
 #pragma unroll
     for (int c = 0; c < 3; ++c)
@@ -215,11 +245,21 @@ ibk_node_gather(int64_t n_nodes, int64_t ne8, const int32_t *__restrict__ adj,
     }
 }
 
+ib_status ibk_fe_precompute(ib_ctx *c, cudaStream_t st)
+{
+    if (c->n_elems == 0) return IB_OK;
+    ibk_fe_geometry<<<ib_blocks(c->n_elems * 8, 256), 256, 0, st>>>(c->n_elems, c->n_nodes, c->d_conn, c->d_X, c->d_geo,
+                                                                   c->d_status);
+    c->launches++;
+    IB_CUDA_TRY(cudaGetLastError());
+    return IB_OK;
+}
+
 ib_status ibk_fe_force(ib_ctx *c, const double *x, double *B, double *Fhat, cudaStream_t st)
 {
     if (c->n_elems > 0) {
         int64_t nt = c->n_elems * 8;
-        ibk_fe_gauss<<<ib_blocks(nt, 256), 256, 0, st>>>(c->n_elems, c->n_nodes, c->d_conn, c->d_X, x,
+        ibk_fe_gauss<<<ib_blocks(nt, 256), 256, 0, st>>>(c->n_elems, c->n_nodes, c->d_conn, c->d_geo, x,
                                                          c->d_fib, c->d_mat_id, c->d_mats, c->d_Ce,
                                                          c->d_status);
         c->launches++;
