@@ -112,11 +112,31 @@ __device__ __forceinline__ double ib_face_lerp(double w00, double w10, double w0
     return __fma_rn(w11, v6, __fma_rn(w01, v4, __fma_rn(w10, v2, __dmul_rn(w00, v0))));
 }
 
-template <int SCATTER>
+// STAGE: uniform nsub with 4 <= n2*n3 dividing 256 -- the CTA's 256 rows are 256/(n2 n3) whole elements,
+// whose node positions (and force coefficients) are staged once in shared memory instead of being
+// gathered by every row.
+template <int SCATTER, int STAGE>
 __global__ void __launch_bounds__(256)
 ibk_bin_mesh(ib_bin_params pr)
 {
     const unsigned full = 0xffffffffu;
+    __shared__ double s_nd[STAGE ? 64 * 8 * 6 : 1];       // [element of the CTA][local node][x0 x1 x2 F0 F1 F2]
+    if (STAGE) {
+        const int rpe = pr.un2 * pr.un3, epc = 256 / rpe;
+        const int64_t e_first = (int64_t)blockIdx.x * epc;
+        for (int i = threadIdx.x; i < epc * 8; i += 256) {
+            const int64_t ee = e_first + (i >> 3);
+            if (ee < pr.n_elems) {
+                const int nd = __ldg(pr.conn + ee * 8 + (i & 7));
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    s_nd[i * 6 + c] = __ldg(pr.x + (int64_t)c * pr.n_nodes + nd);
+                    if (SCATTER && pr.Fhat) s_nd[i * 6 + 3 + c] = __ldg(pr.Fhat + (int64_t)c * pr.n_nodes + nd);
+                }
+            }
+        }
+        __syncthreads();
+    }
     int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     bool live = row < pr.n_rows;
     int64_t e = 0, p0 = 0;
@@ -140,11 +160,16 @@ ibk_bin_mesh(ib_bin_params pr)
     double L[3] = {0, 0, 0}, D[3] = {0, 0, 0}, LF[3] = {0, 0, 0}, DF[3] = {0, 0, 0};
     bool finite = true;
     if (live) {
-        int nd[8];
-        const int4 *cp = reinterpret_cast<const int4 *>(pr.conn + e * 8);
-        int4 c0 = __ldg(cp), c1 = __ldg(cp + 1);
-        nd[0] = c0.x; nd[1] = c0.y; nd[2] = c0.z; nd[3] = c0.w;
-        nd[4] = c1.x; nd[5] = c1.y; nd[6] = c1.z; nd[7] = c1.w;
+        int nd[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+        const double *sn = s_nd;
+        if (STAGE) {
+            sn = s_nd + (int)(e - (int64_t)blockIdx.x * (256 / (pr.un2 * pr.un3))) * 48;
+        } else {
+            const int4 *cp = reinterpret_cast<const int4 *>(pr.conn + e * 8);
+            int4 c0 = __ldg(cp), c1 = __ldg(cp + 1);
+            nd[0] = c0.x; nd[1] = c0.y; nd[2] = c0.z; nd[3] = c0.w;
+            nd[4] = c1.x; nd[5] = c1.y; nd[6] = c1.z; nd[7] = c1.w;
+        }
         // N-weights of the row: 1/2 (1 +- xi) with xi = -1 + (2m+1)/n  ->  (m + 1/2)/n and its complement
         double b1 = ((double)m2 + 0.5) * (1.0 / (double)n2), g1 = ((double)m3 + 0.5) * (1.0 / (double)n3);
         double b0 = 1.0 - b1, g0 = 1.0 - g1;
@@ -154,14 +179,17 @@ ibk_bin_mesh(ib_bin_params pr)
             const double *xc = pr.x + (int64_t)c * pr.n_nodes;
             double v[8];
 #pragma unroll
-            for (int a = 0; a < 8; ++a) { v[a] = __ldg(xc + nd[a]); finite = finite && isfinite(v[a]); }
+            for (int a = 0; a < 8; ++a) {
+                v[a] = STAGE ? sn[a * 6 + c] : __ldg(xc + nd[a]);
+                finite = finite && isfinite(v[a]);
+            }
             L[c] = ib_face_lerp(w00, w10, w01, w11, v[0], v[2], v[4], v[6]);
             double R = ib_face_lerp(w00, w10, w01, w11, v[1], v[3], v[5], v[7]);
             D[c] = __dsub_rn(R, L[c]);
             if (SCATTER && pr.Fhat) {
                 const double *fc = pr.Fhat + (int64_t)c * pr.n_nodes;
 #pragma unroll
-                for (int a = 0; a < 8; ++a) v[a] = __ldg(fc + nd[a]);
+                for (int a = 0; a < 8; ++a) v[a] = STAGE ? sn[a * 6 + 3 + c] : __ldg(fc + nd[a]);
                 LF[c] = ib_face_lerp(w00, w10, w01, w11, v[0], v[2], v[4], v[6]);
                 DF[c] = ib_face_lerp(w00, w10, w01, w11, v[1], v[3], v[5], v[7]) - LF[c];
             }
@@ -333,9 +361,12 @@ ib_status ibk_bin_points(ib_ctx *c, int mesh, const double *xp, const double *Gp
     pr.tile_cur = c->d_tile_cur; pr.sx = c->d_sx; pr.sG = c->d_sG; pr.sid = c->d_sid;
     pr.Up = Up; pr.status = c->d_status;
     const int64_t nthr = mesh ? c->n_rows : P;
+    const int rpe = c->un[1] * c->un[2];
+    const bool stage = c->un[0] > 0 && rpe >= 4 && 256 % rpe == 0;
     if (phases & 1) {
         IB_CUDA_TRY(cudaMemsetAsync(c->d_tile_cur, 0, (size_t)n_tiles * sizeof(int32_t), st));
-        if (mesh) ibk_bin_mesh<0><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
+        if (mesh && stage) ibk_bin_mesh<0, 1><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
+        else if (mesh) ibk_bin_mesh<0, 0><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
         else ibk_bin_cloud<0><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
         const int nsb = (n_tiles + SCT * SCI - 1) / (SCT * SCI);
         int2 *partial = reinterpret_cast<int2 *>(c->d_tile_count + 16);
@@ -344,7 +375,8 @@ ib_status ibk_bin_points(ib_ctx *c, int mesh, const double *xp, const double *Gp
         c->launches += 3;
     }
     if (phases & 2) {
-        if (mesh) ibk_bin_mesh<1><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
+        if (mesh && stage) ibk_bin_mesh<1, 1><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
+        else if (mesh) ibk_bin_mesh<1, 0><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
         else ibk_bin_cloud<1><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
         c->launches += 1;
     }
