@@ -145,6 +145,43 @@ ibk_restrict_rows(int64_t n_rows, int64_t P, int n1r, int n2, int n3, const doub
     }
     const double x2 = ib_subxi(m2, n2), x3 = ib_subxi(m3, n3);
     const double b[2] = {0.5 * (1.0 - x2), 0.5 * (1.0 + x2)}, g[2] = {0.5 * (1.0 - x3), 0.5 * (1.0 + x3)};
+    if (N1 == 4 && n2 == 4 && n3 == 4) {
+        // 4 x 4 rows per element = 16 adjacent lanes, r = m2 + 4 m3.  Transposing reduction: at each
+        // step a lane keeps the half of its values whose target index bit equals its own lane bit and
+        // sends the other half (15 double shuffles instead of 96).
+        const bool r0 = r & 1, r1 = r & 2, r2 = r & 4;
+        const unsigned full = 0xffffffffu;
+        const double lv = live ? 1.0 : 0.0;
+        double s1[2][3];                               // [ia][c], target ja = r0
+#pragma unroll
+        for (int ia = 0; ia < 2; ++ia)
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const double Ai = lv * (ia ? A1[c] : A0[c]);
+                const double keep = (r0 ? b[1] : b[0]) * Ai, send = (r0 ? b[0] : b[1]) * Ai;
+                s1[ia][c] = keep + __shfl_xor_sync(full, send, 1);
+            }
+        double s2[3];                                  // [c], target ia = r1
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const double keep = r1 ? s1[1][c] : s1[0][c], send = r1 ? s1[0][c] : s1[1][c];
+            s2[c] = keep + __shfl_xor_sync(full, send, 2);
+        }
+        double s3[3];                                  // [c], target ka = r2
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const double keep = (r2 ? g[1] : g[0]) * s2[c], send = (r2 ? g[0] : g[1]) * s2[c];
+            s3[c] = keep + __shfl_xor_sync(full, send, 4);
+        }
+#pragma unroll
+        for (int c = 0; c < 3; ++c) s3[c] += __shfl_xor_sync(full, s3[c], 8);
+        if (live && !(r & 8)) {
+            const int a = (r1 ? 1 : 0) + (r0 ? 2 : 0) + (r2 ? 4 : 0);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) Ce[c * ne8 + e * 8 + a] = s3[c];
+        }
+        return;
+    }
     double v[8][3];
 #pragma unroll
     for (int a = 0; a < 8; ++a) {

@@ -131,6 +131,7 @@ ibk_tiled_kernel(ib_tiled_params pr)
         for (int d = 0; d < 3; ++d) h0[d] = ib_wrap(TT * t3[d] - 2, n[d]);
 
         // ---- halo load, zero the accumulators ---------------------------------------------------
+#ifndef IB_NO_HALO
         if (DO_INTERP) {
             for (int idx = tid; idx < 3 * TH3; idx += TB) {
                 int c = idx >> 9, r = idx & 511;
@@ -139,6 +140,7 @@ ibk_tiled_kernel(ib_tiled_params pr)
                 su[c * SU3 + (r >> 6) * SZ + (r & 63)] = __ldg(pr.fld[c] + ((int64_t)k * n[1] + j) * n[0] + i);
             }
         }
+#endif
 
         {
             // ---- stage the chunk, count points per half-cell -----------------------------------
@@ -196,10 +198,12 @@ ibk_tiled_kernel(ib_tiled_params pr)
                 if (tid == TB - 1) oc_start[NOC] = ex;
             }
             __syncthreads();
+#ifndef IB_NO_PASS2
             for (int i = tid; i < cn; i += TB) {
                 int key = ib_octant_key(sxi[i], sxi[CH + i], sxi[2 * CH + i]);
                 sidx[atomicAdd(&oc_cur[key], 1)] = (unsigned short)i;
             }
+#endif
             // ---- points per work item, order items by count (descending) -----------------------
             for (int it = tid; it < NITEM; it += TB) {
                 int c, l[3], lo[3], hi[3];
