@@ -116,11 +116,11 @@ __device__ __forceinline__ double ib_face_lerp(double w00, double w10, double w0
 // whose node positions (and force coefficients) are staged once in shared memory instead of being
 // gathered by every row.
 template <int SCATTER, int STAGE>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, 4)
 ibk_bin_mesh(ib_bin_params pr)
 {
     const unsigned full = 0xffffffffu;
-    __shared__ double s_nd[STAGE ? 64 * 8 * 6 : 1];       // [element of the CTA][local node][x0 x1 x2 F0 F1 F2]
+    __shared__ double s_nd[STAGE ? 16 * 8 * 6 : 1];       // [element of the CTA][local node][x0 x1 x2 F0 F1 F2]
     if (STAGE) {
         const int rpe = pr.un2 * pr.un3, epc = 256 / rpe;
         const int64_t e_first = (int64_t)blockIdx.x * epc;
@@ -362,7 +362,7 @@ ib_status ibk_bin_points(ib_ctx *c, int mesh, const double *xp, const double *Gp
     pr.Up = Up; pr.status = c->d_status;
     const int64_t nthr = mesh ? c->n_rows : P;
     const int rpe = c->un[1] * c->un[2];
-    const bool stage = c->un[0] > 0 && rpe >= 4 && 256 % rpe == 0;
+    const bool stage = c->un[0] > 0 && rpe >= 16 && 256 % rpe == 0;     // <= 16 elements per CTA fit the staging array
     if (phases & 1) {
         IB_CUDA_TRY(cudaMemsetAsync(c->d_tile_cur, 0, (size_t)n_tiles * sizeof(int32_t), st));
         if (mesh && stage) ibk_bin_mesh<0, 1><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);

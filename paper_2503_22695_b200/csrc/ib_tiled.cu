@@ -112,11 +112,13 @@ ibk_tiled_kernel(ib_tiled_params pr)
     if (tid == 0) {
         const int w = atomicAdd(&pr.counters[1], 1);
         s_work = (w < pr.counters[0]) ? __ldg(pr.work + w) : make_int4(-1, 0, 0, 0);
+        s_next = 0;
     }
+    for (int i = tid; i < NOC; i += TB) oc_cur[i] = 0;
+    for (int i = tid; i < 68; i += TB) bins[i] = 0;
     __syncthreads();
     for (;;) {
-        const int4 wk = s_work;
-        __syncthreads();
+        const int4 wk = s_work;                      // published by the barrier that ended the previous item
         if (wk.x < 0) break;
         // the next work item is claimed and read now; its latency hides behind this item's processing
         int4 nwk = make_int4(-1, 0, 0, 0);
@@ -144,10 +146,6 @@ ibk_tiled_kernel(ib_tiled_params pr)
 
         {
             // ---- stage the chunk, count points per half-cell -----------------------------------
-            for (int i = tid; i < NOC; i += TB) oc_cur[i] = 0;
-            for (int i = tid; i < 68; i += TB) bins[i] = 0;
-            if (tid == 0) s_next = 0;
-            __syncthreads();
             {
                 double xr[CH / TB][3];                   // all loads of the chunk in flight at once
 #pragma unroll
@@ -242,6 +240,10 @@ ibk_tiled_kernel(ib_tiled_params pr)
             }
             __syncthreads();
             const int nitems = s_nitems;
+            // the half-cell cursors and the count bins are dead from here on: reset them for the next
+            // work item (their next use lies behind the barriers that end this one)
+            for (int i = tid; i < NOC; i += TB) oc_cur[i] = 0;
+            for (int i = tid; i < 68; i += TB) bins[i] = 0;
 
             // ---- the items --------------------------------------------------------------------------
             double *mystg = stg + (wid * 8 + grp) * GSTRIDE;
@@ -417,7 +419,8 @@ ibk_tiled_kernel(ib_tiled_params pr)
                 }
             }
         }
-        if (tid == 0) s_work = nwk;
+        __syncthreads();                              // every warp has left the item loop and read s_work
+        if (tid == 0) { s_work = nwk; s_next = 0; }
         __syncthreads();                              // buffers are reused by the next work item
     }
 }
