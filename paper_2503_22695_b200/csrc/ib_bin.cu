@@ -290,7 +290,7 @@ __device__ __forceinline__ void ib_block_scan2(int &a, int &b, int *ws, int *wl,
     b = wl[wid] + ib - b;
 }
 
-__device__ __forceinline__ int ib_chunks(int c) { return (c + IB_CHUNK - 1) / IB_CHUNK; }
+__device__ __forceinline__ int ib_chunks(int c) { return c < IB_SMALL_TILE ? 0 : (c + IB_CHUNK - 1) / IB_CHUNK; }
 
 __global__ void __launch_bounds__(SCT)
 ibk_tile_partials(const int32_t *__restrict__ tile_cur, int n_tiles, int2 *__restrict__ partial)
@@ -311,10 +311,11 @@ ibk_tile_partials(const int32_t *__restrict__ tile_cur, int n_tiles, int2 *__res
 // start offsets and cursors of the tiles, and the work list: one entry per chunk of <= IB_CHUNK records
 __global__ void __launch_bounds__(SCT)
 ibk_tile_scan(int32_t *__restrict__ tile_cur, int n_tiles, const int2 *__restrict__ partial,
-              int32_t *__restrict__ tile_start, int4 *__restrict__ work, int32_t *__restrict__ counters)
+              int32_t *__restrict__ tile_start, int4 *__restrict__ work, int32_t *__restrict__ small_rec,
+              int32_t *__restrict__ counters)
 {
     __shared__ int ws[33], wl[33];
-    __shared__ int base_s, base_l;
+    __shared__ int base_s, base_l, base_m;
     if (threadIdx.x < 32) {
         int s = 0, l = 0;
         for (int b = threadIdx.x; b < (int)blockIdx.x; b += 32) { int2 p = partial[b]; s += p.x; l += p.y; }
@@ -336,7 +337,27 @@ ibk_tile_scan(int32_t *__restrict__ tile_cur, int n_tiles, const int2 *__restric
         const int cnt[4] = {c.x, c.y, c.z, c.w}, beg[4] = {st.x, st.y, st.z, st.w};
 #pragma unroll
         for (int k = 0; k < 4; ++k)
-            for (int o = 0; o < cnt[k]; o += IB_CHUNK) work[l++] = make_int4(t0 + k, beg[k] + o, min(IB_CHUNK, cnt[k] - o), 0);
+            for (int o = 0; o < cnt[k] && cnt[k] >= IB_SMALL_TILE; o += IB_CHUNK) work[l++] = make_int4(t0 + k, beg[k] + o, min(IB_CHUNK, cnt[k] - o), 0);
+    }
+    {   // records of sparsely filled tiles: a compact list (order across CTAs is whatever the atomic gives)
+        int m = 0, zero = 0, tm, tz;
+        if (t0 < n_tiles)
+            m = (c.x < IB_SMALL_TILE ? c.x : 0) + (c.y < IB_SMALL_TILE ? c.y : 0) + (c.z < IB_SMALL_TILE ? c.z : 0) +
+                (c.w < IB_SMALL_TILE ? c.w : 0);
+        ib_block_scan2(m, zero, ws, wl, tm, tz);
+        if (threadIdx.x == 0) base_m = tm ? atomicAdd(&counters[2], tm) : 0;
+        __syncthreads();
+        if (t0 < n_tiles) {
+            m += base_m;
+            const int cnt[4] = {c.x, c.y, c.z, c.w};
+            int r = s;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                if (cnt[k] < IB_SMALL_TILE)
+                    for (int o = 0; o < cnt[k]; ++o) small_rec[m++] = r + o;
+                r += cnt[k];
+            }
+        }
     }
     if (blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) {
         tile_start[n_tiles] = base_s + ts;
@@ -365,13 +386,14 @@ ib_status ibk_bin_points(ib_ctx *c, int mesh, const double *xp, const double *Gp
     const bool stage = c->un[0] > 0 && rpe >= 16 && 256 % rpe == 0;     // <= 16 elements per CTA fit the staging array
     if (phases & 1) {
         IB_CUDA_TRY(cudaMemsetAsync(c->d_tile_cur, 0, (size_t)n_tiles * sizeof(int32_t), st));
+        IB_CUDA_TRY(cudaMemsetAsync(c->d_tile_count, 0, 4 * sizeof(int32_t), st));
         if (mesh && stage) ibk_bin_mesh<0, 1><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
         else if (mesh) ibk_bin_mesh<0, 0><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
         else ibk_bin_cloud<0><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
         const int nsb = (n_tiles + SCT * SCI - 1) / (SCT * SCI);
         int2 *partial = reinterpret_cast<int2 *>(c->d_tile_count + 16);
         ibk_tile_partials<<<nsb, SCT, 0, st>>>(c->d_tile_cur, n_tiles, partial);
-        ibk_tile_scan<<<nsb, SCT, 0, st>>>(c->d_tile_cur, n_tiles, partial, c->d_tile_start, c->d_work, c->d_tile_count);
+        ibk_tile_scan<<<nsb, SCT, 0, st>>>(c->d_tile_cur, n_tiles, partial, c->d_tile_start, c->d_work, c->d_small_rec, c->d_tile_count);
         c->launches += 3;
     }
     if (phases & 2) {
@@ -391,6 +413,8 @@ ib_status ibk_bin_reserve(ib_ctx *c, int64_t P)
     if (c->d_sG) cudaFree(c->d_sG);
     if (c->d_sid) cudaFree(c->d_sid);
     if (c->d_work) cudaFree(c->d_work);
+    if (c->d_small_rec) cudaFree(c->d_small_rec);
+    c->d_small_rec = nullptr;
     c->d_sx = c->d_sG = nullptr; c->d_sid = nullptr; c->d_work = nullptr;
     c->bin_cap = 0;
     int64_t cap = P + P / 8 + 1024;
@@ -399,6 +423,7 @@ ib_status ibk_bin_reserve(ib_ctx *c, int64_t P)
     if (cudaMalloc(&c->d_sid, (size_t)cap * sizeof(int32_t)) != cudaSuccess) return IB_ERR_ALLOC;
     c->work_cap = c->n_cells / (BT * BT * BT) + cap / IB_CHUNK + 8;
     if (cudaMalloc(&c->d_work, (size_t)c->work_cap * sizeof(int4)) != cudaSuccess) return IB_ERR_ALLOC;
+    if (cudaMalloc(&c->d_small_rec, (size_t)cap * sizeof(int32_t)) != cudaSuccess) return IB_ERR_ALLOC;
     c->bin_cap = cap;
     return IB_OK;
 }

@@ -7,6 +7,7 @@
 
 #define IB_TILE 8              // tile edge of the binning key (A21)
 #define IB_TILE_CELLS 512
+#define IB_SMALL_TILE 32         // tiles with fewer points skip the tile kernel: their points go one by one (ib_point.cuh)
 #define IB_CHUNK 1728            // points per work item of the tile kernel (ib_bin.cu emits the work list)
 
 // ---------------------------------------------------------------------------------------------
@@ -52,6 +53,7 @@ struct ib_ctx {
     int32_t *d_tile_start;     // [n_tiles+1]
     int4 *d_work;              // work list of the tile kernel: {tile, first record, points, 0} per chunk
     int64_t work_cap;
+    int32_t *d_small_rec;      // records of tiles with < IB_SMALL_TILE points (count in d_tile_count[2])
     int32_t *d_tile_count;     // [0] number of non-empty tiles, [1] work counter
     int64_t bin_cap;
     double *d_sx, *d_sG;       // [3][P] point records grouped by tile

@@ -1,0 +1,67 @@
+// ib_point.cuh -- one point against the grid, no shared memory: delta weights in registers,
+// sum-factorised contraction, grid read through L1/L2, spread with native fp64 global reductions.
+// Used by variant 0 (ib_spread_interp.cu) and for the points of sparsely filled tiles (ib_tiled.cu).
+#pragma once
+#include "ib_common.cuh"
+
+struct ib_stencil {
+    int ix[2][4], iy[2][4], iz[2][4];      // wrapped indices, [0] face-aligned, [1] centre-aligned
+    double wx[2][4], wy[2][4], wz[2][4];
+};
+
+__device__ __forceinline__ void ib_axis(double x, double x0, double h, double inv_h, int n,
+                                        int idx[2][4], double wt[2][4])
+{
+    double sf = ib_scaled(x, x0, h, inv_h);
+#pragma unroll
+    for (int o = 0; o < 2; ++o) {
+        double s = o ? sf - 0.5 : sf;
+        double fl = floor(s);
+        ib_phi4(s - fl, wt[o]);
+        int i0 = ib_wrap((int)fl - 1, n);
+#pragma unroll
+        for (int m = 0; m < 4; ++m) {
+            int i = i0 + m;
+            idx[o][m] = i >= n ? i - n : i;
+        }
+    }
+}
+
+// G[c] (already divided by h^3) is spread to frc[c]; U[c] receives the interpolated fld[c].
+template <int DO_SPREAD, int DO_INTERP>
+__device__ __forceinline__ void ib_point_direct(double x, double y, double z, const double G[3],
+                                                const double *const fld[3], double *const frc[3],
+                                                const ib_grid_desc &g, double inv_h, double U[3])
+{
+    ib_stencil s;
+    ib_axis(x, g.x0, g.h, inv_h, g.nx, s.ix, s.wx);
+    ib_axis(y, g.y0, g.h, inv_h, g.ny, s.iy, s.wy);
+    ib_axis(z, g.z0, g.h, inv_h, g.nz, s.iz, s.wz);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const int ox = (c == 0) ? 0 : 1, oy = (c == 1) ? 0 : 1, oz = (c == 2) ? 0 : 1;
+        double acc = 0.0;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            double gk = DO_SPREAD ? G[c] * s.wz[oz][k] : 0.0;
+            double ak = 0.0;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                int64_t row = ((int64_t)s.iz[oz][k] * g.ny + s.iy[oy][j]) * g.nx;
+                if (DO_INTERP) {
+                    double r = 0.0;
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) r = fma(__ldg(fld[c] + row + s.ix[ox][i]), s.wx[ox][i], r);
+                    ak = fma(r, s.wy[oy][j], ak);
+                }
+                if (DO_SPREAD) {
+                    double gjk = gk * s.wy[oy][j];
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) atomicAdd(frc[c] + row + s.ix[ox][i], gjk * s.wx[ox][i]);
+                }
+            }
+            if (DO_INTERP) acc = fma(ak, s.wz[oz][k], acc);
+        }
+        U[c] = acc;
+    }
+}

@@ -6,30 +6,7 @@
 // variant 0 (this file, ibk_point_*): one thread per point, weights in registers, sum-factorised
 //   contraction, grid read through L1/L2, spread with native fp64 global reductions (RED.ADD.F64).
 // variant 1 (ib_tiled.cu): points sorted by Eulerian cell, shared-memory halo tile per 8^3 tile.
-#include "ib_common.cuh"
-
-struct ib_stencil {
-    int ix[2][4], iy[2][4], iz[2][4];      // wrapped indices, [0] face-aligned, [1] centre-aligned
-    double wx[2][4], wy[2][4], wz[2][4];
-};
-
-__device__ __forceinline__ void ib_axis(double x, double x0, double h, double inv_h, int n,
-                                        int idx[2][4], double wt[2][4])
-{
-    double sf = ib_scaled(x, x0, h, inv_h);
-#pragma unroll
-    for (int o = 0; o < 2; ++o) {
-        double s = o ? sf - 0.5 : sf;
-        double fl = floor(s);
-        ib_phi4(s - fl, wt[o]);
-        int i0 = ib_wrap((int)fl - 1, n);
-#pragma unroll
-        for (int m = 0; m < 4; ++m) {
-            int i = i0 + m;
-            idx[o][m] = i >= n ? i - n : i;
-        }
-    }
-}
+#include "ib_point.cuh"
 
 template <int DO_SPREAD, int DO_INTERP>
 __global__ void __launch_bounds__(128)
@@ -46,41 +23,13 @@ ibk_point_kernel(int64_t P, const double *__restrict__ xp, const double *__restr
         if (DO_INTERP) { Up[p] = 0.0; Up[P + p] = 0.0; Up[2 * P + p] = 0.0; }
         return;
     }
-    ib_stencil s;
-    ib_axis(x, g.x0, g.h, inv_h, g.nx, s.ix, s.wx);
-    ib_axis(y, g.y0, g.h, inv_h, g.ny, s.iy, s.wy);
-    ib_axis(z, g.z0, g.h, inv_h, g.nz, s.iz, s.wz);
     const double ih3 = inv_h * inv_h * inv_h;
-#pragma unroll
-    for (int c = 0; c < 3; ++c) {
-        const int ox = (c == 0) ? 0 : 1, oy = (c == 1) ? 0 : 1, oz = (c == 2) ? 0 : 1;
-        const double *fld = (c == 0) ? u : (c == 1) ? v : w;
-        double *frc = (c == 0) ? fu : (c == 1) ? fv : fw;
-        double Gc = DO_SPREAD ? __ldg(Gp + c * P + p) * ih3 : 0.0;
-        double acc = 0.0;
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            double gk = Gc * s.wz[oz][k];
-            double ak = 0.0;
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                int64_t row = ((int64_t)s.iz[oz][k] * g.ny + s.iy[oy][j]) * g.nx;
-                if (DO_INTERP) {
-                    double r = 0.0;
-#pragma unroll
-                    for (int i = 0; i < 4; ++i) r = fma(__ldg(fld + row + s.ix[ox][i]), s.wx[ox][i], r);
-                    ak = fma(r, s.wy[oy][j], ak);
-                }
-                if (DO_SPREAD) {
-                    double gjk = gk * s.wy[oy][j];
-#pragma unroll
-                    for (int i = 0; i < 4; ++i) atomicAdd(frc + row + s.ix[ox][i], gjk * s.wx[ox][i]);
-                }
-            }
-            if (DO_INTERP) acc = fma(ak, s.wz[oz][k], acc);
-        }
-        if (DO_INTERP) Up[c * P + p] = acc;
-    }
+    double G[3] = {0, 0, 0}, U[3];
+    if (DO_SPREAD) { G[0] = __ldg(Gp + p) * ih3; G[1] = __ldg(Gp + P + p) * ih3; G[2] = __ldg(Gp + 2 * P + p) * ih3; }
+    const double *const fld[3] = {u, v, w};
+    double *const frc[3] = {fu, fv, fw};
+    ib_point_direct<DO_SPREAD, DO_INTERP>(x, y, z, G, fld, frc, g, inv_h, U);
+    if (DO_INTERP) { Up[p] = U[0]; Up[P + p] = U[1]; Up[2 * P + p] = U[2]; }
 }
 
 ib_status ibk_spread_interp(ib_ctx *c, const double *xp, const double *Gp, int64_t P,

@@ -17,7 +17,7 @@
 // and exchanged through a 464-byte shared-memory staging record.  Force is reduced in registers
 // over all points of the item, then in shared memory over the items of the tile (fp64 CAS adds:
 // no native shared fp64 add), then ONE global RED.ADD.F64 per touched face of the halo.
-#include "ib_common.cuh"
+#include "ib_point.cuh"
 
 #define TT 4                    // tile edge in cells
 #define TH 8                    // halo edge
@@ -426,6 +426,25 @@ ibk_tiled_kernel(ib_tiled_params pr)
 }
 
 
+// Points of tiles with fewer than IB_SMALL_TILE points are not worth a halo and a sort: one thread per
+// point of the compact list written by ibk_tile_scan, every point treated directly against the grid.
+template <int DO_SPREAD, int DO_INTERP>
+__global__ void __launch_bounds__(128)
+ibk_small_tiles(ib_tiled_params pr, const int32_t *__restrict__ small_rec, const int32_t *__restrict__ counters)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= counters[2]) return;
+    const int64_t P = pr.P;
+    const int r = __ldg(small_rec + i);
+    double G[3] = {0, 0, 0}, U[3];
+    if (DO_SPREAD) { G[0] = pr.sG[r] * pr.ih3; G[1] = pr.sG[P + r] * pr.ih3; G[2] = pr.sG[2 * P + r] * pr.ih3; }
+    ib_point_direct<DO_SPREAD, DO_INTERP>(pr.sx[r], pr.sx[P + r], pr.sx[2 * P + r], G, pr.fld, pr.frc, pr.g, pr.inv_h, U);
+    if (DO_INTERP) {
+        const int id = pr.sid[r];
+        pr.Up[id] = U[0]; pr.Up[P + id] = U[1]; pr.Up[2 * P + id] = U[2];
+    }
+}
+
 template <int S, int I>
 static ib_status launch_tiled(ib_ctx *c, const ib_tiled_params &pr, cudaStream_t st)
 {
@@ -444,7 +463,10 @@ static ib_status launch_tiled(ib_ctx *c, const ib_tiled_params &pr, cudaStream_t
         sms = prop.multiProcessorCount;
     }
     ibk_tiled_kernel<S, I><<<sms * 2, TB, smem, st>>>(pr);
-    c->launches++;
+    // at most IB_SMALL_TILE-1 such records per tile, and never more than P
+    const int64_t nsmall_max = min((int64_t)pr.P, (c->n_cells / (TT * TT * TT)) * (int64_t)(IB_SMALL_TILE - 1));
+    ibk_small_tiles<S, I><<<ib_blocks(nsmall_max, 128), 128, 0, st>>>(pr, c->d_small_rec, c->d_tile_count);
+    c->launches += 2;
     return IB_OK;
 }
 
