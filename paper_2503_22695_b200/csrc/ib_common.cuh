@@ -8,7 +8,7 @@
 #define IB_TILE 8              // tile edge of the binning key (A21)
 #define IB_TILE_CELLS 512
 #define IB_SMALL_TILE 32         // tiles with fewer points skip the tile kernel: their points go one by one (ib_point.cuh)
-#define IB_CHUNK 1728            // points per work item of the tile kernel (ib_bin.cu emits the work list)
+#define IB_CHUNK 1920            // points per work item of the tile kernel (ib_bin.cu emits the work list)
 
 // ---------------------------------------------------------------------------------------------
 // host-side context

@@ -25,6 +25,7 @@
 #define NOC 512                 // half-cells per tile (8^3)
 #define NITEM 300               // 3 components x (4*5*5) shifted cells
 #define TB 192                  // threads per CTA (2 CTAs/SM at <= 168 registers)
+#define NCTA 2
 #define NWARP (TB / 32)
 #define CH IB_CHUNK             // points staged per work item (9 per thread)
 #define REC 14                  // staging record: wx[4] wy[4] wz[4] G pad (doubles)
@@ -85,19 +86,19 @@ __device__ __forceinline__ int ib_octant_key(double a, double b, double c)
 }
 
 template <int DO_SPREAD, int DO_INTERP>
-__global__ void __launch_bounds__(TB, 2)
+__global__ void __launch_bounds__(TB, NCTA)
 ibk_tiled_kernel(ib_tiled_params pr)
 {
     extern __shared__ __align__(16) double smem[];
     double *su = smem;                                   // [3][8][SZ] halo of u,v,w
     double *sxi = su + 3 * SU3;                          // [3][CH] tile-relative scaled coordinates
     double *stg = sxi + 3 * CH;                          // [NWARP*8][GSTRIDE]
-    int *oc_start = (int *)(stg + NWARP * 8 * GSTRIDE);  // [516]
-    int *oc_cur = oc_start + 516;                        // [512]
-    int *item_cnt = oc_cur + NOC;                        // [NITEM]
-    int *order = item_cnt + NITEM;                       // [NITEM]
-    int *bins = order + NITEM;                           // [68]
-    unsigned short *sidx = (unsigned short *)(bins + 68);// [CH]
+    int *oc_cur = (int *)(stg + NWARP * 8 * GSTRIDE);    // [512]
+    int *bins = oc_cur + NOC;                            // [68]
+    unsigned short *oc_start = (unsigned short *)(bins + 68);   // [516]
+    unsigned short *item_cnt = oc_start + 516;           // [NITEM]
+    unsigned short *order = item_cnt + NITEM;            // [NITEM]
+    unsigned short *sidx = order + NITEM;                // [CH]
     __shared__ int s_nitems, s_next;
     __shared__ int4 s_work;
     __shared__ int wsum[NWARP];
@@ -450,7 +451,7 @@ static ib_status launch_tiled(ib_ctx *c, const ib_tiled_params &pr, cudaStream_t
 {
     static int configured = 0;
     const size_t smem = (size_t)(3 * SU3 + 3 * CH + NWARP * 8 * GSTRIDE) * sizeof(double) +
-                        (516 + NOC + 2 * NITEM + 68) * sizeof(int) + CH * sizeof(unsigned short);
+                        (NOC + 68) * sizeof(int) + (516 + 2 * NITEM + CH) * sizeof(unsigned short);
     static_assert(CH % TB == 0, "chunk must be a whole number of points per thread");
     if (!configured) {
         IB_CUDA_TRY(cudaFuncSetAttribute(ibk_tiled_kernel<S, I>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -462,7 +463,7 @@ static ib_status launch_tiled(ib_ctx *c, const ib_tiled_params &pr, cudaStream_t
         IB_CUDA_TRY(cudaGetDeviceProperties(&prop, c->device));
         sms = prop.multiProcessorCount;
     }
-    ibk_tiled_kernel<S, I><<<sms * 2, TB, smem, st>>>(pr);
+    ibk_tiled_kernel<S, I><<<sms * NCTA, TB, smem, st>>>(pr);
     // at most IB_SMALL_TILE-1 such records per tile, and never more than P
     const int64_t nsmall_max = min((int64_t)pr.P, (c->n_cells / (TT * TT * TT)) * (int64_t)(IB_SMALL_TILE - 1));
     ibk_small_tiles<S, I><<<ib_blocks(nsmall_max, 128), 128, 0, st>>>(pr, c->d_small_rec, c->d_tile_count);
