@@ -132,6 +132,18 @@ ib_status ib_coupling_step(ib_ctx *ctx, const double *x, const double *u, const 
                            const double *w, double *fu, double *fv, double *fw, double *Un,
                            double *B, void *stream);
 
+/* NEXT-1: one time step of the paper's explicit coupling, Eq.(16), with a
+ * frozen velocity field -- the same operators in the paper's order:
+ *   U^IB = I(X^n, u^n)                      interpolate at the CURRENT positions (L173), project to the
+ *                                           nodes (L233-237)                       -> Un [3][n_nodes]
+ *   x_new = x + dt * Un                     move the structure (L173)             -> x_new [3][n_nodes]
+ *   B = fe_force(x_new)                     F^{n+1} from P^{n+1} (L169, L191)     -> B (may be NULL)
+ *   f = E(X^n, F^{n+1})                     spread with deltas centred at the OLD positions x (L171, L193)
+ * fu,fv,fw are overwritten. x_new must not alias x. */
+ib_status ib_step_eq16(ib_ctx *ctx, const double *x, const double *u, const double *v, const double *w,
+                       double dt, double *x_new, double *fu, double *fv, double *fw, double *Un, double *B,
+                       void *stream);
+
 /* Same step with HOST buffers: copies x,u,v,w host->device, runs the step, copies fu,fv,fw,Un
  * (and B if non-NULL) device->host, all on `stream`, then synchronises it. Buffers should be
  * pinned for full PCIe rate. */

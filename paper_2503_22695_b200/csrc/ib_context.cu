@@ -411,6 +411,65 @@ extern "C" ib_status ib_coupling_step(ib_ctx *c, const double *x, const double *
     return s;
 }
 
+__global__ void ibk_axpy(int64_t n, const double *__restrict__ x, double a, const double *__restrict__ y,
+                         double *__restrict__ out)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = fma(a, y[i], x[i]);
+}
+
+extern "C" ib_status ib_step_eq16(ib_ctx *c, const double *x, const double *u, const double *v, const double *w,
+                                  double dt, double *x_new, double *fu, double *fv, double *fw, double *Un,
+                                  double *B, void *stream)
+{
+    ib_status s = enter(c, stream);
+    if (s != IB_OK) return s;
+    if (!x || !u || !v || !w || !x_new || x_new == x || !fu || !fv || !fw || !Un || !std::isfinite(dt))
+        return IB_ERR_INVALID_ARG;
+    cudaStream_t st = ST(stream);
+    double *Bd = B ? B : c->d_B;
+    const int64_t n3 = 3 * c->n_nodes;
+    // 1. U^IB = I(X^n, u^n), projected to the nodes
+    if (c->nodal) {
+        if (c->n_nodes > 0) s = ibk_spread_interp(c, x, nullptr, c->n_nodes, u, v, w, nullptr, nullptr, nullptr, Un, 0, st);
+    } else {
+        if (c->n_points > 0) {
+            if (c->variant == 1)
+                s = ibk_tiled_spread_interp(c, 1, nullptr, nullptr, c->n_points, x, nullptr, u, v, w, nullptr, nullptr,
+                                            nullptr, c->d_Up, 0, st);
+            else {
+                s = ibk_points(c, x, nullptr, c->d_xp, nullptr, st);
+                if (s == IB_OK) s = ibk_spread_interp(c, c->d_xp, nullptr, c->n_points, u, v, w, nullptr, nullptr, nullptr,
+                                                      c->d_Up, 0, st);
+            }
+        }
+        if (s == IB_OK) s = ibk_restrict(c, c->d_Up, Un, st);
+    }
+    if (s != IB_OK) return s;
+    // 2. x_new = x + dt Un
+    if (n3 > 0) {
+        ibk_axpy<<<ib_blocks(n3, 256), 256, 0, st>>>(n3, x, dt, Un, x_new);
+        c->launches++;
+    }
+    // 3. F^{n+1} at the new positions
+    s = ibk_fe_force(c, x_new, Bd, c->nodal ? nullptr : c->d_Fhat, st);
+    if (s != IB_OK) return s;
+    // 4. f = E(X^n, F^{n+1}): spread at the OLD positions
+    const size_t gb = (size_t)c->n_cells * sizeof(double);
+    if (c->nodal) return ibk_spread_interp(c, x, Bd, c->n_nodes, nullptr, nullptr, nullptr, fu, fv, fw, nullptr, 0, st);
+    if (c->variant == 1) {
+        IB_CUDA_TRY(cudaMemsetAsync(fu, 0, gb, st));
+        IB_CUDA_TRY(cudaMemsetAsync(fv, 0, gb, st));
+        IB_CUDA_TRY(cudaMemsetAsync(fw, 0, gb, st));
+        if (c->n_points == 0) return IB_OK;
+        return ibk_tiled_spread_interp(c, 1, nullptr, nullptr, c->n_points, x, c->d_Fhat, nullptr, nullptr, nullptr, fu, fv,
+                                       fw, nullptr, 0, st);
+    }
+    s = ibk_points(c, x, c->d_Fhat, c->d_xp, c->d_Gp, st);
+    if (s != IB_OK) return s;
+    return ibk_spread_interp(c, c->d_xp, c->d_Gp, c->n_points, nullptr, nullptr, nullptr, fu, fv, fw, nullptr, 0, st);
+}
+
 extern "C" ib_status ib_coupling_step_host(ib_ctx *c, const double *x_h, const double *u_h, const double *v_h,
                                            const double *w_h, double *fu_h, double *fv_h, double *fw_h,
                                            double *Un_h, double *B_h, void *stream)

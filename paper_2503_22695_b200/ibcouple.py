@@ -20,7 +20,7 @@ STATUS = {0: "IB_OK", 1: "IB_ERR_INVALID_ARG", 2: "IB_ERR_UNSUPPORTED", 3: "IB_E
 
 EXPORTS = ["ib_create", "ib_destroy", "ib_num_points", "ib_num_nodes", "ib_num_elems", "ib_fe_force",
            "ib_points", "ib_restrict", "ib_bin_sort", "ib_spread", "ib_interp", "ib_coupling_step",
-           "ib_coupling_step_host", "ib_check", "ib_launch_count", "ib_set_variant", "ib_probe_dfma",
+           "ib_coupling_step_host", "ib_step_eq16", "ib_check", "ib_launch_count", "ib_set_variant", "ib_probe_dfma",
            "ib_profile_enable", "ib_profile_read",
            "ib_status_string"]
 
@@ -69,6 +69,7 @@ def lib():
         L.ib_interp.argtypes = [vp, vp, i64, vp, vp, vp, vp, vp]
         L.ib_coupling_step.argtypes = [vp] * 11
         L.ib_coupling_step_host.argtypes = [vp] * 11
+        L.ib_step_eq16.argtypes = [vp] * 5 + [C.c_double] + [vp] * 7
         L.ib_check.argtypes = [vp, C.POINTER(i64)]
         L.ib_set_variant.argtypes = [vp, i32]
         L.ib_profile_enable.argtypes = [vp, i32]
@@ -195,6 +196,10 @@ class Context:
     def ib_coupling_step(self, x, u, v, w, fu, fv, fw, Un, B=None, stream=None):
         _chk(lib().ib_coupling_step(self._h, _dp(x), _dp(u), _dp(v), _dp(w), _dp(fu), _dp(fv), _dp(fw), _dp(Un),
                                     _dp(B), _stream(stream)), "ib_coupling_step")
+
+    def ib_step_eq16(self, x, u, v, w, dt, x_new, fu, fv, fw, Un, B=None, stream=None):
+        _chk(lib().ib_step_eq16(self._h, _dp(x), _dp(u), _dp(v), _dp(w), float(dt), _dp(x_new), _dp(fu), _dp(fv),
+                                _dp(fw), _dp(Un), _dp(B), _stream(stream)), "ib_step_eq16")
 
     def ib_coupling_step_host(self, x, u, v, w, fu, fv, fw, Un, B=None, stream=None):
         """All tensors are (pinned) HOST tensors."""

@@ -283,3 +283,42 @@ def test_c5_top_of_sweep_invariants_and_sampled_outputs(ib, orc):
     _close(xs, xp_ref, "C5 sampled xp")
     _close(Up, orc.interp(_grid(orc, wl), xp_ref, wl.u, wl.v, wl.w), "C5 sampled U")
     ctx.close()
+
+
+# ---- NEXT-1: the paper's explicit coupling order, Eq.(16) L165-173 --------------------------------
+@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("name,nodal", [("C1", False), ("LV-small", False), ("C1", True)])
+def test_step_eq16_matches_oracle_composition(ib, orc, name, nodal, variant):
+    """U = I(X^n,u^n) -> nodes; x_new = x + dt U; B = fe_force(x_new); f = E(X^n, F^{n+1}) with the
+    deltas at the OLD positions.  The oracle side composes its own operators in that order."""
+    import torch
+    wl = CONFIGS[name]()
+    dt = 2e-3 * wl.h                                       # |u| <= 16: moves nodes by a few % of h
+    g = _grid(orc, wl)
+    nsub = None if nodal else wl.nsub
+    if nodal:
+        Un_r = orc.interp(g, wl.x, wl.u, wl.v, wl.w)
+    else:
+        xp, Wp, wa = orc.points(wl.conn, wl.X, wl.x, wl.nsub)
+        Un_r = orc.restrict(wl.conn, wl.nsub, wa, Wp, orc.interp(g, xp, wl.u, wl.v, wl.w))
+    x_new_r = wl.x + dt * Un_r
+    B_r = orc.fe_force(wl.conn, wl.X, x_new_r, wl.fibers, wl.mat_id, wl.mats)["B"]
+    f_r = orc.spread(g, wl.x, B_r) if nodal else orc.spread(g, xp, orc.prolong(wl.conn, wl.nsub, wa, Wp, B_r))
+
+    ctx = ib.Context.from_workload(wl, nodal=nodal)
+    ctx.ib_set_variant(variant)
+    f = [torch.full((wl.n_cells,), 5.0, dtype=torch.float64, device="cuda") for _ in range(3)]
+    Un, B, x_new = (torch.empty((3, wl.n_nodes), dtype=torch.float64, device="cuda") for _ in range(3))
+    ctx.ib_step_eq16(_t(wl.x), _t(wl.u), _t(wl.v), _t(wl.w), dt, x_new, *f, Un, B)
+    ctx.check()
+    _close(Un, Un_r, "eq16 Un")
+    _close(x_new, x_new_r, "eq16 x_new")
+    # B is compared at matching positions: feed the oracle the GPU's own x_new so that the comparison
+    # does not amplify the 1e-16 differences of x_new by the stiffness kappa
+    B_g = orc.fe_force(wl.conn, wl.X, x_new.cpu().numpy(), wl.fibers, wl.mat_id, wl.mats)["B"]
+    _close(B, B_g, "eq16 B")
+    f_g = orc.spread(g, wl.x, B_g) if nodal else orc.spread(g, xp, orc.prolong(wl.conn, wl.nsub, wa, Wp, B_g))
+    for c in range(3):
+        _close(f[c], f_g[c], f"eq16 f{c}")
+        assert rel_l2(f_g[c], f_r[c]) < 1e-8              # and the two oracle runs agree to conditioning
+    ctx.close()
