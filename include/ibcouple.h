@@ -60,14 +60,20 @@ typedef struct {
     int32_t periodic;
 } ib_grid_desc;
 
-typedef enum { IB_LAW_NEOHOOKEAN = 0, IB_LAW_HO = 1 } ib_law;
+typedef enum { IB_LAW_NEOHOOKEAN = 0, IB_LAW_HO = 1, IB_LAW_MSR = 2, IB_LAW_FR2 = 3 } ib_law;
 
 /* Material row. HO (Eq.(12)-(15)): a,b isotropic; af,bf / as_,bs fibre and sheet; afs,bfs
  * coupling; kappa = kappa_stab of U(J) = kappa/2 (ln J)^2 (L94). neo-Hookean (L441-445):
- * a = mu (= 2 alpha), b = 0, fibre constants ignored. */
+ * a = mu (= 2 alpha), b = 0, fibre constants ignored.
+ * NEXT-2 laws: IB_LAW_MSR, modified standard reinforcing model Eq.(7): a = G_T (b = 0),
+ * af = G_L, bf = E_L.  IB_LAW_FR2, fibre-reinforced model 2 Eq.(10)-(11) L136-141: a = 2 C10 C01,
+ * b = C01, af, bf, fibre term on I4f without the tension switch.  Fibre-reinforced model 1,
+ * Eq.(8)-(9) L128-134, is IB_LAW_HO with a = 2 C1, b = 0, as_ = afs = 0.
+ * Ta: active tension T_a(t) of L317-331, P += Ta (1 + 4.9 (sqrt(I4f) - 1)) F e_f (x) e_f; 0 = passive. */
 typedef struct {
     int32_t law;
     double a, b, af, bf, as_, bs, afs, bfs, kappa;
+    double Ta;
 } ib_material;
 
 /* Static mesh description; all pointers are HOST pointers, copied by ib_create. */

@@ -20,7 +20,7 @@ _lib = None
 
 class Material(C.Structure):
     _fields_ = [("law", C.c_int32)] + [(k, C.c_double) for k in
-                                       ("a", "b", "af", "bf", "as_", "bs", "afs", "bfs", "kappa")]
+                                       ("a", "b", "af", "bf", "as_", "bs", "afs", "bfs", "kappa", "Ta")]
 
 
 class Grid(C.Structure):
@@ -68,6 +68,7 @@ def make_materials(mats):
         arr[i].law = int(m["law"])
         for k in ("a", "b", "af", "bf", "as_", "bs", "afs", "bfs", "kappa"):
             setattr(arr[i], k, float(m[k]))
+        arr[i].Ta = float(m.get("Ta", 0.0))
     return arr
 
 

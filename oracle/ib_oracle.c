@@ -34,8 +34,10 @@
 typedef long double ld;
 
 typedef struct {
-    int32_t law;            /* 0 neo-Hookean, 1 Holzapfel-Ogden */
+    int32_t law;            /* 0 neo-Hookean, 1 Holzapfel-Ogden, 2 modified standard reinforcing (Eq.7),
+                               3 fibre-reinforced model 2 (Eq.10-11) */
     double a, b, af, bf, as_, bs, afs, bfs, kappa;
+    double Ta;              /* active tension T_a(t) of L317-331 (0 = passive) */
 } oracle_material;
 
 typedef struct {
@@ -176,6 +178,48 @@ static int pk1_l(const oracle_material *m, const ld F[3][3], const ld ef[3], con
             for (int c = 0; c < 3; ++c)
                 for (int K = 0; K < 3; ++K) P[c][K] += c2 * (Ff[c] * es[K] + Fs[c] * ef[K]);
         }
+    }
+    /* Modified standard reinforcing model Psi_1 / P_1, Eq.(7) L119-124 (NEXT-2): a = G_T (b = 0),
+     * af = G_L, bf = E_L:
+     *   Psi += (G_T-G_L)/2 (2 I4f - I5f - 1) + (E_L+G_T-4G_L)/8 (I4f-1)^2,  I5f = e_f.(C^2 e_f) (L104)
+     *   P   += (G_T-G_L)(2 F ef(x)ef - F ef (x) C ef - F C ef (x) ef) + (E_L+G_T-4G_L)/2 (I4f-1) F ef(x)ef */
+    if (m->law == 2) {
+        ld GT = m->a, GL = m->af, EL = m->bf;
+        ld Ff[3], Cf[3], FCf[3];
+        for (int c = 0; c < 3; ++c) Ff[c] = F[c][0] * ef[0] + F[c][1] * ef[1] + F[c][2] * ef[2];
+        for (int K = 0; K < 3; ++K) Cf[K] = F[0][K] * Ff[0] + F[1][K] * Ff[1] + F[2][K] * Ff[2];   /* C ef = F^T F ef */
+        for (int c = 0; c < 3; ++c) FCf[c] = F[c][0] * Cf[0] + F[c][1] * Cf[1] + F[c][2] * Cf[2];
+        ld I4f = Ff[0] * Ff[0] + Ff[1] * Ff[1] + Ff[2] * Ff[2];
+        ld I5f = Cf[0] * Cf[0] + Cf[1] * Cf[1] + Cf[2] * Cf[2];
+        ld k2 = EL + GT - 4.0L * GL;
+        W += 0.5L * (GT - GL) * (2.0L * I4f - I5f - 1.0L) + 0.125L * k2 * (I4f - 1.0L) * (I4f - 1.0L);
+        for (int c = 0; c < 3; ++c)
+            for (int K = 0; K < 3; ++K)
+                P[c][K] += (GT - GL) * (2.0L * Ff[c] * ef[K] - Ff[c] * Cf[K] - FCf[c] * ef[K])
+                         + 0.5L * k2 * (I4f - 1.0L) * Ff[c] * ef[K];
+    }
+    /* Fibre-reinforced model 2, Psi_3 / P_3, Eq.(10)-(11) L136-141 (NEXT-2; reading A4: C_01 in the
+     * exponent of P_3): isotropic part = the exponential term above with a = 2 C10 C01, b = C01
+     * and the "-1" of Eq.(10), i.e. an offset C10 = a/(2b), restored; fibre term on I4f itself, NO switch:
+     *   Psi += af/(2bf)(exp[bf (I4f-1)^2] - 1),  P += 2 af (I4f-1) exp[bf (I4f-1)^2] F ef(x)ef */
+    if (m->law == 3 && b != 0.0L) W -= a / (2.0L * b);
+    if (m->law == 3 && m->af != 0.0) {
+        ld Ff[3];
+        for (int c = 0; c < 3; ++c) Ff[c] = F[c][0] * ef[0] + F[c][1] * ef[1] + F[c][2] * ef[2];
+        ld d = Ff[0] * Ff[0] + Ff[1] * Ff[1] + Ff[2] * Ff[2] - 1.0L, ex = expl((ld)m->bf * d * d);
+        W += (m->bf != 0.0) ? (ld)m->af / (2.0L * (ld)m->bf) * (ex - 1.0L) : 0.5L * (ld)m->af * d * d;
+        for (int c = 0; c < 3; ++c)
+            for (int K = 0; K < 3; ++K) P[c][K] += 2.0L * (ld)m->af * d * ex * Ff[c] * ef[K];
+    }
+    /* Active stress (L317-331, NEXT-2): P^a = F S_a, S_a = T e_f (x) e_f, T = T_a (1 + 4.9 (sqrt(I4f) - 1)).
+     * Not hyperelastic: it has no energy, psi is the passive energy only. */
+    if (m->Ta != 0.0) {
+        ld Ff[3];
+        for (int c = 0; c < 3; ++c) Ff[c] = F[c][0] * ef[0] + F[c][1] * ef[1] + F[c][2] * ef[2];
+        ld I4f = Ff[0] * Ff[0] + Ff[1] * Ff[1] + Ff[2] * Ff[2];
+        ld T = (ld)m->Ta * (1.0L + 4.9L * (sqrtl(I4f) - 1.0L));
+        for (int c = 0; c < 3; ++c)
+            for (int K = 0; K < 3; ++K) P[c][K] += T * Ff[c] * ef[K];
     }
     if (psi) *psi = W;
     return 0;

@@ -137,7 +137,7 @@ extern "C" ib_status ib_create(ib_ctx **out, const ib_grid_desc *g, const ib_mes
     if (m->n_elems > 0 && (!m->conn || !m->X_ref || !m->mats || m->n_mats <= 0)) return IB_ERR_INVALID_ARG;
     if (m->n_nodes > 0 && !m->X_ref) return IB_ERR_INVALID_ARG;
     for (int i = 0; i < m->n_mats; ++i)
-        if (m->mats[i].law != IB_LAW_NEOHOOKEAN && m->mats[i].law != IB_LAW_HO) return IB_ERR_INVALID_ARG;
+        if (m->mats[i].law < IB_LAW_NEOHOOKEAN || m->mats[i].law > IB_LAW_FR2) return IB_ERR_INVALID_ARG;
 
     // host-side validation and topology
     const int64_t nn = m->n_nodes, ne = m->n_elems;

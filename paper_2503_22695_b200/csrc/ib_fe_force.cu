@@ -9,7 +9,7 @@
 // no CSR, no assembled operator).
 #include "ib_common.cuh"
 
-// first Piola-Kirchhoff stress. Readings A2 (F^-T in the isotropic term), A3 (symmetric I8 term),
+// first Piola-Kirchhoff stress (HO, NH; NEXT-2: Eq.(7), Eq.(10)-(11), active stress). Readings A2 (F^-T in the isotropic term), A3 (symmetric I8 term),
 // A6 (NH: a = mu, b = 0), A9 (I4* = max(I4,1)). Returns J.
 __device__ __forceinline__ double ib_pk1(const ib_material &m, const double F[3][3], const double ef[3],
                                          const double es[3], double P[3][3])
@@ -44,20 +44,41 @@ __device__ __forceinline__ double ib_pk1(const ib_material &m, const double F[3]
     for (int c = 0; c < 3; ++c)
 #pragma unroll
         for (int K = 0; K < 3; ++K) P[c][K] = fma(ciso, F[c][K], cvol * cof[c][K]);
-    if (m.law == IB_LAW_HO) {
+    if (m.law != IB_LAW_NEOHOOKEAN || m.Ta != 0.0) {
         double Ff[3], Fs[3];
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
             Ff[c] = F[c][0] * ef[0] + F[c][1] * ef[1] + F[c][2] * ef[2];
             Fs[c] = F[c][0] * es[0] + F[c][1] * es[1] + F[c][2] * es[2];
         }
-        double I4f = Ff[0] * Ff[0] + Ff[1] * Ff[1] + Ff[2] * Ff[2];
-        double I4s = Fs[0] * Fs[0] + Fs[1] * Fs[1] + Fs[2] * Fs[2];
-        double I8 = Ff[0] * Fs[0] + Ff[1] * Fs[1] + Ff[2] * Fs[2];
-        double df = fmax(I4f, 1.0) - 1.0, ds = fmax(I4s, 1.0) - 1.0;
-        double cf = (m.af != 0.0 && df > 0.0) ? 2.0 * m.af * df * exp(m.bf * df * df) : 0.0;
-        double cs = (m.as_ != 0.0 && ds > 0.0) ? 2.0 * m.as_ * ds * exp(m.bs * ds * ds) : 0.0;
-        double cfs = (m.afs != 0.0) ? m.afs * I8 * exp(m.bfs * I8 * I8) : 0.0;
+        const double I4f = Ff[0] * Ff[0] + Ff[1] * Ff[1] + Ff[2] * Ff[2];
+        double cf = 0.0, cs = 0.0, cfs = 0.0;              // coefficients of Ff(x)ef, Fs(x)es, Ff(x)es + Fs(x)ef
+        if (m.law == IB_LAW_HO) {
+            double I4s = Fs[0] * Fs[0] + Fs[1] * Fs[1] + Fs[2] * Fs[2];
+            double I8 = Ff[0] * Fs[0] + Ff[1] * Fs[1] + Ff[2] * Fs[2];
+            double df = fmax(I4f, 1.0) - 1.0, ds = fmax(I4s, 1.0) - 1.0;
+            cf = (m.af != 0.0 && df > 0.0) ? 2.0 * m.af * df * exp(m.bf * df * df) : 0.0;
+            cs = (m.as_ != 0.0 && ds > 0.0) ? 2.0 * m.as_ * ds * exp(m.bs * ds * ds) : 0.0;
+            cfs = (m.afs != 0.0) ? m.afs * I8 * exp(m.bfs * I8 * I8) : 0.0;
+        } else if (m.law == IB_LAW_FR2) {
+            // Eq.(11): fibre term on I4f itself, no tension switch
+            double df = I4f - 1.0;
+            cf = (m.af != 0.0) ? 2.0 * m.af * df * exp(m.bf * df * df) : 0.0;
+        } else if (m.law == IB_LAW_MSR) {
+            // Eq.(7): a = G_T, af = G_L, bf = E_L;  (G_T-G_L)(2 Ff(x)ef - Ff(x)C ef - F C ef(x)ef) + k2/2 (I4f-1) Ff(x)ef
+            const double gd = m.a - m.af, k2 = m.bf + m.a - 4.0 * m.af;
+            double Cf[3], FCf[3];
+#pragma unroll
+            for (int K = 0; K < 3; ++K) Cf[K] = F[0][K] * Ff[0] + F[1][K] * Ff[1] + F[2][K] * Ff[2];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) FCf[c] = F[c][0] * Cf[0] + F[c][1] * Cf[1] + F[c][2] * Cf[2];
+            cf = 2.0 * gd + 0.5 * k2 * (I4f - 1.0);
+#pragma unroll
+            for (int c = 0; c < 3; ++c)
+#pragma unroll
+                for (int K = 0; K < 3; ++K) P[c][K] -= gd * (Ff[c] * Cf[K] + FCf[c] * ef[K]);
+        }
+        if (m.Ta != 0.0) cf += m.Ta * (1.0 + 4.9 * (sqrt(I4f) - 1.0));          // active stress, L317-331
 #pragma unroll
         for (int c = 0; c < 3; ++c)
 #pragma unroll

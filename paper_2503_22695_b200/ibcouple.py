@@ -38,7 +38,7 @@ class GridDesc(C.Structure):
 
 class Material(C.Structure):
     _fields_ = [("law", C.c_int32)] + [(k, C.c_double) for k in
-                                       ("a", "b", "af", "bf", "as_", "bs", "afs", "bfs", "kappa")]
+                                       ("a", "b", "af", "bf", "as_", "bs", "afs", "bfs", "kappa", "Ta")]
 
 
 class MeshDesc(C.Structure):
@@ -124,6 +124,7 @@ class Context:
             marr[i].law = int(m["law"])
             for k in ("a", "b", "af", "bf", "as_", "bs", "afs", "bfs", "kappa"):
                 setattr(marr[i], k, float(m[k]))
+            marr[i].Ta = float(m.get("Ta", 0.0))
         g = GridDesc(int(nx), int(ny), int(nz), float(h), float(origin[0]), float(origin[1]), float(origin[2]),
                      int(periodic))
         md = MeshDesc(X.shape[1] if X.ndim == 2 else 0, conn.shape[0],

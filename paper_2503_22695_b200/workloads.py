@@ -26,15 +26,17 @@ SEED_ROOT = 250322695
 
 LAW_NEOHOOKEAN = 0
 LAW_HO = 1
+LAW_MSR = 2          # modified standard reinforcing model, Eq.(7): a=G_T, af=G_L, bf=E_L
+LAW_FR2 = 3          # fibre-reinforced model 2, Eq.(10)-(11): a=2 C10 C01, b=C01, af, bf (no tension switch)
 
 # local node a = ia + 2*ja + 4*ka  (SURVEY.md §8 "Mesh")
 _LOCAL = np.array([[a & 1, (a >> 1) & 1, (a >> 2) & 1] for a in range(8)], dtype=np.int64)
 
 
-def material(law, a=0.0, b=0.0, af=0.0, bf=0.0, as_=0.0, bs=0.0, afs=0.0, bfs=0.0, kappa=0.0):
+def material(law, a=0.0, b=0.0, af=0.0, bf=0.0, as_=0.0, bs=0.0, afs=0.0, bfs=0.0, kappa=0.0, Ta=0.0):
     """One row of the material table (ib_material in include/ibcouple.h). NH: a=mu, b=0."""
     return dict(law=int(law), a=float(a), b=float(b), af=float(af), bf=float(bf), as_=float(as_),
-                bs=float(bs), afs=float(afs), bfs=float(bfs), kappa=float(kappa))
+                bs=float(bs), afs=float(afs), bfs=float(bfs), kappa=float(kappa), Ta=float(Ta))
 
 
 @dataclass

@@ -322,3 +322,31 @@ def test_step_eq16_matches_oracle_composition(ib, orc, name, nodal, variant):
         _close(f[c], f_g[c], f"eq16 f{c}")
         assert rel_l2(f_g[c], f_r[c]) < 1e-8              # and the two oracle runs agree to conditioning
     ctx.close()
+
+
+def test_fe_force_next2_laws_and_active_stress(ib, orc):
+    """NEXT-2: Eq.(7), Eq.(8)-(9) as an HO special case, Eq.(10)-(11), and the active stress of L317-331,
+    mixed element by element on a distorted block."""
+    import torch
+    conn, X, x, fib = distorted_block(5, 4, 3, seed=21, cur_noise=0.04)
+    ne, nn = conn.shape[0], X.shape[1]
+    mats = [W.material(W.LAW_MSR, a=8e4, af=1.6e5, bf=2.0e6, kappa=4e6),
+            W.material(W.LAW_HO, a=34.0, b=0.0, af=31.0, bf=4.0, kappa=1e3),                  # Eq.(8)-(9)
+            W.material(W.LAW_FR2, a=2 * 1.21 * 7.99, b=7.99, af=24.23, bf=57.62, kappa=1e3),
+            W.material(W.LAW_HO, Ta=60.0, **W.HO_LV),                                          # active myocardium
+            W.material(W.LAW_NEOHOOKEAN, a=100.0, kappa=1e3, Ta=5.0)]
+    mid = (np.arange(ne) % len(mats)).astype(np.int32)
+    ctx = ib.Context(16, 16, 16, 1 / 16, (0, 0, 0), conn, X, fib, mid, None, mats)
+    B = torch.empty((3, nn), dtype=torch.float64, device="cuda")
+    ctx.ib_fe_force(_t(x), B)
+    ctx.check()
+    ref = orc.fe_force(conn, X, x, fib, mid, mats)
+    _close(B, ref["B"], "NEXT-2 laws B")
+    # each law alone, so that a wrong branch cannot hide behind the stiffest material
+    for k, m in enumerate(mats):
+        c1 = ib.Context(16, 16, 16, 1 / 16, (0, 0, 0), conn, X, fib, None, None, [m])
+        c1.ib_fe_force(_t(x), B)
+        c1.check()
+        _close(B, orc.fe_force(conn, X, x, fib, np.zeros(ne, np.int32), [m])["B"], f"law {k} B")
+        c1.close()
+    ctx.close()

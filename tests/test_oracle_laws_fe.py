@@ -299,3 +299,91 @@ def test_generated_configs_are_valid(orc):
         lo = np.array(wl.origin) + 4 * wl.h   # full-size 6h margins: tests/test_workloads.py
         hi = np.array(wl.origin) + (np.array([wl.nx, wl.ny, wl.nz]) - 4) * wl.h
         assert np.all(wl.x.min(axis=1) > lo) and np.all(wl.x.max(axis=1) < hi)
+
+
+# ---- NEXT-2: the paper's other constitutive laws and the active stress ------------------------------
+# Table 1 (L273-285)-like magnitudes for Eq.(7); Table 4 (L410-421) recast for Eq.(10)-(11)
+MSR = W.material(W.LAW_MSR, a=8e4, af=1.6e5, bf=2.0e6, kappa=4e6)          # G_T, G_L, E_L
+FR2 = W.material(W.LAW_FR2, a=2 * 1.21 * 7.99, b=7.99, af=24.23, bf=57.62, kappa=1e3)
+
+
+@pytest.mark.parametrize("mat", [MSR, FR2], ids=["MSR_eq7", "FR2_eq10"])
+def test_next2_laws_P_is_dPsi_dF_and_objective(orc, mat):
+    rng = np.random.default_rng(5)
+    for trial in range(6):
+        F = np.eye(3) + 0.12 * rng.normal(size=(3, 3))
+        ef = rng.normal(size=3)
+        ef /= np.linalg.norm(ef)
+        es = np.cross(ef, rng.normal(size=3))
+        es /= np.linalg.norm(es)
+        P, psi = orc.pk1(mat, F, ef, es)
+        Pfd = _fd_P(orc, mat, F, ef, es)
+        assert np.max(np.abs(P - Pfd)) < 2e-8 * np.max(np.abs(P)), trial       # Eq.(7) / Eq.(11) with A4
+        S = P @ F.T
+        assert np.max(np.abs(S - S.T)) < 1e-12 * np.max(np.abs(S))
+        Q = rotation(trial)
+        Pq, psiq = orc.pk1(mat, Q @ F, ef, es)
+        assert abs(psiq - psi) < 1e-12 * max(abs(psi), 1e-30)
+        assert np.max(np.abs(Pq - Q @ P)) < 1e-12 * np.max(np.abs(P))
+    P, psi = orc.pk1(mat, np.eye(3), np.array([1.0, 0, 0]), np.array([0, 1.0, 0]))
+    assert np.max(np.abs(P)) < 1e-9 * mat["kappa"] and abs(psi) < 1e-12          # stress-free reference
+
+
+def test_next2_closed_forms(orc):
+    ex, ey = np.array([1.0, 0, 0]), np.array([0, 1.0, 0])
+    # Eq.(7) on F = diag(l, 1, 1), fibre along x: I4 = l^2, I5 = l^4;
+    # P11 = iso11 + (G_T-G_L)(2l - 2l^3) + (E_L+G_T-4G_L)/2 (l^2-1) l, other entries = isotropic part
+    l = 1.07
+    F = np.diag([l, 1.0, 1.0])
+    P, psi = orc.pk1(MSR, F, ex, ey)
+    P_iso, psi_iso = orc.pk1(W.material(W.LAW_NEOHOOKEAN, a=MSR["a"], kappa=MSR["kappa"]), F)
+    GT, GL, EL = MSR["a"], MSR["af"], MSR["bf"]
+    add = (GT - GL) * (2 * l - 2 * l ** 3) + 0.5 * (EL + GT - 4 * GL) * (l * l - 1) * l
+    expect = P_iso.copy()
+    expect[0, 0] += add
+    assert np.allclose(P, expect, rtol=1e-13, atol=1e-9)
+    assert abs(psi - psi_iso - (0.5 * (GT - GL) * (2 * l * l - l ** 4 - 1) + 0.125 * (EL + GT - 4 * GL) * (l * l - 1) ** 2)) < 1e-9
+    # Eq.(8)-(9) is the HO law with a = 2 C1, b = 0 and only the fibre family: same numbers as Eq.(9) typed out
+    C1, af, bf, kap = 17.0, 31.0, 4.0, 1e3
+    m = W.material(W.LAW_HO, a=2 * C1, b=0.0, af=af, bf=bf, kappa=kap)
+    P, _ = orc.pk1(m, F, ex, ey)
+    J, I1 = l, l * l + 2
+    Fit = np.diag([1 / l, 1.0, 1.0])
+    P9 = 2 * C1 * J ** (-2 / 3) * (F - I1 / 3 * Fit) + 2 * af * (l * l - 1) * np.exp(bf * (l * l - 1) ** 2) * l * np.outer(ex, ex) \
+        + kap * np.log(J) * Fit
+    assert np.allclose(P, P9, rtol=1e-13, atol=1e-12)
+    # Eq.(11) has no tension switch: a compressed fibre pushes back (HO's I4* would give exactly zero)
+    lc = 0.9
+    Fc = np.diag([lc, 1.0, 1.0])
+    Pc, _ = orc.pk1(FR2, Fc, ex, ey)
+    Pc0, _ = orc.pk1(W.material(W.LAW_FR2, a=FR2["a"], b=FR2["b"], kappa=FR2["kappa"]), Fc, ex, ey)
+    d = lc * lc - 1
+    assert abs((Pc - Pc0)[0, 0] - 2 * FR2["af"] * d * np.exp(FR2["bf"] * d * d) * lc) < 1e-12
+    assert (Pc - Pc0)[0, 0] < 0 and np.count_nonzero(Pc - Pc0) == 1
+
+
+def test_active_stress_closed_form(orc):
+    """L317-331: P^a = F S_a, S_a = T e_f (x) e_f, T = T_a (1 + 4.9 (sqrt(I4f) - 1))."""
+    ex, ey = np.array([1.0, 0, 0]), np.array([0, 1.0, 0])
+    Ta, l = 60.0, 1.15
+    F = np.diag([l, 0.95, 1.0])
+    passive = dict(HO)
+    active = dict(HO, Ta=Ta)
+    P0, w0 = orc.pk1(passive, F, ex, ey)
+    P1, w1 = orc.pk1(active, F, ex, ey)
+    expect = np.zeros((3, 3))
+    expect[0, 0] = Ta * (1 + 4.9 * (l - 1)) * l
+    assert np.allclose(P1 - P0, expect, rtol=0, atol=1e-12) and w1 == w0
+    # general F and fibre: the added first Piola stress is T (F ef)(x)ef and keeps P F^T symmetric
+    rng = np.random.default_rng(2)
+    F = np.eye(3) + 0.2 * rng.normal(size=(3, 3))
+    ef = rng.normal(size=3)
+    ef /= np.linalg.norm(ef)
+    es = np.cross(ef, rng.normal(size=3))
+    es /= np.linalg.norm(es)
+    dP = orc.pk1(active, F, ef, es)[0] - orc.pk1(passive, F, ef, es)[0]
+    S = np.linalg.solve(F, dP)                                  # second Piola-Kirchhoff S_a = F^-1 P^a
+    T = Ta * (1 + 4.9 * (np.linalg.norm(F @ ef) - 1))
+    assert np.allclose(S, T * np.outer(ef, ef), rtol=1e-11, atol=1e-11)
+    # at the reference configuration the active tension is T_a along the fibre
+    assert np.allclose(orc.pk1(active, np.eye(3), ex, ey)[0], Ta * np.outer(ex, ex), atol=1e-10)
