@@ -334,7 +334,7 @@ def run_ours(args):
                            "input_sha256": wl.sha256()},
                 "clocks": clocks,
                 "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                        "steps": e2e_steps, "api": "ib_coupling_step_host (pinned host buffers)"},
+                        "steps": e2e_steps, "api": "ib_coupling_step_host (pinned host buffers; spread and interpolation pipelined around the copies on two streams)"},
                 "gpu_launches": int(launches),
                 "wall_s_timed_region": t_wall,
                 "roofline": roofline,

@@ -151,8 +151,9 @@ ib_status ib_step_eq16(ib_ctx *ctx, const double *x, const double *u, const doub
                        void *stream);
 
 /* Same step with HOST buffers: copies x,u,v,w host->device, runs the step, copies fu,fv,fw,Un
- * (and B if non-NULL) device->host, all on `stream`, then synchronises it. Buffers should be
- * pinned for full PCIe rate. */
+ * (and B if non-NULL) device->host, then synchronises. Buffers should be pinned for full PCIe rate.
+ * In the default variant the force side (which needs only x) runs while u,v,w are still being
+ * copied on the context's side stream, and fu,fv,fw travel back while the velocity side runs. */
 ib_status ib_coupling_step_host(ib_ctx *ctx, const double *x_host, const double *u_host,
                                 const double *v_host, const double *w_host, double *fu_host,
                                 double *fv_host, double *fw_host, double *Un_host, double *B_host,

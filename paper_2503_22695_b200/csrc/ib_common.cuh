@@ -64,7 +64,7 @@ struct ib_ctx {
     long long *d_status;
     cudaStream_t last_stream;
     cudaStream_t side;         // internal stream: work that needs only the positions overlaps the FE force
-    cudaEvent_t ev_fork, ev_join;
+    cudaEvent_t ev_fork, ev_join, ev_aux;
     int64_t launches;
     // optional per-phase event timing
     int profile;
@@ -203,5 +203,8 @@ ib_status ibk_tiled_spread_interp(ib_ctx *c, int mesh, const double *xp, const d
                                   const double *x, const double *Fhat,
                                   const double *u, const double *v, const double *w,
                                   double *fu, double *fv, double *fw, double *Up, int counted, cudaStream_t st);
+ib_status ibk_tiled_launch(ib_ctx *c, int64_t P, int do_spread, int do_interp,
+                           const double *u, const double *v, const double *w,
+                           double *fu, double *fv, double *fw, double *Up, cudaStream_t st);
 ib_status ibk_bin_points(ib_ctx *c, int mesh, const double *xp, const double *Gp, int64_t P,
                          const double *x, const double *Fhat, double *Up, int phases, cudaStream_t st);

@@ -112,6 +112,7 @@ extern "C" ib_status ib_destroy(ib_ctx *c)
     if (c->side) cudaStreamDestroy(c->side);
     if (c->ev_fork) cudaEventDestroy(c->ev_fork);
     if (c->ev_join) cudaEventDestroy(c->ev_join);
+    if (c->ev_aux) cudaEventDestroy(c->ev_aux);
     if (c->prof) {
         double ms[IB_PHASE_COUNT];
         int64_t n[IB_PHASE_COUNT];
@@ -219,7 +220,8 @@ extern "C" ib_status ib_create(ib_ctx **out, const ib_grid_desc *g, const ib_mes
     TRY(dev_alloc((void **)&c->d_status, 2 * sizeof(long long)));
     if (s == IB_OK && (cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) != cudaSuccess ||
                        cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
-                       cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess))
+                       cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess ||
+                       cudaEventCreateWithFlags(&c->ev_aux, cudaEventDisableTiming) != cudaSuccess))
         s = IB_ERR_CUDA;
     if (s == IB_OK) s = reset_status(c, 0);
     if (s == IB_OK) s = ibk_sort_reserve(c, c->n_points);
@@ -487,19 +489,59 @@ extern "C" ib_status ib_coupling_step_host(ib_ctx *c, const double *x_h, const d
         for (auto b : gbufs) if (a == IB_OK) a = dev_alloc((void **)b, gb);
         if (a != IB_OK) return a;
     }
+    const bool pipelined = c->variant == 1 && !c->nodal && !c->profile && c->n_points > 0;
+    if (!pipelined) {
+        IB_CUDA_TRY(cudaMemcpyAsync(c->d_hx, x_h, nb, cudaMemcpyHostToDevice, st));
+        IB_CUDA_TRY(cudaMemcpyAsync(c->d_hu, u_h, gb, cudaMemcpyHostToDevice, st));
+        IB_CUDA_TRY(cudaMemcpyAsync(c->d_hv, v_h, gb, cudaMemcpyHostToDevice, st));
+        IB_CUDA_TRY(cudaMemcpyAsync(c->d_hw, w_h, gb, cudaMemcpyHostToDevice, st));
+        s = ib_coupling_step(c, c->d_hx, c->d_hu, c->d_hv, c->d_hw, c->d_hfu, c->d_hfv, c->d_hfw, c->d_hUn,
+                             B_h ? c->d_hB : nullptr, stream);
+        if (s != IB_OK) return s;
+        IB_CUDA_TRY(cudaMemcpyAsync(fu_h, c->d_hfu, gb, cudaMemcpyDeviceToHost, st));
+        IB_CUDA_TRY(cudaMemcpyAsync(fv_h, c->d_hfv, gb, cudaMemcpyDeviceToHost, st));
+        IB_CUDA_TRY(cudaMemcpyAsync(fw_h, c->d_hfw, gb, cudaMemcpyDeviceToHost, st));
+        IB_CUDA_TRY(cudaMemcpyAsync(Un_h, c->d_hUn, nb, cudaMemcpyDeviceToHost, st));
+        if (B_h) IB_CUDA_TRY(cudaMemcpyAsync(B_h, c->d_hB, nb, cudaMemcpyDeviceToHost, st));
+        IB_CUDA_TRY(cudaStreamSynchronize(st));
+        return IB_OK;
+    }
+    // Pipelined: the force side of the step needs only x, so it runs while u,v,w are still crossing the
+    // bus on the side stream; f goes back to the host (side stream) while the velocity side runs.
+    //   st   : H2D x | zero f, bin, FE force, scatter, SPREAD | (wait uvw) INTERP, restrict | D2H Un, B
+    //   side : H2D u,v,w ............................... | (wait spread) D2H fu,fv,fw
+    cudaStream_t s2 = c->side;
+    double *Bd = B_h ? c->d_hB : c->d_B;
+    IB_CUDA_TRY(cudaEventRecord(c->ev_fork, st));             // orders the side stream after earlier work on st
+    IB_CUDA_TRY(cudaStreamWaitEvent(s2, c->ev_fork, 0));
     IB_CUDA_TRY(cudaMemcpyAsync(c->d_hx, x_h, nb, cudaMemcpyHostToDevice, st));
-    IB_CUDA_TRY(cudaMemcpyAsync(c->d_hu, u_h, gb, cudaMemcpyHostToDevice, st));
-    IB_CUDA_TRY(cudaMemcpyAsync(c->d_hv, v_h, gb, cudaMemcpyHostToDevice, st));
-    IB_CUDA_TRY(cudaMemcpyAsync(c->d_hw, w_h, gb, cudaMemcpyHostToDevice, st));
-    s = ib_coupling_step(c, c->d_hx, c->d_hu, c->d_hv, c->d_hw, c->d_hfu, c->d_hfv, c->d_hfw, c->d_hUn,
-                         B_h ? c->d_hB : nullptr, stream);
+    IB_CUDA_TRY(cudaMemcpyAsync(c->d_hu, u_h, gb, cudaMemcpyHostToDevice, s2));
+    IB_CUDA_TRY(cudaMemcpyAsync(c->d_hv, v_h, gb, cudaMemcpyHostToDevice, s2));
+    IB_CUDA_TRY(cudaMemcpyAsync(c->d_hw, w_h, gb, cudaMemcpyHostToDevice, s2));
+    IB_CUDA_TRY(cudaEventRecord(c->ev_join, s2));             // u,v,w are on the device
+    IB_CUDA_TRY(cudaMemsetAsync(c->d_hfu, 0, gb, st));
+    IB_CUDA_TRY(cudaMemsetAsync(c->d_hfv, 0, gb, st));
+    IB_CUDA_TRY(cudaMemsetAsync(c->d_hfw, 0, gb, st));
+    s = ibk_bin_reserve(c, c->n_points);
+    if (s == IB_OK) s = ibk_bin_points(c, 1, nullptr, nullptr, c->n_points, c->d_hx, nullptr, nullptr, 1, st);
+    if (s == IB_OK) s = ibk_fe_force(c, c->d_hx, Bd, c->d_Fhat, st);
+    if (s == IB_OK) s = ibk_bin_points(c, 1, nullptr, nullptr, c->n_points, c->d_hx, c->d_Fhat, c->d_Up, 2, st);
+    if (s == IB_OK) s = ibk_tiled_launch(c, c->n_points, 1, 0, nullptr, nullptr, nullptr, c->d_hfu, c->d_hfv, c->d_hfw,
+                                         nullptr, st);
     if (s != IB_OK) return s;
-    IB_CUDA_TRY(cudaMemcpyAsync(fu_h, c->d_hfu, gb, cudaMemcpyDeviceToHost, st));
-    IB_CUDA_TRY(cudaMemcpyAsync(fv_h, c->d_hfv, gb, cudaMemcpyDeviceToHost, st));
-    IB_CUDA_TRY(cudaMemcpyAsync(fw_h, c->d_hfw, gb, cudaMemcpyDeviceToHost, st));
+    IB_CUDA_TRY(cudaEventRecord(c->ev_aux, st));              // f is complete
+    IB_CUDA_TRY(cudaStreamWaitEvent(s2, c->ev_aux, 0));
+    IB_CUDA_TRY(cudaMemcpyAsync(fu_h, c->d_hfu, gb, cudaMemcpyDeviceToHost, s2));
+    IB_CUDA_TRY(cudaMemcpyAsync(fv_h, c->d_hfv, gb, cudaMemcpyDeviceToHost, s2));
+    IB_CUDA_TRY(cudaMemcpyAsync(fw_h, c->d_hfw, gb, cudaMemcpyDeviceToHost, s2));
+    IB_CUDA_TRY(cudaStreamWaitEvent(st, c->ev_join, 0));
+    s = ibk_tiled_launch(c, c->n_points, 0, 1, c->d_hu, c->d_hv, c->d_hw, nullptr, nullptr, nullptr, c->d_Up, st);
+    if (s == IB_OK) s = ibk_restrict(c, c->d_Up, c->d_hUn, st);
+    if (s != IB_OK) return s;
     IB_CUDA_TRY(cudaMemcpyAsync(Un_h, c->d_hUn, nb, cudaMemcpyDeviceToHost, st));
     if (B_h) IB_CUDA_TRY(cudaMemcpyAsync(B_h, c->d_hB, nb, cudaMemcpyDeviceToHost, st));
     IB_CUDA_TRY(cudaStreamSynchronize(st));
+    IB_CUDA_TRY(cudaStreamSynchronize(s2));
     return IB_OK;
 }
 

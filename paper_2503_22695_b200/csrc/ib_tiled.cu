@@ -486,6 +486,17 @@ ib_status ibk_tiled_spread_interp(ib_ctx *c, int mesh, const double *xp, const d
     ib_prof_end(c, IB_PHASE_SORT, st);
     if (rs != IB_OK) return rs;
 
+    return ibk_tiled_launch(c, P, spread, Up != nullptr, u, v, w, fu, fv, fw, Up, st);
+}
+
+// The tile kernel (and the direct path of the sparse tiles) over records that are already binned.
+// Spreading and interpolation may be launched separately over the same records (ib_coupling_step_host
+// overlaps them with the host copies): the work counter is reset on the stream before every launch.
+ib_status ibk_tiled_launch(ib_ctx *c, int64_t P, int do_spread, int do_interp,
+                           const double *u, const double *v, const double *w,
+                           double *fu, double *fv, double *fw, double *Up, cudaStream_t st)
+{
+    ib_status rs = IB_OK;
     ib_tiled_params pr;
     pr.sx = c->d_sx; pr.sG = c->d_sG; pr.sid = c->d_sid; pr.P = P;
     pr.fld[0] = u; pr.fld[1] = v; pr.fld[2] = w;
@@ -493,9 +504,10 @@ ib_status ibk_tiled_spread_interp(ib_ctx *c, int mesh, const double *xp, const d
     pr.Up = Up;
     pr.work = c->d_work; pr.counters = c->d_tile_count;
     pr.g = c->grid; pr.inv_h = c->inv_h; pr.ih3 = c->inv_h * c->inv_h * c->inv_h;
+    IB_CUDA_TRY(cudaMemsetAsync(c->d_tile_count + 1, 0, sizeof(int32_t), st));
     ib_prof_begin(c, IB_PHASE_SPREAD_INTERP, st);
-    if (spread && Up) rs = launch_tiled<1, 1>(c, pr, st);
-    else if (spread) rs = launch_tiled<1, 0>(c, pr, st);
+    if (do_spread && do_interp) rs = launch_tiled<1, 1>(c, pr, st);
+    else if (do_spread) rs = launch_tiled<1, 0>(c, pr, st);
     else rs = launch_tiled<0, 1>(c, pr, st);
     ib_prof_end(c, IB_PHASE_SPREAD_INTERP, st);
     if (rs != IB_OK) return rs;

@@ -198,19 +198,26 @@ def test_error_latch_inverted_element_and_nan(ib):
     ctx.close()
 
 
-def test_host_entry_point_matches_device_path(ib):
+@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("name", ["C1", "LV-small"])
+def test_host_entry_point_matches_device_path(ib, name, variant):
+    """ib_coupling_step_host (variant 1: spread and interpolation pipelined around the host copies on two
+    streams) gives what the device-pointer step gives."""
     import torch
-    wl = W.config1()
+    wl = CONFIGS[name]()
     ctx = ib.Context.from_workload(wl)
-    dev = _run_step(ib, wl, 0)
+    dev = _run_step(ib, wl, variant)
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
-    outs = [torch.empty(wl.n_cells, dtype=torch.float64).pin_memory() for _ in range(3)]
+    outs = [torch.full((wl.n_cells,), 9.0, dtype=torch.float64).pin_memory() for _ in range(3)]
     Un = torch.empty((3, wl.n_nodes), dtype=torch.float64).pin_memory()
     B = torch.empty((3, wl.n_nodes), dtype=torch.float64).pin_memory()
-    ctx.ib_set_variant(0)
-    ctx.ib_coupling_step_host(pin(wl.x), pin(wl.u), pin(wl.v), pin(wl.w), *outs, Un, B)
+    ctx.ib_set_variant(variant)
+    for _ in range(2):                                            # twice: buffers and events are reused
+        ctx.ib_coupling_step_host(pin(wl.x), pin(wl.u), pin(wl.v), pin(wl.w), *outs, Un, B)
+    ctx.check()
     assert np.array_equal(B.numpy(), dev["B"])
-    _close(outs[0].numpy(), dev["fu"], "host fu")
+    for k, o in zip(("fu", "fv", "fw"), outs):
+        _close(o.numpy(), dev[k], f"host {k}")
     _close(Un.numpy(), dev["Un"], "host Un")
     ctx.close()
 
