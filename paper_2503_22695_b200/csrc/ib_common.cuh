@@ -65,6 +65,8 @@ struct ib_ctx {
     cudaStream_t last_stream;
     cudaStream_t side;         // internal stream: work that needs only the positions overlaps the FE force
     cudaEvent_t ev_fork, ev_join, ev_aux;
+    cudaStream_t side2;        // the direct path of the sparse tiles runs beside the tile kernel
+    cudaEvent_t ev_sfork, ev_sjoin;
     int64_t launches;
     // optional per-phase event timing
     int profile;

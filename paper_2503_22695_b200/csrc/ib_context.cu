@@ -113,6 +113,9 @@ extern "C" ib_status ib_destroy(ib_ctx *c)
     if (c->ev_fork) cudaEventDestroy(c->ev_fork);
     if (c->ev_join) cudaEventDestroy(c->ev_join);
     if (c->ev_aux) cudaEventDestroy(c->ev_aux);
+    if (c->side2) cudaStreamDestroy(c->side2);
+    if (c->ev_sfork) cudaEventDestroy(c->ev_sfork);
+    if (c->ev_sjoin) cudaEventDestroy(c->ev_sjoin);
     if (c->prof) {
         double ms[IB_PHASE_COUNT];
         int64_t n[IB_PHASE_COUNT];
@@ -221,7 +224,10 @@ extern "C" ib_status ib_create(ib_ctx **out, const ib_grid_desc *g, const ib_mes
     if (s == IB_OK && (cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) != cudaSuccess ||
                        cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
                        cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess ||
-                       cudaEventCreateWithFlags(&c->ev_aux, cudaEventDisableTiming) != cudaSuccess))
+                       cudaEventCreateWithFlags(&c->ev_aux, cudaEventDisableTiming) != cudaSuccess ||
+                       cudaStreamCreateWithFlags(&c->side2, cudaStreamNonBlocking) != cudaSuccess ||
+                       cudaEventCreateWithFlags(&c->ev_sfork, cudaEventDisableTiming) != cudaSuccess ||
+                       cudaEventCreateWithFlags(&c->ev_sjoin, cudaEventDisableTiming) != cudaSuccess))
         s = IB_ERR_CUDA;
     if (s == IB_OK) s = reset_status(c, 0);
     if (s == IB_OK) s = ibk_sort_reserve(c, c->n_points);

@@ -463,10 +463,18 @@ static ib_status launch_tiled(ib_ctx *c, const ib_tiled_params &pr, cudaStream_t
         IB_CUDA_TRY(cudaGetDeviceProperties(&prop, c->device));
         sms = prop.multiProcessorCount;
     }
-    ibk_tiled_kernel<S, I><<<sms * NCTA, TB, smem, st>>>(pr);
-    // at most IB_SMALL_TILE-1 such records per tile, and never more than P
+    // the few points of sparsely filled tiles go one by one on a second stream, beside the tile kernel
     const int64_t nsmall_max = min((int64_t)pr.P, (c->n_cells / (TT * TT * TT)) * (int64_t)(IB_SMALL_TILE - 1));
-    ibk_small_tiles<S, I><<<ib_blocks(nsmall_max, 128), 128, 0, st>>>(pr, c->d_small_rec, c->d_tile_count);
+    const bool beside = !c->profile;
+    cudaStream_t s3 = beside ? c->side2 : st;
+    if (beside) {
+        IB_CUDA_TRY(cudaEventRecord(c->ev_sfork, st));
+        IB_CUDA_TRY(cudaStreamWaitEvent(s3, c->ev_sfork, 0));
+    }
+    ibk_small_tiles<S, I><<<ib_blocks(nsmall_max, 128), 128, 0, s3>>>(pr, c->d_small_rec, c->d_tile_count);
+    if (beside) IB_CUDA_TRY(cudaEventRecord(c->ev_sjoin, s3));
+    ibk_tiled_kernel<S, I><<<sms * NCTA, TB, smem, st>>>(pr);
+    if (beside) IB_CUDA_TRY(cudaStreamWaitEvent(st, c->ev_sjoin, 0));
     c->launches += 2;
     return IB_OK;
 }
