@@ -19,7 +19,7 @@
  *       nx, ny, nz must be multiples of 8 (tile edge of the binning key).
  *   node arrays X_ref, x, B, Un : component-major [3][n_nodes] doubles.
  *   point arrays xp, Gp, Up     : component-major [3][P] doubles.
- *   conn [n_elems][8] int32, local node a = ia + 2 ja + 4 ka (Q1 hexahedron);
+ *   conn [n_elems][8] int32, local node a = ia + 2 ja + 4 ka (Q1 hexahedron; [n_elems][4] for P1 tets);
  *   fibers [6][n_elems] doubles = (e_f, e_s) per element, unit and orthogonal;
  *   nsub [n_elems][3] int32 sub-point counts (n1,n2,n3) per element, each in 1..8.
  *
@@ -86,7 +86,11 @@ typedef struct {
     const int32_t *nsub;      /* [n_elems][3] or NULL = nodal rule of L241 (points=nodes)*/
     const ib_material *mats;  /* [n_mats]                                                */
     int32_t n_mats;
+    int32_t elem_type;        /* IB_ELEM_HEX8 (0): conn [n_elems][8]; IB_ELEM_TET4 (1), NEXT-3: P1
+                                 tetrahedra, conn [n_elems][4] with det [X1-X0,X2-X0,X3-X0] > 0, one
+                                 quadrature point, nodal coupling only (nsub must be NULL, L241)  */
 } ib_mesh_desc;
+enum { IB_ELEM_HEX8 = 0, IB_ELEM_TET4 = 1 };
 
 /* Create a context: validates, copies the mesh, builds the node->element adjacency (at most 8
  * incident elements per node), and precomputes on the device the sub-point weights W_s =

@@ -102,9 +102,11 @@ def fe_force(conn, X, x, fibers, mat_id, mats, want=("B", "energy", "minJ")):
     mat_id = _i32(mat_id)
     B = np.empty((3, nn))
     E, mj, bad = C.c_double(0), C.c_double(0), C.c_int64(-1)
-    rc = lib().oracle_fe_force(C.c_int64(nn), C.c_int64(ne), _p(conn, C.c_int32), _p(X), _p(x),
-                               _p(fibers), _p(mat_id, C.c_int32), make_materials(mats), _p(B),
-                               C.byref(E), C.byref(mj), C.byref(bad))
+    # conn [ne,8]: Q1 hexahedra; conn [ne,4]: P1 tetrahedra (NEXT-3)
+    fn = lib().oracle_fe_force_tet if conn.shape[1] == 4 else lib().oracle_fe_force
+    rc = fn(C.c_int64(nn), C.c_int64(ne), _p(conn, C.c_int32), _p(X), _p(x),
+            _p(fibers), _p(mat_id, C.c_int32), make_materials(mats), _p(B),
+            C.byref(E), C.byref(mj), C.byref(bad))
     return dict(B=B, energy=E.value, minJ=mj.value, rc=rc, first_bad=bad.value)
 
 

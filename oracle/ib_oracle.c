@@ -311,6 +311,78 @@ int oracle_fe_force(int64_t n_nodes, int64_t n_elems, const int32_t *conn, const
 }
 
 /* ------------------------------------------------------------------------------------------
+ * O2t FE nodal force on P1 (4-node, linear) tetrahedra -- NEXT-3: the paper's cardiac meshes are
+ * tetrahedral (L372, L447) and coupled by the nodal rule (L241, L466).  Same weak form (Eq.(20)
+ * L191; L249-251) with N_0 = 1-xi-eta-zeta, N_1 = xi, N_2 = eta, N_3 = zeta:
+ *   J0_{I d} = sum_a X_{a,I} dN_a/dxi_d = [X_1-X_0, X_2-X_0, X_3-X_0],  G_a = J0^-T grad_xi N_a,
+ *   one quadrature point (F is constant per element), weight w = det J0 / 6 (the element volume),
+ *   F = sum_a x_a (x) G_a,  B_{a,c} -= sum_J P_{cJ} G_{a,J} w,  energy = sum_e Psi(F_e) w_e.
+ * conn is [n_elems][4].  Returns 0, or 1 with *first_bad = element id if det J0 <= 0 or J <= 0.
+ * ---------------------------------------------------------------------------------------- */
+int oracle_fe_force_tet(int64_t n_nodes, int64_t n_elems, const int32_t *conn, const double *X,
+                        const double *x, const double *fibers, const int32_t *mat_id,
+                        const oracle_material *mats, double *B, double *energy, double *minJ,
+                        int64_t *first_bad)
+{
+    static const ld dNt[4][3] = {{-1, -1, -1}, {1, 0, 0}, {0, 1, 0}, {0, 0, 1}};
+    ld *Bl = (ld *)calloc((size_t)(3 * n_nodes), sizeof(ld));
+    ld E = 0.0L, mj = INFINITY;
+    int rc = 0;
+    for (int64_t e = 0; e < n_elems && !rc; ++e) {
+        ld Xe[4][3], xe[4][3], ef[3] = {1, 0, 0}, es[3] = {0, 1, 0};
+        for (int a = 0; a < 4; ++a)
+            for (int c = 0; c < 3; ++c) {
+                Xe[a][c] = X[c * n_nodes + conn[e * 4 + a]];
+                xe[a][c] = x[c * n_nodes + conn[e * 4 + a]];
+            }
+        if (fibers)
+            for (int c = 0; c < 3; ++c) { ef[c] = fibers[c * n_elems + e]; es[c] = fibers[(3 + c) * n_elems + e]; }
+        const oracle_material *m = &mats[mat_id ? mat_id[e] : 0];
+        ld J0[3][3], J0i[3][3];
+        for (int I = 0; I < 3; ++I)
+            for (int d = 0; d < 3; ++d) {
+                ld s = 0.0L;
+                for (int a = 0; a < 4; ++a) s += Xe[a][I] * dNt[a][d];
+                J0[I][d] = s;
+            }
+        ld dj = inv3(J0, J0i);
+        if (!(dj > 0.0L)) { rc = 1; if (first_bad) *first_bad = e; break; }
+        ld w = dj / 6.0L;
+        ld G[4][3];
+        for (int a = 0; a < 4; ++a)
+            for (int I = 0; I < 3; ++I) {
+                ld s = 0.0L;
+                for (int d = 0; d < 3; ++d) s += J0i[d][I] * dNt[a][d];
+                G[a][I] = s;
+            }
+        ld F[3][3], P[3][3], W;
+        for (int c = 0; c < 3; ++c)
+            for (int I = 0; I < 3; ++I) {
+                ld s = 0.0L;
+                for (int a = 0; a < 4; ++a) s += xe[a][c] * G[a][I];
+                F[c][I] = s;
+            }
+        if (pk1_l(m, F, ef, es, P, &W)) { rc = 1; if (first_bad) *first_bad = e; break; }
+        ld J = det3(F);
+        if (J < mj) mj = J;
+        E += W * w;
+        for (int a = 0; a < 4; ++a) {
+            int64_t n = conn[e * 4 + a];
+            for (int c = 0; c < 3; ++c) {
+                ld s = 0.0L;
+                for (int I = 0; I < 3; ++I) s += P[c][I] * G[a][I];
+                Bl[c * n_nodes + n] -= s * w;
+            }
+        }
+    }
+    for (int64_t i = 0; i < 3 * n_nodes; ++i) B[i] = (double)Bl[i];
+    if (energy) *energy = (double)E;
+    if (minJ) *minJ = (double)mj;
+    free(Bl);
+    return rc;
+}
+
+/* ------------------------------------------------------------------------------------------
  * O4  force points, lumped weights, prolongation; O7 restriction.
  * Reading A13 (Griffith-Luo style quadrature coupling; PAPER.md L233-237 projection, L241 nodal
  * weights w_q = int phi_q): with sub-point rule {xi_s, W_s} per element,

@@ -30,7 +30,9 @@ struct ib_ctx {
     int32_t *d_nsub;           // [n_elems][3]
     int64_t *d_pt_off;         // [n_elems+1]
     ib_material *d_mats;
-    int32_t *d_adj;            // [8][n_nodes] slot = e*8+a or -1 (ELL, ascending element id)
+    int elem_type, npe;        // IB_ELEM_HEX8 / IB_ELEM_TET4, nodes per element
+    int32_t *d_adj;            // hex: [8][n_nodes] slot = e*8+a or -1 (ELL, ascending element id)
+    int32_t *d_node_off, *d_node_slot;   // tets: CSR node -> slots e*4+a (ascending), valence is unbounded
     double *d_Wp;              // [P] sub-point weights W_s
     double *d_wa;              // [n_nodes] lumped weights
     double *d_geo;             // [10][8 n_elems] reference J0^-1 and det J0 per Gauss point

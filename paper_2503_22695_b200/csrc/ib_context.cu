@@ -102,7 +102,7 @@ extern "C" ib_status ib_destroy(ib_ctx *c)
     if (!c) return IB_ERR_INVALID_ARG;
     cudaSetDevice(c->device);
     void *ptrs[] = {c->d_conn, c->d_X, c->d_fib, c->d_mat_id, c->d_nsub, c->d_pt_off, c->d_mats, c->d_adj,
-                    c->d_Wp, c->d_wa, c->d_geo, c->d_Ce, c->d_Fhat, c->d_B, c->d_xp, c->d_Gp, c->d_Up, c->d_key[0],
+                    c->d_Wp, c->d_wa, c->d_geo, c->d_node_off, c->d_node_slot, c->d_Ce, c->d_Fhat, c->d_B, c->d_xp, c->d_Gp, c->d_Up, c->d_key[0],
                     c->d_key[1], c->d_val[0], c->d_val[1], c->d_hist, c->d_tile_cur, c->d_tile_start, c->d_work, c->d_small_rec,
                     c->d_row_off, c->d_sx, c->d_sG, c->d_sid,
                     c->d_tile_count, c->d_hx, c->d_hu, c->d_hv, c->d_hw, c->d_hfu, c->d_hfv, c->d_hfw,
@@ -139,6 +139,9 @@ extern "C" ib_status ib_create(ib_ctx **out, const ib_grid_desc *g, const ib_mes
     if (!g->periodic) return IB_ERR_UNSUPPORTED;
     if (m->n_nodes < 0 || m->n_elems < 0 || m->n_nodes > INT32_MAX || m->n_elems > INT32_MAX / 8) return IB_ERR_INVALID_ARG;
     if (m->n_elems > 0 && (!m->conn || !m->X_ref || !m->mats || m->n_mats <= 0)) return IB_ERR_INVALID_ARG;
+    if (m->elem_type != IB_ELEM_HEX8 && m->elem_type != IB_ELEM_TET4) return IB_ERR_INVALID_ARG;
+    if (m->elem_type == IB_ELEM_TET4 && m->nsub) return IB_ERR_UNSUPPORTED;      // tets: nodal coupling only
+    const int npe = m->elem_type == IB_ELEM_TET4 ? 4 : 8;
     if (m->n_nodes > 0 && !m->X_ref) return IB_ERR_INVALID_ARG;
     for (int i = 0; i < m->n_mats; ++i)
         if (m->mats[i].law < IB_LAW_NEOHOOKEAN || m->mats[i].law > IB_LAW_FR2) return IB_ERR_INVALID_ARG;
@@ -160,18 +163,27 @@ extern "C" ib_status ib_create(ib_ctx **out, const ib_grid_desc *g, const ib_mes
             if (m->nsub[3 * e] != m->nsub[0] || m->nsub[3 * e + 1] != m->nsub[1] || m->nsub[3 * e + 2] != m->nsub[2])
                 uniform = 0;
     }
-    std::vector<int32_t> adj((size_t)8 * (nn > 0 ? nn : 1), -1);
+    std::vector<int32_t> adj((size_t)8 * (nn > 0 ? nn : 1), -1), node_off((size_t)nn + 1, 0), node_slot;
     {
-        std::vector<unsigned char> cnt((size_t)(nn > 0 ? nn : 1), 0);
+        std::vector<int32_t> cnt((size_t)(nn > 0 ? nn : 1), 0);
         for (int64_t e = 0; e < ne; ++e) {
             if (m->mat_id && (m->mat_id[e] < 0 || m->mat_id[e] >= m->n_mats)) return IB_ERR_INVALID_ARG;
-            for (int a = 0; a < 8; ++a) {
-                int32_t n = m->conn[e * 8 + a];
+            for (int a = 0; a < npe; ++a) {
+                int32_t n = m->conn[e * npe + a];
                 if (n < 0 || n >= nn) return IB_ERR_INVALID_ARG;
-                if (cnt[n] >= 8) return IB_ERR_UNSUPPORTED;
-                adj[(size_t)cnt[n] * nn + n] = (int32_t)(e * 8 + a);      // ascending element id
+                if (npe == 8) {
+                    if (cnt[n] >= 8) return IB_ERR_UNSUPPORTED;
+                    adj[(size_t)cnt[n] * nn + n] = (int32_t)(e * 8 + a);      // ascending element id
+                }
                 cnt[n]++;
             }
+        }
+        if (npe == 4) {                                   // CSR: tets share nodes with any number of neighbours
+            for (int64_t n = 0; n < nn; ++n) node_off[n + 1] = node_off[n] + cnt[n];
+            node_slot.resize((size_t)ne * 4 + 1);
+            std::vector<int32_t> cur(node_off.begin(), node_off.end() - 1);
+            for (int64_t e = 0; e < ne; ++e)
+                for (int a = 0; a < 4; ++a) node_slot[cur[m->conn[e * 4 + a]]++] = (int32_t)(e * 4 + a);
         }
     }
 
@@ -191,11 +203,13 @@ extern "C" ib_status ib_create(ib_ctx **out, const ib_grid_desc *g, const ib_mes
     c->n_rows = roff[ne];
     if (uniform) { c->un[0] = m->nsub[0]; c->un[1] = m->nsub[1]; c->un[2] = m->nsub[2]; }
     c->n_mats = m->n_mats;
+    c->elem_type = m->elem_type;
+    c->npe = npe;
     c->variant = 1;
 
     ib_status s = IB_OK;
 #define TRY(x) do { if (s == IB_OK) s = (x); } while (0)
-    TRY(dev_upload(&c->d_conn, m->conn, (size_t)ne * 8));
+    TRY(dev_upload(&c->d_conn, m->conn, (size_t)ne * npe));
     TRY(dev_upload(&c->d_X, m->X_ref, (size_t)nn * 3));
     if (m->fibers) TRY(dev_upload(&c->d_fib, m->fibers, (size_t)ne * 6));
     if (m->mat_id) TRY(dev_upload(&c->d_mat_id, m->mat_id, (size_t)ne));
@@ -203,6 +217,10 @@ extern "C" ib_status ib_create(ib_ctx **out, const ib_grid_desc *g, const ib_mes
     TRY(dev_upload(&c->d_pt_off, off.data(), (size_t)ne + 1));
     TRY(dev_upload(&c->d_mats, m->mats, (size_t)(m->n_mats > 0 ? m->n_mats : 0)));
     TRY(dev_upload(&c->d_adj, adj.data(), (size_t)8 * (nn > 0 ? nn : 1)));
+    if (npe == 4) {
+        TRY(dev_upload(&c->d_node_off, node_off.data(), (size_t)nn + 1));
+        TRY(dev_upload(&c->d_node_slot, node_slot.data(), node_slot.size()));
+    }
     const size_t P = (size_t)c->n_points;
     TRY(dev_alloc((void **)&c->d_wa, (size_t)nn * sizeof(double)));
     TRY(dev_alloc((void **)&c->d_Ce, (size_t)ne * 24 * sizeof(double)));
@@ -233,7 +251,7 @@ extern "C" ib_status ib_create(ib_ctx **out, const ib_grid_desc *g, const ib_mes
     if (s == IB_OK) s = ibk_sort_reserve(c, c->n_points);
     if (s == IB_OK) s = ibk_bin_reserve(c, c->n_points);
     if (s == IB_OK) s = ibk_precompute_weights(c, 0);
-    if (s == IB_OK) s = ibk_fe_precompute(c, 0);
+    if (s == IB_OK && npe == 8) s = ibk_fe_precompute(c, 0);
     if (s == IB_OK && cudaDeviceSynchronize() != cudaSuccess) s = IB_ERR_CUDA;
 #undef TRY
     if (s == IB_OK) {

@@ -266,6 +266,90 @@ ibk_node_gather(int64_t n_nodes, int64_t ne8, const int32_t *__restrict__ adj,
     }
 }
 
+// ---- NEXT-3: P1 tetrahedra ---------------------------------------------------------------------------
+// One thread per element: F is constant, one quadrature point with weight det J0 / 6 (the volume).
+// J0 = [X1-X0, X2-X0, X3-X0]; G_a = J0^-T grad_xi N_a (grad_xi N = (-1,-1,-1), e1, e2, e3);
+// F = sum_a x_a (x) G_a = [x1-x0, x2-x0, x3-x0] J0^-1;  node a >= 1 gets -w P G_a, node 0 the negative sum.
+__global__ void __launch_bounds__(128)
+ibk_fe_tet(int64_t n_elems, int64_t n_nodes, const int32_t *__restrict__ conn, const double *__restrict__ X,
+           const double *__restrict__ x, const double *__restrict__ fib, const int32_t *__restrict__ mat_id,
+           const ib_material *__restrict__ mats, double *__restrict__ Ce, long long *status)
+{
+    int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= n_elems) return;
+    const int4 nd = __ldg(reinterpret_cast<const int4 *>(conn) + e);
+    const int n4[4] = {nd.x, nd.y, nd.z, nd.w};
+    double Xe[4][3], xe[4][3];
+    bool finite = true;
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            Xe[a][c] = __ldg(X + c * n_nodes + n4[a]);
+            xe[a][c] = __ldg(x + c * n_nodes + n4[a]);
+            finite = finite && isfinite(xe[a][c]);
+        }
+    double J0[3][3], Ds[3][3];                      // [I][d] = X_{d+1,I} - X_{0,I}
+#pragma unroll
+    for (int I = 0; I < 3; ++I)
+#pragma unroll
+        for (int d = 0; d < 3; ++d) { J0[I][d] = Xe[d + 1][I] - Xe[0][I]; Ds[I][d] = xe[d + 1][I] - xe[0][I]; }
+    const double dj = ib_det3(J0), rd = 1.0 / dj;
+    double Ji[3][3];                                 // J0^-1 (rows d, cols I)
+    Ji[0][0] = (J0[1][1] * J0[2][2] - J0[1][2] * J0[2][1]) * rd;
+    Ji[0][1] = (J0[0][2] * J0[2][1] - J0[0][1] * J0[2][2]) * rd;
+    Ji[0][2] = (J0[0][1] * J0[1][2] - J0[0][2] * J0[1][1]) * rd;
+    Ji[1][0] = (J0[1][2] * J0[2][0] - J0[1][0] * J0[2][2]) * rd;
+    Ji[1][1] = (J0[0][0] * J0[2][2] - J0[0][2] * J0[2][0]) * rd;
+    Ji[1][2] = (J0[0][2] * J0[1][0] - J0[0][0] * J0[1][2]) * rd;
+    Ji[2][0] = (J0[1][0] * J0[2][1] - J0[1][1] * J0[2][0]) * rd;
+    Ji[2][1] = (J0[0][1] * J0[2][0] - J0[0][0] * J0[2][1]) * rd;
+    Ji[2][2] = (J0[0][0] * J0[1][1] - J0[0][1] * J0[1][0]) * rd;
+    double F[3][3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+#pragma unroll
+        for (int I = 0; I < 3; ++I) F[c][I] = Ds[c][0] * Ji[0][I] + Ds[c][1] * Ji[1][I] + Ds[c][2] * Ji[2][I];
+    double ef[3] = {1.0, 0.0, 0.0}, es[3] = {0.0, 1.0, 0.0};
+    if (fib) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) { ef[c] = __ldg(fib + c * n_elems + e); es[c] = __ldg(fib + (3 + c) * n_elems + e); }
+    }
+    ib_material m = mats[mat_id ? __ldg(mat_id + e) : 0];
+    double P[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
+    double J = ib_pk1(m, F, ef, es, P);
+    if (!finite) ib_latch(status, IB_ERR_NONFINITE, e);
+    else if (!(dj > 0.0) || !(J > 0.0)) ib_latch(status, IB_ERR_INVERTED_ELEMENT, e);
+    const double w = dj * (1.0 / 6.0);
+    const int64_t ne4 = n_elems * 4;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        double s0 = 0.0;
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {               // node d+1: G = row d of J0^-1
+            double v = -w * (P[c][0] * Ji[d][0] + P[c][1] * Ji[d][1] + P[c][2] * Ji[d][2]);
+            Ce[c * ne4 + e * 4 + d + 1] = v;
+            s0 -= v;
+        }
+        Ce[c * ne4 + e * 4] = s0;
+    }
+}
+
+// Per node: sum its element contributions through the CSR adjacency in ascending slot order.
+__global__ void __launch_bounds__(256)
+ibk_node_gather_csr(int64_t n_nodes, int64_t ne4, const int32_t *__restrict__ off, const int32_t *__restrict__ slot,
+                    const double *__restrict__ Ce, double *__restrict__ B)
+{
+    int64_t n = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= n_nodes) return;
+    double s0 = 0.0, s1 = 0.0, s2 = 0.0;
+    for (int k = __ldg(off + n); k < __ldg(off + n + 1); ++k) {
+        int sl = __ldg(slot + k);
+        s0 += __ldg(Ce + sl); s1 += __ldg(Ce + ne4 + sl); s2 += __ldg(Ce + 2 * ne4 + sl);
+    }
+    B[n] = s0; B[n_nodes + n] = s1; B[2 * n_nodes + n] = s2;
+}
+
 ib_status ibk_fe_precompute(ib_ctx *c, cudaStream_t st)
 {
     if (c->n_elems == 0) return IB_OK;
@@ -278,6 +362,20 @@ ib_status ibk_fe_precompute(ib_ctx *c, cudaStream_t st)
 
 ib_status ibk_fe_force(ib_ctx *c, const double *x, double *B, double *Fhat, cudaStream_t st)
 {
+    if (c->elem_type == IB_ELEM_TET4) {                   // nodal coupling only: Fhat is never needed
+        if (c->n_elems > 0) {
+            ibk_fe_tet<<<ib_blocks(c->n_elems, 128), 128, 0, st>>>(c->n_elems, c->n_nodes, c->d_conn, c->d_X, x, c->d_fib,
+                                                                  c->d_mat_id, c->d_mats, c->d_Ce, c->d_status);
+            c->launches++;
+        }
+        if (c->n_nodes > 0) {
+            ibk_node_gather_csr<<<ib_blocks(c->n_nodes, 256), 256, 0, st>>>(c->n_nodes, c->n_elems * 4, c->d_node_off,
+                                                                            c->d_node_slot, c->d_Ce, B);
+            c->launches++;
+        }
+        IB_CUDA_TRY(cudaGetLastError());
+        return IB_OK;
+    }
     if (c->n_elems > 0) {
         int64_t nt = c->n_elems * 8;
         ibk_fe_gauss<<<ib_blocks(nt, 256), 256, 0, st>>>(c->n_elems, c->n_nodes, c->d_conn, c->d_geo, x,

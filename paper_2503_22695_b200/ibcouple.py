@@ -44,7 +44,7 @@ class Material(C.Structure):
 class MeshDesc(C.Structure):
     _fields_ = [("n_nodes", C.c_int64), ("n_elems", C.c_int64), ("conn", C.c_void_p), ("X_ref", C.c_void_p),
                 ("fibers", C.c_void_p), ("mat_id", C.c_void_p), ("nsub", C.c_void_p), ("mats", C.c_void_p),
-                ("n_mats", C.c_int32)]
+                ("n_mats", C.c_int32), ("elem_type", C.c_int32)]
 
 
 def lib():
@@ -132,7 +132,7 @@ class Context:
                       None if fibers is None else fibers.ctypes.data,
                       None if mat_id is None else mat_id.ctypes.data,
                       None if nsub is None else nsub.ctypes.data,
-                      C.cast(marr, C.c_void_p), len(mats))
+                      C.cast(marr, C.c_void_p), len(mats), 1 if (conn.ndim == 2 and conn.shape[1] == 4) else 0)
         _chk(L.ib_create(C.byref(self._h), C.byref(g), C.byref(md), self.device), "ib_create")
         self.nx, self.ny, self.nz, self.h = int(nx), int(ny), int(nz), float(h)
         self.n_cells = self.nx * self.ny * self.nz

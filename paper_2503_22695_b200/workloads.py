@@ -100,6 +100,20 @@ def block_connectivity(n1, n2, n3, periodic2=False):
     return conn, (N1, N2, N3)
 
 
+def tets_from_hexes(conn_hex, X):
+    """Kuhn split of every hexahedron into 6 tetrahedra along the diagonal (local nodes 0-7), each
+    ordered so that det [X1-X0, X2-X0, X3-X0] > 0.  Inputs only: the P1 meshes of NEXT-3 stand in for the
+    paper's tetrahedral valve meshes (L372, L447)."""
+    loc = np.array([[0, 1, 3, 7], [0, 3, 2, 7], [0, 2, 6, 7], [0, 6, 4, 7], [0, 4, 5, 7], [0, 5, 1, 7]])
+    tets = conn_hex[:, loc].reshape(-1, 4).astype(np.int64)
+    P = X[:, tets]                                   # [3, nt, 4]
+    d = np.einsum("in,in->n", np.cross((P[:, :, 1] - P[:, :, 0]).T, (P[:, :, 2] - P[:, :, 0]).T).T,
+                  P[:, :, 3] - P[:, :, 0])
+    neg = d < 0
+    tets[neg] = tets[neg][:, [0, 2, 1, 3]]
+    return tets.astype(np.int32)
+
+
 def _orient(conn, X):
     """Make every element right-handed (positive reference Jacobian at the centroid) by
     swapping the local xi_1 direction when the mean-edge triple product is negative."""

@@ -357,3 +357,54 @@ def test_fe_force_next2_laws_and_active_stress(ib, orc):
         _close(B, orc.fe_force(conn, X, x, fib, np.zeros(ne, np.int32), [m])["B"], f"law {k} B")
         c1.close()
     ctx.close()
+
+
+# ---- NEXT-3: P1 tetrahedra with the paper's nodal coupling (L241-257, L372, L447) -------------------
+def test_tet_mesh_force_and_nodal_coupling_step(ib, orc):
+    import torch
+    conn_hex, X, x, _ = distorted_block(6, 5, 4, size=(0.3, 0.25, 0.2), seed=31, ref_noise=0.1, cur_noise=0.05)
+    tets = W.tets_from_hexes(conn_hex, X)
+    ne, nn = tets.shape[0], X.shape[1]
+    assert np.bincount(tets.ravel()).max() > 8                   # valence beyond the hex ELL width
+    rng = np.random.default_rng(7)
+    ef = rng.normal(size=(3, ne))
+    ef /= np.linalg.norm(ef, axis=0)
+    es = np.cross(ef.T, rng.normal(size=(ne, 3))).T
+    es /= np.linalg.norm(es, axis=0)
+    fib = np.concatenate([ef, es])
+    mats = [W.material(W.LAW_NEOHOOKEAN, a=1e4, kappa=1e6), W.material(W.LAW_HO, Ta=20.0, **W.HO_LV),
+            W.material(W.LAW_FR2, a=2 * 1.21 * 7.99, b=7.99, af=24.23, bf=57.62, kappa=1e3)]
+    mid = (np.arange(ne) % 3).astype(np.int32)
+    n, h, org = (32, 32, 32), 1 / 32, (0.0, 0.0, 0.0)
+    g = orc.make_grid(*n, h, org)
+    uvw = np.random.default_rng(8).normal(size=(3, n[0] * n[1] * n[2]))
+    ref_B = orc.fe_force(tets, X, x, fib, mid, mats)["B"]
+    ref_f = orc.spread(g, x, ref_B)
+    ref_U = orc.interp(g, x, *uvw)
+    for variant in (0, 1):
+        ctx = ib.Context(*n, h, org, tets, X, fib, mid, None, mats)
+        ctx.ib_set_variant(variant)
+        B = torch.empty((3, nn), dtype=torch.float64, device="cuda")
+        ctx.ib_fe_force(_t(x), B)
+        ctx.check()
+        _close(B, ref_B, "tet B")
+        B2 = torch.empty_like(B)
+        ctx.ib_fe_force(_t(x), B2)
+        assert torch.equal(B, B2)                                 # CSR node gather: bit-reproducible
+        f = [torch.full((g.nx * g.ny * g.nz,), 2.0, dtype=torch.float64, device="cuda") for _ in range(3)]
+        Un = torch.empty((3, nn), dtype=torch.float64, device="cuda")
+        ctx.ib_coupling_step(_t(x), _t(uvw[0]), _t(uvw[1]), _t(uvw[2]), *f, Un, B)
+        ctx.check()
+        for c in range(3):
+            _close(f[c], ref_f[c], f"tet v{variant} f{c}")
+        _close(Un, ref_U, f"tet v{variant} Un")
+        # inverted tetrahedron is latched
+        xi = x.copy()
+        t0 = tets[5]
+        xi[:, t0[3]] = 2 * x[:, t0[0]] - x[:, t0[3]] + (x[:, t0[1]] - x[:, t0[0]])
+        ctx.ib_fe_force(_t(xi), B)
+        assert ctx.ib_check()[0] == 5
+        ctx.close()
+    # sub-point coupling is not defined for tetrahedra
+    with pytest.raises(ib.IbError):
+        ib.Context(*n, h, org, tets, X, fib, mid, np.ones((ne, 3), np.int32), mats)

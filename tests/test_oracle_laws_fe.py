@@ -387,3 +387,73 @@ def test_active_stress_closed_form(orc):
     assert np.allclose(S, T * np.outer(ef, ef), rtol=1e-11, atol=1e-11)
     # at the reference configuration the active tension is T_a along the fibre
     assert np.allclose(orc.pk1(active, np.eye(3), ex, ey)[0], Ta * np.outer(ex, ex), atol=1e-10)
+
+
+# ---- NEXT-3: P1 tetrahedra (the paper's valve meshes are tetrahedral, L372 / L447) ------------------
+def _tet_block(seed=3):
+    conn, X, x, fib = distorted_block(3, 3, 2, seed=seed, ref_noise=0.12, cur_noise=0.06)
+    tets = W.tets_from_hexes(conn, X)
+    rng = np.random.default_rng(seed)
+    ef = rng.normal(size=(3, tets.shape[0]))
+    ef /= np.linalg.norm(ef, axis=0)
+    es = np.cross(ef.T, rng.normal(size=(tets.shape[0], 3))).T
+    es /= np.linalg.norm(es, axis=0)
+    return tets, X, x, np.concatenate([ef, es])
+
+
+def test_tet_single_element_closed_form(orc):
+    """Unit right tetrahedron, x = F0 X: the force on node a is -V P(F0) grad N_a with V = 1/6 and
+    grad N = (-1,-1,-1), e_x, e_y, e_z."""
+    X = np.array([[0.0, 1, 0, 0], [0, 0, 1, 0], [0, 0, 0, 1]])
+    conn = np.array([[0, 1, 2, 3]], dtype=np.int32)
+    F0 = np.array([[1.1, 0.05, 0.0], [0.0, 0.95, 0.1], [0.02, 0.0, 1.03]])
+    x = F0 @ X
+    out = orc.fe_force(conn, X, x, None, None, [NH])
+    P, psi = orc.pk1(NH, F0)
+    G = np.array([[-1.0, -1, -1], [1, 0, 0], [0, 1, 0], [0, 0, 1]]).T          # [I, a]
+    assert np.allclose(out["B"], -(P @ G) / 6.0, rtol=1e-13, atol=1e-9)
+    assert abs(out["energy"] - psi / 6.0) < 1e-12 * psi and abs(out["minJ"] - np.linalg.det(F0)) < 1e-14
+    assert orc.fe_force(conn[:, [0, 2, 1, 3]], X, x, None, None, [NH])["rc"] == 1   # inverted reference
+
+
+@pytest.mark.parametrize("mat", [NH, HO], ids=["NH", "HO"])
+def test_tet_force_is_minus_energy_gradient_and_balances(orc, mat):
+    tets, X, x, fib = _tet_block()
+    out = orc.fe_force(tets, X, x, fib, None, [mat])
+    assert out["rc"] == 0 and out["minJ"] > 0.3
+    B = out["B"]
+    rng = np.random.default_rng(0)
+    eps = 1e-6 * 0.1
+    for _ in range(12):
+        c, n = rng.integers(0, 3), rng.integers(0, X.shape[1])
+        xp, xm = x.copy(), x.copy()
+        xp[c, n] += eps
+        xm[c, n] -= eps
+        fd = -(orc.fe_force(tets, X, xp, fib, None, [mat])["energy"]
+               - orc.fe_force(tets, X, xm, fib, None, [mat])["energy"]) / (2 * eps)
+        assert abs(fd - B[c, n]) < 2e-7 * np.max(np.abs(B)), (c, n)
+    assert np.max(np.abs(B.sum(axis=1))) < 1e-12 * np.max(np.abs(B))                       # no net force
+    assert np.max(np.abs(np.cross(x.T, B.T).sum(axis=0))) < 1e-11 * np.max(np.abs(B))      # no net torque
+
+
+def test_tet_rigid_motion_patch_and_volume(orc):
+    tets, X, x, fib = _tet_block(seed=4)
+    # total volume of the 6-tet split against the hex oracle's lumped weights of the same block
+    conn_hex, Xh, _, _ = distorted_block(3, 3, 2, seed=4, ref_noise=0.12, cur_noise=0.06)
+    vol_hex = orc.nodal_weights(conn_hex, Xh).sum()
+    P = X[:, tets]
+    vol_tet = np.einsum("in,in->n", np.cross((P[:, :, 1] - P[:, :, 0]).T, (P[:, :, 2] - P[:, :, 0]).T).T,
+                        P[:, :, 3] - P[:, :, 0]).sum() / 6.0
+    assert vol_tet > 0 and abs(vol_tet - vol_hex) < 0.02 * vol_hex   # planar-face split vs trilinear faces: close, not equal
+    # rigid motion: zero force
+    Q, t = rotation(5), np.array([[0.3], [-0.2], [0.1]])
+    B = orc.fe_force(tets, X, Q @ X + t, fib, None, [HO])["B"]
+    assert np.max(np.abs(B)) < 1e-12 * HO["kappa"] * 0.1 ** 2
+    # patch test: homogeneous deformation -> every node not on the boundary of the block is in balance
+    F0 = np.array([[1.05, 0.08, -0.02], [0.01, 0.97, 0.05], [-0.03, 0.02, 1.04]])
+    B = orc.fe_force(tets, X, F0 @ X, None, None, [NH])["B"]
+    N1, N2, N3 = 4, 4, 3
+    k, j, i = np.meshgrid(np.arange(N3), np.arange(N2), np.arange(N1), indexing="ij")
+    interior = ((i > 0) & (i < N1 - 1) & (j > 0) & (j < N2 - 1) & (k > 0) & (k < N3 - 1)).ravel()
+    assert interior.sum() == 4
+    assert np.max(np.abs(B[:, interior])) < 1e-11 * np.max(np.abs(B[:, ~interior]))
