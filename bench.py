@@ -233,7 +233,11 @@ def run_ours(args):
     fu, fv, fw = (torch.empty(wl.n_cells, dtype=torch.float64, device=dev) for _ in range(3))
     Un = torch.empty((3, wl.n_nodes), dtype=torch.float64, device=dev)
     flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)       # 512 MiB > 126 MB L2
-    stream = torch.cuda.current_stream()
+    # a stream of our own: the legacy default stream cannot be captured, and the library replays the
+    # step as one CUDA graph from the third call on (include/ibcouple.h, ib_set_graph)
+    stream = torch.cuda.Stream(device=dev)
+    torch.cuda.synchronize()
+    torch.cuda.set_stream(stream)
 
     def barrier():
         torch.cuda.synchronize()

@@ -175,6 +175,12 @@ int64_t ib_launch_count(const ib_ctx *ctx);
  * Default 1. Returns IB_ERR_INVALID_ARG for other values. */
 ib_status ib_set_variant(ib_ctx *ctx, int32_t variant);
 
+/* CUDA graph replay of ib_coupling_step (default on): when the call comes in a second time with the same
+ * pointers on the same non-default stream, the step's ~16 launches on three streams are captured once
+ * and replayed with one cudaGraphLaunch afterwards (the small configs are launch-latency bound). The
+ * legacy default stream cannot be captured: there the step is always enqueued kernel by kernel. */
+ib_status ib_set_graph(ib_ctx *ctx, int32_t on);
+
 /* Per-phase device timing with CUDA events recorded on the launching stream (used by bench.py for
  * the roofline of the dominant kernel). Phases of ib_coupling_step / ib_spread / ib_interp: */
 enum { IB_PHASE_FE_FORCE = 0, IB_PHASE_POINTS = 1, IB_PHASE_SORT = 2, IB_PHASE_SPREAD_INTERP = 3,

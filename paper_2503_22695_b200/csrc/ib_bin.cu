@@ -409,6 +409,7 @@ ib_status ibk_bin_points(ib_ctx *c, int mesh, const double *xp, const double *Gp
 ib_status ibk_bin_reserve(ib_ctx *c, int64_t P)
 {
     if (P <= c->bin_cap) return IB_OK;
+    c->gstate = 0;                                  // a captured step holds the old buffers
     if (c->d_sx) cudaFree(c->d_sx);
     if (c->d_sG) cudaFree(c->d_sG);
     if (c->d_sid) cudaFree(c->d_sid);

@@ -70,6 +70,11 @@ struct ib_ctx {
     cudaStream_t side2;        // the direct path of the sparse tiles runs beside the tile kernel
     cudaEvent_t ev_sfork, ev_sjoin;
     int64_t launches;
+    // CUDA graph of ib_coupling_step (replayed when the same pointers come in again on a capturable stream)
+    int graph_on, gstate;      // gstate: 0 none, 1 key seen once (ran eagerly), 2 captured
+    cudaGraphExec_t gexec;
+    const void *gkey[11];
+    int64_t g_launches;
     // optional per-phase event timing
     int profile;
     void *prof;                // std::vector<ib_prof_rec>* (ib_context.cu)

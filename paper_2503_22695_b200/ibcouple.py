@@ -20,7 +20,7 @@ STATUS = {0: "IB_OK", 1: "IB_ERR_INVALID_ARG", 2: "IB_ERR_UNSUPPORTED", 3: "IB_E
 
 EXPORTS = ["ib_create", "ib_destroy", "ib_num_points", "ib_num_nodes", "ib_num_elems", "ib_fe_force",
            "ib_points", "ib_restrict", "ib_bin_sort", "ib_spread", "ib_interp", "ib_coupling_step",
-           "ib_coupling_step_host", "ib_step_eq16", "ib_check", "ib_launch_count", "ib_set_variant", "ib_probe_dfma",
+           "ib_coupling_step_host", "ib_step_eq16", "ib_check", "ib_launch_count", "ib_set_variant", "ib_set_graph", "ib_probe_dfma",
            "ib_profile_enable", "ib_profile_read",
            "ib_status_string"]
 
@@ -72,6 +72,7 @@ def lib():
         L.ib_step_eq16.argtypes = [vp] * 5 + [C.c_double] + [vp] * 7
         L.ib_check.argtypes = [vp, C.POINTER(i64)]
         L.ib_set_variant.argtypes = [vp, i32]
+        L.ib_set_graph.argtypes = [vp, i32]
         L.ib_profile_enable.argtypes = [vp, i32]
         L.ib_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(i64)]
         L.ib_probe_dfma.argtypes = [i32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
@@ -159,6 +160,9 @@ class Context:
     # ---- the C ABI, same names ---------------------------------------------------------------
     def ib_set_variant(self, variant):
         _chk(lib().ib_set_variant(self._h, int(variant)), "ib_set_variant")
+
+    def ib_set_graph(self, on=True):
+        _chk(lib().ib_set_graph(self._h, int(bool(on))), "ib_set_graph")
 
     PHASES = ("fe_force", "points", "sort", "spread_interp", "restrict", "zero")
 
