@@ -290,10 +290,12 @@ __device__ __forceinline__ void ib_block_scan2(int &a, int &b, int *ws, int *wl,
     b = wl[wid] + ib - b;
 }
 
-__device__ __forceinline__ int ib_chunks(int c) { return c < IB_SMALL_TILE ? 0 : (c + IB_CHUNK - 1) / IB_CHUNK; }
+// chunk = points per work item: IB_CHUNK (the tile kernel's staging capacity) for large clouds, smaller
+// for small ones so that a few densely filled tiles still spread over many CTAs
+__device__ __forceinline__ int ib_chunks(int c, int chunk) { return c < IB_SMALL_TILE ? 0 : (c + chunk - 1) / chunk; }
 
 __global__ void __launch_bounds__(SCT)
-ibk_tile_partials(const int32_t *__restrict__ tile_cur, int n_tiles, int2 *__restrict__ partial)
+ibk_tile_partials(const int32_t *__restrict__ tile_cur, int n_tiles, int chunk, int2 *__restrict__ partial)
 {
     __shared__ int ws[33], wl[33];
     const int t0 = (blockIdx.x * SCT + threadIdx.x) * SCI;
@@ -301,7 +303,7 @@ ibk_tile_partials(const int32_t *__restrict__ tile_cur, int n_tiles, int2 *__res
     if (t0 < n_tiles) {
         int4 c = *reinterpret_cast<const int4 *>(tile_cur + t0);
         s = c.x + c.y + c.z + c.w;
-        l = ib_chunks(c.x) + ib_chunks(c.y) + ib_chunks(c.z) + ib_chunks(c.w);
+        l = ib_chunks(c.x, chunk) + ib_chunks(c.y, chunk) + ib_chunks(c.z, chunk) + ib_chunks(c.w, chunk);
     }
     int ts, tl;
     ib_block_scan2(s, l, ws, wl, ts, tl);
@@ -310,7 +312,7 @@ ibk_tile_partials(const int32_t *__restrict__ tile_cur, int n_tiles, int2 *__res
 
 // start offsets and cursors of the tiles, and the work list: one entry per chunk of <= IB_CHUNK records
 __global__ void __launch_bounds__(SCT)
-ibk_tile_scan(int32_t *__restrict__ tile_cur, int n_tiles, const int2 *__restrict__ partial,
+ibk_tile_scan(int32_t *__restrict__ tile_cur, int n_tiles, int chunk, const int2 *__restrict__ partial,
               int32_t *__restrict__ tile_start, int4 *__restrict__ work, int32_t *__restrict__ small_rec,
               int32_t *__restrict__ counters)
 {
@@ -326,7 +328,7 @@ ibk_tile_scan(int32_t *__restrict__ tile_cur, int n_tiles, const int2 *__restric
     const int t0 = (blockIdx.x * SCT + threadIdx.x) * SCI;
     int4 c = make_int4(0, 0, 0, 0);
     if (t0 < n_tiles) c = *reinterpret_cast<const int4 *>(tile_cur + t0);
-    int s = c.x + c.y + c.z + c.w, l = ib_chunks(c.x) + ib_chunks(c.y) + ib_chunks(c.z) + ib_chunks(c.w);
+    int s = c.x + c.y + c.z + c.w, l = ib_chunks(c.x, chunk) + ib_chunks(c.y, chunk) + ib_chunks(c.z, chunk) + ib_chunks(c.w, chunk);
     int ts, tl;
     ib_block_scan2(s, l, ws, wl, ts, tl);          // includes the barrier that publishes base_s/base_l
     s += base_s; l += base_l;
@@ -337,7 +339,7 @@ ibk_tile_scan(int32_t *__restrict__ tile_cur, int n_tiles, const int2 *__restric
         const int cnt[4] = {c.x, c.y, c.z, c.w}, beg[4] = {st.x, st.y, st.z, st.w};
 #pragma unroll
         for (int k = 0; k < 4; ++k)
-            for (int o = 0; o < cnt[k] && cnt[k] >= IB_SMALL_TILE; o += IB_CHUNK) work[l++] = make_int4(t0 + k, beg[k] + o, min(IB_CHUNK, cnt[k] - o), 0);
+            for (int o = 0; o < cnt[k] && cnt[k] >= IB_SMALL_TILE; o += chunk) work[l++] = make_int4(t0 + k, beg[k] + o, min(chunk, cnt[k] - o), 0);
     }
     {   // records of sparsely filled tiles: a compact list (order across CTAs is whatever the atomic gives)
         int m = 0, zero = 0, tm, tz;
@@ -392,8 +394,11 @@ ib_status ibk_bin_points(ib_ctx *c, int mesh, const double *xp, const double *Gp
         else ibk_bin_cloud<0><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
         const int nsb = (n_tiles + SCT * SCI - 1) / (SCT * SCI);
         int2 *partial = reinterpret_cast<int2 *>(c->d_tile_count + 16);
-        ibk_tile_partials<<<nsb, SCT, 0, st>>>(c->d_tile_cur, n_tiles, partial);
-        ibk_tile_scan<<<nsb, SCT, 0, st>>>(c->d_tile_cur, n_tiles, partial, c->d_tile_start, c->d_work, c->d_small_rec, c->d_tile_count);
+        // ~4 work items per resident CTA of the tile kernel when the cloud is small
+        int chunk = (int)((P / 1200 + 63) / 64 * 64);
+        chunk = chunk < 192 ? 192 : (chunk > IB_CHUNK ? IB_CHUNK : chunk);
+        ibk_tile_partials<<<nsb, SCT, 0, st>>>(c->d_tile_cur, n_tiles, chunk, partial);
+        ibk_tile_scan<<<nsb, SCT, 0, st>>>(c->d_tile_cur, n_tiles, chunk, partial, c->d_tile_start, c->d_work, c->d_small_rec, c->d_tile_count);
         c->launches += 3;
     }
     if (phases & 2) {
@@ -422,7 +427,7 @@ ib_status ibk_bin_reserve(ib_ctx *c, int64_t P)
     if (cudaMalloc(&c->d_sx, (size_t)cap * 3 * sizeof(double)) != cudaSuccess) return IB_ERR_ALLOC;
     if (cudaMalloc(&c->d_sG, (size_t)cap * 3 * sizeof(double)) != cudaSuccess) return IB_ERR_ALLOC;
     if (cudaMalloc(&c->d_sid, (size_t)cap * sizeof(int32_t)) != cudaSuccess) return IB_ERR_ALLOC;
-    c->work_cap = c->n_cells / (BT * BT * BT) + cap / IB_CHUNK + 8;
+    c->work_cap = c->n_cells / (BT * BT * BT) + cap / 192 + 8;
     if (cudaMalloc(&c->d_work, (size_t)c->work_cap * sizeof(int4)) != cudaSuccess) return IB_ERR_ALLOC;
     if (cudaMalloc(&c->d_small_rec, (size_t)cap * sizeof(int32_t)) != cudaSuccess) return IB_ERR_ALLOC;
     c->bin_cap = cap;
