@@ -1,8 +1,9 @@
 // ib_bin.cu -- tile-level counting sort of the Lagrangian force points (SURVEY.md §8(a) a4+a5 fused).
 // Not in the paper (north_star: "points binned and sorted by Eulerian cell").
 //
-// Points are grouped by 4x4x4-cell tile with a counting sort: count pass -> single-CTA scan ->
-// scatter pass that writes the point records (x_s, G_s, id) contiguously per tile.  The order of
+// Points are grouped by 4x4x4-cell tile with a counting sort: count pass -> two-kernel scan (which also
+// emits the tile kernel's work list and the list of points of sparsely filled tiles) -> scatter pass
+// that writes the point records (x_s, G_s, id) contiguously per tile.  The order of
 // points inside a tile is whatever the atomics give; the tile kernel (ib_tiled.cu) sorts them by
 // half-cell in shared memory.  Two point sources:
 //   cloud : xp/Gp arrays given by the caller (ib_spread / ib_interp, nodal rule of L241)

@@ -1,22 +1,25 @@
 // ib_tiled.cu -- variant 1 of spread (Eq.(24)-(26)) and interpolation (Eq.(27)-(29)):
-// points grouped by 4x4x4-cell tile (ib_bin.cu), one CTA per tile with an 8x8x8 shared-memory halo
-// of u,v,w and of the force accumulators, register-resident 4x4x4 stencil slabs.
+// points grouped by 4x4x4-cell tile (ib_bin.cu); persistent CTAs pull chunks of one tile from a work
+// list, keep an 8x8x8 halo of u,v,w in shared memory and hold 4x4x4 stencil windows in registers.
 //
-// Per tile the CTA stages the scaled coordinates of its points in shared memory and sorts them by
-// half-cell ("octant", 8^3 per tile) with a shared-memory counting sort.  Why half-cells: component
-// c lives on its own staggered lattice (MAC grid, L205).  In the direction d == c the 4-point
-// support of a point is fixed by its cell; in the other two it is fixed by the cell of the lattice
-// shifted by h/2.  With the points ordered by half-cell every cell of every shifted lattice is a
-// union of <= 4 contiguous runs, so all points of one work item (shifted cell, component) share ONE
+// Per chunk the CTA stages the tile-relative scaled coordinates of the points in shared memory and
+// sorts them by half-cell ("octant", 8^3 per tile) with a shared-memory counting sort.  Why half-cells:
+// component c lives on its own staggered lattice (MAC grid, L205).  In the direction d == c the
+// 4-point support of a point is fixed by its cell; in the other two it is fixed by the cell of the
+// lattice shifted by h/2.  With the points ordered by half-cell every cell of every shifted lattice is
+// a union of <= 4 contiguous runs, so all points of one work item (shifted cell, component) share ONE
 // 4x4x4 window.
 //
-// Work item = (shifted cell, component).  A group of 4 lanes owns it: lane q keeps the z-plane q of
-// the window -- 16 velocity values and 16 force accumulators -- in registers and loops over the
-// item's points.  Per point and lane: 21 DFMA for interpolation, 21 for spreading; the delta
-// weights of 4 points are computed by the 4 lanes (one point each, one sqrt per 1-D weight set)
-// and exchanged through a 464-byte shared-memory staging record.  Force is reduced in registers
-// over all points of the item, then in shared memory over the items of the tile (fp64 CAS adds:
-// no native shared fp64 add), then ONE global RED.ADD.F64 per touched face of the halo.
+// Work item = (shifted cell, component); items are ordered by point count and pulled by the warps, 8
+// at a time.  A group of 4 lanes owns an item: lane q keeps the x-column q of the window -- 16
+// velocity values and 16 force accumulators -- in registers and loops over the item's points in quads.
+// Per point and lane: 21 DFMA for interpolation, 21 for spreading.  The delta weights of a quad are
+// computed by the 4 lanes (one point each, one branch-free sqrt per 1-D weight set) into a
+// double-buffered shared-memory record while the group consumes the previous quad; index, force and
+// id of the quad after that are already in flight.  Force is reduced in registers over all points of
+// the item and flushed with RED.ADD.F64 straight to the grid: the 4 lanes of a group hit 4 consecutive
+// faces (Blackwell has no native shared-memory fp64 add; the CAS loop measured 34 wavefronts each).
+// Tiles with fewer than IB_SMALL_TILE points skip all of this (ibk_small_tiles, ib_point.cuh).
 #include "ib_point.cuh"
 
 #define TT 4                    // tile edge in cells
