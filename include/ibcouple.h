@@ -175,6 +175,21 @@ int64_t ib_launch_count(const ib_ctx *ctx);
  * Default 1. Returns IB_ERR_INVALID_ARG for other values. */
 ib_status ib_set_variant(ib_ctx *ctx, int32_t variant);
 
+/* NEXT-4: solid boundary loads (Table 3 row "Solid boundary" L398). Once set they are ADDED to
+ * the nodal force by ib_fe_force and by every step (before the force is spread); B is then no longer
+ * bit-reproducible (the surface loads are accumulated with atomics).
+ *  tethers  (L263 "fixed left face ... penalty parameter kappa = 10^6", L425): reading A24, a penalty spring
+ *           to the reference position, B_a += kappa (X_a - x_a) for the listed nodes (host ids, distinct).
+ *  surface  boundary faces, host array [n_faces][nodes_per_face], 4 = bilinear quads in cyclic order,
+ *           3 = linear triangles, normal pointing out of the solid.
+ *  loads    qt0 = q(t) t0 (host, 3 doubles or NULL): dead traction per unit REFERENCE area (L263),
+ *           B_a += q t0 int N_a dA;   p: follower pressure on the CURRENT faces (L303, L315),
+ *           B_a -= p int N_a n da.  Call again every step with the current q(t), p_endo(t).
+ * n = 0 / n_faces = 0 removes the load. */
+ib_status ib_set_tethers(ib_ctx *ctx, int64_t n, const int32_t *node_ids, double kappa);
+ib_status ib_set_surface(ib_ctx *ctx, int64_t n_faces, int32_t nodes_per_face, const int32_t *faces);
+ib_status ib_set_loads(ib_ctx *ctx, const double *qt0, double p);
+
 /* CUDA graph replay of ib_coupling_step (default on): when the call comes in a second time with the same
  * pointers on the same non-default stream, the step's ~16 launches on three streams are captured once
  * and replayed with one cudaGraphLaunch afterwards (the small configs are launch-latency bound). The

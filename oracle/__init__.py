@@ -110,6 +110,26 @@ def fe_force(conn, X, x, fibers, mat_id, mats, want=("B", "energy", "minJ")):
     return dict(B=B, energy=E.value, minJ=mj.value, rc=rc, first_bad=bad.value)
 
 
+def tethers(ids, X, x, kappa, B):
+    """B += kappa (X - x) on the nodes `ids`; returns (B, energy)."""
+    ids, X, x = _i32(ids), _f64(X), _f64(x)
+    B = _f64(B).copy()
+    E = C.c_double(0)
+    lib().oracle_tethers(C.c_int64(X.shape[1]), C.c_int64(ids.size), _p(ids, C.c_int32), _p(X), _p(x),
+                         C.c_double(kappa), _p(B), C.byref(E))
+    return B, E.value
+
+
+def surface_loads(faces, X, x, qt0, p, B):
+    """B += q t0 int N dA (reference faces) - p int N n da (current faces); faces [nf,3] or [nf,4]."""
+    faces, X, x = _i32(faces), _f64(X), _f64(x)
+    B = _f64(B).copy()
+    qt0 = None if qt0 is None else _f64(qt0)
+    lib().oracle_surface_loads(C.c_int64(X.shape[1]), C.c_int64(faces.shape[0]), C.c_int32(faces.shape[1]),
+                               _p(faces, C.c_int32), _p(X), _p(x), _p(qt0), C.c_double(p), _p(B))
+    return B
+
+
 def num_points(n_nodes, n_elems, nsub):
     nsub = _i32(nsub)
     return int(lib().oracle_num_points(C.c_int64(n_nodes), C.c_int64(n_elems), _p(nsub, C.c_int32)))

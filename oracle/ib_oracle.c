@@ -383,6 +383,78 @@ int oracle_fe_force_tet(int64_t n_nodes, int64_t n_elems, const int32_t *conn, c
 }
 
 /* ------------------------------------------------------------------------------------------
+ * O9  solid boundary loads (NEXT-4; Table 3 row "Solid boundary" L398).  All ADD to B [3][n_nodes].
+ *  tethers (L263 "fixed left face ... penalty parameter kappa = 10^6", L425): the paper gives only the
+ *    parameter; reading A24: a penalty spring to the reference position, B_a += kappa (X_a - x_a),
+ *    energy kappa/2 sum |x_a - X_a|^2.
+ *  traction (L263): dead load q t0 per unit REFERENCE area on boundary faces, B_a += q t0 int N_a dA.
+ *  pressure (L303, L315 "uniform pressure applied to the endocardial surface"): follower load -p n per
+ *    unit CURRENT area, n the outward normal of the face as oriented, B_a -= p int N_a n da.
+ * Faces: npf = 4 bilinear quads (nodes in cyclic order; 2x2 Gauss, exact for these integrands) or
+ * npf = 3 linear triangles (one point).  n da = d x/d xi x d x/d eta d xi d eta.
+ * ---------------------------------------------------------------------------------------- */
+void oracle_tethers(int64_t n_nodes, int64_t n_t, const int32_t *ids, const double *X, const double *x,
+                    double kappa, double *B, double *energy)
+{
+    ld E = 0.0L;
+    for (int64_t k = 0; k < n_t; ++k)
+        for (int c = 0; c < 3; ++c) {
+            ld d = (ld)x[c * n_nodes + ids[k]] - (ld)X[c * n_nodes + ids[k]];
+            B[c * n_nodes + ids[k]] = (double)((ld)B[c * n_nodes + ids[k]] - (ld)kappa * d);
+            E += 0.5L * (ld)kappa * d * d;
+        }
+    if (energy) *energy = (double)E;
+}
+
+void oracle_surface_loads(int64_t n_nodes, int64_t n_faces, int32_t npf, const int32_t *faces,
+                          const double *X, const double *x, const double *qt0, double p, double *B)
+{
+    const ld g = 0.57735026918962576450914878050196L;
+    for (int64_t f = 0; f < n_faces; ++f) {
+        ld add[4][3] = {{0}};
+        int nq = npf == 4 ? 4 : 1;
+        for (int q = 0; q < nq; ++q) {
+            ld N[4], dNx[4], dNe[4], wq;
+            if (npf == 4) {                          /* cyclic node order (-1,-1),(1,-1),(1,1),(-1,1) */
+                ld xi = (q & 1) ? g : -g, et = (q & 2) ? g : -g;
+                const ld sx[4] = {-1, 1, 1, -1}, se[4] = {-1, -1, 1, 1};
+                for (int a = 0; a < 4; ++a) {
+                    N[a] = 0.25L * (1 + sx[a] * xi) * (1 + se[a] * et);
+                    dNx[a] = 0.25L * sx[a] * (1 + se[a] * et);
+                    dNe[a] = 0.25L * (1 + sx[a] * xi) * se[a];
+                }
+                wq = 1.0L;
+            } else {                                 /* N = (1-xi-eta, xi, eta) at the centroid, weight 1/2 */
+                N[0] = N[1] = N[2] = 1.0L / 3.0L; N[3] = 0;
+                dNx[0] = -1; dNx[1] = 1; dNx[2] = 0; dNx[3] = 0;
+                dNe[0] = -1; dNe[1] = 0; dNe[2] = 1; dNe[3] = 0;
+                wq = 0.5L;
+            }
+            ld tX[2][3] = {{0}}, tx[2][3] = {{0}};
+            for (int a = 0; a < npf; ++a)
+                for (int c = 0; c < 3; ++c) {
+                    int64_t n = faces[f * npf + a];
+                    tX[0][c] += dNx[a] * X[c * n_nodes + n]; tX[1][c] += dNe[a] * X[c * n_nodes + n];
+                    tx[0][c] += dNx[a] * x[c * n_nodes + n]; tx[1][c] += dNe[a] * x[c * n_nodes + n];
+                }
+            ld NX[3] = {tX[0][1] * tX[1][2] - tX[0][2] * tX[1][1], tX[0][2] * tX[1][0] - tX[0][0] * tX[1][2],
+                        tX[0][0] * tX[1][1] - tX[0][1] * tX[1][0]};
+            ld nx[3] = {tx[0][1] * tx[1][2] - tx[0][2] * tx[1][1], tx[0][2] * tx[1][0] - tx[0][0] * tx[1][2],
+                        tx[0][0] * tx[1][1] - tx[0][1] * tx[1][0]};
+            ld dA = sqrtl(NX[0] * NX[0] + NX[1] * NX[1] + NX[2] * NX[2]);
+            for (int a = 0; a < npf; ++a)
+                for (int c = 0; c < 3; ++c)
+                    add[a][c] += wq * N[a] * ((qt0 ? (ld)qt0[c] : 0.0L) * dA - (ld)p * nx[c]);
+        }
+        for (int a = 0; a < npf; ++a)
+            for (int c = 0; c < 3; ++c) {
+                int64_t n = faces[f * npf + a];
+                B[c * n_nodes + n] = (double)((ld)B[c * n_nodes + n] + add[a][c]);
+            }
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
  * O4  force points, lumped weights, prolongation; O7 restriction.
  * Reading A13 (Griffith-Luo style quadrature coupling; PAPER.md L233-237 projection, L241 nodal
  * weights w_q = int phi_q): with sub-point rule {xi_s, W_s} per element,

@@ -70,6 +70,11 @@ struct ib_ctx {
     cudaStream_t side2;        // the direct path of the sparse tiles runs beside the tile kernel
     cudaEvent_t ev_sfork, ev_sjoin;
     int64_t launches;
+    // NEXT-4 boundary loads (ib_set_tethers / ib_set_surface / ib_set_loads)
+    int32_t *d_teth_ids, *d_faces;
+    int64_t n_teth, n_faces;
+    int npf;
+    double kappa_t, qt0[3], p_load;
     // CUDA graph of ib_coupling_step (replayed when the same pointers come in again on a capturable stream)
     int graph_on, gstate;      // gstate: 0 none, 1 key seen once (ran eagerly), 2 captured
     cudaGraphExec_t gexec;

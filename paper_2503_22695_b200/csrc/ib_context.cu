@@ -103,7 +103,7 @@ extern "C" ib_status ib_destroy(ib_ctx *c)
     if (!c) return IB_ERR_INVALID_ARG;
     cudaSetDevice(c->device);
     void *ptrs[] = {c->d_conn, c->d_X, c->d_fib, c->d_mat_id, c->d_nsub, c->d_pt_off, c->d_mats, c->d_adj,
-                    c->d_Wp, c->d_wa, c->d_geo, c->d_node_off, c->d_node_slot, c->d_Ce, c->d_Fhat, c->d_B, c->d_xp, c->d_Gp, c->d_Up, c->d_key[0],
+                    c->d_Wp, c->d_wa, c->d_geo, c->d_node_off, c->d_node_slot, c->d_teth_ids, c->d_faces, c->d_Ce, c->d_Fhat, c->d_B, c->d_xp, c->d_Gp, c->d_Up, c->d_key[0],
                     c->d_key[1], c->d_val[0], c->d_val[1], c->d_hist, c->d_tile_cur, c->d_tile_start, c->d_work, c->d_small_rec,
                     c->d_row_off, c->d_sx, c->d_sG, c->d_sid,
                     c->d_tile_count, c->d_hx, c->d_hu, c->d_hv, c->d_hw, c->d_hfu, c->d_hfv, c->d_hfw,
@@ -277,6 +277,56 @@ extern "C" ib_status ib_set_variant(ib_ctx *c, int32_t variant)
     if (!c || (variant != 0 && variant != 1)) return IB_ERR_INVALID_ARG;
     c->variant = variant;
     c->gstate = 0;
+    return IB_OK;
+}
+
+static ib_status replace_ids(int32_t **dst, const int32_t *src, size_t n)
+{
+    if (*dst) { cudaFree(*dst); *dst = nullptr; }
+    return n ? dev_upload(dst, src, n) : IB_OK;
+}
+
+extern "C" ib_status ib_set_tethers(ib_ctx *c, int64_t n, const int32_t *ids, double kappa)
+{
+    if (!c || n < 0 || (n > 0 && !ids) || !std::isfinite(kappa)) return IB_ERR_INVALID_ARG;
+    for (int64_t k = 0; k < n; ++k)
+        if (ids[k] < 0 || ids[k] >= c->n_nodes) return IB_ERR_INVALID_ARG;
+    if (cudaSetDevice(c->device) != cudaSuccess) return IB_ERR_CUDA;
+    cudaDeviceSynchronize();
+    c->gstate = 0;
+    c->n_teth = 0;
+    ib_status s = replace_ids(&c->d_teth_ids, ids, (size_t)n);
+    if (s != IB_OK) return s;
+    c->n_teth = n;
+    c->kappa_t = kappa;
+    return IB_OK;
+}
+
+extern "C" ib_status ib_set_surface(ib_ctx *c, int64_t n_faces, int32_t npf, const int32_t *faces)
+{
+    if (!c || n_faces < 0 || (n_faces > 0 && (!faces || (npf != 3 && npf != 4)))) return IB_ERR_INVALID_ARG;
+    for (int64_t k = 0; k < n_faces * npf; ++k)
+        if (faces[k] < 0 || faces[k] >= c->n_nodes) return IB_ERR_INVALID_ARG;
+    if (cudaSetDevice(c->device) != cudaSuccess) return IB_ERR_CUDA;
+    cudaDeviceSynchronize();
+    c->gstate = 0;
+    c->n_faces = 0;
+    ib_status s = replace_ids(&c->d_faces, faces, (size_t)(n_faces * npf));
+    if (s != IB_OK) return s;
+    c->n_faces = n_faces;
+    c->npf = npf;
+    return IB_OK;
+}
+
+extern "C" ib_status ib_set_loads(ib_ctx *c, const double *qt0, double p)
+{
+    if (!c || !std::isfinite(p)) return IB_ERR_INVALID_ARG;
+    for (int k = 0; k < 3; ++k) {
+        if (qt0 && !std::isfinite(qt0[k])) return IB_ERR_INVALID_ARG;
+        c->qt0[k] = qt0 ? qt0[k] : 0.0;
+    }
+    c->p_load = p;
+    c->gstate = 0;                                   // the load values are kernel arguments of a captured step
     return IB_OK;
 }
 

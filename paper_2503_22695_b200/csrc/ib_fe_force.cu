@@ -350,6 +350,105 @@ ibk_node_gather_csr(int64_t n_nodes, int64_t ne4, const int32_t *__restrict__ of
     B[n] = s0; B[n_nodes + n] = s1; B[2 * n_nodes + n] = s2;
 }
 
+// ---- NEXT-4: solid boundary loads, added to B ----------------------------------------------------------
+__global__ void __launch_bounds__(256)
+ibk_tethers(int64_t n, int64_t n_nodes, const int32_t *__restrict__ ids, const double *__restrict__ X,
+            const double *__restrict__ x, double kappa, double *__restrict__ B)
+{
+    int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    const int64_t a = ids[k];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) B[c * n_nodes + a] += kappa * (X[c * n_nodes + a] - x[c * n_nodes + a]);
+}
+
+// one thread per face: dead traction q t0 dA on the reference face, follower pressure -p n da on the
+// current face; bilinear quads with 2x2 Gauss points, linear triangles with the centroid rule
+__global__ void __launch_bounds__(128)
+ibk_surface_loads(int64_t n_faces, int npf, int64_t n_nodes, const int32_t *__restrict__ faces,
+                  const double *__restrict__ X, const double *__restrict__ x, double q0, double q1, double q2,
+                  double p, double *__restrict__ B)
+{
+    int64_t f = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (f >= n_faces) return;
+    int nd[4] = {0, 0, 0, 0};
+    double Xf[4][3], xf[4][3];
+    for (int a = 0; a < npf; ++a) {
+        nd[a] = faces[f * npf + a];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) { Xf[a][c] = X[c * n_nodes + nd[a]]; xf[a][c] = x[c * n_nodes + nd[a]]; }
+    }
+    const double qv[3] = {q0, q1, q2};
+    double add[4][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
+    const double g = 0.57735026918962576451;
+    const int nq = npf == 4 ? 4 : 1;
+    for (int q = 0; q < nq; ++q) {
+        double N[4], d1[4], d2[4], wq;
+        if (npf == 4) {
+            const double xi = (q & 1) ? g : -g, et = (q & 2) ? g : -g;
+#pragma unroll
+            for (int a = 0; a < 4; ++a) {
+                const double sx = (a == 1 || a == 2) ? 1.0 : -1.0, se = (a >= 2) ? 1.0 : -1.0;
+                N[a] = 0.25 * (1.0 + sx * xi) * (1.0 + se * et);
+                d1[a] = 0.25 * sx * (1.0 + se * et);
+                d2[a] = 0.25 * (1.0 + sx * xi) * se;
+            }
+            wq = 1.0;
+        } else {
+            N[0] = N[1] = N[2] = 1.0 / 3.0; N[3] = 0.0;
+            d1[0] = -1.0; d1[1] = 1.0; d1[2] = 0.0; d1[3] = 0.0;
+            d2[0] = -1.0; d2[1] = 0.0; d2[2] = 1.0; d2[3] = 0.0;
+            wq = 0.5;
+        }
+        double T1[3] = {0, 0, 0}, T2[3] = {0, 0, 0}, t1[3] = {0, 0, 0}, t2[3] = {0, 0, 0};
+        for (int a = 0; a < npf; ++a)
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                T1[c] = fma(d1[a], Xf[a][c], T1[c]); T2[c] = fma(d2[a], Xf[a][c], T2[c]);
+                t1[c] = fma(d1[a], xf[a][c], t1[c]); t2[c] = fma(d2[a], xf[a][c], t2[c]);
+            }
+        const double NX[3] = {T1[1] * T2[2] - T1[2] * T2[1], T1[2] * T2[0] - T1[0] * T2[2], T1[0] * T2[1] - T1[1] * T2[0]};
+        const double nx[3] = {t1[1] * t2[2] - t1[2] * t2[1], t1[2] * t2[0] - t1[0] * t2[2], t1[0] * t2[1] - t1[1] * t2[0]};
+        const double dA = sqrt(NX[0] * NX[0] + NX[1] * NX[1] + NX[2] * NX[2]);
+        for (int a = 0; a < npf; ++a)
+#pragma unroll
+            for (int c = 0; c < 3; ++c) add[a][c] += wq * N[a] * (qv[c] * dA - p * nx[c]);
+    }
+    for (int a = 0; a < npf; ++a)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) atomicAdd(B + c * n_nodes + nd[a], add[a][c]);
+}
+
+__global__ void __launch_bounds__(256)
+ibk_fhat(int64_t n_nodes, const double *__restrict__ B, const double *__restrict__ wa, double *__restrict__ Fhat)
+{
+    int64_t n = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= n_nodes) return;
+    const double r = 1.0 / wa[n];
+    Fhat[n] = B[n] * r; Fhat[n_nodes + n] = B[n_nodes + n] * r; Fhat[2 * n_nodes + n] = B[2 * n_nodes + n] * r;
+}
+
+static bool ib_has_loads(const ib_ctx *c)
+{
+    return (c->n_teth > 0 && c->kappa_t != 0.0) ||
+           (c->n_faces > 0 && (c->p_load != 0.0 || c->qt0[0] != 0.0 || c->qt0[1] != 0.0 || c->qt0[2] != 0.0));
+}
+
+static ib_status ib_add_loads(ib_ctx *c, const double *x, double *B, cudaStream_t st)
+{
+    if (c->n_teth > 0 && c->kappa_t != 0.0) {
+        ibk_tethers<<<ib_blocks(c->n_teth, 256), 256, 0, st>>>(c->n_teth, c->n_nodes, c->d_teth_ids, c->d_X, x, c->kappa_t, B);
+        c->launches++;
+    }
+    if (c->n_faces > 0 && (c->p_load != 0.0 || c->qt0[0] != 0.0 || c->qt0[1] != 0.0 || c->qt0[2] != 0.0)) {
+        ibk_surface_loads<<<ib_blocks(c->n_faces, 128), 128, 0, st>>>(c->n_faces, c->npf, c->n_nodes, c->d_faces, c->d_X, x,
+                                                                     c->qt0[0], c->qt0[1], c->qt0[2], c->p_load, B);
+        c->launches++;
+    }
+    IB_CUDA_TRY(cudaGetLastError());
+    return IB_OK;
+}
+
 ib_status ibk_fe_precompute(ib_ctx *c, cudaStream_t st)
 {
     if (c->n_elems == 0) return IB_OK;
@@ -374,7 +473,7 @@ ib_status ibk_fe_force(ib_ctx *c, const double *x, double *B, double *Fhat, cuda
             c->launches++;
         }
         IB_CUDA_TRY(cudaGetLastError());
-        return IB_OK;
+        return ib_has_loads(c) ? ib_add_loads(c, x, B, st) : IB_OK;
     }
     if (c->n_elems > 0) {
         int64_t nt = c->n_elems * 8;
@@ -384,9 +483,18 @@ ib_status ibk_fe_force(ib_ctx *c, const double *x, double *B, double *Fhat, cuda
         c->launches++;
     }
     if (c->n_nodes > 0) {
+        const bool loads = ib_has_loads(c);
         ibk_node_gather<<<ib_blocks(c->n_nodes, 256), 256, 0, st>>>(c->n_nodes, c->n_elems * 8, c->d_adj,
-                                                                    c->d_Ce, c->d_wa, B, Fhat);
+                                                                    c->d_Ce, c->d_wa, B, loads ? nullptr : Fhat);
         c->launches++;
+        if (loads) {                                          // Fhat = B / w_a must see the boundary loads too
+            ib_status s = ib_add_loads(c, x, B, st);
+            if (s != IB_OK) return s;
+            if (Fhat) {
+                ibk_fhat<<<ib_blocks(c->n_nodes, 256), 256, 0, st>>>(c->n_nodes, B, c->d_wa, Fhat);
+                c->launches++;
+            }
+        }
     }
     IB_CUDA_TRY(cudaGetLastError());
     return IB_OK;

@@ -20,7 +20,7 @@ STATUS = {0: "IB_OK", 1: "IB_ERR_INVALID_ARG", 2: "IB_ERR_UNSUPPORTED", 3: "IB_E
 
 EXPORTS = ["ib_create", "ib_destroy", "ib_num_points", "ib_num_nodes", "ib_num_elems", "ib_fe_force",
            "ib_points", "ib_restrict", "ib_bin_sort", "ib_spread", "ib_interp", "ib_coupling_step",
-           "ib_coupling_step_host", "ib_step_eq16", "ib_check", "ib_launch_count", "ib_set_variant", "ib_set_graph", "ib_probe_dfma",
+           "ib_coupling_step_host", "ib_step_eq16", "ib_check", "ib_launch_count", "ib_set_variant", "ib_set_graph", "ib_set_tethers", "ib_set_surface", "ib_set_loads", "ib_probe_dfma",
            "ib_profile_enable", "ib_profile_read",
            "ib_status_string"]
 
@@ -73,6 +73,9 @@ def lib():
         L.ib_check.argtypes = [vp, C.POINTER(i64)]
         L.ib_set_variant.argtypes = [vp, i32]
         L.ib_set_graph.argtypes = [vp, i32]
+        L.ib_set_tethers.argtypes = [vp, i64, vp, C.c_double]
+        L.ib_set_surface.argtypes = [vp, i64, i32, vp]
+        L.ib_set_loads.argtypes = [vp, vp, C.c_double]
         L.ib_profile_enable.argtypes = [vp, i32]
         L.ib_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(i64)]
         L.ib_probe_dfma.argtypes = [i32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
@@ -160,6 +163,19 @@ class Context:
     # ---- the C ABI, same names ---------------------------------------------------------------
     def ib_set_variant(self, variant):
         _chk(lib().ib_set_variant(self._h, int(variant)), "ib_set_variant")
+
+    def ib_set_tethers(self, node_ids, kappa):
+        ids = np.ascontiguousarray(node_ids, dtype=np.int32)
+        _chk(lib().ib_set_tethers(self._h, ids.size, ids.ctypes.data if ids.size else None, float(kappa)), "ib_set_tethers")
+
+    def ib_set_surface(self, faces):
+        f = np.ascontiguousarray(faces, dtype=np.int32)
+        npf = f.shape[1] if f.ndim == 2 and f.size else 4
+        _chk(lib().ib_set_surface(self._h, f.shape[0] if f.size else 0, npf, f.ctypes.data if f.size else None), "ib_set_surface")
+
+    def ib_set_loads(self, qt0=None, p=0.0):
+        q = None if qt0 is None else np.ascontiguousarray(qt0, dtype=np.float64)
+        _chk(lib().ib_set_loads(self._h, None if q is None else q.ctypes.data, float(p)), "ib_set_loads")
 
     def ib_set_graph(self, on=True):
         _chk(lib().ib_set_graph(self._h, int(bool(on))), "ib_set_graph")

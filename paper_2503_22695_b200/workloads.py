@@ -114,6 +114,21 @@ def tets_from_hexes(conn_hex, X):
     return tets.astype(np.int32)
 
 
+_HEX_FACES = np.array([[0, 4, 6, 2], [1, 3, 7, 5], [0, 1, 5, 4], [2, 6, 7, 3], [0, 2, 3, 1], [4, 5, 7, 6]])
+_TET_FACES = np.array([[1, 2, 3], [0, 3, 2], [0, 1, 3], [0, 2, 1]])
+
+
+def boundary_faces(conn):
+    """Faces that belong to exactly one element, nodes in cyclic order with the normal pointing out of the
+    element (right-handed elements): [nf,4] for hexahedra, [nf,3] for tetrahedra.  Inputs for the surface
+    loads of NEXT-4 (pressure on the endocardium L303, traction on the Cook membrane's face L263)."""
+    loc = _HEX_FACES if conn.shape[1] == 8 else _TET_FACES
+    faces = conn[:, loc].reshape(-1, loc.shape[1])
+    key = np.sort(faces, axis=1)
+    _, inv, cnt = np.unique(key, axis=0, return_inverse=True, return_counts=True)
+    return np.ascontiguousarray(faces[cnt[inv.ravel()] == 1]).astype(np.int32)
+
+
 def _orient(conn, X):
     """Make every element right-handed (positive reference Jacobian at the centroid) by
     swapping the local xi_1 direction when the mean-edge triple product is negative."""

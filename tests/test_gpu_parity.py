@@ -443,3 +443,53 @@ def test_graph_replay_matches_eager_step(ib, orc):
             assert max_abs_scaled(Un2.cpu().numpy(), eager["Un"]) <= 1e-12
         st.synchronize()
         ctx.close()
+
+
+# ---- NEXT-4: solid boundary loads ---------------------------------------------------------------------
+@pytest.mark.parametrize("kind", ["hex-sub", "hex-nodal", "tet"])
+def test_boundary_loads_enter_force_and_step(ib, orc, kind):
+    """Tethers (L263, L425), dead traction (L263) and follower pressure (L303, L315) are added to B by
+    ib_fe_force and reach the grid through the step (Fhat = B / w_a includes them)."""
+    import torch
+    conn, X, x, fib = distorted_block(5, 4, 3, size=(0.3, 0.25, 0.2), seed=41, ref_noise=0.1, cur_noise=0.05)
+    if kind == "tet":
+        conn = W.tets_from_hexes(conn, X)
+        fib = None
+    ne, nn = conn.shape[0], X.shape[1]
+    nsub = np.tile([3, 2, 2], (ne, 1)).astype(np.int32) if kind == "hex-sub" else None
+    mats = [W.material(W.LAW_NEOHOOKEAN, a=80.0, kappa=4e4)]
+    faces = W.boundary_faces(conn)
+    left = np.unique(faces[np.all(X[0, faces] < X[0].min() + 0.03, axis=1)])
+    qt0, p, kap = np.array([0.0, 6.25, -1.0]), 14.53, 1e6
+    B_r = orc.fe_force(conn, X, x, fib, None, mats)["B"]
+    B_r, _ = orc.tethers(left, X, x, kap, B_r)
+    B_r = orc.surface_loads(faces, X, x, qt0, p, B_r)
+    n, h, org = (32, 32, 32), 1 / 32, (0.0, 0.0, 0.0)
+    g = orc.make_grid(*n, h, org)
+    if nsub is None:
+        f_r = orc.spread(g, x, B_r)
+    else:
+        xp, Wp, wa = orc.points(conn, X, x, nsub)
+        f_r = orc.spread(g, xp, orc.prolong(conn, nsub, wa, Wp, B_r))
+    ctx = ib.Context(*n, h, org, conn, X, fib, None, nsub, mats)
+    ctx.ib_set_tethers(left, kap)
+    ctx.ib_set_surface(faces)
+    ctx.ib_set_loads(qt0, p)
+    B = torch.empty((3, nn), dtype=torch.float64, device="cuda")
+    ctx.ib_fe_force(_t(x), B)
+    ctx.check()
+    _close(B, B_r, f"{kind} loaded B")
+    ncell = n[0] * n[1] * n[2]
+    uvw = np.random.default_rng(2).normal(size=(3, ncell))
+    f = [torch.empty(ncell, dtype=torch.float64, device="cuda") for _ in range(3)]
+    Un = torch.empty((3, nn), dtype=torch.float64, device="cuda")
+    ctx.ib_coupling_step(_t(x), _t(uvw[0]), _t(uvw[1]), _t(uvw[2]), *f, Un, B)
+    ctx.check()
+    for c in range(3):
+        _close(f[c], f_r[c], f"{kind} loaded f{c}")
+    # loads off again: back to the plain elastic force
+    ctx.ib_set_tethers([], 0.0)
+    ctx.ib_set_loads(None, 0.0)
+    ctx.ib_fe_force(_t(x), B)
+    _close(B, orc.fe_force(conn, X, x, fib, None, mats)["B"], f"{kind} unloaded B")
+    ctx.close()

@@ -457,3 +457,74 @@ def test_tet_rigid_motion_patch_and_volume(orc):
     interior = ((i > 0) & (i < N1 - 1) & (j > 0) & (j < N2 - 1) & (k > 0) & (k < N3 - 1)).ravel()
     assert interior.sum() == 4
     assert np.max(np.abs(B[:, interior])) < 1e-11 * np.max(np.abs(B[:, ~interior]))
+
+
+# ---- NEXT-4: solid boundary loads (Table 3 "Solid boundary", L263, L303, L315, L425) ----------------
+def _enclosed_volume(faces, x):
+    """(1/3) closed-surface integral of x.n da, 2x2 Gauss per bilinear quad / centroid rule per triangle
+    -- a formula of its own (divergence theorem), not the oracle's load integral."""
+    V = 0.0
+    g = 1 / np.sqrt(3)
+    for f in faces:
+        P = x[:, f]
+        if len(f) == 3:
+            n = np.cross(P[:, 1] - P[:, 0], P[:, 2] - P[:, 0])
+            V += np.dot(P.mean(axis=1), n) / 2 / 3
+        else:
+            for xi in (-g, g):
+                for et in (-g, g):
+                    sx, se = np.array([-1, 1, 1, -1]), np.array([-1, -1, 1, 1])
+                    N = 0.25 * (1 + sx * xi) * (1 + se * et)
+                    tx = P @ (0.25 * sx * (1 + se * et))
+                    te = P @ (0.25 * (1 + sx * xi) * se)
+                    V += np.dot(P @ N, np.cross(tx, te)) / 3
+    return V
+
+
+@pytest.mark.parametrize("kind", ["hex", "tet"])
+def test_boundary_loads_pins(orc, kind):
+    conn, X, x, _ = distorted_block(3, 3, 2, seed=12, ref_noise=0.1, cur_noise=0.06)
+    if kind == "tet":
+        conn = W.tets_from_hexes(conn, X)
+    faces = W.boundary_faces(conn)
+    assert faces.shape == ((2 * (9 + 6 + 6), 4) if kind == "hex" else (4 * (9 + 6 + 6), 3))
+    nn = X.shape[1]
+    zero = np.zeros((3, nn))
+    # closed surface: the enclosed volume is the element volume (orientation is outward)
+    vol = orc.nodal_weights(*distorted_block(3, 3, 2, seed=12, ref_noise=0.1, cur_noise=0.06)[:2]).sum()
+    if kind == "tet":
+        Pt = X[:, conn]
+        vol = np.einsum("in,in->n", np.cross((Pt[:, :, 1] - Pt[:, :, 0]).T, (Pt[:, :, 2] - Pt[:, :, 0]).T).T,
+                        Pt[:, :, 3] - Pt[:, :, 0]).sum() / 6
+    assert abs(_enclosed_volume(faces, X) - vol) < 1e-12 * vol
+    # pressure: follower load -p n da on a closed surface = -p dV/dx, no net force, no net torque
+    p = 3.7
+    Bp = orc.surface_loads(faces, X, x, None, p, zero)
+    rng = np.random.default_rng(1)
+    eps = 1e-6 * 0.1
+    for _ in range(10):
+        c, n = rng.integers(0, 3), rng.integers(0, nn)
+        xp, xm = x.copy(), x.copy()
+        xp[c, n] += eps
+        xm[c, n] -= eps
+        fd = -p * (_enclosed_volume(faces, xp) - _enclosed_volume(faces, xm)) / (2 * eps)
+        assert abs(fd - Bp[c, n]) < 1e-7 * np.max(np.abs(Bp)), (c, n)
+    assert np.max(np.abs(Bp.sum(axis=1))) < 1e-13 * np.max(np.abs(Bp)) * nn
+    assert np.max(np.abs(np.cross(x.T, Bp.T).sum(axis=0))) < 1e-12 * np.max(np.abs(Bp)) * nn
+    # traction: dead load q t0 per unit reference area: total = q t0 * area; on the flat undistorted block the
+    # face x = const has area 0.3 x 0.2 and each of its 4 x 3 nodes gets its lumped share
+    conn0, X0, _, _ = distorted_block(3, 3, 2, seed=12, ref_noise=0.0, cur_noise=0.0)
+    if kind == "tet":
+        conn0 = W.tets_from_hexes(conn0, X0)
+    f0 = W.boundary_faces(conn0)
+    right = f0[np.all(np.abs(X0[0, f0] - X0[0].max()) < 1e-12, axis=1)]
+    qt0 = np.array([0.0, 6.25, 0.0])
+    Bt = orc.surface_loads(right, X0, X0 * 1.3, qt0, 0.0, np.zeros_like(X0))       # current config is irrelevant
+    assert np.allclose(Bt.sum(axis=1), qt0 * 0.3 * 0.2, rtol=1e-13, atol=1e-15)
+    assert np.count_nonzero(Bt[1]) == 12 and np.all(Bt[[0, 2]] == 0)
+    # tethers: penalty spring to the reference position, B = -dE/dx with E = kappa/2 sum |x-X|^2
+    ids = np.unique(faces[np.all(np.abs(X[0, faces] - X[0].min()) < 0.05, axis=1)])[:7]
+    Bk, E = orc.tethers(ids, X, x, 1e6, zero)
+    assert np.allclose(Bk[:, ids], 1e6 * (X - x)[:, ids], rtol=1e-14) and np.count_nonzero(Bk) == 3 * ids.size
+    assert abs(E - 0.5e6 * np.sum((x - X)[:, ids] ** 2)) < 1e-12 * E
+    assert np.array_equal(orc.tethers(ids, X, X, 1e6, zero)[0], zero)
