@@ -7,7 +7,9 @@
 
 #define IB_TILE 8              // tile edge of the binning key (A21)
 #define IB_TILE_CELLS 512
-#define IB_SMALL_TILE 32         // tiles with fewer points skip the tile kernel: their points go one by one (ib_point.cuh)
+#ifndef IB_SMALL_TILE
+#define IB_SMALL_TILE 64         // tiles with fewer points skip the tile kernel: their points go one by one (ib_point.cuh)
+#endif
 #define IB_CHUNK 1920            // points per work item of the tile kernel (ib_bin.cu emits the work list)
 
 // ---------------------------------------------------------------------------------------------
