@@ -108,30 +108,28 @@ __device__ __forceinline__ void ib_latch(long long *status, int code, long long 
     atomicMin(&status[1], id);
 }
 
-// Peskin 4-point kernel (PAPER.md L52 -> ref.1): the four weights of the support that starts at
-// i0 = floor(s) - 1, with r = s - floor(s) in [0,1):
-//   phi(1+r) = (3-2r-q)/8, phi(r) = (3-2r+q)/8, phi(1-r) = (1+2r+q)/8, phi(2-r) = (1+2r-q)/8,
-//   q = sqrt(1+4r-4r^2)  (one square root serves all four).
-// sqrt(a) for a in [1,2] (the argument 1+4r-4r^2 of the kernel): float rsqrt seed, two Goldschmidt
-// steps and a final residual correction -- no special cases, no branches; error <= 1 ulp.
-__device__ __forceinline__ double ib_sqrt12(double a)
+// sqrt(a) for a in [1/64, 1/32] (the argument (1+4r-4r^2)/64 of the kernel): float rsqrt seed (~2^-22),
+// one Goldschmidt step (~2^-43) and one residual correction (~2^-85, i.e. rounding level) -- no special
+// cases, no branches, 7 fp64 operations.
+__device__ __forceinline__ double ib_sqrt_seeded(double a)
 {
     float yf;
-    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(yf) : "f"((float)a));       // one MUFU.RSQ, ~22 good bits
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(yf) : "f"((float)a));       // one MUFU.RSQ
     double y = (double)yf;
     double g = a * y, h = 0.5 * y;
     double r = fma(-g, h, 0.5);
     g = fma(g, r, g);
     h = fma(h, r, h);
-    r = fma(-g, h, 0.5);
-    g = fma(g, r, g);
-    h = fma(h, r, h);
     return fma(fma(-g, g, a), h, g);
 }
 
+// Peskin 4-point kernel (PAPER.md L52 -> ref.1): the four weights of the support that starts at
+// i0 = floor(s) - 1, with r = s - floor(s) in [0,1):
+//   phi(1+r) = (3-2r-q)/8, phi(r) = (3-2r+q)/8, phi(1-r) = (1+2r+q)/8, phi(2-r) = (1+2r-q)/8,
+//   q = sqrt(1+4r-4r^2)  (one square root serves all four; q/8 = sqrt((1+4r-4r^2)/64) directly).
 __device__ __forceinline__ void ib_phi4(double r, double w[4])
 {
-    double q = ib_sqrt12(fma(4.0 * r, 1.0 - r, 1.0)) * 0.125;
+    double q = ib_sqrt_seeded(fma(0.0625 * r, 1.0 - r, 0.015625));
     double a = fma(-0.25, r, 0.375);
     double b = fma(0.25, r, 0.125);
     w[0] = a - q;
