@@ -398,7 +398,7 @@ ib_status ibk_bin_points(ib_ctx *c, int mesh, const double *xp, const double *Gp
         // ~4 work items per resident CTA of the tile kernel when the cloud is small
         int chunk = (int)((P / 1200 + 63) / 64 * 64);
         chunk = chunk < 192 ? 192 : (chunk > IB_CHUNK ? IB_CHUNK : chunk);
-        ibk_tile_partials<<<nsb, SCT, 0, st>>>(c->d_tile_cur, n_tiles, chunk, partial);
+        if (nsb > 1) ibk_tile_partials<<<nsb, SCT, 0, st>>>(c->d_tile_cur, n_tiles, chunk, partial);   // one CTA needs no partial sums
         ibk_tile_scan<<<nsb, SCT, 0, st>>>(c->d_tile_cur, n_tiles, chunk, partial, c->d_tile_start, c->d_work, c->d_small_rec, c->d_tile_count);
         c->launches += 3;
     }
