@@ -313,11 +313,25 @@ def run_ours(args):
         dfma_peak, _ = ibcouple.probe_dfma(local)
         # dominant kernel: points' 72 B + grid 48 B/cell of the algorithmic bytes belong to it
         dom_bytes = 72 * wl.n_points + 48 * wl.n_cells
-        roofline = {"bound": "hbm", "kernel": "spread+interp (" + ("tiled" if args.variant else "per-point") + ")",
-                    "achieved": dom_bytes / (dom_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
-                    "frac": dom_bytes / (dom_ms * 1e-3) / 1e9 / hbm_peak, "traffic": ncu_traffic_bytes(wl.name),
-                    "peak_source": hbm_src, "kernel_ms": dom_ms,
-                    "algorithmic_bytes_per_launch": dom_bytes,
+        # The dominant kernel is bound by the plain fp64 ALUs, not by HBM: the top-level
+        # roofline is the ALU one -- algorithmic flops = 2 x 600 DFMA slots per force point (SURVEY.md
+        # §8(d): weights 100 + interpolation 252 + spreading 252), peak derived from the unit count and
+        # the clock (64 DFMA/clk/SM x SMs x max SM clock; ib_probe_dfma measures 92 % of it).  The HBM
+        # roofline BASELINE.json's metric names is reported beside it under "hbm".
+        dom_slots = 600 * wl.n_points
+        sms = torch.cuda.get_device_properties(local).multi_processor_count
+        sm_hz = 1e6 * float(clocks.get("sm_max_mhz") or 1965.0)
+        alu_peak_tf = 2.0 * 64 * sms * sm_hz / 1e12
+        dom_tf = 2.0 * dom_slots / (dom_ms * 1e-3) / 1e12
+        roofline = {"bound": "alu", "kernel": "spread+interp (" + ("tiled" if args.variant else "per-point") + ")",
+                    "achieved": dom_tf, "peak": alu_peak_tf, "unit": "TFLOP/s", "frac": dom_tf / alu_peak_tf,
+                    "traffic": ncu_traffic_bytes(wl.name),
+                    "peak_source": f"derived: 64 DFMA/clk/SM x {sms} SMs x {sm_hz / 1e6:.0f} MHz x 2 flop (fp64 vector pipe); "
+                                   f"ib_probe_dfma measured {2 * dfma_peak / 1e12:.1f} TFLOP/s in this run",
+                    "kernel_ms": dom_ms, "algorithmic_flops_per_launch": 2 * dom_slots,
+                    "hbm": {"achieved": dom_bytes / (dom_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                            "frac": dom_bytes / (dom_ms * 1e-3) / 1e9 / hbm_peak, "peak_source": hbm_src,
+                            "algorithmic_bytes_per_launch": dom_bytes},
                     "step": {"algorithmic_bytes": abytes, "achieved_GBps": abytes / (step_ms * 1e-3) / 1e9,
                              "frac_of_hbm_peak": abytes / (step_ms * 1e-3) / 1e9 / hbm_peak},
                     "alu": {"dfma_slots_per_step": dfma_slots(wl), "dfma_peak_per_s": dfma_peak,
