@@ -493,3 +493,32 @@ def test_boundary_loads_enter_force_and_step(ib, orc, kind):
     ctx.ib_fe_force(_t(x), B)
     _close(B, orc.fe_force(conn, X, x, fib, None, mats)["B"], f"{kind} unloaded B")
     ctx.close()
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_spread_interp_heavy_contention(ib, orc, variant):
+    """Degenerate clouds: 60,000 points inside ONE cell (32 chunks of one tile, every item crowded, all
+    atomics on the same 3 x 64 faces), many exactly coincident points, and a cloud of exactly one point."""
+    import torch
+    n, h, org = (16, 16, 24), 0.1, (0.0, -0.5, 1.0)
+    ctx = ib.Context(*n, h, org, np.zeros((0, 8), np.int32), np.zeros((3, 0)), None, None, None, [])
+    ctx.ib_set_variant(variant)
+    g = orc.make_grid(*n, h, org)
+    rng = np.random.default_rng(11)
+    ncell = n[0] * n[1] * n[2]
+    uvw = rng.normal(size=(3, ncell))
+    for P, where in ((60000, "cell"), (4096, "same"), (1, "same")):
+        base = np.asarray(org) + h * np.array([15.0, 0.0, 23.0])            # a corner cell: supports wrap in x, y and z
+        xp = base[:, None] + (rng.uniform(0, h, (3, P)) if where == "cell" else np.full((3, P), 0.37 * h))
+        G = rng.normal(size=(3, P))
+        f = [torch.empty(ncell, dtype=torch.float64, device="cuda") for _ in range(3)]
+        Up = torch.empty((3, P), dtype=torch.float64, device="cuda")
+        ctx.ib_spread(_t(xp), _t(G), P, *f, accumulate=0)
+        ctx.ib_interp(_t(xp), P, _t(uvw[0]), _t(uvw[1]), _t(uvw[2]), Up)
+        ctx.check()
+        fr = orc.spread(g, xp, G)
+        for c in range(3):
+            _close(f[c], fr[c], f"contention {where} {P} f{c}")
+            assert abs(h ** 3 * float(f[c].sum()) - G[c].sum()) <= 1e-11 * np.abs(G[c]).sum()
+        _close(Up, orc.interp(g, xp, *uvw), f"contention {where} {P} U")
+    ctx.close()
