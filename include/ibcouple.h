@@ -88,9 +88,12 @@ typedef struct {
     int32_t n_mats;
     int32_t elem_type;        /* IB_ELEM_HEX8 (0): conn [n_elems][8]; IB_ELEM_TET4 (1), NEXT-3: P1
                                  tetrahedra, conn [n_elems][4] with det [X1-X0,X2-X0,X3-X0] > 0, one
-                                 quadrature point, nodal coupling only (nsub must be NULL, L241)  */
+                                 quadrature point, nodal coupling only (nsub must be NULL, L241);
+                                 IB_ELEM_TET10 (2): P2 tetrahedra (L265), conn [n_elems][10] = 4 vertices then the
+                                 mid-edge nodes of edges 01,12,02,03,13,23; 4-point degree-2 rule (reading A25);
+                                 nodal coupling only */
 } ib_mesh_desc;
-enum { IB_ELEM_HEX8 = 0, IB_ELEM_TET4 = 1 };
+enum { IB_ELEM_HEX8 = 0, IB_ELEM_TET4 = 1, IB_ELEM_TET10 = 2 };
 
 /* Create a context: validates, copies the mesh, builds the node->element adjacency (at most 8
  * incident elements per node), and precomputes on the device the sub-point weights W_s =

@@ -102,8 +102,8 @@ def fe_force(conn, X, x, fibers, mat_id, mats, want=("B", "energy", "minJ")):
     mat_id = _i32(mat_id)
     B = np.empty((3, nn))
     E, mj, bad = C.c_double(0), C.c_double(0), C.c_int64(-1)
-    # conn [ne,8]: Q1 hexahedra; conn [ne,4]: P1 tetrahedra (NEXT-3)
-    fn = lib().oracle_fe_force_tet if conn.shape[1] == 4 else lib().oracle_fe_force
+    # conn [ne,8]: Q1 hexahedra; conn [ne,4]: P1 tetrahedra; conn [ne,10]: P2 tetrahedra (NEXT-3)
+    fn = {4: lib().oracle_fe_force_tet, 10: lib().oracle_fe_force_tet10}.get(conn.shape[1], lib().oracle_fe_force)
     rc = fn(C.c_int64(nn), C.c_int64(ne), _p(conn, C.c_int32), _p(X), _p(x),
             _p(fibers), _p(mat_id, C.c_int32), make_materials(mats), _p(B),
             C.byref(E), C.byref(mj), C.byref(bad))

@@ -383,6 +383,95 @@ int oracle_fe_force_tet(int64_t n_nodes, int64_t n_elems, const int32_t *conn, c
 }
 
 /* ------------------------------------------------------------------------------------------
+ * O2q FE nodal force on P2 (10-node, quadratic) tetrahedra -- NEXT-3, second half: "the forces and
+ * displacements are discretized using P2 finite elements" (Cook's membrane, L265).  Barycentric
+ * coordinates l0 = 1-xi-eta-zeta, l1 = xi, l2 = eta, l3 = zeta; nodes 0-3 vertices, 4-9 the edge
+ * mid-points (01, 12, 02, 03, 13, 23):
+ *   N_v = l_v (2 l_v - 1),   N_(ab) = 4 l_a l_b,   grad_xi by the product rule,
+ *   J0 = sum_a X_a (x) grad_xi N_a (per quadrature point: edges may be curved), G_a = J0^-T grad_xi N_a,
+ *   F = sum_a x_a (x) G_a,  B_{a,c} -= sum_J P_{cJ} G_{a,J} w,  w = det J0 * w_q  (Eq.(20)).
+ * The paper does not name the quadrature rule; reading A25: the 4-point degree-2 rule, points
+ * (a,b,b,b) and permutations in barycentric coordinates, a = (5+3 sqrt5)/20, b = (5-sqrt5)/20, w_q = 1/24.
+ * conn is [n_elems][10].
+ * ---------------------------------------------------------------------------------------- */
+static void p2_shape(const ld l[4], ld dN[10][3])
+{
+    static const ld dl[4][3] = {{-1, -1, -1}, {1, 0, 0}, {0, 1, 0}, {0, 0, 1}};
+    static const int ea[6] = {0, 1, 0, 0, 1, 2}, eb[6] = {1, 2, 2, 3, 3, 3};
+    for (int v = 0; v < 4; ++v)
+        for (int d = 0; d < 3; ++d) dN[v][d] = (4.0L * l[v] - 1.0L) * dl[v][d];
+    for (int e = 0; e < 6; ++e)
+        for (int d = 0; d < 3; ++d) dN[4 + e][d] = 4.0L * (l[ea[e]] * dl[eb[e]][d] + l[eb[e]] * dl[ea[e]][d]);
+}
+
+int oracle_fe_force_tet10(int64_t n_nodes, int64_t n_elems, const int32_t *conn, const double *X,
+                          const double *x, const double *fibers, const int32_t *mat_id,
+                          const oracle_material *mats, double *B, double *energy, double *minJ,
+                          int64_t *first_bad)
+{
+    const ld qa = (5.0L + 3.0L * sqrtl(5.0L)) / 20.0L, qb = (5.0L - sqrtl(5.0L)) / 20.0L;
+    ld *Bl = (ld *)calloc((size_t)(3 * n_nodes), sizeof(ld));
+    ld E = 0.0L, mj = INFINITY;
+    int rc = 0;
+    for (int64_t e = 0; e < n_elems && !rc; ++e) {
+        ld Xe[10][3], xe[10][3], ef[3] = {1, 0, 0}, es[3] = {0, 1, 0};
+        for (int a = 0; a < 10; ++a)
+            for (int c = 0; c < 3; ++c) {
+                Xe[a][c] = X[c * n_nodes + conn[e * 10 + a]];
+                xe[a][c] = x[c * n_nodes + conn[e * 10 + a]];
+            }
+        if (fibers)
+            for (int c = 0; c < 3; ++c) { ef[c] = fibers[c * n_elems + e]; es[c] = fibers[(3 + c) * n_elems + e]; }
+        const oracle_material *m = &mats[mat_id ? mat_id[e] : 0];
+        for (int q = 0; q < 4; ++q) {
+            ld l[4] = {qb, qb, qb, qb}, dN[10][3], J0[3][3], J0i[3][3];
+            l[q] = qa;
+            p2_shape(l, dN);
+            for (int I = 0; I < 3; ++I)
+                for (int d = 0; d < 3; ++d) {
+                    ld s2 = 0.0L;
+                    for (int a = 0; a < 10; ++a) s2 += Xe[a][I] * dN[a][d];
+                    J0[I][d] = s2;
+                }
+            ld dj = inv3(J0, J0i);
+            if (!(dj > 0.0L)) { rc = 1; if (first_bad) *first_bad = e; break; }
+            ld w = dj / 24.0L;
+            ld G[10][3];
+            for (int a = 0; a < 10; ++a)
+                for (int I = 0; I < 3; ++I) {
+                    ld s2 = 0.0L;
+                    for (int d = 0; d < 3; ++d) s2 += J0i[d][I] * dN[a][d];
+                    G[a][I] = s2;
+                }
+            ld F[3][3], P[3][3], W;
+            for (int c = 0; c < 3; ++c)
+                for (int I = 0; I < 3; ++I) {
+                    ld s2 = 0.0L;
+                    for (int a = 0; a < 10; ++a) s2 += xe[a][c] * G[a][I];
+                    F[c][I] = s2;
+                }
+            if (pk1_l(m, F, ef, es, P, &W)) { rc = 1; if (first_bad) *first_bad = e; break; }
+            ld J = det3(F);
+            if (J < mj) mj = J;
+            E += W * w;
+            for (int a = 0; a < 10; ++a) {
+                int64_t n = conn[e * 10 + a];
+                for (int c = 0; c < 3; ++c) {
+                    ld s2 = 0.0L;
+                    for (int I = 0; I < 3; ++I) s2 += P[c][I] * G[a][I];
+                    Bl[c * n_nodes + n] -= s2 * w;
+                }
+            }
+        }
+    }
+    for (int64_t i = 0; i < 3 * n_nodes; ++i) B[i] = (double)Bl[i];
+    if (energy) *energy = (double)E;
+    if (minJ) *minJ = (double)mj;
+    free(Bl);
+    return rc;
+}
+
+/* ------------------------------------------------------------------------------------------
  * O9  solid boundary loads (NEXT-4; Table 3 row "Solid boundary" L398).  All ADD to B [3][n_nodes].
  *  tethers (L263 "fixed left face ... penalty parameter kappa = 10^6", L425): the paper gives only the
  *    parameter; reading A24: a penalty spring to the reference position, B_a += kappa (X_a - x_a),

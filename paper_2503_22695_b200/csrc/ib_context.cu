@@ -141,9 +141,9 @@ extern "C" ib_status ib_create(ib_ctx **out, const ib_grid_desc *g, const ib_mes
     if (!g->periodic) return IB_ERR_UNSUPPORTED;
     if (m->n_nodes < 0 || m->n_elems < 0 || m->n_nodes > INT32_MAX || m->n_elems > INT32_MAX / 8) return IB_ERR_INVALID_ARG;
     if (m->n_elems > 0 && (!m->conn || !m->X_ref || !m->mats || m->n_mats <= 0)) return IB_ERR_INVALID_ARG;
-    if (m->elem_type != IB_ELEM_HEX8 && m->elem_type != IB_ELEM_TET4) return IB_ERR_INVALID_ARG;
-    if (m->elem_type == IB_ELEM_TET4 && m->nsub) return IB_ERR_UNSUPPORTED;      // tets: nodal coupling only
-    const int npe = m->elem_type == IB_ELEM_TET4 ? 4 : 8;
+    if (m->elem_type < IB_ELEM_HEX8 || m->elem_type > IB_ELEM_TET10) return IB_ERR_INVALID_ARG;
+    if (m->elem_type != IB_ELEM_HEX8 && m->nsub) return IB_ERR_UNSUPPORTED;       // tets: nodal coupling only
+    const int npe = m->elem_type == IB_ELEM_TET4 ? 4 : (m->elem_type == IB_ELEM_TET10 ? 10 : 8);
     if (m->n_nodes > 0 && !m->X_ref) return IB_ERR_INVALID_ARG;
     for (int i = 0; i < m->n_mats; ++i)
         if (m->mats[i].law < IB_LAW_NEOHOOKEAN || m->mats[i].law > IB_LAW_FR2) return IB_ERR_INVALID_ARG;
@@ -180,12 +180,12 @@ extern "C" ib_status ib_create(ib_ctx **out, const ib_grid_desc *g, const ib_mes
                 cnt[n]++;
             }
         }
-        if (npe == 4) {                                   // CSR: tets share nodes with any number of neighbours
+        if (npe != 8) {                                   // CSR: tets share nodes with any number of neighbours
             for (int64_t n = 0; n < nn; ++n) node_off[n + 1] = node_off[n] + cnt[n];
-            node_slot.resize((size_t)ne * 4 + 1);
+            node_slot.resize((size_t)ne * npe + 1);
             std::vector<int32_t> cur(node_off.begin(), node_off.end() - 1);
             for (int64_t e = 0; e < ne; ++e)
-                for (int a = 0; a < 4; ++a) node_slot[cur[m->conn[e * 4 + a]]++] = (int32_t)(e * 4 + a);
+                for (int a = 0; a < npe; ++a) node_slot[cur[m->conn[e * npe + a]]++] = (int32_t)(e * npe + a);
         }
     }
 
@@ -220,13 +220,13 @@ extern "C" ib_status ib_create(ib_ctx **out, const ib_grid_desc *g, const ib_mes
     TRY(dev_upload(&c->d_pt_off, off.data(), (size_t)ne + 1));
     TRY(dev_upload(&c->d_mats, m->mats, (size_t)(m->n_mats > 0 ? m->n_mats : 0)));
     TRY(dev_upload(&c->d_adj, adj.data(), (size_t)8 * (nn > 0 ? nn : 1)));
-    if (npe == 4) {
+    if (npe != 8) {
         TRY(dev_upload(&c->d_node_off, node_off.data(), (size_t)nn + 1));
         TRY(dev_upload(&c->d_node_slot, node_slot.data(), node_slot.size()));
     }
     const size_t P = (size_t)c->n_points;
     TRY(dev_alloc((void **)&c->d_wa, (size_t)nn * sizeof(double)));
-    TRY(dev_alloc((void **)&c->d_Ce, (size_t)ne * 24 * sizeof(double)));
+    TRY(dev_alloc((void **)&c->d_Ce, (size_t)ne * 3 * (npe > 8 ? npe : 8) * sizeof(double)));
     TRY(dev_alloc((void **)&c->d_geo, (size_t)ne * 80 * sizeof(double)));
     TRY(dev_alloc((void **)&c->d_Fhat, (size_t)nn * 3 * sizeof(double)));
     TRY(dev_alloc((void **)&c->d_B, (size_t)nn * 3 * sizeof(double)));

@@ -335,6 +335,90 @@ ibk_fe_tet(int64_t n_elems, int64_t n_nodes, const int32_t *__restrict__ conn, c
     }
 }
 
+// P2 (10-node) tetrahedra, L265: one thread per (element, quadrature point), the 4 points of the
+// degree-2 rule (reading A25) in 4 adjacent lanes; N_v = l_v (2 l_v - 1), N_(ab) = 4 l_a l_b with the
+// mid-edge nodes in the order 01, 12, 02, 03, 13, 23; the 10 x 3 nodal contributions of the 4 points
+// are summed with a butterfly over the 4 lanes.
+__global__ void __launch_bounds__(128)
+ibk_fe_tet10(int64_t n_elems, int64_t n_nodes, const int32_t *__restrict__ conn, const double *__restrict__ X,
+             const double *__restrict__ x, const double *__restrict__ fib, const int32_t *__restrict__ mat_id,
+             const ib_material *__restrict__ mats, double *__restrict__ Ce, long long *status)
+{
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t e = t >> 2;
+    const int q = (int)(t & 3);
+    const bool live = e < n_elems;
+    const int64_t ee = live ? e : n_elems - 1;
+    const double qa = 0.58541019662496845446, qb = 0.13819660112501051518;      // (5 +- 3 sqrt5)/20, (5 - sqrt5)/20
+    const double l[4] = {q == 0 ? qa : qb, q == 1 ? qa : qb, q == 2 ? qa : qb, q == 3 ? qa : qb};
+    const double dl[4][3] = {{-1, -1, -1}, {1, 0, 0}, {0, 1, 0}, {0, 0, 1}};
+    const int ea[6] = {0, 1, 0, 0, 1, 2}, eb[6] = {1, 2, 2, 3, 3, 3};
+    double dN[10][3];
+#pragma unroll
+    for (int v = 0; v < 4; ++v)
+#pragma unroll
+        for (int d = 0; d < 3; ++d) dN[v][d] = (4.0 * l[v] - 1.0) * dl[v][d];
+#pragma unroll
+    for (int k = 0; k < 6; ++k)
+#pragma unroll
+        for (int d = 0; d < 3; ++d) dN[4 + k][d] = 4.0 * (l[ea[k]] * dl[eb[k]][d] + l[eb[k]] * dl[ea[k]][d]);
+    double J0[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}}, Fx[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
+    bool finite = true;
+#pragma unroll
+    for (int a = 0; a < 10; ++a) {
+        const int nd = __ldg(conn + ee * 10 + a);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const double Xa = __ldg(X + c * n_nodes + nd), xa = __ldg(x + c * n_nodes + nd);
+            finite = finite && isfinite(xa);
+#pragma unroll
+            for (int d = 0; d < 3; ++d) { J0[c][d] = fma(Xa, dN[a][d], J0[c][d]); Fx[c][d] = fma(xa, dN[a][d], Fx[c][d]); }
+        }
+    }
+    const double dj = ib_det3(J0), rd = 1.0 / dj;
+    double Ji[3][3];
+    Ji[0][0] = (J0[1][1] * J0[2][2] - J0[1][2] * J0[2][1]) * rd;
+    Ji[0][1] = (J0[0][2] * J0[2][1] - J0[0][1] * J0[2][2]) * rd;
+    Ji[0][2] = (J0[0][1] * J0[1][2] - J0[0][2] * J0[1][1]) * rd;
+    Ji[1][0] = (J0[1][2] * J0[2][0] - J0[1][0] * J0[2][2]) * rd;
+    Ji[1][1] = (J0[0][0] * J0[2][2] - J0[0][2] * J0[2][0]) * rd;
+    Ji[1][2] = (J0[0][2] * J0[1][0] - J0[0][0] * J0[1][2]) * rd;
+    Ji[2][0] = (J0[1][0] * J0[2][1] - J0[1][1] * J0[2][0]) * rd;
+    Ji[2][1] = (J0[0][1] * J0[2][0] - J0[0][0] * J0[2][1]) * rd;
+    Ji[2][2] = (J0[0][0] * J0[1][1] - J0[0][1] * J0[1][0]) * rd;
+    double F[3][3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+#pragma unroll
+        for (int I = 0; I < 3; ++I) F[c][I] = Fx[c][0] * Ji[0][I] + Fx[c][1] * Ji[1][I] + Fx[c][2] * Ji[2][I];
+    double ef[3] = {1.0, 0.0, 0.0}, es[3] = {0.0, 1.0, 0.0};
+    if (fib) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) { ef[c] = __ldg(fib + c * n_elems + ee); es[c] = __ldg(fib + (3 + c) * n_elems + ee); }
+    }
+    ib_material m = mats[mat_id ? __ldg(mat_id + ee) : 0];
+    double P[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
+    const double J = ib_pk1(m, F, ef, es, P);
+    if (live && !finite) ib_latch(status, IB_ERR_NONFINITE, e);
+    else if (live && (!(dj > 0.0) || !(J > 0.0))) ib_latch(status, IB_ERR_INVERTED_ELEMENT, e);
+    const double w = dj * (1.0 / 24.0);
+    double Q[3][3];                                  // Q_{c d} = -w sum_I P_{cI} Ji[d][I]
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+#pragma unroll
+        for (int d = 0; d < 3; ++d) Q[c][d] = -w * (P[c][0] * Ji[d][0] + P[c][1] * Ji[d][1] + P[c][2] * Ji[d][2]);
+    const int64_t ne10 = n_elems * 10;
+#pragma unroll
+    for (int a = 0; a < 10; ++a)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            double v = Q[c][0] * dN[a][0] + Q[c][1] * dN[a][1] + Q[c][2] * dN[a][2];
+            v += __shfl_xor_sync(0xffffffffu, v, 1);
+            v += __shfl_xor_sync(0xffffffffu, v, 2);
+            if (live && ((a * 3 + c) & 3) == q) Ce[c * ne10 + e * 10 + a] = v;
+        }
+}
+
 // Per node: sum its element contributions through the CSR adjacency in ascending slot order.
 __global__ void __launch_bounds__(256)
 ibk_node_gather_csr(int64_t n_nodes, int64_t ne4, const int32_t *__restrict__ off, const int32_t *__restrict__ slot,
@@ -461,14 +545,19 @@ ib_status ibk_fe_precompute(ib_ctx *c, cudaStream_t st)
 
 ib_status ibk_fe_force(ib_ctx *c, const double *x, double *B, double *Fhat, cudaStream_t st)
 {
-    if (c->elem_type == IB_ELEM_TET4) {                   // nodal coupling only: Fhat is never needed
+    if (c->elem_type != IB_ELEM_HEX8) {                   // nodal coupling only: Fhat is never needed
         if (c->n_elems > 0) {
-            ibk_fe_tet<<<ib_blocks(c->n_elems, 128), 128, 0, st>>>(c->n_elems, c->n_nodes, c->d_conn, c->d_X, x, c->d_fib,
-                                                                  c->d_mat_id, c->d_mats, c->d_Ce, c->d_status);
+            if (c->elem_type == IB_ELEM_TET4)
+                ibk_fe_tet<<<ib_blocks(c->n_elems, 128), 128, 0, st>>>(c->n_elems, c->n_nodes, c->d_conn, c->d_X, x, c->d_fib,
+                                                                      c->d_mat_id, c->d_mats, c->d_Ce, c->d_status);
+            else
+                ibk_fe_tet10<<<ib_blocks(c->n_elems * 4, 128), 128, 0, st>>>(c->n_elems, c->n_nodes, c->d_conn, c->d_X, x,
+                                                                            c->d_fib, c->d_mat_id, c->d_mats, c->d_Ce,
+                                                                            c->d_status);
             c->launches++;
         }
         if (c->n_nodes > 0) {
-            ibk_node_gather_csr<<<ib_blocks(c->n_nodes, 256), 256, 0, st>>>(c->n_nodes, c->n_elems * 4, c->d_node_off,
+            ibk_node_gather_csr<<<ib_blocks(c->n_nodes, 256), 256, 0, st>>>(c->n_nodes, c->n_elems * c->npe, c->d_node_off,
                                                                             c->d_node_slot, c->d_Ce, B);
             c->launches++;
         }

@@ -136,7 +136,7 @@ class Context:
                       None if fibers is None else fibers.ctypes.data,
                       None if mat_id is None else mat_id.ctypes.data,
                       None if nsub is None else nsub.ctypes.data,
-                      C.cast(marr, C.c_void_p), len(mats), 1 if (conn.ndim == 2 and conn.shape[1] == 4) else 0)
+                      C.cast(marr, C.c_void_p), len(mats), {4: 1, 10: 2}.get(conn.shape[1] if conn.ndim == 2 else 8, 0))
         _chk(L.ib_create(C.byref(self._h), C.byref(g), C.byref(md), self.device), "ib_create")
         self.nx, self.ny, self.nz, self.h = int(nx), int(ny), int(nz), float(h)
         self.n_cells = self.nx * self.ny * self.nz

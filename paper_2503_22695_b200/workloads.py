@@ -114,6 +114,19 @@ def tets_from_hexes(conn_hex, X):
     return tets.astype(np.int32)
 
 
+def p2_from_tets(tets, X):
+    """Quadratic (10-node) tetrahedra from linear ones: one new node at the middle of every edge, local
+    order 0-3 vertices, 4-9 edges (01, 12, 02, 03, 13, 23).  Returns (conn10 [nt,10], X10 [3, nn + n_edges]).
+    Stands in for the paper's P2 Cook-membrane mesh (L265)."""
+    pairs = np.array([[0, 1], [1, 2], [0, 2], [0, 3], [1, 3], [2, 3]])
+    e = np.sort(tets[:, pairs].reshape(-1, 2), axis=1)
+    uniq, inv = np.unique(e, axis=0, return_inverse=True)
+    nn = X.shape[1]
+    Xm = 0.5 * (X[:, uniq[:, 0]] + X[:, uniq[:, 1]])
+    conn10 = np.concatenate([tets, nn + inv.reshape(-1, 6)], axis=1).astype(np.int32)
+    return conn10, np.ascontiguousarray(np.concatenate([X, Xm], axis=1))
+
+
 _HEX_FACES = np.array([[0, 4, 6, 2], [1, 3, 7, 5], [0, 1, 5, 4], [2, 6, 7, 3], [0, 2, 3, 1], [4, 5, 7, 6]])
 _TET_FACES = np.array([[1, 2, 3], [0, 3, 2], [0, 1, 3], [0, 2, 1]])
 

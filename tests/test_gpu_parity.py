@@ -522,3 +522,40 @@ def test_spread_interp_heavy_contention(ib, orc, variant):
             assert abs(h ** 3 * float(f[c].sum()) - G[c].sum()) <= 1e-11 * np.abs(G[c]).sum()
         _close(Up, orc.interp(g, xp, *uvw), f"contention {where} {P} U")
     ctx.close()
+
+
+def test_p2_tet_mesh_force_and_nodal_step(ib, orc):
+    """NEXT-3, second half: P2 tetrahedra (L265) with curved edges, mixed laws, nodal coupling."""
+    import torch
+    conn_hex, X, _, _ = distorted_block(5, 4, 3, size=(0.3, 0.25, 0.2), seed=51, ref_noise=0.1, cur_noise=0.0)
+    c10, X10 = W.p2_from_tets(W.tets_from_hexes(conn_hex, X), X)
+    rng = np.random.default_rng(5)
+    X10[:, X.shape[1]:] += 0.003 * rng.uniform(-1, 1, (3, X10.shape[1] - X.shape[1]))      # curved edges
+    x10 = X10 + 0.004 * rng.uniform(-1, 1, X10.shape)
+    ne, nn = c10.shape[0], X10.shape[1]
+    ef = rng.normal(size=(3, ne))
+    ef /= np.linalg.norm(ef, axis=0)
+    es = np.cross(ef.T, rng.normal(size=(ne, 3))).T
+    es /= np.linalg.norm(es, axis=0)
+    fib = np.concatenate([ef, es])
+    mats = [W.material(W.LAW_MSR, a=8e4, af=1.6e5, bf=2.0e6, kappa=4e6),                    # Cook's membrane law
+            W.material(W.LAW_HO, Ta=20.0, **W.HO_LV), W.material(W.LAW_NEOHOOKEAN, a=1e4, kappa=1e6)]
+    mid = (np.arange(ne) % 3).astype(np.int32)
+    n, h, org = (32, 32, 32), 1 / 32, (0.0, 0.0, 0.0)
+    g = orc.make_grid(*n, h, org)
+    uvw = rng.normal(size=(3, n[0] * n[1] * n[2]))
+    ref_B = orc.fe_force(c10, X10, x10, fib, mid, mats)["B"]
+    ctx = ib.Context(*n, h, org, c10, X10, fib, mid, None, mats)
+    B = torch.empty((3, nn), dtype=torch.float64, device="cuda")
+    ctx.ib_fe_force(_t(x10), B)
+    ctx.check()
+    _close(B, ref_B, "P2 B")
+    f = [torch.empty(n[0] * n[1] * n[2], dtype=torch.float64, device="cuda") for _ in range(3)]
+    Un = torch.empty((3, nn), dtype=torch.float64, device="cuda")
+    ctx.ib_coupling_step(_t(x10), _t(uvw[0]), _t(uvw[1]), _t(uvw[2]), *f, Un, B)
+    ctx.check()
+    ref_f = orc.spread(g, x10, ref_B)
+    for c in range(3):
+        _close(f[c], ref_f[c], f"P2 f{c}")
+    _close(Un, orc.interp(g, x10, *uvw), "P2 Un")
+    ctx.close()

@@ -528,3 +528,84 @@ def test_boundary_loads_pins(orc, kind):
     assert np.allclose(Bk[:, ids], 1e6 * (X - x)[:, ids], rtol=1e-14) and np.count_nonzero(Bk) == 3 * ids.size
     assert abs(E - 0.5e6 * np.sum((x - X)[:, ids] ** 2)) < 1e-12 * E
     assert np.array_equal(orc.tethers(ids, X, X, 1e6, zero)[0], zero)
+
+
+# ---- NEXT-3, second half: P2 tetrahedra (Cook's membrane is discretised with P2 elements, L265) -----
+def _p2_block(seed=6, bend=0.0):
+    conn, X, x, _ = distorted_block(3, 2, 2, seed=seed, ref_noise=0.1, cur_noise=0.0)
+    tets = W.tets_from_hexes(conn, X)
+    c10, X10 = W.p2_from_tets(tets, X)
+    rng = np.random.default_rng(seed)
+    if bend:                                              # curved edges: move the mid-edge nodes a little
+        X10[:, X.shape[1]:] += bend * rng.uniform(-1, 1, (3, X10.shape[1] - X.shape[1]))
+    x10 = X10 + 0.006 * rng.uniform(-1, 1, X10.shape)
+    return c10, X10, x10
+
+
+def test_p2_single_element_closed_form(orc):
+    """Straight-sided P2 tetrahedron under x = F0 X: int grad N_vertex = 0 and int grad N_(ab) =
+    V (grad l_a + grad l_b), so the vertices carry no force and edge (ab) carries -V P (grad l_a + grad l_b)."""
+    X4 = np.array([[0.0, 1.2, 0.1, 0.2], [0.0, 0.1, 0.9, 0.3], [0.0, 0.0, 0.2, 1.1]])
+    c10, X10 = W.p2_from_tets(np.array([[0, 1, 2, 3]], dtype=np.int32), X4)
+    F0 = np.array([[1.1, 0.05, 0.0], [0.0, 0.95, 0.1], [0.02, 0.0, 1.03]])
+    out = orc.fe_force(c10, X10, F0 @ X10, None, None, [NH])
+    P, psi = orc.pk1(NH, F0)
+    D = np.stack([X4[:, 1] - X4[:, 0], X4[:, 2] - X4[:, 0], X4[:, 3] - X4[:, 0]], axis=1)
+    V = np.linalg.det(D) / 6
+    gl = np.linalg.inv(D)                                  # rows: grad l_1, grad l_2, grad l_3
+    gl = np.vstack([-gl.sum(axis=0), gl])                  # grad l_0 = -(sum)
+    B = out["B"]
+    assert np.max(np.abs(B[:, :4])) < 1e-10 * np.max(np.abs(B))
+    for k, (a, b) in enumerate([(0, 1), (1, 2), (0, 2), (0, 3), (1, 3), (2, 3)]):
+        assert np.allclose(B[:, c10[0, 4 + k]], -V * P @ (gl[a] + gl[b]), rtol=1e-12, atol=1e-9)
+    assert abs(out["energy"] - psi * V) < 1e-12 * psi * V
+
+
+@pytest.mark.parametrize("mat", [NH, HO], ids=["NH", "HO"])
+def test_p2_force_is_minus_energy_gradient_and_balances(orc, mat):
+    c10, X10, x10 = _p2_block(bend=0.004)
+    ne = c10.shape[0]
+    rng = np.random.default_rng(3)
+    ef = rng.normal(size=(3, ne))
+    ef /= np.linalg.norm(ef, axis=0)
+    es = np.cross(ef.T, rng.normal(size=(ne, 3))).T
+    es /= np.linalg.norm(es, axis=0)
+    fib = np.concatenate([ef, es])
+    out = orc.fe_force(c10, X10, x10, fib, None, [mat])
+    assert out["rc"] == 0 and out["minJ"] > 0.5
+    B = out["B"]
+    eps = 1e-7
+    for _ in range(12):
+        c, n = rng.integers(0, 3), rng.integers(0, X10.shape[1])
+        xp, xm = x10.copy(), x10.copy()
+        xp[c, n] += eps
+        xm[c, n] -= eps
+        fd = -(orc.fe_force(c10, X10, xp, fib, None, [mat])["energy"]
+               - orc.fe_force(c10, X10, xm, fib, None, [mat])["energy"]) / (2 * eps)
+        assert abs(fd - B[c, n]) < 5e-7 * np.max(np.abs(B)), (c, n)
+    assert np.max(np.abs(B.sum(axis=1))) < 1e-11 * np.max(np.abs(B))
+    assert np.max(np.abs(np.cross(x10.T, B.T).sum(axis=0))) < 1e-10 * np.max(np.abs(B))
+
+
+def test_p2_rigid_motion_and_patch(orc):
+    c10, X10, _ = _p2_block(seed=9)
+    Q, t = rotation(6), np.array([[0.1], [0.4], [-0.3]])
+    B = orc.fe_force(c10, X10, Q @ X10 + t, None, None, [HO])["B"]
+    assert np.max(np.abs(B)) < 1e-12 * HO["kappa"] * 0.1 ** 2
+    F0 = np.array([[1.04, 0.06, -0.02], [0.01, 0.98, 0.04], [-0.03, 0.02, 1.03]])
+    B = orc.fe_force(c10, X10, F0 @ X10, None, None, [NH])["B"]
+    # nodes strictly inside the block (vertices and mid-edge nodes): in balance under a homogeneous deformation
+    lo, hi = X10.min(axis=1, keepdims=True), X10.max(axis=1, keepdims=True)
+    conn_hex, Xh, _, _ = distorted_block(3, 2, 2, seed=9, ref_noise=0.1, cur_noise=0.0)
+    faces = W.boundary_faces(W.tets_from_hexes(conn_hex, Xh))
+    on_bnd = np.zeros(X10.shape[1], bool)
+    on_bnd[np.unique(faces)] = True
+    tets = c10[:, :4]
+    pairs = np.array([[0, 1], [1, 2], [0, 2], [0, 3], [1, 3], [2, 3]])
+    fe = {tuple(sorted(p)) for f in faces for p in ((f[0], f[1]), (f[1], f[2]), (f[0], f[2]))}
+    for t_, row in zip(tets, c10):
+        for k, (a, b) in enumerate(pairs):
+            if tuple(sorted((t_[a], t_[b]))) in fe:
+                on_bnd[row[4 + k]] = True
+    assert (~on_bnd).sum() >= 5
+    assert np.max(np.abs(B[:, ~on_bnd])) < 1e-10 * np.max(np.abs(B[:, on_bnd]))
