@@ -45,15 +45,18 @@ typedef struct ib_ctx ib_ctx;
 typedef enum {
     IB_OK = 0,
     IB_ERR_INVALID_ARG = 1,      /* NULL pointer, negative size, h <= 0, bad mat_id / nsub / dims      */
-    IB_ERR_UNSUPPORTED = 2,      /* periodic == 0; node shared by more than 8 elements                  */
+    IB_ERR_UNSUPPORTED = 2,      /* hex node shared by more than 8 elements; sub-points on tetrahedra   */
     IB_ERR_ALLOC = 3,            /* cudaMalloc / malloc failed                                          */
     IB_ERR_CUDA = 4,             /* a CUDA runtime call failed (no device, launch error)                */
     IB_ERR_INVERTED_ELEMENT = 5, /* det J0 <= 0 or J <= 0 at a Gauss point (reported by ib_check)       */
     IB_ERR_NONFINITE = 6,        /* NaN/Inf position (reported by ib_check)                             */
-    IB_ERR_OUT_OF_DOMAIN = 7     /* reserved for bounded (non-periodic) grids                           */
+    IB_ERR_OUT_OF_DOMAIN = 7     /* point outside a bounded (periodic == 0) grid (reported by ib_check) */
 } ib_status;
 
-/* Uniform MAC grid. periodic must be 1. */
+/* Uniform MAC grid. periodic = 1: indices wrap in all three directions (the configs).
+ * periodic = 0 (NEXT-4; the paper's box has Dirichlet walls, L200; reading A26): the arrays hold the faces
+ * 0..n-1 of every component, a delta support that reaches outside is truncated, and a point outside
+ * [x0, x0 + n h) is skipped (U = 0) and latched as IB_ERR_OUT_OF_DOMAIN. */
 typedef struct {
     int32_t nx, ny, nz;
     double h, x0, y0, z0;

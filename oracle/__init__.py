@@ -25,7 +25,8 @@ class Material(C.Structure):
 
 class Grid(C.Structure):
     _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32),
-                ("h", C.c_double), ("x0", C.c_double), ("y0", C.c_double), ("z0", C.c_double)]
+                ("h", C.c_double), ("x0", C.c_double), ("y0", C.c_double), ("z0", C.c_double),
+                ("periodic", C.c_int32)]
 
 
 def build(force=False):
@@ -72,8 +73,9 @@ def make_materials(mats):
     return arr
 
 
-def make_grid(nx, ny, nz, h, origin=(0.0, 0.0, 0.0)):
-    return Grid(int(nx), int(ny), int(nz), float(h), float(origin[0]), float(origin[1]), float(origin[2]))
+def make_grid(nx, ny, nz, h, origin=(0.0, 0.0, 0.0), periodic=1):
+    return Grid(int(nx), int(ny), int(nz), float(h), float(origin[0]), float(origin[1]), float(origin[2]),
+                int(periodic))
 
 
 def phi(r):

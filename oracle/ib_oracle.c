@@ -43,6 +43,9 @@ typedef struct {
 typedef struct {
     int32_t nx, ny, nz;
     double h, x0, y0, z0;
+    int32_t periodic;       /* 1: indices wrap (configs); 0: bounded box (PAPER.md L200 Dirichlet walls), NEXT-4:
+                               reading A26 -- the arrays hold faces 0..n-1 of every component, a support that
+                               reaches outside is truncated (those faces belong to the wall / do not exist) */
 } oracle_grid;
 
 /* ------------------------------------------------------------------------------------------
@@ -690,6 +693,12 @@ void oracle_restrict(int64_t n_nodes, int64_t n_elems, const int32_t *conn, cons
 static const ld OFFS[3][3] = {{0.0L, 0.5L, 0.5L}, {0.5L, 0.0L, 0.5L}, {0.5L, 0.5L, 0.0L}};
 
 static int64_t wrapi(int64_t i, int64_t n) { i %= n; return i < 0 ? i + n : i; }
+/* index of a support face: wrapped (periodic) or -1 if it lies outside a bounded grid */
+static int64_t facei(const oracle_grid *g, int64_t i, int64_t n)
+{
+    if (g->periodic) return wrapi(i, n);
+    return (i < 0 || i >= n) ? -1 : i;
+}
 
 static void support(const oracle_grid *g, int c, const ld xpt[3], int64_t i0[3], ld wt[3][4])
 {
@@ -719,7 +728,8 @@ void oracle_spread(const oracle_grid *g, int64_t P, const double *xp, const doub
             for (int m3 = 0; m3 < 4; ++m3)
                 for (int m2 = 0; m2 < 4; ++m2)
                     for (int m1 = 0; m1 < 4; ++m1) {
-                        int64_t i = wrapi(i0[0] + m1, g->nx), j = wrapi(i0[1] + m2, g->ny), k = wrapi(i0[2] + m3, g->nz);
+                        int64_t i = facei(g, i0[0] + m1, g->nx), j = facei(g, i0[1] + m2, g->ny), k = facei(g, i0[2] + m3, g->nz);
+                        if (i < 0 || j < 0 || k < 0) continue;
                         acc[(k * g->ny + j) * g->nx + i] += G * wt[0][m1] * wt[1][m2] * wt[2][m3] / h3;
                     }
         }
@@ -741,7 +751,8 @@ void oracle_interp(const oracle_grid *g, int64_t P, const double *xp, const doub
             for (int m3 = 0; m3 < 4; ++m3)
                 for (int m2 = 0; m2 < 4; ++m2)
                     for (int m1 = 0; m1 < 4; ++m1) {
-                        int64_t i = wrapi(i0[0] + m1, g->nx), j = wrapi(i0[1] + m2, g->ny), k = wrapi(i0[2] + m3, g->nz);
+                        int64_t i = facei(g, i0[0] + m1, g->nx), j = facei(g, i0[1] + m2, g->ny), k = facei(g, i0[2] + m3, g->nz);
+                        if (i < 0 || j < 0 || k < 0) continue;
                         s += (ld)f[c][(k * g->ny + j) * g->nx + i] * wt[0][m1] * wt[1][m2] * wt[2][m3];
                     }
             Up[c * P + p] = (double)s;
@@ -772,7 +783,8 @@ void oracle_spread_brute(const oracle_grid *g, int64_t P, const double *xp, cons
                     face_coord(g, c, i, j, k, xf);
                     for (int64_t p = 0; p < P; ++p) {
                         ld wgt = 1.0L;
-                        for (int d = 0; d < 3; ++d) wgt *= phi_l(min_image(xf[d] - (ld)xp[d * P + p], L[d]) / h);
+                        for (int d = 0; d < 3; ++d)
+                            wgt *= phi_l((g->periodic ? min_image(xf[d] - (ld)xp[d * P + p], L[d]) : xf[d] - (ld)xp[d * P + p]) / h);
                         s += (ld)Gp[c * P + p] * wgt / (h * h * h);
                     }
                     f[c][(k * g->ny + j) * g->nx + i] = (double)s;
@@ -792,7 +804,8 @@ void oracle_interp_brute(const oracle_grid *g, int64_t P, const double *xp, cons
                     for (int64_t i = 0; i < g->nx; ++i) {
                         ld xf[3], wgt = 1.0L;
                         face_coord(g, c, i, j, k, xf);
-                        for (int d = 0; d < 3; ++d) wgt *= phi_l(min_image(xf[d] - (ld)xp[d * P + p], L[d]) / h);
+                        for (int d = 0; d < 3; ++d)
+                            wgt *= phi_l((g->periodic ? min_image(xf[d] - (ld)xp[d * P + p], L[d]) : xf[d] - (ld)xp[d * P + p]) / h);
                         s += (ld)f[c][(k * g->ny + j) * g->nx + i] * wgt;
                     }
             Up[c * P + p] = (double)s;

@@ -82,6 +82,12 @@ ibk_bin_cloud(ib_bin_params pr)
                 if (pr.Up) { pr.Up[p] = 0.0; pr.Up[P + p] = 0.0; pr.Up[2 * P + p] = 0.0; }
             }
             valid = false;
+        } else if (!pr.g.periodic && !ib_in_box(x, y, z, pr.g, pr.inv_h)) {
+            if (SCATTER) {
+                ib_latch(pr.status, IB_ERR_OUT_OF_DOMAIN, p);
+                if (pr.Up) { pr.Up[p] = 0.0; pr.Up[P + p] = 0.0; pr.Up[2 * P + p] = 0.0; }
+            }
+            valid = false;
         }
     }
     int tile = valid ? ib_tile_of(x, y, z, pr.g, pr.inv_h) : 0;
@@ -213,9 +219,10 @@ ibk_bin_mesh(ib_bin_params pr)
     if (live) {
         for (int j = 0; j < n1; ++j) {
             double t = ((double)j + 0.5) * rn1;
-            int tl = ib_tile_of(__fma_rn(t, D[0], L[0]), __fma_rn(t, D[1], L[1]), __fma_rn(t, D[2], L[2]), pr.g, pr.inv_h);
+            const double xj = __fma_rn(t, D[0], L[0]), yj = __fma_rn(t, D[1], L[1]), zj = __fma_rn(t, D[2], L[2]);
+            int tl = ib_tile_of(xj, yj, zj, pr.g, pr.inv_h);
             if (j == 0) tile0 = tl;
-            same = same && (tl == tile0);
+            same = same && (tl == tile0) && (pr.g.periodic || ib_in_box(xj, yj, zj, pr.g, pr.inv_h));
         }
     }
     const bool warp_same = __all_sync(full, same) && __all_sync(full, !live || n1 == nmax);
@@ -242,6 +249,13 @@ ibk_bin_mesh(ib_bin_params pr)
         int pos;
         if (warp_same) pos = base + j * pstride;
         else {
+            if (valid && !pr.g.periodic && !ib_in_box(x, y, z, pr.g, pr.inv_h)) {      // outside a bounded grid
+                if (SCATTER) {
+                    ib_latch(pr.status, IB_ERR_OUT_OF_DOMAIN, e);
+                    if (pr.Up) { pr.Up[p0 + j] = 0.0; pr.Up[pr.P + p0 + j] = 0.0; pr.Up[2 * pr.P + p0 + j] = 0.0; }
+                }
+                valid = false;
+            }
             int tile = valid ? ib_tile_of(x, y, z, pr.g, pr.inv_h) : 0;
             pos = ib_bin_slot<SCATTER>(valid, tile, pr.tile_cur);
         }

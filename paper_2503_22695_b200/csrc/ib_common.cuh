@@ -165,6 +165,14 @@ __device__ __forceinline__ int ib_cell(double x, double x0, double inv_h, int n)
     return (int)c;
 }
 
+// bounded grid (periodic == 0, reading A26): is the point inside the box [x0, x0 + n h)^3 ?
+__device__ __forceinline__ bool ib_in_box(double x, double y, double z, const ib_grid_desc &g, double inv_h)
+{
+    const double fx = floor(__dmul_rn(__dsub_rn(x, g.x0), inv_h)), fy = floor(__dmul_rn(__dsub_rn(y, g.y0), inv_h)),
+                 fz = floor(__dmul_rn(__dsub_rn(z, g.z0), inv_h));
+    return fx >= 0.0 && fx < (double)g.nx && fy >= 0.0 && fy < (double)g.ny && fz >= 0.0 && fz < (double)g.nz;
+}
+
 // Q1 shape functions at xi (local node a = ia + 2 ja + 4 ka)
 __device__ __forceinline__ void ib_shape(double x0, double x1, double x2, double N[8])
 {

@@ -138,7 +138,6 @@ extern "C" ib_status ib_create(ib_ctx **out, const ib_grid_desc *g, const ib_mes
     if (!(g->h > 0.0) || !std::isfinite(g->h) || !std::isfinite(g->x0) || !std::isfinite(g->y0) || !std::isfinite(g->z0))
         return IB_ERR_INVALID_ARG;
     if ((int64_t)g->nx * g->ny * g->nz > (int64_t)INT32_MAX) return IB_ERR_INVALID_ARG;
-    if (!g->periodic) return IB_ERR_UNSUPPORTED;
     if (m->n_nodes < 0 || m->n_elems < 0 || m->n_nodes > INT32_MAX || m->n_elems > INT32_MAX / 8) return IB_ERR_INVALID_ARG;
     if (m->n_elems > 0 && (!m->conn || !m->X_ref || !m->mats || m->n_mats <= 0)) return IB_ERR_INVALID_ARG;
     if (m->elem_type < IB_ELEM_HEX8 || m->elem_type > IB_ELEM_TET10) return IB_ERR_INVALID_ARG;

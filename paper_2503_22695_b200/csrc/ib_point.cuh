@@ -9,7 +9,8 @@ struct ib_stencil {
     double wx[2][4], wy[2][4], wz[2][4];
 };
 
-__device__ __forceinline__ void ib_axis(double x, double x0, double h, double inv_h, int n,
+// periodic == 0: faces outside 0..n-1 do not exist (index -1: skipped by the caller)
+__device__ __forceinline__ void ib_axis(double x, double x0, double h, double inv_h, int n, int periodic,
                                         int idx[2][4], double wt[2][4])
 {
     double sf = ib_scaled(x, x0, h, inv_h);
@@ -18,11 +19,19 @@ __device__ __forceinline__ void ib_axis(double x, double x0, double h, double in
         double s = o ? sf - 0.5 : sf;
         double fl = floor(s);
         ib_phi4(s - fl, wt[o]);
-        int i0 = ib_wrap((int)fl - 1, n);
+        if (periodic) {
+            int i0 = ib_wrap((int)fl - 1, n);
 #pragma unroll
-        for (int m = 0; m < 4; ++m) {
-            int i = i0 + m;
-            idx[o][m] = i >= n ? i - n : i;
+            for (int m = 0; m < 4; ++m) {
+                int i = i0 + m;
+                idx[o][m] = i >= n ? i - n : i;
+            }
+        } else {
+#pragma unroll
+            for (int m = 0; m < 4; ++m) {
+                int i = (int)fl - 1 + m;
+                idx[o][m] = (i < 0 || i >= n) ? -1 : i;
+            }
         }
     }
 }
@@ -34,9 +43,9 @@ __device__ __forceinline__ void ib_point_direct(double x, double y, double z, co
                                                 const ib_grid_desc &g, double inv_h, double U[3])
 {
     ib_stencil s;
-    ib_axis(x, g.x0, g.h, inv_h, g.nx, s.ix, s.wx);
-    ib_axis(y, g.y0, g.h, inv_h, g.ny, s.iy, s.wy);
-    ib_axis(z, g.z0, g.h, inv_h, g.nz, s.iz, s.wz);
+    ib_axis(x, g.x0, g.h, inv_h, g.nx, g.periodic, s.ix, s.wx);
+    ib_axis(y, g.y0, g.h, inv_h, g.ny, g.periodic, s.iy, s.wy);
+    ib_axis(z, g.z0, g.h, inv_h, g.nz, g.periodic, s.iz, s.wz);
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         const int ox = (c == 0) ? 0 : 1, oy = (c == 1) ? 0 : 1, oz = (c == 2) ? 0 : 1;
@@ -47,17 +56,20 @@ __device__ __forceinline__ void ib_point_direct(double x, double y, double z, co
             double ak = 0.0;
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
+                if (s.iz[oz][k] < 0 || s.iy[oy][j] < 0) continue;           // outside a bounded grid
                 int64_t row = ((int64_t)s.iz[oz][k] * g.ny + s.iy[oy][j]) * g.nx;
                 if (DO_INTERP) {
                     double r = 0.0;
 #pragma unroll
-                    for (int i = 0; i < 4; ++i) r = fma(__ldg(fld[c] + row + s.ix[ox][i]), s.wx[ox][i], r);
+                    for (int i = 0; i < 4; ++i)
+                        if (s.ix[ox][i] >= 0) r = fma(__ldg(fld[c] + row + s.ix[ox][i]), s.wx[ox][i], r);
                     ak = fma(r, s.wy[oy][j], ak);
                 }
                 if (DO_SPREAD) {
                     double gjk = gk * s.wy[oy][j];
 #pragma unroll
-                    for (int i = 0; i < 4; ++i) atomicAdd(frc[c] + row + s.ix[ox][i], gjk * s.wx[ox][i]);
+                    for (int i = 0; i < 4; ++i)
+                        if (s.ix[ox][i] >= 0) atomicAdd(frc[c] + row + s.ix[ox][i], gjk * s.wx[ox][i]);
                 }
             }
             if (DO_INTERP) acc = fma(ak, s.wz[oz][k], acc);

@@ -23,6 +23,11 @@ ibk_point_kernel(int64_t P, const double *__restrict__ xp, const double *__restr
         if (DO_INTERP) { Up[p] = 0.0; Up[P + p] = 0.0; Up[2 * P + p] = 0.0; }
         return;
     }
+    if (!g.periodic && !ib_in_box(x, y, z, g, inv_h)) {
+        ib_latch(status, IB_ERR_OUT_OF_DOMAIN, p);
+        if (DO_INTERP) { Up[p] = 0.0; Up[P + p] = 0.0; Up[2 * P + p] = 0.0; }
+        return;
+    }
     const double ih3 = inv_h * inv_h * inv_h;
     double G[3] = {0, 0, 0}, U[3];
     if (DO_SPREAD) { G[0] = __ldg(Gp + p) * ih3; G[1] = __ldg(Gp + P + p) * ih3; G[2] = __ldg(Gp + 2 * P + p) * ih3; }

@@ -88,7 +88,8 @@ __device__ __forceinline__ int ib_octant_key(double a, double b, double c)
     return (hz * 8 + hy) * 8 + hx;
 }
 
-template <int DO_SPREAD, int DO_INTERP>
+// PER: periodic grid (compile-time, so that the periodic kernel carries none of the wall predicates)
+template <int DO_SPREAD, int DO_INTERP, int PER>
 __global__ void __launch_bounds__(TB, NCTA)
 ibk_tiled_kernel(ib_tiled_params pr)
 {
@@ -134,7 +135,7 @@ ibk_tiled_kernel(ib_tiled_params pr)
         const int t3[3] = {tile % ntx, (tile / ntx) % nty, tile / (ntx * nty)};
         int h0[3];                                       // halo origin (global index of halo entry 0), wrapped
 #pragma unroll
-        for (int d = 0; d < 3; ++d) h0[d] = ib_wrap(TT * t3[d] - 2, n[d]);
+        for (int d = 0; d < 3; ++d) h0[d] = PER ? ib_wrap(TT * t3[d] - 2, n[d]) : TT * t3[d] - 2;
 
         // ---- halo load, zero the accumulators ---------------------------------------------------
 #ifndef IB_NO_HALO
@@ -142,8 +143,11 @@ ibk_tiled_kernel(ib_tiled_params pr)
             for (int idx = tid; idx < 3 * TH3; idx += TB) {
                 int c = idx >> 9, r = idx & 511;
                 int i = h0[0] + (r & 7), j = h0[1] + ((r >> 3) & 7), k = h0[2] + (r >> 6);
-                i -= (i >= n[0]) ? n[0] : 0; j -= (j >= n[1]) ? n[1] : 0; k -= (k >= n[2]) ? n[2] : 0;
-                su[c * SU3 + (r >> 6) * SZ + (r & 63)] = __ldg(pr.fld[c] + ((int64_t)k * n[1] + j) * n[0] + i);
+                double val = 0.0;                        // faces outside a bounded grid read as zero (never used: weight dropped)
+                if (PER) { i -= (i >= n[0]) ? n[0] : 0; j -= (j >= n[1]) ? n[1] : 0; k -= (k >= n[2]) ? n[2] : 0; }
+                if (PER || (i >= 0 && i < n[0] && j >= 0 && j < n[1] && k >= 0 && k < n[2]))
+                    val = __ldg(pr.fld[c] + ((int64_t)k * n[1] + j) * n[0] + i);
+                su[c * SU3 + (r >> 6) * SZ + (r & 63)] = val;
             }
         }
 #endif
@@ -405,12 +409,19 @@ ibk_tiled_kernel(ib_tiled_params pr)
                 if (DO_SPREAD && have) {
 #endif
                     // lane q flushes x-column q: for every (y,z) the 4 lanes of the group hit 4 consecutive faces
-                    int gi = h0[0] + o3[0] + q; gi -= (gi >= n[0]) ? n[0] : 0;
+                    // (bounded grid: faces outside 0..n-1 do not exist -- their share of the force is dropped, A26)
+                    constexpr bool per = PER != 0;
+                    int gi = h0[0] + o3[0] + q;
+                    if (per) gi -= (gi >= n[0]) ? n[0] : 0;
+                    const bool xin = per || (gi >= 0 && gi < n[0]);
                     int gj[4], gk[4];
+                    bool jin[4], kin[4];
 #pragma unroll
                     for (int m = 0; m < 4; ++m) {
-                        gj[m] = h0[1] + o3[1] + m; gj[m] -= (gj[m] >= n[1]) ? n[1] : 0;
-                        gk[m] = h0[2] + o3[2] + m; gk[m] -= (gk[m] >= n[2]) ? n[2] : 0;
+                        gj[m] = h0[1] + o3[1] + m; gk[m] = h0[2] + o3[2] + m;
+                        if (per) { gj[m] -= (gj[m] >= n[1]) ? n[1] : 0; gk[m] -= (gk[m] >= n[2]) ? n[2] : 0; }
+                        jin[m] = per || (gj[m] >= 0 && gj[m] < n[1]);
+                        kin[m] = per || (gk[m] >= 0 && gk[m] < n[2]);
                     }
                     double *fp = pr.frc[c] + gi;
                     int ok[4], oj[4];                                  // 32-bit face offsets (n_cells < 2^31)
@@ -419,7 +430,8 @@ ibk_tiled_kernel(ib_tiled_params pr)
 #pragma unroll
                     for (int i = 0; i < 4; ++i)
 #pragma unroll
-                        for (int j = 0; j < 4; ++j) atomicAdd(fp + (ok[i] + oj[j]), ff[j][i]);
+                        for (int j = 0; j < 4; ++j)
+                            if (xin && kin[i] && jin[j]) atomicAdd(fp + (ok[i] + oj[j]), ff[j][i]);
                 }
             }
         }
@@ -449,15 +461,15 @@ ibk_small_tiles(ib_tiled_params pr, const int32_t *__restrict__ small_rec, const
     }
 }
 
-template <int S, int I>
-static ib_status launch_tiled(ib_ctx *c, const ib_tiled_params &pr, cudaStream_t st)
+template <int S, int I, int PER>
+static ib_status launch_tiled_p(ib_ctx *c, const ib_tiled_params &pr, cudaStream_t st)
 {
     static int configured = 0;
     const size_t smem = (size_t)(3 * SU3 + 3 * CH + NWARP * 8 * GSTRIDE) * sizeof(double) +
                         (NOC + 68) * sizeof(int) + (516 + 2 * NITEM + CH) * sizeof(unsigned short);
     static_assert(CH % TB == 0, "chunk must be a whole number of points per thread");
     if (!configured) {
-        IB_CUDA_TRY(cudaFuncSetAttribute(ibk_tiled_kernel<S, I>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        IB_CUDA_TRY(cudaFuncSetAttribute(ibk_tiled_kernel<S, I, PER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         configured = 1;
     }
     static int sms = 0;
@@ -476,10 +488,16 @@ static ib_status launch_tiled(ib_ctx *c, const ib_tiled_params &pr, cudaStream_t
     }
     ibk_small_tiles<S, I><<<ib_blocks(nsmall_max, 128), 128, 0, s3>>>(pr, c->d_small_rec, c->d_tile_count);
     if (beside) IB_CUDA_TRY(cudaEventRecord(c->ev_sjoin, s3));
-    ibk_tiled_kernel<S, I><<<sms * NCTA, TB, smem, st>>>(pr);
+    ibk_tiled_kernel<S, I, PER><<<sms * NCTA, TB, smem, st>>>(pr);
     if (beside) IB_CUDA_TRY(cudaStreamWaitEvent(st, c->ev_sjoin, 0));
     c->launches += 2;
     return IB_OK;
+}
+
+template <int S, int I>
+static ib_status launch_tiled(ib_ctx *c, const ib_tiled_params &pr, cudaStream_t st)
+{
+    return c->grid.periodic ? launch_tiled_p<S, I, 1>(c, pr, st) : launch_tiled_p<S, I, 0>(c, pr, st);
 }
 
 // mesh != 0: points are the sub-points of the mesh at node positions x with force coefficients Fhat

@@ -559,3 +559,53 @@ def test_p2_tet_mesh_force_and_nodal_step(ib, orc):
         _close(f[c], ref_f[c], f"P2 f{c}")
     _close(Un, orc.interp(g, x10, *uvw), "P2 Un")
     ctx.close()
+
+
+# ---- NEXT-4, second half: bounded (non-periodic) grid, supports truncated at the walls (A26) -------
+@pytest.mark.parametrize("variant", [0, 1])
+def test_bounded_grid_cloud_and_mesh(ib, orc, variant):
+    import torch
+    n, h, org = (24, 16, 32), 0.05, (-0.4, 0.1, 0.3)
+    L = np.array(n) * h
+    g = orc.make_grid(*n, h, org, periodic=0)
+    rng = np.random.default_rng(13)
+    ncell = n[0] * n[1] * n[2]
+    uvw = rng.normal(size=(3, ncell))
+    # a cloud filling the box right up to the walls (dense near two corners), one point outside
+    P = 30011
+    xp = np.asarray(org)[:, None] + rng.uniform(0.0, 1.0, (3, P)) * L[:, None]
+    xp[:, :4000] = np.asarray(org)[:, None] + rng.uniform(0.0, 1.9 * h, (3, 4000))
+    xp[:, 4000:8000] = (np.asarray(org) + L)[:, None] - rng.uniform(1e-9, 1.9 * h, (3, 4000))
+    G = rng.normal(size=(3, P))
+    ctx = ib.Context(*n, h, org, np.zeros((0, 8), np.int32), np.zeros((3, 0)), None, None, None, [], periodic=0)
+    ctx.ib_set_variant(variant)
+    f = [torch.empty(ncell, dtype=torch.float64, device="cuda") for _ in range(3)]
+    Up = torch.empty((3, P), dtype=torch.float64, device="cuda")
+    ctx.ib_spread(_t(xp), _t(G), P, *f, accumulate=0)
+    ctx.ib_interp(_t(xp), P, _t(uvw[0]), _t(uvw[1]), _t(uvw[2]), Up)
+    ctx.check()
+    fr = orc.spread(g, xp, G)
+    for c in range(3):
+        _close(f[c], fr[c], f"bounded v{variant} f{c}")
+    _close(Up, orc.interp(g, xp, *uvw), f"bounded v{variant} U")
+    xo = xp.copy()
+    xo[0, 17] = org[0] - 0.3 * h                                  # outside the box: latched, skipped, U = 0
+    ctx.ib_interp(_t(xo), P, _t(uvw[0]), _t(uvw[1]), _t(uvw[2]), Up)
+    code, bad = ctx.ib_check()
+    assert code == 7 and bad == 17 and float(Up[:, 17].abs().max()) == 0.0
+    ctx.close()
+    # a structure pushed into the corner of the box: sub-point coupling through the whole step
+    wl = W.config1()
+    shift = np.asarray(wl.origin) - wl.X.min(axis=1) + 0.3 * wl.h         # 0.3 h from three walls
+    X, x = wl.X + shift[:, None], wl.x + shift[:, None]
+    gb = orc.make_grid(wl.nx, wl.ny, wl.nz, wl.h, wl.origin, periodic=0)
+    ref = orc.coupling_step(gb, wl.conn, X, wl.fibers, wl.mat_id, wl.nsub, wl.mats, x, wl.u, wl.v, wl.w)
+    ctx = ib.Context(wl.nx, wl.ny, wl.nz, wl.h, wl.origin, wl.conn, X, wl.fibers, wl.mat_id, wl.nsub, wl.mats, periodic=0)
+    ctx.ib_set_variant(variant)
+    fo = [torch.empty(wl.n_cells, dtype=torch.float64, device="cuda") for _ in range(3)]
+    Un, B = (torch.empty((3, wl.n_nodes), dtype=torch.float64, device="cuda") for _ in range(2))
+    ctx.ib_coupling_step(_t(x), _t(wl.u), _t(wl.v), _t(wl.w), *fo, Un, B)
+    ctx.check()
+    for k, t in (("B", B), ("fu", fo[0]), ("fv", fo[1]), ("fw", fo[2]), ("Un", Un)):
+        _close(t, ref[k], f"bounded step v{variant} {k}")
+    ctx.close()

@@ -190,3 +190,40 @@ def test_bin_sort_keys_and_stability(orc):
     # empty input
     k0, p0 = orc.bin_sort(g, np.zeros((3, 0)))
     assert k0.size == 0 and p0.size == 0
+
+
+# ---- NEXT-4, second half: bounded (non-periodic) grid, reading A26 --------------------------------
+def test_bounded_grid_truncates_supports(orc):
+    """periodic=0: faces 0..n-1 exist, a support reaching outside is cut.  Pins: brute force over all
+    faces with plain (not minimum-image) distances; identical to the periodic result away from the walls;
+    a point half a cell from the wall keeps exactly the in-box share of its force (closed form)."""
+    n, h, org = (8, 12, 8), 0.125, (-0.5, 0.0, 1.0)
+    gb, gp = orc.make_grid(*n, h, org, periodic=0), orc.make_grid(*n, h, org, periodic=1)
+    rng = np.random.default_rng(4)
+    L = np.array(n) * h
+    P = 60
+    xp = np.asarray(org)[:, None] + rng.uniform(0.0, 1.0, (3, P)) * L[:, None]      # anywhere in the box, walls included
+    G = rng.normal(size=(3, P))
+    uvw = rng.normal(size=(3, n[0] * n[1] * n[2]))
+    f, fb = orc.spread(gb, xp, G), orc.spread(gb, xp, G, brute=True)
+    for c in range(3):
+        assert np.max(np.abs(f[c] - fb[c])) < 1e-13 * np.max(np.abs(fb[c]))
+    U, Ub = orc.interp(gb, xp, *uvw), orc.interp(gb, xp, *uvw, brute=True)
+    assert np.max(np.abs(U - Ub)) < 1e-14 * np.max(np.abs(Ub))
+    # adjointness survives the truncation (the same faces are dropped on both sides)
+    lhs = h ** 3 * sum(np.dot(f[c], uvw[c]) for c in range(3))
+    assert abs(lhs - np.sum(G * U)) < 1e-13 * np.sum(np.abs(G * U))
+    # interior points (>= 2.5 h from every wall): same as periodic
+    inner = np.asarray(org)[:, None] + 2.5 * h + rng.uniform(0, 1, (3, P)) * (L - 5 * h)[:, None]
+    for a, b in zip(orc.spread(gb, inner, G), orc.spread(gp, inner, G)):
+        assert np.array_equal(a, b)
+    assert np.array_equal(orc.interp(gb, inner, *uvw), orc.interp(gp, inner, *uvw))
+    # closed form: point at the centre of the corner cell (0,0,0), force (1,1,1).
+    # face-aligned weights [a,b,b,a] at faces -1..2 -> the face -1 is outside: share 1-a, a = (2-sqrt2)/8;
+    # centre-aligned weights [1/4,1/2,1/4,0] at -1..2 -> share 3/4
+    x1 = (np.asarray(org) + 0.5 * h)[:, None]
+    f1 = orc.spread(gb, x1, np.ones((3, 1)))
+    al = (2 - np.sqrt(2)) / 8
+    for c in range(3):
+        assert abs(h ** 3 * f1[c].sum() - (1 - al) * 0.75 * 0.75) < 1e-15
+    assert abs(h ** 3 * orc.spread(gp, x1, np.ones((3, 1)))[0].sum() - 1.0) < 1e-15       # periodic keeps all of it
