@@ -38,8 +38,12 @@ def test_argument_validation_without_a_gpu():
     assert L.ib_create(ctypes.byref(h), ctypes.byref(g), ctypes.byref(md), 0) == 1
     g = ibcouple.GridDesc(32, 32, 32, -0.1, 0, 0, 0, 1)
     assert L.ib_create(ctypes.byref(h), ctypes.byref(g), ctypes.byref(md), 0) == 1
-    g = ibcouple.GridDesc(32, 32, 32, 0.1, 0, 0, 0, 0)          # bounded grids: unsupported
-    assert L.ib_create(ctypes.byref(h), ctypes.byref(g), ctypes.byref(md), 0) == 2
+    g = ibcouple.GridDesc(32, 32, 32, 0.1, 0, 0, 0, 0)          # a bounded grid is fine ...
+    dummy = (ctypes.c_int32 * 3)(1, 1, 1)
+    md_t = ibcouple.MeshDesc(0, 0, None, None, None, None, ctypes.cast(dummy, ctypes.c_void_p), None, 0, 1)
+    assert L.ib_create(ctypes.byref(h), ctypes.byref(g), ctypes.byref(md_t), 0) == 2     # ... sub-points on tets are not
+    md_bad = ibcouple.MeshDesc(0, 0, None, None, None, None, None, None, 0, 7)            # unknown element type
+    assert L.ib_create(ctypes.byref(h), ctypes.byref(g), ctypes.byref(md_bad), 0) == 1
     assert L.ib_create(None, ctypes.byref(g), ctypes.byref(md), 0) == 1
     assert L.ib_fe_force(None, None, None, None) == 1
     assert L.ib_destroy(None) == 1
