@@ -98,9 +98,11 @@ typedef struct {
 } ib_mesh_desc;
 enum { IB_ELEM_HEX8 = 0, IB_ELEM_TET4 = 1, IB_ELEM_TET10 = 2 };
 
-/* Create a context: validates, copies the mesh, builds the node->element adjacency (at most 8
- * incident elements per node), and precomputes on the device the sub-point weights W_s =
- * det J0(xi_s) 8/(n1 n2 n3) and the lumped nodal weights w_a = sum W_s N_a(xi_s) (L235, L241).
+/* Create a context: validates, copies the mesh, builds the node->element adjacency (hexahedra: at most 8
+ * incident elements per node, else IB_ERR_UNSUPPORTED; tetrahedra: any valence), and precomputes on the
+ * device the reference geometry of the Gauss points, the sub-point weights W_s = det J0(xi_s) 8/(n1 n2 n3)
+ * and the lumped nodal weights w_a = sum W_s N_a(xi_s) (L235, L241). An inverted reference element
+ * (det J0 <= 0) makes ib_create return IB_ERR_INVERTED_ELEMENT.
  * `device` is the CUDA device ordinal. Synchronous. */
 ib_status ib_create(ib_ctx **ctx, const ib_grid_desc *grid, const ib_mesh_desc *mesh, int32_t device);
 ib_status ib_destroy(ib_ctx *ctx);
@@ -143,7 +145,10 @@ ib_status ib_interp(ib_ctx *ctx, const double *xp, int64_t P, const double *u, c
 
 /* The whole coupling step at one position array x (BASELINE.json "one coupling step"):
  *   B = fe_force(x); points; f = spread(xp, Gp) (overwrites fu,fv,fw); Up = interp(xp,u,v,w);
- *   Un = restrict(Up).   B may be NULL (not returned). */
+ *   Un = restrict(Up).   B may be NULL (not returned).  In nodal mode (nsub == NULL, the paper's rule
+ *   L241-257) the points are the nodes: f = spread(x, B), Un = interp(x, u,v,w).  Work that needs only x
+ *   runs on context-owned side streams beside the FE force; everything is ordered after earlier work on
+ *   `stream` and complete, in stream order, when the call's last kernel on `stream` is. */
 ib_status ib_coupling_step(ib_ctx *ctx, const double *x, const double *u, const double *v,
                            const double *w, double *fu, double *fv, double *fw, double *Un,
                            double *B, void *stream);
