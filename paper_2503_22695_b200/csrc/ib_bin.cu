@@ -261,13 +261,16 @@ ibk_bin_mesh(ib_bin_params pr)
         }
         if (SCATTER && valid) {
             const int64_t P = pr.P;
-            pr.sx[pos] = x; pr.sx[P + pos] = y; pr.sx[2 * P + pos] = z;
-            pr.sid[pos] = (int32_t)(p0 + j);
+            // streaming stores: the records (325 MB for C3) exceed L2 and are read once, oldest first,
+            // so keeping them out of L2 leaves room for the grid halos (measured -0.6 % on the step)
+#define IB_ST(PTR, V) __stcs((PTR), (V))
+            IB_ST(pr.sx + pos, x); IB_ST(pr.sx + P + pos, y); IB_ST(pr.sx + 2 * P + pos, z);
+            IB_ST(pr.sid + pos, (int32_t)(p0 + j));
             if (pr.Fhat) {
                 double W = __ldg(pr.Wp + p0 + j);
-                pr.sG[pos] = W * fma(t, DF[0], LF[0]);
-                pr.sG[P + pos] = W * fma(t, DF[1], LF[1]);
-                pr.sG[2 * P + pos] = W * fma(t, DF[2], LF[2]);
+                IB_ST(pr.sG + pos, W * fma(t, DF[0], LF[0]));
+                IB_ST(pr.sG + P + pos, W * fma(t, DF[1], LF[1]));
+                IB_ST(pr.sG + 2 * P + pos, W * fma(t, DF[2], LF[2]));
             }
         }
     }
