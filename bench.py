@@ -280,6 +280,19 @@ def run_ours(args):
     prof = ctx.ib_profile_read()
     ctx.ib_profile_enable(False)
     value, t_dev = whole_job_value(wl.n_points, args.steps, float(np.sum(ms)) * 1e-3, world, dev)
+    # run-to-run deviation: the REDs of the spreading reorder the sums, so three
+    # untimed runs on the same inputs are compared; B and the bin counts are order-free
+    runs = []
+    for _ in range(3):
+        step()
+        torch.cuda.synchronize()
+        runs.append([a.clone() for a in (fu, fv, fw, Un)])
+    dev_rr = {}
+    for k, name in enumerate(("fu", "fv", "fw", "Un")):
+        scale = float(runs[0][k].abs().max())
+        d = max(float((runs[i][k] - runs[0][k]).abs().max()) for i in (1, 2))
+        dev_rr[name] = d / scale if scale > 0 else 0.0
+    del runs
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
@@ -352,9 +365,10 @@ def run_ours(args):
                            "input_sha256": wl.sha256()},
                 "clocks": clocks,
                 "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                        "steps": e2e_steps, "api": "ib_coupling_step_host (pinned host buffers; spread and interpolation pipelined around the copies on two streams)"},
+                        "steps": e2e_steps, "api": "ib_coupling_step_host (pinned host buffers; the step is pipelined in 8 z-slabs: H2D of u,v,w, fused spread + interpolate per slab, D2H of the finished f layers)"},
                 "gpu_launches": int(launches),
                 "wall_s_timed_region": t_wall,
+                "run_to_run": {"runs": 3, "max_abs_dev_over_max_abs": dev_rr},
                 "roofline": roofline,
                 "cpu_baseline": {"value": s["n_points"] / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
                                  "sample": sample}}

@@ -332,7 +332,7 @@ ibk_tile_partials(const int32_t *__restrict__ tile_cur, int n_tiles, int chunk, 
 __global__ void __launch_bounds__(SCT)
 ibk_tile_scan(int32_t *__restrict__ tile_cur, int n_tiles, int chunk, const int2 *__restrict__ partial,
               int32_t *__restrict__ tile_start, int4 *__restrict__ work, int32_t *__restrict__ small_rec,
-              int32_t *__restrict__ counters)
+              int32_t *__restrict__ counters, int slab_tiles)
 {
     __shared__ int ws[33], wl[33];
     __shared__ int base_s, base_l, base_m;
@@ -350,6 +350,9 @@ ibk_tile_scan(int32_t *__restrict__ tile_cur, int n_tiles, int chunk, const int2
     int ts, tl;
     ib_block_scan2(s, l, ws, wl, ts, tl);          // includes the barrier that publishes base_s/base_l
     s += base_s; l += base_l;
+    // first work item of every slab of slab_tiles tiles (a multiple of SCI): ib_coupling_step_host launches
+    // the tile kernel slab by slab so that the copies of f overlap the spreading of the next slab
+    if (t0 < n_tiles && t0 % slab_tiles == 0) counters[IB_SLAB0 + t0 / slab_tiles] = l;
     if (t0 < n_tiles) {
         int4 st = make_int4(s, s + c.x, s + c.x + c.y, s + c.x + c.y + c.z);
         *reinterpret_cast<int4 *>(tile_start + t0) = st;
@@ -383,6 +386,7 @@ ibk_tile_scan(int32_t *__restrict__ tile_cur, int n_tiles, int chunk, const int2
         tile_start[n_tiles] = base_s + ts;
         counters[0] = base_l + tl;
         counters[1] = 0;
+        for (int k = (n_tiles + slab_tiles - 1) / slab_tiles; k <= IB_MAX_SLABS; ++k) counters[IB_SLAB0 + k] = base_l + tl;
     }
 }
 
@@ -411,12 +415,13 @@ ib_status ibk_bin_points(ib_ctx *c, int mesh, const double *xp, const double *Gp
         else if (mesh) ibk_bin_mesh<0, 0><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
         else ibk_bin_cloud<0><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
         const int nsb = (n_tiles + SCT * SCI - 1) / (SCT * SCI);
-        int2 *partial = reinterpret_cast<int2 *>(c->d_tile_count + 16);
+        int2 *partial = reinterpret_cast<int2 *>(c->d_tile_count + IB_TILE_HDR);
         // ~4 work items per resident CTA of the tile kernel when the cloud is small
         int chunk = (int)((P / 1200 + 63) / 64 * 64);
         chunk = chunk < 192 ? 192 : (chunk > IB_CHUNK ? IB_CHUNK : chunk);
         if (nsb > 1) ibk_tile_partials<<<nsb, SCT, 0, st>>>(c->d_tile_cur, n_tiles, chunk, partial);   // one CTA needs no partial sums
-        ibk_tile_scan<<<nsb, SCT, 0, st>>>(c->d_tile_cur, n_tiles, chunk, partial, c->d_tile_start, c->d_work, c->d_small_rec, c->d_tile_count);
+        ibk_tile_scan<<<nsb, SCT, 0, st>>>(c->d_tile_cur, n_tiles, chunk, partial, c->d_tile_start, c->d_work, c->d_small_rec, c->d_tile_count,
+                                           ib_slab_tiles(c));
         c->launches += 3;
     }
     if (phases & 2) {

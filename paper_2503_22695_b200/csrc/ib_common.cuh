@@ -11,6 +11,13 @@
 #define IB_SMALL_TILE 64         // tiles with fewer points skip the tile kernel: their points go one by one (ib_point.cuh)
 #endif
 #define IB_CHUNK 1920            // points per work item of the tile kernel (ib_bin.cu emits the work list)
+#define IB_SLAB0 4                // d_tile_count[IB_SLAB0 + k] = first work item of z-slab k (ib_tile_scan)
+#define IB_MAX_SLABS 32
+#define IB_SLABC0 40              // d_tile_count[IB_SLABC0 + k] = work counter of slab k
+#define IB_TILE_HDR 80            // ints of d_tile_count before the partial sums of the scan
+#ifndef IB_HOST_SLABS
+#define IB_HOST_SLABS 8           // z-slabs ib_coupling_step_host cuts the spreading into
+#endif
 
 // ---------------------------------------------------------------------------------------------
 // host-side context
@@ -71,6 +78,9 @@ struct ib_ctx {
     cudaEvent_t ev_fork, ev_join, ev_aux;
     cudaStream_t side2;        // the direct path of the sparse tiles runs beside the tile kernel
     cudaEvent_t ev_sfork, ev_sjoin;
+    cudaStream_t side3;        // ib_coupling_step_host: f goes back to the host slab by slab on this stream
+    cudaStream_t side4;        // ... and the odd slabs of the tile kernel run on this one
+    cudaEvent_t ev_slab[IB_MAX_SLABS], ev_h2d[IB_MAX_SLABS];
     int64_t launches;
     // NEXT-4 boundary loads (ib_set_tethers / ib_set_surface / ib_set_loads)
     int32_t *d_teth_ids, *d_faces;
@@ -86,6 +96,27 @@ struct ib_ctx {
     int profile;
     void *prof;                // std::vector<ib_prof_rec>* (ib_context.cu)
 };
+
+// z-slabs of the tile list (tiles are numbered z-major): tile layers per slab and tiles per slab.  The
+// scan handles 4 tiles per thread, so a tile layer must be a multiple of 4 tiles; otherwise one slab.
+static inline int ib_slab_layers(const ib_ctx *c)
+{
+    const int ntz = c->grid.nz / 4, per = (c->grid.nx / 4) * (c->grid.ny / 4);
+    const int K = ntz / 2 < IB_HOST_SLABS ? ntz / 2 : IB_HOST_SLABS;     // at least two tile layers per slab
+    if (per % 4 != 0 || K < 2) return ntz;
+    return (ntz + K - 1) / K;
+}
+static inline int ib_slab_tiles(const ib_ctx *c)
+{
+    const int per = (c->grid.nx / 4) * (c->grid.ny / 4);
+    const int t = ib_slab_layers(c) * per;
+    return (t + 3) / 4 * 4;
+}
+static inline int ib_slab_count(const ib_ctx *c)
+{
+    const int ntz = c->grid.nz / 4, L = ib_slab_layers(c);
+    return (ntz + L - 1) / L;
+}
 
 void ib_prof_begin(ib_ctx *c, int phase, cudaStream_t st);
 void ib_prof_end(ib_ctx *c, int phase, cudaStream_t st);
@@ -226,6 +257,9 @@ ib_status ibk_tiled_spread_interp(ib_ctx *c, int mesh, const double *xp, const d
                                   const double *u, const double *v, const double *w,
                                   double *fu, double *fv, double *fw, double *Up, int counted, cudaStream_t st);
 ib_status ibk_tiled_launch(ib_ctx *c, int64_t P, int do_spread, int do_interp,
+                           const double *u, const double *v, const double *w,
+                           double *fu, double *fv, double *fw, double *Up, int slab, cudaStream_t st);
+ib_status ibk_small_launch(ib_ctx *c, int64_t P, int do_spread, int do_interp,
                            const double *u, const double *v, const double *w,
                            double *fu, double *fv, double *fw, double *Up, cudaStream_t st);
 ib_status ibk_bin_points(ib_ctx *c, int mesh, const double *xp, const double *Gp, int64_t P,

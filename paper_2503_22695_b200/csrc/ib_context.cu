@@ -118,6 +118,12 @@ extern "C" ib_status ib_destroy(ib_ctx *c)
     if (c->side2) cudaStreamDestroy(c->side2);
     if (c->ev_sfork) cudaEventDestroy(c->ev_sfork);
     if (c->ev_sjoin) cudaEventDestroy(c->ev_sjoin);
+    if (c->side3) cudaStreamDestroy(c->side3);
+    if (c->side4) cudaStreamDestroy(c->side4);
+    for (cudaEvent_t e : c->ev_h2d)
+        if (e) cudaEventDestroy(e);
+    for (cudaEvent_t e : c->ev_slab)
+        if (e) cudaEventDestroy(e);
     if (c->prof) {
         double ms[IB_PHASE_COUNT];
         int64_t n[IB_PHASE_COUNT];
@@ -239,7 +245,7 @@ extern "C" ib_status ib_create(ib_ctx **out, const ib_grid_desc *g, const ib_mes
     TRY(dev_alloc((void **)&c->d_tile_cur, (size_t)(n_tiles + 4) * sizeof(int32_t)));
     TRY(dev_alloc((void **)&c->d_tile_start, (size_t)(n_tiles + 4) * sizeof(int32_t)));
     TRY(dev_upload(&c->d_row_off, roff.data(), (size_t)ne + 1));
-    TRY(dev_alloc((void **)&c->d_tile_count, (size_t)(16 + 2 * (n_tiles / 4096 + 2)) * sizeof(int32_t)));
+    TRY(dev_alloc((void **)&c->d_tile_count, (size_t)(IB_TILE_HDR + 2 * (n_tiles / 4096 + 2)) * sizeof(int32_t)));
     TRY(dev_alloc((void **)&c->d_status, 2 * sizeof(long long)));
     if (s == IB_OK && (cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) != cudaSuccess ||
                        cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
@@ -249,6 +255,13 @@ extern "C" ib_status ib_create(ib_ctx **out, const ib_grid_desc *g, const ib_mes
                        cudaEventCreateWithFlags(&c->ev_sfork, cudaEventDisableTiming) != cudaSuccess ||
                        cudaEventCreateWithFlags(&c->ev_sjoin, cudaEventDisableTiming) != cudaSuccess))
         s = IB_ERR_CUDA;
+    if (s == IB_OK && (cudaStreamCreateWithFlags(&c->side3, cudaStreamNonBlocking) != cudaSuccess ||
+                       cudaStreamCreateWithFlags(&c->side4, cudaStreamNonBlocking) != cudaSuccess))
+        s = IB_ERR_CUDA;
+    for (int k = 0; k < IB_MAX_SLABS && s == IB_OK; ++k)
+        if (cudaEventCreateWithFlags(&c->ev_slab[k], cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&c->ev_h2d[k], cudaEventDisableTiming) != cudaSuccess)
+            s = IB_ERR_CUDA;
     if (s == IB_OK) s = reset_status(c, 0);
     if (s == IB_OK) s = ibk_sort_reserve(c, c->n_points);
     if (s == IB_OK) s = ibk_bin_reserve(c, c->n_points);
@@ -601,6 +614,15 @@ extern "C" ib_status ib_coupling_step(ib_ctx *c, const double *x, const double *
     return coupling_step_body(c, x, u, v, w, fu, fv, fw, Un, B, st);
 }
 
+// -DIB_HOST_TRACE (through IB_NVCC_EXTRA): time stamps of the pipelined host step on its three streams
+#ifdef IB_HOST_TRACE
+#include <cstdio>
+struct ib_trace { cudaEvent_t e[96]; const char *name[96]; int n; };
+#define IB_TR(STREAM, NAME) do { cudaEventCreate(&tr.e[tr.n]); cudaEventRecord(tr.e[tr.n], (STREAM)); tr.name[tr.n++] = (NAME); } while (0)
+#else
+#define IB_TR(STREAM, NAME) do { } while (0)
+#endif
+
 extern "C" ib_status ib_coupling_step_host(ib_ctx *c, const double *x_h, const double *u_h, const double *v_h,
                                            const double *w_h, double *fu_h, double *fv_h, double *fw_h,
                                            double *Un_h, double *B_h, void *stream)
@@ -635,42 +657,114 @@ extern "C" ib_status ib_coupling_step_host(ib_ctx *c, const double *x_h, const d
         IB_CUDA_TRY(cudaStreamSynchronize(st));
         return IB_OK;
     }
-    // Pipelined: the force side of the step needs only x, so it runs while u,v,w are still crossing the
-    // bus on the side stream; f goes back to the host (side stream) while the velocity side runs.
-    //   st   : H2D x | zero f, bin, FE force, scatter, SPREAD | (wait uvw) INTERP, restrict | D2H Un, B
-    //   side : H2D u,v,w ............................... | (wait spread) D2H fu,fv,fw
-    cudaStream_t s2 = c->side;
+    // Pipelined in z-slabs of the tile list (tiles are numbered z-major).  The force side of the step needs
+    // only x, so it runs while u,v,w cross the bus, slab by slab, on a side stream.  The fused
+    // spread + interpolate kernel of slab k needs the velocity layers of slabs k-1..k+1 only (halo = 2 cells)
+    // and a point reaches at most 2 cells beyond its own 4-cell tile layer, so after slab k every z-layer
+    // below the last tile layer of that slab is final and goes back to the host on a third stream while the
+    // next slabs run; the first tile layer (periodic wrap of the last slab) goes last.  Consecutive slabs
+    // alternate between two streams so that the tail of one kernel is filled by the next.
+    //   st / side4 : H2D x | zero f, bin, FE force, scatter | SPREAD+INTERP slab 0 | 1 | ... | restrict | D2H Un, B
+    //   side       : H2D u,v,w wrap layers | slab 0 | slab 1 | ...
+    //   side2      :                        sparse tiles: spread            ...           interpolate
+    //   side3      :                                            D2H f layers of slab 0 | slab 1 | ...
+    cudaStream_t s2 = c->side, s3 = c->side3, s4 = c->side4, ss = c->side2;
     double *Bd = B_h ? c->d_hB : c->d_B;
-    IB_CUDA_TRY(cudaEventRecord(c->ev_fork, st));             // orders the side stream after earlier work on st
-    IB_CUDA_TRY(cudaStreamWaitEvent(s2, c->ev_fork, 0));
+#ifdef IB_HOST_TRACE
+    ib_trace tr; tr.n = 0;
+#endif
+    const int K = ib_slab_count(c), nz = c->grid.nz, zs = 4 * ib_slab_layers(c);
+    const size_t plane = (size_t)c->grid.nx * c->grid.ny, pb = plane * sizeof(double);
+    const int z_first = nz < 4 ? nz : 4;          // wrap margin: the last z_first layers come first, the first go back last
+    IB_TR(st, "start");
+    // x first: the force side waits for it, and the copy engine serves the H2D copies of all streams in turn
     IB_CUDA_TRY(cudaMemcpyAsync(c->d_hx, x_h, nb, cudaMemcpyHostToDevice, st));
-    IB_CUDA_TRY(cudaMemcpyAsync(c->d_hu, u_h, gb, cudaMemcpyHostToDevice, s2));
-    IB_CUDA_TRY(cudaMemcpyAsync(c->d_hv, v_h, gb, cudaMemcpyHostToDevice, s2));
-    IB_CUDA_TRY(cudaMemcpyAsync(c->d_hw, w_h, gb, cudaMemcpyHostToDevice, s2));
-    IB_CUDA_TRY(cudaEventRecord(c->ev_join, s2));             // u,v,w are on the device
+    IB_CUDA_TRY(cudaEventRecord(c->ev_fork, st));             // orders the side streams after x and earlier work on st
+    IB_CUDA_TRY(cudaStreamWaitEvent(s2, c->ev_fork, 0));
+    {
+        const double *uh[3] = {u_h, v_h, w_h};
+        double *ud[3] = {c->d_hu, c->d_hv, c->d_hw};
+        for (int d = 0; d < 3 && K > 1; ++d)
+            IB_CUDA_TRY(cudaMemcpyAsync(ud[d] + (nz - z_first) * plane, uh[d] + (nz - z_first) * plane, z_first * pb,
+                                        cudaMemcpyHostToDevice, s2));
+        for (int k = 0; k < K; ++k) {
+            const int z0 = zs * k, z1 = (k == K - 1) ? (K > 1 ? nz - z_first : nz) : zs * (k + 1);
+            for (int d = 0; d < 3 && z1 > z0; ++d)
+                IB_CUDA_TRY(cudaMemcpyAsync(ud[d] + z0 * plane, uh[d] + z0 * plane, (size_t)(z1 - z0) * pb,
+                                            cudaMemcpyHostToDevice, s2));
+            IB_CUDA_TRY(cudaEventRecord(c->ev_h2d[k], s2));
+            IB_TR(s2, "uvw slab on device");
+        }
+    }
+    IB_TR(st, "x on device");
     IB_CUDA_TRY(cudaMemsetAsync(c->d_hfu, 0, gb, st));
     IB_CUDA_TRY(cudaMemsetAsync(c->d_hfv, 0, gb, st));
     IB_CUDA_TRY(cudaMemsetAsync(c->d_hfw, 0, gb, st));
     s = ibk_bin_reserve(c, c->n_points);
     if (s == IB_OK) s = ibk_bin_points(c, 1, nullptr, nullptr, c->n_points, c->d_hx, nullptr, nullptr, 1, st);
+    IB_TR(st, "zero + count + scan");
     if (s == IB_OK) s = ibk_fe_force(c, c->d_hx, Bd, c->d_Fhat, st);
+    IB_TR(st, "FE force");
     if (s == IB_OK) s = ibk_bin_points(c, 1, nullptr, nullptr, c->n_points, c->d_hx, c->d_Fhat, c->d_Up, 2, st);
-    if (s == IB_OK) s = ibk_tiled_launch(c, c->n_points, 1, 0, nullptr, nullptr, nullptr, c->d_hfu, c->d_hfv, c->d_hfw,
-                                         nullptr, st);
+    IB_TR(st, "scatter");
     if (s != IB_OK) return s;
-    IB_CUDA_TRY(cudaEventRecord(c->ev_aux, st));              // f is complete
-    IB_CUDA_TRY(cudaStreamWaitEvent(s2, c->ev_aux, 0));
-    IB_CUDA_TRY(cudaMemcpyAsync(fu_h, c->d_hfu, gb, cudaMemcpyDeviceToHost, s2));
-    IB_CUDA_TRY(cudaMemcpyAsync(fv_h, c->d_hfv, gb, cudaMemcpyDeviceToHost, s2));
-    IB_CUDA_TRY(cudaMemcpyAsync(fw_h, c->d_hfw, gb, cudaMemcpyDeviceToHost, s2));
-    IB_CUDA_TRY(cudaStreamWaitEvent(st, c->ev_join, 0));
-    s = ibk_tiled_launch(c, c->n_points, 0, 1, c->d_hu, c->d_hv, c->d_hw, nullptr, nullptr, nullptr, c->d_Up, st);
-    if (s == IB_OK) s = ibk_restrict(c, c->d_Up, c->d_hUn, st);
+    IB_CUDA_TRY(cudaEventRecord(c->ev_aux, st));              // the records are binned
+    IB_CUDA_TRY(cudaStreamWaitEvent(ss, c->ev_aux, 0));
+    IB_CUDA_TRY(cudaStreamWaitEvent(s4, c->ev_aux, 0));
+    s = ibk_small_launch(c, c->n_points, 1, 0, nullptr, nullptr, nullptr, c->d_hfu, c->d_hfv, c->d_hfw, nullptr, ss);
+    if (s != IB_OK) return s;
+    IB_CUDA_TRY(cudaEventRecord(c->ev_sjoin, ss));            // the sparse tiles are spread
+    IB_CUDA_TRY(cudaStreamWaitEvent(s3, c->ev_sjoin, 0));
+    {
+        double *fh[3] = {fu_h, fv_h, fw_h}, *fd[3] = {c->d_hfu, c->d_hfv, c->d_hfw};
+        int z_done = z_first;
+        for (int k = 0; k < K; ++k) {
+            cudaStream_t sk = (k & 1) ? s4 : st;
+            IB_CUDA_TRY(cudaStreamWaitEvent(sk, c->ev_h2d[k + 1 < K ? k + 1 : K - 1], 0));
+            s = ibk_tiled_launch(c, c->n_points, 1, 1, c->d_hu, c->d_hv, c->d_hw, c->d_hfu, c->d_hfv, c->d_hfw,
+                                 c->d_Up, k, sk);
+            if (s != IB_OK) return s;
+            IB_CUDA_TRY(cudaEventRecord(c->ev_slab[k], sk));
+            IB_TR(sk, "spread + interp slab");
+            int z_end = (k == K - 1) ? nz : zs * (k + 1) - 4;
+            if (z_end > nz) z_end = nz;
+            if (z_end < z_done) z_end = z_done;
+            IB_CUDA_TRY(cudaStreamWaitEvent(s3, c->ev_slab[k], 0));
+            for (int d = 0; d < 3 && z_end > z_done; ++d)
+                IB_CUDA_TRY(cudaMemcpyAsync(fh[d] + z_done * plane, fd[d] + z_done * plane, (size_t)(z_end - z_done) * pb,
+                                            cudaMemcpyDeviceToHost, s3));
+            z_done = z_end;
+            IB_TR(s3, "f slab on host");
+        }
+        for (int d = 0; d < 3 && z_first > 0; ++d)
+            IB_CUDA_TRY(cudaMemcpyAsync(fh[d], fd[d], z_first * pb, cudaMemcpyDeviceToHost, s3));
+        IB_TR(s3, "f on host");
+    }
+    IB_CUDA_TRY(cudaStreamWaitEvent(ss, c->ev_h2d[K - 1], 0));
+    s = ibk_small_launch(c, c->n_points, 0, 1, c->d_hu, c->d_hv, c->d_hw, nullptr, nullptr, nullptr, c->d_Up, ss);
+    if (s != IB_OK) return s;
+    IB_CUDA_TRY(cudaEventRecord(c->ev_sfork, ss));            // the sparse tiles are interpolated
+    IB_CUDA_TRY(cudaStreamWaitEvent(st, c->ev_sfork, 0));
+    for (int k = 1; k < K; k += 2) IB_CUDA_TRY(cudaStreamWaitEvent(st, c->ev_slab[k], 0));
+    IB_TR(st, "all slabs");
+    s = ibk_restrict(c, c->d_Up, c->d_hUn, st);
+    IB_TR(st, "restrict");
     if (s != IB_OK) return s;
     IB_CUDA_TRY(cudaMemcpyAsync(Un_h, c->d_hUn, nb, cudaMemcpyDeviceToHost, st));
     if (B_h) IB_CUDA_TRY(cudaMemcpyAsync(B_h, c->d_hB, nb, cudaMemcpyDeviceToHost, st));
+    IB_TR(st, "Un on host");
     IB_CUDA_TRY(cudaStreamSynchronize(st));
     IB_CUDA_TRY(cudaStreamSynchronize(s2));
+    IB_CUDA_TRY(cudaStreamSynchronize(s3));
+#ifdef IB_HOST_TRACE
+    for (int i = 0; i < tr.n; ++i) {
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, tr.e[0], tr.e[i]);
+        fprintf(stderr, "[ib host trace] %8.3f ms  %s\n", ms, tr.name[i]);
+        if (i) cudaEventDestroy(tr.e[i]);
+    }
+    cudaEventDestroy(tr.e[0]);
+#endif
     return IB_OK;
 }
 

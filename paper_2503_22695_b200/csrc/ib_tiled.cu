@@ -46,7 +46,8 @@ struct ib_tiled_params {
     double *frc[3];
     double *Up;
     const int4 *work;           // {tile, first record, points, 0} per chunk
-    int32_t *counters;          // [0] number of work items, [1] work counter
+    int32_t *counters;          // [0] number of work items, [1] work counter, [3] zero, [IB_SLAB0 + k] first item of slab k
+    int wb, we, wc;             // this launch covers the work items counters[wb] <= w < counters[we]; counters[wc] counts them
     ib_grid_desc g;
     double inv_h, ih3;
 };
@@ -115,8 +116,8 @@ ibk_tiled_kernel(ib_tiled_params pr)
     const int64_t P = pr.P;
 
     if (tid == 0) {
-        const int w = atomicAdd(&pr.counters[1], 1);
-        s_work = (w < pr.counters[0]) ? __ldg(pr.work + w) : make_int4(-1, 0, 0, 0);
+        const int w = pr.counters[pr.wb] + atomicAdd(&pr.counters[pr.wc], 1);
+        s_work = (w < pr.counters[pr.we]) ? __ldg(pr.work + w) : make_int4(-1, 0, 0, 0);
         s_next = 0;
     }
     for (int i = tid; i < NOC; i += TB) oc_cur[i] = 0;
@@ -128,8 +129,8 @@ ibk_tiled_kernel(ib_tiled_params pr)
         // the next work item is claimed and read now; its latency hides behind this item's processing
         int4 nwk = make_int4(-1, 0, 0, 0);
         if (tid == 0) {
-            const int w = atomicAdd(&pr.counters[1], 1);
-            if (w < pr.counters[0]) nwk = __ldg(pr.work + w);
+            const int w = pr.counters[pr.wb] + atomicAdd(&pr.counters[pr.wc], 1);
+            if (w < pr.counters[pr.we]) nwk = __ldg(pr.work + w);
         }
         const int tile = wk.x, cb = wk.y, cn = wk.z;
         const int t3[3] = {tile % ntx, (tile / ntx) % nty, tile / (ntx * nty)};
@@ -462,7 +463,7 @@ ibk_small_tiles(ib_tiled_params pr, const int32_t *__restrict__ small_rec, const
 }
 
 template <int S, int I, int PER>
-static ib_status launch_tiled_p(ib_ctx *c, const ib_tiled_params &pr, cudaStream_t st)
+static ib_status launch_tiled_p(ib_ctx *c, const ib_tiled_params &pr, bool with_small, cudaStream_t st)
 {
     static int configured = 0;
     const size_t smem = (size_t)(3 * SU3 + 3 * CH + NWARP * 8 * GSTRIDE) * sizeof(double) +
@@ -480,24 +481,24 @@ static ib_status launch_tiled_p(ib_ctx *c, const ib_tiled_params &pr, cudaStream
     }
     // the few points of sparsely filled tiles go one by one on a second stream, beside the tile kernel
     const int64_t nsmall_max = min((int64_t)pr.P, (c->n_cells / (TT * TT * TT)) * (int64_t)(IB_SMALL_TILE - 1));
-    const bool beside = !c->profile;
+    const bool beside = !c->profile && with_small;
     cudaStream_t s3 = beside ? c->side2 : st;
     if (beside) {
         IB_CUDA_TRY(cudaEventRecord(c->ev_sfork, st));
         IB_CUDA_TRY(cudaStreamWaitEvent(s3, c->ev_sfork, 0));
     }
-    ibk_small_tiles<S, I><<<ib_blocks(nsmall_max, 128), 128, 0, s3>>>(pr, c->d_small_rec, c->d_tile_count);
+    if (with_small) ibk_small_tiles<S, I><<<ib_blocks(nsmall_max, 128), 128, 0, s3>>>(pr, c->d_small_rec, c->d_tile_count);
     if (beside) IB_CUDA_TRY(cudaEventRecord(c->ev_sjoin, s3));
     ibk_tiled_kernel<S, I, PER><<<sms * NCTA, TB, smem, st>>>(pr);
     if (beside) IB_CUDA_TRY(cudaStreamWaitEvent(st, c->ev_sjoin, 0));
-    c->launches += 2;
+    c->launches += with_small ? 2 : 1;
     return IB_OK;
 }
 
 template <int S, int I>
-static ib_status launch_tiled(ib_ctx *c, const ib_tiled_params &pr, cudaStream_t st)
+static ib_status launch_tiled(ib_ctx *c, const ib_tiled_params &pr, bool with_small, cudaStream_t st)
 {
-    return c->grid.periodic ? launch_tiled_p<S, I, 1>(c, pr, st) : launch_tiled_p<S, I, 0>(c, pr, st);
+    return c->grid.periodic ? launch_tiled_p<S, I, 1>(c, pr, with_small, st) : launch_tiled_p<S, I, 0>(c, pr, with_small, st);
 }
 
 // mesh != 0: points are the sub-points of the mesh at node positions x with force coefficients Fhat
@@ -515,31 +516,61 @@ ib_status ibk_tiled_spread_interp(ib_ctx *c, int mesh, const double *xp, const d
     ib_prof_end(c, IB_PHASE_SORT, st);
     if (rs != IB_OK) return rs;
 
-    return ibk_tiled_launch(c, P, spread, Up != nullptr, u, v, w, fu, fv, fw, Up, st);
+    return ibk_tiled_launch(c, P, spread, Up != nullptr, u, v, w, fu, fv, fw, Up, -1, st);
 }
 
-// The tile kernel (and the direct path of the sparse tiles) over records that are already binned.
-// Spreading and interpolation may be launched separately over the same records (ib_coupling_step_host
-// overlaps them with the host copies): the work counter is reset on the stream before every launch.
-ib_status ibk_tiled_launch(ib_ctx *c, int64_t P, int do_spread, int do_interp,
-                           const double *u, const double *v, const double *w,
-                           double *fu, double *fv, double *fw, double *Up, cudaStream_t st)
+static void fill_params(ib_ctx *c, ib_tiled_params &pr, int64_t P, const double *u, const double *v, const double *w,
+                        double *fu, double *fv, double *fw, double *Up, int slab)
 {
-    ib_status rs = IB_OK;
-    ib_tiled_params pr;
     pr.sx = c->d_sx; pr.sG = c->d_sG; pr.sid = c->d_sid; pr.P = P;
     pr.fld[0] = u; pr.fld[1] = v; pr.fld[2] = w;
     pr.frc[0] = fu; pr.frc[1] = fv; pr.frc[2] = fw;
     pr.Up = Up;
     pr.work = c->d_work; pr.counters = c->d_tile_count;
+    pr.wb = slab < 0 ? 3 : IB_SLAB0 + slab;
+    pr.we = slab < 0 ? 0 : IB_SLAB0 + slab + 1;
+    pr.wc = slab < 0 ? 1 : IB_SLABC0 + slab;
     pr.g = c->grid; pr.inv_h = c->inv_h; pr.ih3 = c->inv_h * c->inv_h * c->inv_h;
-    IB_CUDA_TRY(cudaMemsetAsync(c->d_tile_count + 1, 0, sizeof(int32_t), st));
+}
+
+// The tile kernel (and the direct path of the sparse tiles) over records that are already binned.
+// Spreading and interpolation may be launched separately over the same records (ib_coupling_step_host
+// overlaps them with the host copies): the work counter is reset on the stream before every launch.
+// slab < 0: all work items, and the sparse tiles beside them; slab k >= 0: the work items of z-slab k only
+// (the tile layers [k L, (k+1) L), L = ib_slab_layers) with a work counter of its own, so that slabs may run
+// on different streams at once; the sparse tiles are then the caller's to launch (ibk_small_launch).
+ib_status ibk_tiled_launch(ib_ctx *c, int64_t P, int do_spread, int do_interp,
+                           const double *u, const double *v, const double *w,
+                           double *fu, double *fv, double *fw, double *Up, int slab, cudaStream_t st)
+{
+    ib_status rs = IB_OK;
+    ib_tiled_params pr;
+    fill_params(c, pr, P, u, v, w, fu, fv, fw, Up, slab);
+    const bool with_small = slab < 0;
+    IB_CUDA_TRY(cudaMemsetAsync(c->d_tile_count + pr.wc, 0, sizeof(int32_t), st));
     ib_prof_begin(c, IB_PHASE_SPREAD_INTERP, st);
-    if (do_spread && do_interp) rs = launch_tiled<1, 1>(c, pr, st);
-    else if (do_spread) rs = launch_tiled<1, 0>(c, pr, st);
-    else rs = launch_tiled<0, 1>(c, pr, st);
+    if (do_spread && do_interp) rs = launch_tiled<1, 1>(c, pr, with_small, st);
+    else if (do_spread) rs = launch_tiled<1, 0>(c, pr, with_small, st);
+    else rs = launch_tiled<0, 1>(c, pr, with_small, st);
     ib_prof_end(c, IB_PHASE_SPREAD_INTERP, st);
     if (rs != IB_OK) return rs;
+    IB_CUDA_TRY(cudaGetLastError());
+    return IB_OK;
+}
+
+// the direct path of the sparse tiles alone, on the given stream
+ib_status ibk_small_launch(ib_ctx *c, int64_t P, int do_spread, int do_interp,
+                           const double *u, const double *v, const double *w,
+                           double *fu, double *fv, double *fw, double *Up, cudaStream_t st)
+{
+    ib_tiled_params pr;
+    fill_params(c, pr, P, u, v, w, fu, fv, fw, Up, -1);
+    const int64_t nsmall_max = min((int64_t)P, (c->n_cells / (TT * TT * TT)) * (int64_t)(IB_SMALL_TILE - 1));
+    const int nb = ib_blocks(nsmall_max, 128);
+    if (do_spread && do_interp) ibk_small_tiles<1, 1><<<nb, 128, 0, st>>>(pr, c->d_small_rec, c->d_tile_count);
+    else if (do_spread) ibk_small_tiles<1, 0><<<nb, 128, 0, st>>>(pr, c->d_small_rec, c->d_tile_count);
+    else ibk_small_tiles<0, 1><<<nb, 128, 0, st>>>(pr, c->d_small_rec, c->d_tile_count);
+    c->launches += 1;
     IB_CUDA_TRY(cudaGetLastError());
     return IB_OK;
 }

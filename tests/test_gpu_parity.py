@@ -222,6 +222,42 @@ def test_host_entry_point_matches_device_path(ib, name, variant):
     ctx.close()
 
 
+@pytest.mark.parametrize("case", ["wrap", "bounded", "one-slab"])
+def test_host_step_slabs_against_oracle(ib, orc, case):
+    """ib_coupling_step_host cuts the step into z-slabs (copies of u,v,w and f overlap the tile kernel):
+    a structure across the periodic z wrap (first and last slab share points), a bounded grid with the
+    structure in a corner, and a grid too thin for more than one slab, each against the oracle."""
+    import torch
+    wl = W.config1()
+    nz, periodic = wl.nz, 1
+    org = np.asarray(wl.origin, dtype=np.float64).copy()
+    if case == "wrap":
+        shift = np.array([0.0, 0.0, 0.5 * wl.nz * wl.h + 0.37 * wl.h])      # the slab sits on the z wrap
+    elif case == "bounded":
+        shift = org - wl.X.min(axis=1) + 0.3 * wl.h
+        periodic = 0
+    else:
+        nz = 8
+        shift = np.zeros(3)
+        org[2] = 0.5 * (wl.X[2].min() + wl.X[2].max()) - 4 * wl.h + 0.21 * wl.h
+    X, x = wl.X + shift[:, None], wl.x + shift[:, None]
+    ncell = wl.nx * wl.ny * nz
+    u, v, w = (np.ascontiguousarray(a.reshape(wl.nz, wl.ny, wl.nx)[:nz].reshape(-1)) for a in (wl.u, wl.v, wl.w))
+    g = orc.make_grid(wl.nx, wl.ny, nz, wl.h, tuple(org), periodic=periodic)
+    ref = orc.coupling_step(g, wl.conn, X, wl.fibers, wl.mat_id, wl.nsub, wl.mats, x, u, v, w)
+    ctx = ib.Context(wl.nx, wl.ny, nz, wl.h, tuple(org), wl.conn, X, wl.fibers, wl.mat_id, wl.nsub, wl.mats, periodic=periodic)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    outs = [torch.full((ncell,), 9.0, dtype=torch.float64).pin_memory() for _ in range(3)]
+    Un = torch.empty((3, wl.n_nodes), dtype=torch.float64).pin_memory()
+    B = torch.empty((3, wl.n_nodes), dtype=torch.float64).pin_memory()
+    for _ in range(2):
+        ctx.ib_coupling_step_host(pin(x), pin(u), pin(v), pin(w), *outs, Un, B)
+    ctx.check()
+    for k, t in (("B", B), ("fu", outs[0]), ("fv", outs[1]), ("fw", outs[2]), ("Un", Un)):
+        _close(t.numpy(), ref[k], f"host slabs {case} {k}")
+    ctx.close()
+
+
 # ---- full sizes, in the launch configuration bench.py times --------------------------------------
 FULL = {
     "C3": lambda: W.config3(),                       # the bench workload: whole oracle step (~20 s)
