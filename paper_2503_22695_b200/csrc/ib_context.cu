@@ -659,15 +659,15 @@ extern "C" ib_status ib_coupling_step_host(ib_ctx *c, const double *x_h, const d
     }
     // Pipelined in z-slabs of the tile list (tiles are numbered z-major).  The force side of the step needs
     // only x, so it runs while u,v,w cross the bus, slab by slab, on a side stream.  The fused
-    // spread + interpolate kernel of slab k needs the velocity layers of slabs k-1..k+1 only (halo = 2 cells)
+    // spread + interpolate kernel of slab k needs the velocity layers of slab k and 2 more on either side
     // and a point reaches at most 2 cells beyond its own 4-cell tile layer, so after slab k every z-layer
     // below the last tile layer of that slab is final and goes back to the host on a third stream while the
     // next slabs run; the first tile layer (periodic wrap of the last slab) goes last.  Consecutive slabs
     // alternate between two streams so that the tail of one kernel is filled by the next.
-    //   st / side4 : H2D x | zero f, bin, FE force, scatter | SPREAD+INTERP slab 0 | 1 | ... | restrict | D2H Un, B
-    //   side       : H2D u,v,w wrap layers | slab 0 | slab 1 | ...
-    //   side2      :                        sparse tiles: spread            ...           interpolate
-    //   side3      :                                            D2H f layers of slab 0 | slab 1 | ...
+    //   st / side4 : H2D x | FE force | scatter, sparse tiles: spread | SPREAD+INTERP slab 0 | 1 | ... | restrict | D2H Un, B
+    //   side       :       H2D u,v,w wrap layers + slab 0 | slab 1 | ...
+    //   side2      :       zero f, count pass, scan                      ...      sparse tiles: interpolate
+    //   side3      :                                                        D2H f layers of slab 0 | slab 1 | ...
     cudaStream_t s2 = c->side, s3 = c->side3, s4 = c->side4, ss = c->side2;
     double *Bd = B_h ? c->d_hB : c->d_B;
 #ifdef IB_HOST_TRACE
@@ -687,8 +687,11 @@ extern "C" ib_status ib_coupling_step_host(ib_ctx *c, const double *x_h, const d
         for (int d = 0; d < 3 && K > 1; ++d)
             IB_CUDA_TRY(cudaMemcpyAsync(ud[d] + (nz - z_first) * plane, uh[d] + (nz - z_first) * plane, z_first * pb,
                                         cudaMemcpyHostToDevice, s2));
+        // copy k ends 4 layers into slab k+1: with the wrap layers it is all that the kernel of slab k reads
+        const int z_last = K > 1 ? nz - z_first : nz;
         for (int k = 0; k < K; ++k) {
-            const int z0 = zs * k, z1 = (k == K - 1) ? (K > 1 ? nz - z_first : nz) : zs * (k + 1);
+            const int z0 = k == 0 ? 0 : (zs * k + 4 < z_last ? zs * k + 4 : z_last);
+            const int z1 = (k == K - 1 || zs * (k + 1) + 4 > z_last) ? z_last : zs * (k + 1) + 4;
             for (int d = 0; d < 3 && z1 > z0; ++d)
                 IB_CUDA_TRY(cudaMemcpyAsync(ud[d] + z0 * plane, uh[d] + z0 * plane, (size_t)(z1 - z0) * pb,
                                             cudaMemcpyHostToDevice, s2));
@@ -697,30 +700,31 @@ extern "C" ib_status ib_coupling_step_host(ib_ctx *c, const double *x_h, const d
         }
     }
     IB_TR(st, "x on device");
-    IB_CUDA_TRY(cudaMemsetAsync(c->d_hfu, 0, gb, st));
-    IB_CUDA_TRY(cudaMemsetAsync(c->d_hfv, 0, gb, st));
-    IB_CUDA_TRY(cudaMemsetAsync(c->d_hfw, 0, gb, st));
+    // zero-fill of f and the count pass of the binning beside the FE force, as in ib_coupling_step
+    IB_CUDA_TRY(cudaStreamWaitEvent(ss, c->ev_fork, 0));
+    IB_CUDA_TRY(cudaMemsetAsync(c->d_hfu, 0, gb, ss));
+    IB_CUDA_TRY(cudaMemsetAsync(c->d_hfv, 0, gb, ss));
+    IB_CUDA_TRY(cudaMemsetAsync(c->d_hfw, 0, gb, ss));
     s = ibk_bin_reserve(c, c->n_points);
-    if (s == IB_OK) s = ibk_bin_points(c, 1, nullptr, nullptr, c->n_points, c->d_hx, nullptr, nullptr, 1, st);
-    IB_TR(st, "zero + count + scan");
+    if (s == IB_OK) s = ibk_bin_points(c, 1, nullptr, nullptr, c->n_points, c->d_hx, nullptr, nullptr, 1, ss);
+    IB_CUDA_TRY(cudaEventRecord(c->ev_join, ss));
+    IB_TR(ss, "zero + count + scan");
     if (s == IB_OK) s = ibk_fe_force(c, c->d_hx, Bd, c->d_Fhat, st);
     IB_TR(st, "FE force");
+    IB_CUDA_TRY(cudaStreamWaitEvent(st, c->ev_join, 0));
     if (s == IB_OK) s = ibk_bin_points(c, 1, nullptr, nullptr, c->n_points, c->d_hx, c->d_Fhat, c->d_Up, 2, st);
     IB_TR(st, "scatter");
+    // the sparse tiles are spread before the first slab: beside it they would find no free SM until it ends
+    if (s == IB_OK) s = ibk_small_launch(c, c->n_points, 1, 0, nullptr, nullptr, nullptr, c->d_hfu, c->d_hfv, c->d_hfw, nullptr, st);
     if (s != IB_OK) return s;
     IB_CUDA_TRY(cudaEventRecord(c->ev_aux, st));              // the records are binned
-    IB_CUDA_TRY(cudaStreamWaitEvent(ss, c->ev_aux, 0));
     IB_CUDA_TRY(cudaStreamWaitEvent(s4, c->ev_aux, 0));
-    s = ibk_small_launch(c, c->n_points, 1, 0, nullptr, nullptr, nullptr, c->d_hfu, c->d_hfv, c->d_hfw, nullptr, ss);
-    if (s != IB_OK) return s;
-    IB_CUDA_TRY(cudaEventRecord(c->ev_sjoin, ss));            // the sparse tiles are spread
-    IB_CUDA_TRY(cudaStreamWaitEvent(s3, c->ev_sjoin, 0));
     {
         double *fh[3] = {fu_h, fv_h, fw_h}, *fd[3] = {c->d_hfu, c->d_hfv, c->d_hfw};
         int z_done = z_first;
         for (int k = 0; k < K; ++k) {
             cudaStream_t sk = (k & 1) ? s4 : st;
-            IB_CUDA_TRY(cudaStreamWaitEvent(sk, c->ev_h2d[k + 1 < K ? k + 1 : K - 1], 0));
+            IB_CUDA_TRY(cudaStreamWaitEvent(sk, c->ev_h2d[k], 0));
             s = ibk_tiled_launch(c, c->n_points, 1, 1, c->d_hu, c->d_hv, c->d_hw, c->d_hfu, c->d_hfv, c->d_hfw,
                                  c->d_Up, k, sk);
             if (s != IB_OK) return s;
@@ -740,6 +744,7 @@ extern "C" ib_status ib_coupling_step_host(ib_ctx *c, const double *x_h, const d
             IB_CUDA_TRY(cudaMemcpyAsync(fh[d], fd[d], z_first * pb, cudaMemcpyDeviceToHost, s3));
         IB_TR(s3, "f on host");
     }
+    IB_CUDA_TRY(cudaStreamWaitEvent(ss, c->ev_aux, 0));
     IB_CUDA_TRY(cudaStreamWaitEvent(ss, c->ev_h2d[K - 1], 0));
     s = ibk_small_launch(c, c->n_points, 0, 1, c->d_hu, c->d_hv, c->d_hw, nullptr, nullptr, nullptr, c->d_Up, ss);
     if (s != IB_OK) return s;
