@@ -222,7 +222,7 @@ def test_host_entry_point_matches_device_path(ib, name, variant):
     ctx.close()
 
 
-@pytest.mark.parametrize("case", ["wrap", "bounded", "one-slab"])
+@pytest.mark.parametrize("case", ["wrap", "bounded", "one-slab", "pageable"])
 def test_host_step_slabs_against_oracle(ib, orc, case):
     """ib_coupling_step_host cuts the step into z-slabs (copies of u,v,w and f overlap the tile kernel):
     a structure across the periodic z wrap (first and last slab share points), a bounded grid with the
@@ -236,6 +236,8 @@ def test_host_step_slabs_against_oracle(ib, orc, case):
     elif case == "bounded":
         shift = org - wl.X.min(axis=1) + 0.3 * wl.h
         periodic = 0
+    elif case == "pageable":                      # plain (unpinned) host memory: slower copies, same answer
+        shift = np.zeros(3)
     else:
         nz = 8
         shift = np.zeros(3)
@@ -246,10 +248,10 @@ def test_host_step_slabs_against_oracle(ib, orc, case):
     g = orc.make_grid(wl.nx, wl.ny, nz, wl.h, tuple(org), periodic=periodic)
     ref = orc.coupling_step(g, wl.conn, X, wl.fibers, wl.mat_id, wl.nsub, wl.mats, x, u, v, w)
     ctx = ib.Context(wl.nx, wl.ny, nz, wl.h, tuple(org), wl.conn, X, wl.fibers, wl.mat_id, wl.nsub, wl.mats, periodic=periodic)
-    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
-    outs = [torch.full((ncell,), 9.0, dtype=torch.float64).pin_memory() for _ in range(3)]
-    Un = torch.empty((3, wl.n_nodes), dtype=torch.float64).pin_memory()
-    B = torch.empty((3, wl.n_nodes), dtype=torch.float64).pin_memory()
+    pin = (lambda a: torch.from_numpy(np.array(a, order="C"))) if case == "pageable" else \
+          (lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory())
+    outs = [pin(np.full(ncell, 9.0)) for _ in range(3)]
+    Un, B = pin(np.empty((3, wl.n_nodes))), pin(np.empty((3, wl.n_nodes)))
     for _ in range(2):
         ctx.ib_coupling_step_host(pin(x), pin(u), pin(v), pin(w), *outs, Un, B)
     ctx.check()
