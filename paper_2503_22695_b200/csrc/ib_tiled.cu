@@ -56,11 +56,28 @@ struct ib_tiled_params {
 // nx = 4 if c == 0 else 5, ny = 4 if c == 1 else 5; compile-time constant divisors only)
 __device__ __forceinline__ void ib_item_decode(int it, int &c, int l[3])
 {
+    // written without branches: the compiler merges a three-way branch into selects of the DIVISORS and
+    // then divides by a run-time value (three I2F/MUFU.RCP sequences per item in the SASS)
     c = it / 100;
-    int r = it - c * 100;
-    if (c == 0) { l[0] = r % 4; l[1] = (r / 4) % 5; l[2] = r / 20; }
-    else if (c == 1) { l[0] = r % 5; l[1] = (r / 5) % 4; l[2] = r / 20; }
-    else { l[0] = r % 5; l[1] = (r / 5) % 5; l[2] = r / 25; }
+    const int r = it - c * 100;
+    const int q20 = r / 20, q25 = r / 25;
+    l[2] = (c == 2) ? q25 : q20;
+    const int rem = r - ((c == 2) ? 25 * q25 : 20 * q20);      // index in the z-plane: nx*ny = 20 or 25
+    const int q5 = rem / 5;
+    l[1] = (c == 0) ? (rem >> 2) : q5;
+    l[0] = (c == 0) ? (rem & 3) : rem - 5 * q5;
+}
+
+// the same, packed into 11 bits for the sorted item list (the item loop unpacks instead of dividing)
+__device__ __forceinline__ unsigned short ib_item_code(int it)
+{
+    int c, l[3];
+    ib_item_decode(it, c, l);
+    return (unsigned short)(c | (l[0] << 2) | (l[1] << 5) | (l[2] << 8));
+}
+__device__ __forceinline__ void ib_item_unpack(int code, int &c, int l[3])
+{
+    c = code & 3; l[0] = (code >> 2) & 7; l[1] = (code >> 5) & 7; l[2] = code >> 8;
 }
 
 // half-cell range [lo,hi] (clipped to the tile) covered by shifted cell l in direction d of comp c
@@ -89,6 +106,11 @@ __device__ __forceinline__ int ib_octant_key(double a, double b, double c)
     return (hz * 8 + hy) * 8 + hx;
 }
 
+__device__ __forceinline__ void ib_prefetch_l2(const void *p)
+{
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+}
+
 // PER: periodic grid (compile-time, so that the periodic kernel carries none of the wall predicates)
 template <int DO_SPREAD, int DO_INTERP, int PER>
 __global__ void __launch_bounds__(TB, NCTA)
@@ -105,7 +127,7 @@ ibk_tiled_kernel(ib_tiled_params pr)
     unsigned short *order = item_cnt + NITEM;            // [NITEM]
     unsigned short *sidx = order + NITEM;                // [CH]
     __shared__ int s_nitems, s_next;
-    __shared__ int4 s_work;
+    __shared__ int4 s_work, s_nwk;
     __shared__ int wsum[NWARP];
 
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -131,8 +153,20 @@ ibk_tiled_kernel(ib_tiled_params pr)
         if (tid == 0) {
             const int w = pr.counters[pr.wb] + atomicAdd(&pr.counters[pr.wc], 1);
             if (w < pr.counters[pr.we]) nwk = __ldg(pr.work + w);
+            s_nwk = nwk;                                 // read behind the next barrier (prefetch of its records)
         }
         const int tile = wk.x, cb = wk.y, cn = wk.z;
+#ifndef IB_NO_PF
+        // this chunk's forces and ids are first needed after the staging and the sort: pull them into L2 now
+        // (one 128-byte line per 16 doubles / 32 ids; the item loop then waits on L2, not on DRAM)
+        if (16 * tid < cn) {
+            if (DO_SPREAD) {
+#pragma unroll
+                for (int d = 0; d < 3; ++d) ib_prefetch_l2(pr.sG + (int64_t)d * P + cb + 16 * tid);
+            }
+            if (DO_INTERP && 32 * tid < cn) ib_prefetch_l2(pr.sid + cb + 32 * tid);
+        }
+#endif
         const int t3[3] = {tile % ntx, (tile / ntx) % nty, tile / (ntx * nty)};
         int h0[3];                                       // halo origin (global index of halo entry 0), wrapped
 #pragma unroll
@@ -179,6 +213,17 @@ ibk_tiled_kernel(ib_tiled_params pr)
                 }
             }
             __syncthreads();
+#ifndef IB_NO_PF
+            {                                            // the next chunk's coordinates -> L2 while this one is processed
+                const int4 nx4 = s_nwk;
+                if (nx4.x >= 0) {
+                    for (int i = 16 * tid; i < 3 * CH; i += 16 * TB) {
+                        const int d = i / CH, o = i - d * CH;          // CH is a multiple of 16
+                        if (o < nx4.z) ib_prefetch_l2(pr.sx + (int64_t)d * P + nx4.y + o);
+                    }
+                }
+            }
+#endif
             {                                            // exclusive scan of the 512 counts, SCK per thread
                 constexpr int SCK = (NOC + TB - 1) / TB;
                 int v[SCK], s = 0;
@@ -245,7 +290,7 @@ ibk_tiled_kernel(ib_tiled_params pr)
             __syncthreads();
             for (int it = tid; it < NITEM; it += TB) {
                 int cnt = item_cnt[it];
-                if (cnt > 0) order[atomicAdd(&bins[min(cnt, NBIN - 1)], 1)] = it;
+                if (cnt > 0) order[atomicAdd(&bins[min(cnt, NBIN - 1)], 1)] = ib_item_code(it);
             }
             __syncthreads();
             const int nitems = s_nitems;
@@ -267,7 +312,7 @@ ibk_tiled_kernel(ib_tiled_params pr)
                 const int wi = base + grp;
                 const bool have = wi < nitems;
                 int c = 0, l[3] = {0, 0, 0};
-                if (have) ib_item_decode(order[wi], c, l);
+                if (have) ib_item_unpack(order[wi], c, l);
                 // runs of the half-cell order that make up this item
                 int rstart[4], rend[4], npts = 0;
                 {
