@@ -195,7 +195,9 @@ ib_status ib_set_variant(ib_ctx *ctx, int32_t variant);
  *  tethers  (L263 "fixed left face ... penalty parameter kappa = 10^6", L425): reading A24, a penalty spring
  *           to the reference position, B_a += kappa (X_a - x_a) for the listed nodes (host ids, distinct).
  *  surface  boundary faces, host array [n_faces][nodes_per_face], 4 = bilinear quads in cyclic order,
- *           3 = linear triangles, normal pointing out of the solid.
+ *           3 = linear triangles, 6 = quadratic triangles (3 vertices, then the middles of the edges
+ *           v0v1, v1v2, v2v0; reading A27: symmetric 6-point rule of degree 4, exact for the pressure term),
+ *           normal pointing out of the solid.
  *  loads    qt0 = q(t) t0 (host, 3 doubles or NULL): dead traction per unit REFERENCE area (L263),
  *           B_a += q t0 int N_a dA;   p: follower pressure on the CURRENT faces (L303, L315),
  *           B_a -= p int N_a n da.  Call again every step with the current q(t), p_endo(t).

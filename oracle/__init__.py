@@ -123,7 +123,7 @@ def tethers(ids, X, x, kappa, B):
 
 
 def surface_loads(faces, X, x, qt0, p, B):
-    """B += q t0 int N dA (reference faces) - p int N n da (current faces); faces [nf,3] or [nf,4]."""
+    """B += q t0 int N dA (reference faces) - p int N n da (current faces); faces [nf,3], [nf,4] or [nf,6] (quadratic triangles)."""
     faces, X, x = _i32(faces), _f64(X), _f64(x)
     B = _f64(B).copy()
     qt0 = None if qt0 is None else _f64(qt0)

@@ -502,11 +502,18 @@ void oracle_surface_loads(int64_t n_nodes, int64_t n_faces, int32_t npf, const i
                           const double *X, const double *x, const double *qt0, double p, double *B)
 {
     const ld g = 0.57735026918962576450914878050196L;
+    /* reading A27: 6-node (quadratic) triangles take the symmetric 6-point rule of degree 4,
+     *   a,b = (8 - sqrt10 +- sqrt(38 - 44 sqrt(2/5)))/18,  w = (620 +- sqrt(213125 - 53320 sqrt10))/3720,
+     * points (t,t), (t,1-2t), (1-2t,t) for t = a (weight w+) and t = b (weight w-), times the area 1/2 of
+     * the reference triangle: exact for the follower pressure (N_a (t1 x t2) has degree 4). */
+    const ld s10 = sqrtl(10.0L), rr = sqrtl(38.0L - 44.0L * sqrtl(0.4L)), tt = sqrtl(213125.0L - 53320.0L * s10);
+    const ld qa = (8.0L - s10 + rr) / 18.0L, qb = (8.0L - s10 - rr) / 18.0L;
+    const ld wa = (620.0L + tt) / 3720.0L, wb = (620.0L - tt) / 3720.0L;
     for (int64_t f = 0; f < n_faces; ++f) {
-        ld add[4][3] = {{0}};
-        int nq = npf == 4 ? 4 : 1;
+        ld add[6][3] = {{0}};
+        int nq = npf == 4 ? 4 : (npf == 6 ? 6 : 1);
         for (int q = 0; q < nq; ++q) {
-            ld N[4], dNx[4], dNe[4], wq;
+            ld N[6] = {0}, dNx[6] = {0}, dNe[6] = {0}, wq;
             if (npf == 4) {                          /* cyclic node order (-1,-1),(1,-1),(1,1),(-1,1) */
                 ld xi = (q & 1) ? g : -g, et = (q & 2) ? g : -g;
                 const ld sx[4] = {-1, 1, 1, -1}, se[4] = {-1, -1, 1, 1};
@@ -516,10 +523,22 @@ void oracle_surface_loads(int64_t n_nodes, int64_t n_faces, int32_t npf, const i
                     dNe[a] = 0.25L * (1 + sx[a] * xi) * se[a];
                 }
                 wq = 1.0L;
+            } else if (npf == 6) {                   /* nodes: vertices 0,1,2, then the middles of 01, 12, 20 */
+                ld t = q < 3 ? qa : qb;
+                int k = q % 3;
+                ld xi = k == 2 ? 1.0L - 2.0L * t : t, et = k == 1 ? 1.0L - 2.0L * t : t;
+                ld l0 = 1.0L - xi - et, l1 = xi, l2 = et;
+                N[0] = l0 * (2 * l0 - 1); N[1] = l1 * (2 * l1 - 1); N[2] = l2 * (2 * l2 - 1);
+                N[3] = 4 * l0 * l1; N[4] = 4 * l1 * l2; N[5] = 4 * l2 * l0;
+                dNx[0] = -(4 * l0 - 1); dNx[1] = 4 * l1 - 1; dNx[2] = 0;
+                dNx[3] = 4 * (l0 - l1); dNx[4] = 4 * l2; dNx[5] = -4 * l2;
+                dNe[0] = -(4 * l0 - 1); dNe[1] = 0; dNe[2] = 4 * l2 - 1;
+                dNe[3] = -4 * l1; dNe[4] = 4 * l1; dNe[5] = 4 * (l0 - l2);
+                wq = 0.5L * (q < 3 ? wa : wb);
             } else {                                 /* N = (1-xi-eta, xi, eta) at the centroid, weight 1/2 */
-                N[0] = N[1] = N[2] = 1.0L / 3.0L; N[3] = 0;
-                dNx[0] = -1; dNx[1] = 1; dNx[2] = 0; dNx[3] = 0;
-                dNe[0] = -1; dNe[1] = 0; dNe[2] = 1; dNe[3] = 0;
+                N[0] = N[1] = N[2] = 1.0L / 3.0L;
+                dNx[0] = -1; dNx[1] = 1; dNx[2] = 0;
+                dNe[0] = -1; dNe[1] = 0; dNe[2] = 1;
                 wq = 0.5L;
             }
             ld tX[2][3] = {{0}}, tx[2][3] = {{0}};

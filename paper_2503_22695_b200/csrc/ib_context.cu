@@ -316,7 +316,7 @@ extern "C" ib_status ib_set_tethers(ib_ctx *c, int64_t n, const int32_t *ids, do
 
 extern "C" ib_status ib_set_surface(ib_ctx *c, int64_t n_faces, int32_t npf, const int32_t *faces)
 {
-    if (!c || n_faces < 0 || (n_faces > 0 && (!faces || (npf != 3 && npf != 4)))) return IB_ERR_INVALID_ARG;
+    if (!c || n_faces < 0 || (n_faces > 0 && (!faces || (npf != 3 && npf != 4 && npf != 6)))) return IB_ERR_INVALID_ARG;
     for (int64_t k = 0; k < n_faces * npf; ++k)
         if (faces[k] < 0 || faces[k] >= c->n_nodes) return IB_ERR_INVALID_ARG;
     if (cudaSetDevice(c->device) != cudaSuccess) return IB_ERR_CUDA;

@@ -503,6 +503,61 @@ ibk_surface_loads(int64_t n_faces, int npf, int64_t n_nodes, const int32_t *__re
         for (int c = 0; c < 3; ++c) atomicAdd(B + c * n_nodes + nd[a], add[a][c]);
 }
 
+// the same for 6-node (quadratic) triangles, the faces of the P2 tetrahedra: nodes = 3 vertices, then the
+// middles of v0v1, v1v2, v2v0; symmetric 6-point rule of degree 4 (reading A27), one thread per face
+__global__ void __launch_bounds__(128)
+ibk_surface_loads_t6(int64_t n_faces, int64_t n_nodes, const int32_t *__restrict__ faces,
+                     const double *__restrict__ X, const double *__restrict__ x, double q0, double q1, double q2,
+                     double p, double *__restrict__ B)
+{
+    int64_t f = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (f >= n_faces) return;
+    int nd[6];
+    double Xf[6][3], xf[6][3], add[6][3];
+#pragma unroll
+    for (int a = 0; a < 6; ++a) {
+        nd[a] = faces[f * 6 + a];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            Xf[a][c] = X[c * n_nodes + nd[a]]; xf[a][c] = x[c * n_nodes + nd[a]];
+            add[a][c] = 0.0;
+        }
+    }
+    const double qv[3] = {q0, q1, q2};
+    // a,b = (8 - sqrt10 +- sqrt(38 - 44 sqrt(2/5)))/18; weights (620 +- sqrt(213125 - 53320 sqrt10))/3720, halved (area 1/2)
+    const double ta = 0.44594849091596488632, tb = 0.091576213509770743460;
+    const double wa = 0.5 * 0.22338158967801146570, wb = 0.5 * 0.10995174365532186764;
+#pragma unroll 1
+    for (int q = 0; q < 6; ++q) {
+        const double t = q < 3 ? ta : tb, wq = q < 3 ? wa : wb;
+        const int k = q < 3 ? q : q - 3;
+        const double xi = (k == 2) ? 1.0 - 2.0 * t : t, et = (k == 1) ? 1.0 - 2.0 * t : t;
+        const double l0 = 1.0 - xi - et, l1 = xi, l2 = et;
+        const double N[6] = {l0 * (2.0 * l0 - 1.0), l1 * (2.0 * l1 - 1.0), l2 * (2.0 * l2 - 1.0), 4.0 * l0 * l1, 4.0 * l1 * l2, 4.0 * l2 * l0};
+        const double d1[6] = {-(4.0 * l0 - 1.0), 4.0 * l1 - 1.0, 0.0, 4.0 * (l0 - l1), 4.0 * l2, -4.0 * l2};
+        const double d2[6] = {-(4.0 * l0 - 1.0), 0.0, 4.0 * l2 - 1.0, -4.0 * l1, 4.0 * l1, 4.0 * (l0 - l2)};
+        double T1[3] = {0, 0, 0}, T2[3] = {0, 0, 0}, t1[3] = {0, 0, 0}, t2[3] = {0, 0, 0};
+#pragma unroll
+        for (int a = 0; a < 6; ++a)
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                T1[c] = fma(d1[a], Xf[a][c], T1[c]); T2[c] = fma(d2[a], Xf[a][c], T2[c]);
+                t1[c] = fma(d1[a], xf[a][c], t1[c]); t2[c] = fma(d2[a], xf[a][c], t2[c]);
+            }
+        const double NX[3] = {T1[1] * T2[2] - T1[2] * T2[1], T1[2] * T2[0] - T1[0] * T2[2], T1[0] * T2[1] - T1[1] * T2[0]};
+        const double nx[3] = {t1[1] * t2[2] - t1[2] * t2[1], t1[2] * t2[0] - t1[0] * t2[2], t1[0] * t2[1] - t1[1] * t2[0]};
+        const double dA = sqrt(NX[0] * NX[0] + NX[1] * NX[1] + NX[2] * NX[2]);
+#pragma unroll
+        for (int a = 0; a < 6; ++a)
+#pragma unroll
+            for (int c = 0; c < 3; ++c) add[a][c] += wq * N[a] * (qv[c] * dA - p * nx[c]);
+    }
+#pragma unroll
+    for (int a = 0; a < 6; ++a)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) atomicAdd(B + c * n_nodes + nd[a], add[a][c]);
+}
+
 __global__ void __launch_bounds__(256)
 ibk_fhat(int64_t n_nodes, const double *__restrict__ B, const double *__restrict__ wa, double *__restrict__ Fhat)
 {
@@ -525,8 +580,12 @@ static ib_status ib_add_loads(ib_ctx *c, const double *x, double *B, cudaStream_
         c->launches++;
     }
     if (c->n_faces > 0 && (c->p_load != 0.0 || c->qt0[0] != 0.0 || c->qt0[1] != 0.0 || c->qt0[2] != 0.0)) {
-        ibk_surface_loads<<<ib_blocks(c->n_faces, 128), 128, 0, st>>>(c->n_faces, c->npf, c->n_nodes, c->d_faces, c->d_X, x,
-                                                                     c->qt0[0], c->qt0[1], c->qt0[2], c->p_load, B);
+        if (c->npf == 6)
+            ibk_surface_loads_t6<<<ib_blocks(c->n_faces, 128), 128, 0, st>>>(c->n_faces, c->n_nodes, c->d_faces, c->d_X, x,
+                                                                            c->qt0[0], c->qt0[1], c->qt0[2], c->p_load, B);
+        else
+            ibk_surface_loads<<<ib_blocks(c->n_faces, 128), 128, 0, st>>>(c->n_faces, c->npf, c->n_nodes, c->d_faces, c->d_X, x,
+                                                                         c->qt0[0], c->qt0[1], c->qt0[2], c->p_load, B);
         c->launches++;
     }
     IB_CUDA_TRY(cudaGetLastError());

@@ -129,15 +129,19 @@ def p2_from_tets(tets, X):
 
 _HEX_FACES = np.array([[0, 4, 6, 2], [1, 3, 7, 5], [0, 1, 5, 4], [2, 6, 7, 3], [0, 2, 3, 1], [4, 5, 7, 6]])
 _TET_FACES = np.array([[1, 2, 3], [0, 3, 2], [0, 1, 3], [0, 2, 1]])
+# the same faces of a 10-node tetrahedron (p2_from_tets order): 3 vertices, then the middles of the edges
+# (v0 v1), (v1 v2), (v2 v0) of the face
+_TET10_FACES = np.array([[1, 2, 3, 5, 9, 8], [0, 3, 2, 7, 9, 6], [0, 1, 3, 4, 8, 7], [0, 2, 1, 6, 5, 4]])
 
 
 def boundary_faces(conn):
     """Faces that belong to exactly one element, nodes in cyclic order with the normal pointing out of the
-    element (right-handed elements): [nf,4] for hexahedra, [nf,3] for tetrahedra.  Inputs for the surface
-    loads of NEXT-4 (pressure on the endocardium L303, traction on the Cook membrane's face L263)."""
-    loc = _HEX_FACES if conn.shape[1] == 8 else _TET_FACES
+    element (right-handed elements): [nf,4] for hexahedra, [nf,3] for linear and [nf,6] for quadratic
+    tetrahedra.  Inputs for the surface loads of NEXT-4 (pressure on the endocardium L303, traction on the
+    Cook membrane's face L263)."""
+    loc = {8: _HEX_FACES, 4: _TET_FACES, 10: _TET10_FACES}[conn.shape[1]]
     faces = conn[:, loc].reshape(-1, loc.shape[1])
-    key = np.sort(faces, axis=1)
+    key = np.sort(faces[:, :3] if conn.shape[1] == 10 else faces, axis=1)
     _, inv, cnt = np.unique(key, axis=0, return_inverse=True, return_counts=True)
     return np.ascontiguousarray(faces[cnt[inv.ravel()] == 1]).astype(np.int32)
 

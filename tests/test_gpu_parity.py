@@ -484,15 +484,21 @@ def test_graph_replay_matches_eager_step(ib, orc):
 
 
 # ---- NEXT-4: solid boundary loads ---------------------------------------------------------------------
-@pytest.mark.parametrize("kind", ["hex-sub", "hex-nodal", "tet"])
+@pytest.mark.parametrize("kind", ["hex-sub", "hex-nodal", "tet", "tet10"])
 def test_boundary_loads_enter_force_and_step(ib, orc, kind):
     """Tethers (L263, L425), dead traction (L263) and follower pressure (L303, L315) are added to B by
     ib_fe_force and reach the grid through the step (Fhat = B / w_a includes them)."""
     import torch
     conn, X, x, fib = distorted_block(5, 4, 3, size=(0.3, 0.25, 0.2), seed=41, ref_noise=0.1, cur_noise=0.05)
-    if kind == "tet":
+    if kind in ("tet", "tet10"):
         conn = W.tets_from_hexes(conn, X)
         fib = None
+    if kind == "tet10":                                           # 6-node faces with curved edges (reading A27)
+        nv = X.shape[1]
+        conn, X = W.p2_from_tets(conn, X)
+        rng = np.random.default_rng(43)
+        X[:, nv:] += 0.004 * rng.uniform(-1, 1, (3, X.shape[1] - nv))
+        x = X + 0.004 * rng.uniform(-1, 1, X.shape)
     ne, nn = conn.shape[0], X.shape[1]
     nsub = np.tile([3, 2, 2], (ne, 1)).astype(np.int32) if kind == "hex-sub" else None
     mats = [W.material(W.LAW_NEOHOOKEAN, a=80.0, kappa=4e4)]

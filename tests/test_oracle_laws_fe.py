@@ -609,3 +609,86 @@ def test_p2_rigid_motion_and_patch(orc):
                 on_bnd[row[4 + k]] = True
     assert (~on_bnd).sum() >= 5
     assert np.max(np.abs(B[:, ~on_bnd])) < 1e-10 * np.max(np.abs(B[:, on_bnd]))
+
+
+# ---- NEXT-4 on P2 meshes: loads on 6-node (quadratic) faces, reading A27 ------------------------------
+_T6_MONO = np.zeros((6, 3, 3))                            # N_a = sum_ij c[a,i,j] xi^i eta^j
+_T6_MONO[0, 0, 0], _T6_MONO[0, 1, 0], _T6_MONO[0, 0, 1] = 1, -3, -3
+_T6_MONO[0, 2, 0], _T6_MONO[0, 1, 1], _T6_MONO[0, 0, 2] = 2, 4, 2
+_T6_MONO[1, 1, 0], _T6_MONO[1, 2, 0] = -1, 2
+_T6_MONO[2, 0, 1], _T6_MONO[2, 0, 2] = -1, 2
+_T6_MONO[3, 1, 0], _T6_MONO[3, 2, 0], _T6_MONO[3, 1, 1] = 4, -4, -4
+_T6_MONO[4, 1, 1] = 4
+_T6_MONO[5, 0, 1], _T6_MONO[5, 1, 1], _T6_MONO[5, 0, 2] = 4, -4, -4
+
+
+def _pmul(a, b):
+    out = np.zeros((a.shape[0] + b.shape[0] - 1, a.shape[1] + b.shape[1] - 1))
+    for i in range(a.shape[0]):
+        for j in range(a.shape[1]):
+            out[i:i + b.shape[0], j:j + b.shape[1]] += a[i, j] * b
+    return out
+
+
+def _pint(a):
+    """integral over the unit triangle: xi^i eta^j -> i! j! / (i + j + 2)!"""
+    from math import factorial as f
+    return sum(a[i, j] * f(i) * f(j) / f(i + j + 2) for i in range(a.shape[0]) for j in range(a.shape[1]))
+
+
+def _t6_volume_exact(faces, x):
+    """(1/3) closed-surface integral of x.(x_xi x x_eta) over quadratic triangles, integrated exactly by
+    polynomial algebra (the integrand has degree 4) -- no quadrature rule involved."""
+    V = 0.0
+    for f in faces:
+        X3 = [np.tensordot(x[c, f], _T6_MONO, axes=(0, 0)) for c in range(3)]           # 3 polynomials [3,3]
+        dxi = [np.pad(q[1:, :] * np.arange(1, 3)[:, None], ((0, 1), (0, 0))) for q in X3]
+        det = [np.pad(q[:, 1:] * np.arange(1, 3)[None, :], ((0, 0), (0, 1))) for q in X3]
+        cr = [_pmul(dxi[1], det[2]) - _pmul(dxi[2], det[1]), _pmul(dxi[2], det[0]) - _pmul(dxi[0], det[2]),
+              _pmul(dxi[0], det[1]) - _pmul(dxi[1], det[0])]
+        V += sum(_pint(_pmul(X3[c], cr[c])) for c in range(3)) / 3
+    return V
+
+
+def test_p2_face_loads_pins(orc):
+    c10, X10, x10 = _p2_block(seed=8, bend=0.012)
+    faces = W.boundary_faces(c10)
+    assert faces.shape == (2 * 2 * (6 + 6 + 4), 6)
+    nn = X10.shape[1]
+    zero = np.zeros((3, nn))
+    # orientation and bookkeeping: with straight edges the closed surface encloses the volume of the tetrahedra
+    c10s, X10s, _ = _p2_block(seed=8, bend=0.0)
+    Pt = X10s[:, c10s[:, :4]]
+    vol = np.einsum("in,in->n", np.cross((Pt[:, :, 1] - Pt[:, :, 0]).T, (Pt[:, :, 2] - Pt[:, :, 0]).T).T,
+                    Pt[:, :, 3] - Pt[:, :, 0]).sum() / 6
+    assert abs(_t6_volume_exact(W.boundary_faces(c10s), X10s) - vol) < 1e-13 * vol
+    # follower pressure on the curved closed surface: B = -p dV/dx (vertex and mid-edge nodes), no net force or torque
+    p = 2.9
+    Bp = orc.surface_loads(faces, X10, x10, None, p, zero)
+    on_surf = np.unique(faces)
+    rng = np.random.default_rng(4)
+    eps = 1e-6
+    for n in rng.choice(on_surf, 12, replace=False):
+        c = rng.integers(0, 3)
+        xp, xm = x10.copy(), x10.copy()
+        xp[c, n] += eps
+        xm[c, n] -= eps
+        fd = -p * (_t6_volume_exact(faces, xp) - _t6_volume_exact(faces, xm)) / (2 * eps)
+        assert abs(fd - Bp[c, n]) < 1e-8 * np.max(np.abs(Bp)), (c, n)
+    assert np.max(np.abs(Bp.sum(axis=1))) < 1e-13 * np.max(np.abs(Bp)) * nn
+    assert np.max(np.abs(np.cross(x10.T, Bp.T).sum(axis=0))) < 1e-12 * np.max(np.abs(Bp)) * nn
+    interior = np.setdiff1d(np.arange(nn), on_surf)
+    assert np.all(Bp[:, interior] == 0)
+    # one flat straight-sided face, closed form: int N_vertex = 0 and int N_mid = A/3, so the vertices carry
+    # nothing and every mid-edge node a third of the load -- pressure along the normal, traction along t0
+    V3 = np.array([[0.1, 1.3, 0.4], [0.2, 0.3, 1.5], [0.0, 0.4, 0.1]])
+    Xf = np.concatenate([V3, 0.5 * (V3[:, [0, 1, 2]] + V3[:, [1, 2, 0]])], axis=1)
+    one = np.arange(6, dtype=np.int32)[None, :]
+    nA = 0.5 * np.cross(V3[:, 1] - V3[:, 0], V3[:, 2] - V3[:, 0])                 # area vector
+    Bf = orc.surface_loads(one, Xf, Xf, None, p, np.zeros((3, 6)))
+    assert np.max(np.abs(Bf[:, :3])) < 1e-15
+    assert np.allclose(Bf[:, 3:], np.repeat((-p * nA / 3)[:, None], 3, axis=1), rtol=1e-14, atol=1e-16)
+    qt0 = np.array([0.5, -2.0, 1.25])
+    Bq = orc.surface_loads(one, Xf, 1.7 * Xf, qt0, 0.0, np.zeros((3, 6)))          # current configuration is irrelevant
+    assert np.max(np.abs(Bq[:, :3])) < 1e-15
+    assert np.allclose(Bq[:, 3:], np.repeat((qt0 * np.linalg.norm(nA) / 3)[:, None], 3, axis=1), rtol=1e-14)
