@@ -510,20 +510,18 @@ ibk_small_tiles(ib_tiled_params pr, const int32_t *__restrict__ small_rec, const
 template <int S, int I, int PER>
 static ib_status launch_tiled_p(ib_ctx *c, const ib_tiled_params &pr, bool with_small, cudaStream_t st)
 {
-    static int configured = 0;
+    static unsigned char configured[64] = {0};           // per device: function attributes belong to the device's context
+    static int sm_count[64] = {0};
+    const int dv = c->device & 63;
     const size_t smem = (size_t)(3 * SU3 + 3 * CH + NWARP * 8 * GSTRIDE) * sizeof(double) +
                         (NOC + 68) * sizeof(int) + (516 + 2 * NITEM + CH) * sizeof(unsigned short);
     static_assert(CH % TB == 0, "chunk must be a whole number of points per thread");
-    if (!configured) {
+    if (!configured[dv]) {
         IB_CUDA_TRY(cudaFuncSetAttribute(ibk_tiled_kernel<S, I, PER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured = 1;
+        configured[dv] = 1;
     }
-    static int sms = 0;
-    if (!sms) {
-        cudaDeviceProp prop;
-        IB_CUDA_TRY(cudaGetDeviceProperties(&prop, c->device));
-        sms = prop.multiProcessorCount;
-    }
+    if (!sm_count[dv]) IB_CUDA_TRY(cudaDeviceGetAttribute(&sm_count[dv], cudaDevAttrMultiProcessorCount, c->device));
+    const int sms = sm_count[dv];
     // the few points of sparsely filled tiles go one by one on a second stream, beside the tile kernel
     const int64_t nsmall_max = min((int64_t)pr.P, (c->n_cells / (TT * TT * TT)) * (int64_t)(IB_SMALL_TILE - 1));
     const bool beside = !c->profile && with_small;
