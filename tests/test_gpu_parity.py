@@ -6,7 +6,7 @@ array (A20); bit-exact for the integer binning/sort permutation.
 import numpy as np
 import pytest
 
-from helpers import distorted_block, max_abs_scaled, rel_l2
+from helpers import distorted_block, max_abs_scaled, rel_l2, rotation
 from paper_2503_22695_b200 import workloads as W
 
 pytestmark = pytest.mark.gpu
@@ -222,7 +222,7 @@ def test_host_entry_point_matches_device_path(ib, name, variant):
     ctx.close()
 
 
-@pytest.mark.parametrize("case", ["wrap", "bounded", "one-slab", "pageable"])
+@pytest.mark.parametrize("case", ["wrap", "bounded", "one-slab", "pageable", "non-cubic"])
 def test_host_step_slabs_against_oracle(ib, orc, case):
     """ib_coupling_step_host cuts the step into z-slabs (copies of u,v,w and f overlap the tile kernel):
     a structure across the periodic z wrap (first and last slab share points), a bounded grid with the
@@ -238,16 +238,28 @@ def test_host_step_slabs_against_oracle(ib, orc, case):
         periodic = 0
     elif case == "pageable":                      # plain (unpinned) host memory: slower copies, same answer
         shift = np.zeros(3)
+    elif case == "non-cubic":                     # 24 x 16 x 40 cells: 5 slabs of 2 tile layers, the slab tilted across them
+        shift = np.zeros(3)
     else:
         nz = 8
         shift = np.zeros(3)
         org[2] = 0.5 * (wl.X[2].min() + wl.X[2].max()) - 4 * wl.h + 0.21 * wl.h
     X, x = wl.X + shift[:, None], wl.x + shift[:, None]
-    ncell = wl.nx * wl.ny * nz
-    u, v, w = (np.ascontiguousarray(a.reshape(wl.nz, wl.ny, wl.nx)[:nz].reshape(-1)) for a in (wl.u, wl.v, wl.w))
-    g = orc.make_grid(wl.nx, wl.ny, nz, wl.h, tuple(org), periodic=periodic)
+    nx, ny = wl.nx, wl.ny
+    if case == "non-cubic":
+        nx, ny, nz = 24, 16, 40
+        org = np.array([0.125, 0.25, -0.125])
+        c0 = 0.5 * (wl.X.min(axis=1) + wl.X.max(axis=1))
+        R = rotation(5)                                       # the slab turned out of its plane: it spans several z-slabs
+        X, x = c0[:, None] + R @ (wl.X - c0[:, None]), c0[:, None] + R @ (wl.x - c0[:, None])
+    ncell = nx * ny * nz
+    if case == "non-cubic":
+        u, v, w = np.random.default_rng(77).normal(size=(3, ncell))
+    else:
+        u, v, w = (np.ascontiguousarray(a.reshape(wl.nz, wl.ny, wl.nx)[:nz].reshape(-1)) for a in (wl.u, wl.v, wl.w))
+    g = orc.make_grid(nx, ny, nz, wl.h, tuple(org), periodic=periodic)
     ref = orc.coupling_step(g, wl.conn, X, wl.fibers, wl.mat_id, wl.nsub, wl.mats, x, u, v, w)
-    ctx = ib.Context(wl.nx, wl.ny, nz, wl.h, tuple(org), wl.conn, X, wl.fibers, wl.mat_id, wl.nsub, wl.mats, periodic=periodic)
+    ctx = ib.Context(nx, ny, nz, wl.h, tuple(org), wl.conn, X, wl.fibers, wl.mat_id, wl.nsub, wl.mats, periodic=periodic)
     pin = (lambda a: torch.from_numpy(np.array(a, order="C"))) if case == "pageable" else \
           (lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory())
     outs = [pin(np.full(ncell, 9.0)) for _ in range(3)]
