@@ -77,3 +77,51 @@ __device__ __forceinline__ void ib_point_direct(double x, double y, double z, co
         U[c] = acc;
     }
 }
+
+// The same with 4 lanes per point, lane q = the q-th face of every x-row of the support: the 4 lanes of a
+// group hit 4 consecutive faces, so a warp's RED or load touches 8-16 sectors instead of 32 (the direct path
+// of the sparse tiles is bound by L2 reduction traffic, not by arithmetic; every lane recomputes the weights).
+// All 4 lanes must call; qmask = the group's lanes.  U is complete in every lane of the group.
+template <int DO_SPREAD, int DO_INTERP>
+__device__ __forceinline__ void ib_point_quad(double x, double y, double z, const double G[3],
+                                              const double *const fld[3], double *const frc[3],
+                                              const ib_grid_desc &g, double inv_h, int q, unsigned qmask, double U[3])
+{
+    ib_stencil s;
+    ib_axis(x, g.x0, g.h, inv_h, g.nx, g.periodic, s.ix, s.wx);
+    ib_axis(y, g.y0, g.h, inv_h, g.ny, g.periodic, s.iy, s.wy);
+    ib_axis(z, g.z0, g.h, inv_h, g.nz, g.periodic, s.iz, s.wz);
+    int ixq[2];
+    double wxq[2];
+#pragma unroll
+    for (int o = 0; o < 2; ++o) {                       // selects, not indexing: the arrays stay in registers
+        ixq[o] = q == 0 ? s.ix[o][0] : q == 1 ? s.ix[o][1] : q == 2 ? s.ix[o][2] : s.ix[o][3];
+        wxq[o] = q == 0 ? s.wx[o][0] : q == 1 ? s.wx[o][1] : q == 2 ? s.wx[o][2] : s.wx[o][3];
+    }
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const int ox = (c == 0) ? 0 : 1, oy = (c == 1) ? 0 : 1, oz = (c == 2) ? 0 : 1;
+        const bool xin = ixq[ox] >= 0;
+        const double gx = DO_SPREAD ? G[c] * wxq[ox] : 0.0;
+        double acc = 0.0;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const double gk = gx * s.wz[oz][k];
+            double ak = 0.0;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                if (s.iz[oz][k] < 0 || s.iy[oy][j] < 0 || !xin) continue;           // outside a bounded grid
+                const int64_t at = ((int64_t)s.iz[oz][k] * g.ny + s.iy[oy][j]) * g.nx + ixq[ox];
+                if (DO_INTERP) ak = fma(__ldg(fld[c] + at), s.wy[oy][j], ak);
+                if (DO_SPREAD) atomicAdd(frc[c] + at, gk * s.wy[oy][j]);
+            }
+            if (DO_INTERP) acc = fma(ak, s.wz[oz][k], acc);
+        }
+        if (DO_INTERP) {
+            acc *= wxq[ox];
+            acc += __shfl_xor_sync(qmask, acc, 1);
+            acc += __shfl_xor_sync(qmask, acc, 2);
+        }
+        U[c] = acc;
+    }
+}

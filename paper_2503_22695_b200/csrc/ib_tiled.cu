@@ -494,17 +494,30 @@ template <int DO_SPREAD, int DO_INTERP>
 __global__ void __launch_bounds__(128)
 ibk_small_tiles(ib_tiled_params pr, const int32_t *__restrict__ small_rec, const int32_t *__restrict__ counters)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= counters[2]) return;
+    // 4 lanes per point (ib_point_quad); the list length is known on the device only, so the grid is sized for
+    // the device and strides over the list
+    const int q = threadIdx.x & 3;
+    const unsigned qmask = 0xFu << (threadIdx.x & 28);
     const int64_t P = pr.P;
-    const int r = __ldg(small_rec + i);
-    double G[3] = {0, 0, 0}, U[3];
-    if (DO_SPREAD) { G[0] = pr.sG[r] * pr.ih3; G[1] = pr.sG[P + r] * pr.ih3; G[2] = pr.sG[2 * P + r] * pr.ih3; }
-    ib_point_direct<DO_SPREAD, DO_INTERP>(pr.sx[r], pr.sx[P + r], pr.sx[2 * P + r], G, pr.fld, pr.frc, pr.g, pr.inv_h, U);
-    if (DO_INTERP) {
-        const int id = pr.sid[r];
-        pr.Up[id] = U[0]; pr.Up[P + id] = U[1]; pr.Up[2 * P + id] = U[2];
+    const int n = counters[2], stride = (gridDim.x * blockDim.x) >> 2;
+    for (int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 2; i < n; i += stride) {
+        const int r = __ldg(small_rec + i);
+        double G[3] = {0, 0, 0}, U[3];
+        if (DO_SPREAD) { G[0] = pr.sG[r] * pr.ih3; G[1] = pr.sG[P + r] * pr.ih3; G[2] = pr.sG[2 * P + r] * pr.ih3; }
+        ib_point_quad<DO_SPREAD, DO_INTERP>(pr.sx[r], pr.sx[P + r], pr.sx[2 * P + r], G, pr.fld, pr.frc, pr.g, pr.inv_h, q, qmask, U);
+        if (DO_INTERP && q == 0) {
+            const int id = pr.sid[r];
+            pr.Up[id] = U[0]; pr.Up[P + id] = U[1]; pr.Up[2 * P + id] = U[2];
+        }
     }
+}
+
+// blocks of the sparse-tile kernel: enough for the longest possible list, at most 16 per SM (grid stride)
+static int ib_small_blocks(int64_t nsmall_max, int sms)
+{
+    const int64_t need = (nsmall_max * 4 + 127) / 128;
+    const int64_t cap = (int64_t)(sms > 0 ? sms : 148) * 16;
+    return (int)(need < 1 ? 1 : (need < cap ? need : cap));
 }
 
 template <int S, int I, int PER>
@@ -530,7 +543,7 @@ static ib_status launch_tiled_p(ib_ctx *c, const ib_tiled_params &pr, bool with_
         IB_CUDA_TRY(cudaEventRecord(c->ev_sfork, st));
         IB_CUDA_TRY(cudaStreamWaitEvent(s3, c->ev_sfork, 0));
     }
-    if (with_small) ibk_small_tiles<S, I><<<ib_blocks(nsmall_max, 128), 128, 0, s3>>>(pr, c->d_small_rec, c->d_tile_count);
+    if (with_small) ibk_small_tiles<S, I><<<ib_small_blocks(nsmall_max, sms), 128, 0, s3>>>(pr, c->d_small_rec, c->d_tile_count);
     if (beside) IB_CUDA_TRY(cudaEventRecord(c->ev_sjoin, s3));
     ibk_tiled_kernel<S, I, PER><<<sms * NCTA, TB, smem, st>>>(pr);
     if (beside) IB_CUDA_TRY(cudaStreamWaitEvent(st, c->ev_sjoin, 0));
@@ -609,7 +622,7 @@ ib_status ibk_small_launch(ib_ctx *c, int64_t P, int do_spread, int do_interp,
     ib_tiled_params pr;
     fill_params(c, pr, P, u, v, w, fu, fv, fw, Up, -1);
     const int64_t nsmall_max = min((int64_t)P, (c->n_cells / (TT * TT * TT)) * (int64_t)(IB_SMALL_TILE - 1));
-    const int nb = ib_blocks(nsmall_max, 128);
+    const int nb = ib_small_blocks(nsmall_max, 0);
     if (do_spread && do_interp) ibk_small_tiles<1, 1><<<nb, 128, 0, st>>>(pr, c->d_small_rec, c->d_tile_count);
     else if (do_spread) ibk_small_tiles<1, 0><<<nb, 128, 0, st>>>(pr, c->d_small_rec, c->d_tile_count);
     else ibk_small_tiles<0, 1><<<nb, 128, 0, st>>>(pr, c->d_small_rec, c->d_tile_count);
