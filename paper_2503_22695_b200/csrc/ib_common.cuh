@@ -16,8 +16,10 @@
 #define IB_SLABC0 40              // d_tile_count[IB_SLABC0 + k] = work counter of slab k
 #define IB_TILE_HDR 80            // ints of d_tile_count before the partial sums of the scan
 #ifndef IB_HOST_SLABS
-#define IB_HOST_SLABS 8           // z-slabs ib_coupling_step_host cuts the spreading into
+#define IB_HOST_SLABS 8           // z-slabs ib_coupling_step_host cuts the step into
 #endif
+static_assert(IB_HOST_SLABS >= 1 && IB_HOST_SLABS <= IB_MAX_SLABS, "IB_HOST_SLABS out of range");
+static_assert(IB_SLAB0 + IB_MAX_SLABS < IB_SLABC0 && IB_SLABC0 + IB_MAX_SLABS <= IB_TILE_HDR, "d_tile_count header layout");
 
 // ---------------------------------------------------------------------------------------------
 // host-side context
