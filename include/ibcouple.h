@@ -170,7 +170,8 @@ ib_status ib_step_eq16(ib_ctx *ctx, const double *x, const double *u, const doub
  * In the default variant the step is pipelined in z-slabs of the grid (up to 8): the force side, which
  * needs only x, runs while u,v,w cross the bus slab by slab; the fused spread + interpolate kernel of a
  * slab starts when the velocity layers of that slab and its neighbours have arrived; the layers of
- * fu,fv,fw that a finished slab can no longer touch travel back while the next slabs run. The host
+ * fu,fv,fw that a finished slab can no longer touch travel back while the next slabs run (layers out of
+ * the structure's reach -- found from the z-range of x_host -- go back as soon as they are zero-filled). The host
  * arrays are therefore written in pieces: none of them is valid before the call returns. */
 ib_status ib_coupling_step_host(ib_ctx *ctx, const double *x_host, const double *u_host,
                                 const double *v_host, const double *w_host, double *fu_host,

@@ -83,6 +83,7 @@ struct ib_ctx {
     cudaStream_t side3;        // ib_coupling_step_host: f goes back to the host slab by slab on this stream
     cudaStream_t side4;        // ... and the odd slabs of the tile kernel run on this one
     cudaEvent_t ev_slab[IB_MAX_SLABS], ev_h2d[IB_MAX_SLABS];
+    cudaEvent_t ev_zero;       // ... f has been zero-filled
     int64_t launches;
     // NEXT-4 boundary loads (ib_set_tethers / ib_set_surface / ib_set_loads)
     int32_t *d_teth_ids, *d_faces;

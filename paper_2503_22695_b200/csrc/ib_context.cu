@@ -122,6 +122,7 @@ extern "C" ib_status ib_destroy(ib_ctx *c)
     if (c->side4) cudaStreamDestroy(c->side4);
     for (cudaEvent_t e : c->ev_h2d)
         if (e) cudaEventDestroy(e);
+    if (c->ev_zero) cudaEventDestroy(c->ev_zero);
     for (cudaEvent_t e : c->ev_slab)
         if (e) cudaEventDestroy(e);
     if (c->prof) {
@@ -255,6 +256,7 @@ extern "C" ib_status ib_create(ib_ctx **out, const ib_grid_desc *g, const ib_mes
                        cudaEventCreateWithFlags(&c->ev_sfork, cudaEventDisableTiming) != cudaSuccess ||
                        cudaEventCreateWithFlags(&c->ev_sjoin, cudaEventDisableTiming) != cudaSuccess))
         s = IB_ERR_CUDA;
+    if (s == IB_OK && cudaEventCreateWithFlags(&c->ev_zero, cudaEventDisableTiming) != cudaSuccess) s = IB_ERR_CUDA;
     if (s == IB_OK && (cudaStreamCreateWithFlags(&c->side3, cudaStreamNonBlocking) != cudaSuccess ||
                        cudaStreamCreateWithFlags(&c->side4, cudaStreamNonBlocking) != cudaSuccess))
         s = IB_ERR_CUDA;
@@ -681,6 +683,20 @@ extern "C" ib_status ib_coupling_step_host(ib_ctx *c, const double *x_h, const d
     IB_CUDA_TRY(cudaMemcpyAsync(c->d_hx, x_h, nb, cudaMemcpyHostToDevice, st));
     IB_CUDA_TRY(cudaEventRecord(c->ev_fork, st));             // orders the side streams after x and earlier work on st
     IB_CUDA_TRY(cudaStreamWaitEvent(s2, c->ev_fork, 0));
+    IB_TR(st, "x on device");
+    // zero-fill of f and the count pass of the binning beside the FE force, as in ib_coupling_step
+    IB_CUDA_TRY(cudaStreamWaitEvent(ss, c->ev_fork, 0));
+    IB_CUDA_TRY(cudaMemsetAsync(c->d_hfu, 0, gb, ss));
+    IB_CUDA_TRY(cudaMemsetAsync(c->d_hfv, 0, gb, ss));
+    IB_CUDA_TRY(cudaMemsetAsync(c->d_hfw, 0, gb, ss));
+    IB_CUDA_TRY(cudaEventRecord(c->ev_zero, ss));             // f is zero
+    s = ibk_bin_reserve(c, c->n_points);
+    if (s == IB_OK) s = ibk_bin_points(c, 1, nullptr, nullptr, c->n_points, c->d_hx, nullptr, nullptr, 1, ss);
+    IB_CUDA_TRY(cudaEventRecord(c->ev_join, ss));
+    IB_TR(ss, "zero + count + scan");
+    if (s == IB_OK) s = ibk_fe_force(c, c->d_hx, Bd, c->d_Fhat, st);
+    IB_TR(st, "FE force");
+    if (s != IB_OK) return s;
     {
         const double *uh[3] = {u_h, v_h, w_h};
         double *ud[3] = {c->d_hu, c->d_hv, c->d_hw};
@@ -699,18 +715,33 @@ extern "C" ib_status ib_coupling_step_host(ib_ctx *c, const double *x_h, const d
             IB_TR(s2, "uvw slab on device");
         }
     }
-    IB_TR(st, "x on device");
-    // zero-fill of f and the count pass of the binning beside the FE force, as in ib_coupling_step
-    IB_CUDA_TRY(cudaStreamWaitEvent(ss, c->ev_fork, 0));
-    IB_CUDA_TRY(cudaMemsetAsync(c->d_hfu, 0, gb, ss));
-    IB_CUDA_TRY(cudaMemsetAsync(c->d_hfv, 0, gb, ss));
-    IB_CUDA_TRY(cudaMemsetAsync(c->d_hfw, 0, gb, ss));
-    s = ibk_bin_reserve(c, c->n_points);
-    if (s == IB_OK) s = ibk_bin_points(c, 1, nullptr, nullptr, c->n_points, c->d_hx, nullptr, nullptr, 1, ss);
-    IB_CUDA_TRY(cudaEventRecord(c->ev_join, ss));
-    IB_TR(ss, "zero + count + scan");
-    if (s == IB_OK) s = ibk_fe_force(c, c->d_hx, Bd, c->d_Fhat, st);
-    IB_TR(st, "FE force");
+    // While the device is busy with all that, the host finds the z-layers the structure can reach: the
+    // sub-points are convex combinations of the nodes, a support reaches less than 3 cells, so outside
+    // [f_lo, f_hi) the force stays the zero it was filled with and goes back right away (the D2H engine has
+    // nothing else to do yet).  Not used when the structure comes within 4 layers of the z-walls (periodic wrap).
+    int f_lo = 0, f_hi = nz;
+    bool band = false;
+    {
+        const double *zh = x_h + 2 * c->n_nodes;
+        double zmin = zh[0], zmax = zh[0];
+        for (int64_t n = 1; n < c->n_nodes; ++n) {
+            zmin = zh[n] < zmin ? zh[n] : zmin;
+            zmax = zh[n] > zmax ? zh[n] : zmax;
+        }
+        const double lo = floor((zmin - c->grid.z0) * c->inv_h) - 4.0, hi = floor((zmax - c->grid.z0) * c->inv_h) + 6.0;
+        if (lo >= (double)z_first && hi <= (double)(nz - z_first) && hi > lo) {      // false for NaN as well
+            f_lo = (int)lo; f_hi = (int)hi; band = true;
+        }
+    }
+    if (band) {
+        double *fh[3] = {fu_h, fv_h, fw_h}, *fd[3] = {c->d_hfu, c->d_hfv, c->d_hfw};
+        IB_CUDA_TRY(cudaStreamWaitEvent(s3, c->ev_zero, 0));
+        for (int d = 0; d < 3; ++d) {
+            IB_CUDA_TRY(cudaMemcpyAsync(fh[d], fd[d], (size_t)f_lo * pb, cudaMemcpyDeviceToHost, s3));
+            IB_CUDA_TRY(cudaMemcpyAsync(fh[d] + f_hi * plane, fd[d] + f_hi * plane, (size_t)(nz - f_hi) * pb, cudaMemcpyDeviceToHost, s3));
+        }
+        IB_TR(s3, "zero layers of f on host");
+    }
     IB_CUDA_TRY(cudaStreamWaitEvent(st, c->ev_join, 0));
     if (s == IB_OK) s = ibk_bin_points(c, 1, nullptr, nullptr, c->n_points, c->d_hx, c->d_Fhat, c->d_Up, 2, st);
     IB_TR(st, "scatter");
@@ -721,7 +752,7 @@ extern "C" ib_status ib_coupling_step_host(ib_ctx *c, const double *x_h, const d
     IB_CUDA_TRY(cudaStreamWaitEvent(s4, c->ev_aux, 0));
     {
         double *fh[3] = {fu_h, fv_h, fw_h}, *fd[3] = {c->d_hfu, c->d_hfv, c->d_hfw};
-        int z_done = z_first;
+        int z_done = band ? f_lo : z_first;
         for (int k = 0; k < K; ++k) {
             cudaStream_t sk = (k & 1) ? s4 : st;
             IB_CUDA_TRY(cudaStreamWaitEvent(sk, c->ev_h2d[k], 0));
@@ -731,7 +762,7 @@ extern "C" ib_status ib_coupling_step_host(ib_ctx *c, const double *x_h, const d
             IB_CUDA_TRY(cudaEventRecord(c->ev_slab[k], sk));
             IB_TR(sk, "spread + interp slab");
             int z_end = (k == K - 1) ? nz : zs * (k + 1) - 4;
-            if (z_end > nz) z_end = nz;
+            if (z_end > f_hi) z_end = f_hi;                   // f_hi = nz without a band
             if (z_end < z_done) z_end = z_done;
             IB_CUDA_TRY(cudaStreamWaitEvent(s3, c->ev_slab[k], 0));
             for (int d = 0; d < 3 && z_end > z_done; ++d)
@@ -740,7 +771,7 @@ extern "C" ib_status ib_coupling_step_host(ib_ctx *c, const double *x_h, const d
             z_done = z_end;
             IB_TR(s3, "f slab on host");
         }
-        for (int d = 0; d < 3 && z_first > 0; ++d)
+        for (int d = 0; d < 3 && z_first > 0 && !band; ++d)
             IB_CUDA_TRY(cudaMemcpyAsync(fh[d], fd[d], z_first * pb, cudaMemcpyDeviceToHost, s3));
         IB_TR(s3, "f on host");
     }
