@@ -490,8 +490,13 @@ ibk_tiled_kernel(ib_tiled_params pr)
 
 // Points of tiles with fewer than IB_SMALL_TILE points are not worth a halo and a sort: one thread per
 // point of the compact list written by ibk_tile_scan, every point treated directly against the grid.
+// 8 resident CTAs = 64 registers, 32 warps per SM: the kernel waits on dependent loads and REDs, not on issue slots,
+// so the few spilled values (<= 170 B) cost less than the warps gain (5/6/8/10/12/16 CTAs measured: DESIGN.md s.9)
+#ifndef IB_SMALL_MINB
+#define IB_SMALL_MINB 8
+#endif
 template <int DO_SPREAD, int DO_INTERP>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(128, IB_SMALL_MINB)
 ibk_small_tiles(ib_tiled_params pr, const int32_t *__restrict__ small_rec, const int32_t *__restrict__ counters)
 {
     // 4 lanes per point (ib_point_quad); the list length is known on the device only, so the grid is sized for
