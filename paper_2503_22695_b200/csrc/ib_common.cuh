@@ -8,7 +8,7 @@
 #define IB_TILE 8              // tile edge of the binning key (A21)
 #define IB_TILE_CELLS 512
 #ifndef IB_SMALL_TILE
-#define IB_SMALL_TILE 64         // tiles with fewer points skip the tile kernel: their points go one by one (ib_point.cuh)
+#define IB_SMALL_TILE 96         // tiles with fewer points skip the tile kernel: their points go one by one (ib_point.cuh); 64/96/128/192 measured
 #endif
 #define IB_CHUNK 1920            // points per work item of the tile kernel (ib_bin.cu emits the work list)
 #define IB_SLAB0 4                // d_tile_count[IB_SLAB0 + k] = first work item of z-slab k (ib_tile_scan)
