@@ -1,10 +1,13 @@
 // ib_bin.cu -- tile-level counting sort of the Lagrangian force points (SURVEY.md §8(a) a4+a5 fused).
 // Not in the paper (north_star: "points binned and sorted by Eulerian cell").
 //
-// Points are grouped by 4x4x4-cell tile with a counting sort: count pass -> two-kernel scan (which also
-// emits the tile kernel's work list and the list of points of sparsely filled tiles) -> scatter pass
-// that writes the point records (x_s, G_s, id) contiguously per tile.  The order of
-// points inside a tile is whatever the atomics give; the tile kernel (ib_tiled.cu) sorts them by
+// Points are grouped by 4x4x4-cell tile, and inside a tile by z-layer of cells, with a counting sort over
+// the bins (tile, layer): count pass -> two-kernel scan (which also emits the tile kernel's work list and
+// the list of points of sparsely filled tiles) -> scatter pass that writes the point records (x_s, G_s,
+// id) contiguously per bin.  A work item of the tile kernel is a run of whole layers of one tile with at
+// most IB_CHUNK points (a layer with more is cut into equal pieces), so the points of a work item are
+// neighbours in space and share their stencil windows however densely a tile is filled.  The order of
+// points inside a bin is whatever the atomics give; the tile kernel (ib_tiled.cu) sorts them by
 // half-cell in shared memory.  Two point sources:
 //   cloud : xp/Gp arrays given by the caller (ib_spread / ib_interp, nodal rule of L241)
 //   mesh  : sub-points generated on the fly from the element nodes -- x_s = sum_a N_a(xi_s) x_a,
@@ -38,10 +41,11 @@ struct ib_bin_params {
     long long *status;
 };
 
+// bin of a point: 4 x (tile index) + (z-layer of the cell inside its tile)
 __device__ __forceinline__ int ib_tile_of(double x, double y, double z, const ib_grid_desc &g, double inv_h)
 {
     int cx = ib_cell(x, g.x0, inv_h, g.nx), cy = ib_cell(y, g.y0, inv_h, g.ny), cz = ib_cell(z, g.z0, inv_h, g.nz);
-    return ((cz >> 2) * (g.ny / BT) + (cy >> 2)) * (g.nx / BT) + (cx >> 2);
+    return ((((cz >> 2) * (g.ny / BT) + (cy >> 2)) * (g.nx / BT) + (cx >> 2)) << 2) | (cz & 3);
 }
 
 // warp-aggregated count / slot allocation; every lane of the warp must call (valid may differ)
@@ -276,10 +280,9 @@ ibk_bin_mesh(ib_bin_params pr)
     }
 }
 
-// ---- scan over the tiles (two small kernels, 4096 tiles per CTA): start offsets, cursors, compacted
-// list of non-empty tiles -----------------------------------------------------------------------------
+// ---- scan over the tiles (two small kernels, one thread per tile = 4 bins): start offsets, cursors, work
+// list, compact list of the records of sparsely filled tiles ------------------------------------------
 #define SCT 1024
-#define SCI 4
 
 __device__ __forceinline__ void ib_block_scan2(int &a, int &b, int *ws, int *wl, int &ta, int &tb)
 {
@@ -308,31 +311,64 @@ __device__ __forceinline__ void ib_block_scan2(int &a, int &b, int *ws, int *wl,
     b = wl[wid] + ib - b;
 }
 
-// chunk = points per work item: IB_CHUNK (the tile kernel's staging capacity) for large clouds, smaller
-// for small ones so that a few densely filled tiles still spread over many CTAs
-__device__ __forceinline__ int ib_chunks(int c, int chunk) { return c < IB_SMALL_TILE ? 0 : (c + chunk - 1) / chunk; }
+// Work items of one tile whose 4 z-layers hold c.x .. c.w points (records start at `first`): runs of whole
+// layers with at most `chunk` points; a layer with more is cut into equal pieces.  chunk = IB_CHUNK (the
+// tile kernel's staging capacity) for large clouds, smaller for small ones so that a few densely filled
+// tiles still spread over many CTAs.  EMIT: write {tile, first record, points, tile coordinates} to work[l ...].
+// Returns the number of work items (0 for a sparsely filled tile: its points go one by one).
+template <int EMIT>
+__device__ __forceinline__ int ib_tile_chunks(const int4 c, int chunk, int tile, int first, int4 *__restrict__ work, int l, int ntx, int nty)
+{
+    const int tw = EMIT ? ((tile % ntx) | (((tile / ntx) % nty) << 10) | ((tile / (ntx * nty)) << 20)) : 0;   // tile coordinates (grids up to 4096 cells an edge)
+    const int cnt[4] = {c.x, c.y, c.z, c.w};
+    if (c.x + c.y + c.z + c.w < IB_SMALL_TILE) return 0;
+    int n = 0, acc = 0, beg = first;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        if (cnt[k] > chunk) {
+            if (acc > 0) {
+                if (EMIT) work[l + n] = make_int4(tile, beg, acc, tw);
+                ++n; beg += acc; acc = 0;
+            }
+            const int pieces = (cnt[k] + chunk - 1) / chunk, per = (cnt[k] + pieces - 1) / pieces;
+            for (int o = 0; o < cnt[k]; o += per) {
+                if (EMIT) work[l + n] = make_int4(tile, beg + o, min(per, cnt[k] - o), tw);
+                ++n;
+            }
+            beg += cnt[k];
+        } else if (acc + cnt[k] > chunk) {
+            if (EMIT) work[l + n] = make_int4(tile, beg, acc, tw);
+            ++n; beg += acc; acc = cnt[k];
+        } else acc += cnt[k];
+    }
+    if (acc > 0) {
+        if (EMIT) work[l + n] = make_int4(tile, beg, acc, tw);
+        ++n;
+    }
+    return n;
+}
 
 __global__ void __launch_bounds__(SCT)
 ibk_tile_partials(const int32_t *__restrict__ tile_cur, int n_tiles, int chunk, int2 *__restrict__ partial)
 {
     __shared__ int ws[33], wl[33];
-    const int t0 = (blockIdx.x * SCT + threadIdx.x) * SCI;
+    const int t = blockIdx.x * SCT + threadIdx.x;
     int s = 0, l = 0;
-    if (t0 < n_tiles) {
-        int4 c = *reinterpret_cast<const int4 *>(tile_cur + t0);
+    if (t < n_tiles) {
+        const int4 c = *reinterpret_cast<const int4 *>(tile_cur + 4 * t);
         s = c.x + c.y + c.z + c.w;
-        l = ib_chunks(c.x, chunk) + ib_chunks(c.y, chunk) + ib_chunks(c.z, chunk) + ib_chunks(c.w, chunk);
+        l = ib_tile_chunks<0>(c, chunk, t, 0, nullptr, 0, 1, 1);
     }
     int ts, tl;
     ib_block_scan2(s, l, ws, wl, ts, tl);
     if (threadIdx.x == 0) partial[blockIdx.x] = make_int2(ts, tl);
 }
 
-// start offsets and cursors of the tiles, and the work list: one entry per chunk of <= IB_CHUNK records
+// start offsets and cursors of the bins, and the work list
 __global__ void __launch_bounds__(SCT)
 ibk_tile_scan(int32_t *__restrict__ tile_cur, int n_tiles, int chunk, const int2 *__restrict__ partial,
               int32_t *__restrict__ tile_start, int4 *__restrict__ work, int32_t *__restrict__ small_rec,
-              int32_t *__restrict__ counters, int slab_tiles)
+              int32_t *__restrict__ counters, int slab_tiles, int ntx, int nty)
 {
     __shared__ int ws[33], wl[33];
     __shared__ int base_s, base_l, base_m;
@@ -343,47 +379,35 @@ ibk_tile_scan(int32_t *__restrict__ tile_cur, int n_tiles, int chunk, const int2
         for (int o = 16; o >= 1; o >>= 1) { s += __shfl_xor_sync(0xffffffffu, s, o); l += __shfl_xor_sync(0xffffffffu, l, o); }
         if (threadIdx.x == 0) { base_s = s; base_l = l; }
     }
-    const int t0 = (blockIdx.x * SCT + threadIdx.x) * SCI;
+    const int t = blockIdx.x * SCT + threadIdx.x;
     int4 c = make_int4(0, 0, 0, 0);
-    if (t0 < n_tiles) c = *reinterpret_cast<const int4 *>(tile_cur + t0);
-    int s = c.x + c.y + c.z + c.w, l = ib_chunks(c.x, chunk) + ib_chunks(c.y, chunk) + ib_chunks(c.z, chunk) + ib_chunks(c.w, chunk);
+    if (t < n_tiles) c = *reinterpret_cast<const int4 *>(tile_cur + 4 * t);
+    const int tot = c.x + c.y + c.z + c.w;
+    int s = tot, l = ib_tile_chunks<0>(c, chunk, t, 0, nullptr, 0, 1, 1);
     int ts, tl;
     ib_block_scan2(s, l, ws, wl, ts, tl);          // includes the barrier that publishes base_s/base_l
     s += base_s; l += base_l;
-    // first work item of every slab of slab_tiles tiles (a multiple of SCI): ib_coupling_step_host launches
-    // the tile kernel slab by slab so that the copies of f overlap the spreading of the next slab
-    if (t0 < n_tiles && t0 % slab_tiles == 0) counters[IB_SLAB0 + t0 / slab_tiles] = l;
-    if (t0 < n_tiles) {
-        int4 st = make_int4(s, s + c.x, s + c.x + c.y, s + c.x + c.y + c.z);
-        *reinterpret_cast<int4 *>(tile_start + t0) = st;
-        *reinterpret_cast<int4 *>(tile_cur + t0) = st;
-        const int cnt[4] = {c.x, c.y, c.z, c.w}, beg[4] = {st.x, st.y, st.z, st.w};
-#pragma unroll
-        for (int k = 0; k < 4; ++k)
-            for (int o = 0; o < cnt[k] && cnt[k] >= IB_SMALL_TILE; o += chunk) work[l++] = make_int4(t0 + k, beg[k] + o, min(chunk, cnt[k] - o), 0);
+    // first work item of every slab of slab_tiles tiles: ib_coupling_step_host launches the tile kernel slab
+    // by slab so that the copies of f overlap the spreading of the next slab
+    if (t < n_tiles && t % slab_tiles == 0) counters[IB_SLAB0 + t / slab_tiles] = l;
+    if (t < n_tiles) {
+        const int4 st = make_int4(s, s + c.x, s + c.x + c.y, s + c.x + c.y + c.z);
+        *reinterpret_cast<int4 *>(tile_start + 4 * t) = st;
+        *reinterpret_cast<int4 *>(tile_cur + 4 * t) = st;
+        ib_tile_chunks<1>(c, chunk, t, s, work, l, ntx, nty);
     }
     {   // records of sparsely filled tiles: a compact list (order across CTAs is whatever the atomic gives)
-        int m = 0, zero = 0, tm, tz;
-        if (t0 < n_tiles)
-            m = (c.x < IB_SMALL_TILE ? c.x : 0) + (c.y < IB_SMALL_TILE ? c.y : 0) + (c.z < IB_SMALL_TILE ? c.z : 0) +
-                (c.w < IB_SMALL_TILE ? c.w : 0);
+        int m = (t < n_tiles && tot < IB_SMALL_TILE) ? tot : 0, zero = 0, tm, tz;
+        const int mine = m;
+        __syncthreads();                           // the first scan's totals have been read by every thread
         ib_block_scan2(m, zero, ws, wl, tm, tz);
         if (threadIdx.x == 0) base_m = tm ? atomicAdd(&counters[2], tm) : 0;
         __syncthreads();
-        if (t0 < n_tiles) {
-            m += base_m;
-            const int cnt[4] = {c.x, c.y, c.z, c.w};
-            int r = s;
-#pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                if (cnt[k] < IB_SMALL_TILE)
-                    for (int o = 0; o < cnt[k]; ++o) small_rec[m++] = r + o;
-                r += cnt[k];
-            }
-        }
+        m += base_m;
+        for (int o = 0; o < mine; ++o) small_rec[m + o] = s + o;
     }
     if (blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) {
-        tile_start[n_tiles] = base_s + ts;
+        tile_start[4 * n_tiles] = base_s + ts;
         counters[0] = base_l + tl;
         counters[1] = 0;
         for (int k = (n_tiles + slab_tiles - 1) / slab_tiles; k <= IB_MAX_SLABS; ++k) counters[IB_SLAB0 + k] = base_l + tl;
@@ -409,19 +433,19 @@ ib_status ibk_bin_points(ib_ctx *c, int mesh, const double *xp, const double *Gp
     const int rpe = c->un[1] * c->un[2];
     const bool stage = c->un[0] > 0 && rpe >= 16 && 256 % rpe == 0;     // <= 16 elements per CTA fit the staging array
     if (phases & 1) {
-        IB_CUDA_TRY(cudaMemsetAsync(c->d_tile_cur, 0, (size_t)n_tiles * sizeof(int32_t), st));
+        IB_CUDA_TRY(cudaMemsetAsync(c->d_tile_cur, 0, (size_t)n_tiles * 4 * sizeof(int32_t), st));
         IB_CUDA_TRY(cudaMemsetAsync(c->d_tile_count, 0, 4 * sizeof(int32_t), st));
         if (mesh && stage) ibk_bin_mesh<0, 1><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
         else if (mesh) ibk_bin_mesh<0, 0><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
         else ibk_bin_cloud<0><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
-        const int nsb = (n_tiles + SCT * SCI - 1) / (SCT * SCI);
+        const int nsb = (n_tiles + SCT - 1) / SCT;
         int2 *partial = reinterpret_cast<int2 *>(c->d_tile_count + IB_TILE_HDR);
         // ~4 work items per resident CTA of the tile kernel when the cloud is small
         int chunk = (int)((P / 1200 + 63) / 64 * 64);
         chunk = chunk < 192 ? 192 : (chunk > IB_CHUNK ? IB_CHUNK : chunk);
         if (nsb > 1) ibk_tile_partials<<<nsb, SCT, 0, st>>>(c->d_tile_cur, n_tiles, chunk, partial);   // one CTA needs no partial sums
         ibk_tile_scan<<<nsb, SCT, 0, st>>>(c->d_tile_cur, n_tiles, chunk, partial, c->d_tile_start, c->d_work, c->d_small_rec, c->d_tile_count,
-                                           ib_slab_tiles(c));
+                                           ib_slab_tiles(c), c->grid.nx / BT, c->grid.ny / BT);
         c->launches += 3;
     }
     if (phases & 2) {
@@ -450,7 +474,10 @@ ib_status ibk_bin_reserve(ib_ctx *c, int64_t P)
     if (cudaMalloc(&c->d_sx, (size_t)cap * 3 * sizeof(double)) != cudaSuccess) return IB_ERR_ALLOC;
     if (cudaMalloc(&c->d_sG, (size_t)cap * 3 * sizeof(double)) != cudaSuccess) return IB_ERR_ALLOC;
     if (cudaMalloc(&c->d_sid, (size_t)cap * sizeof(int32_t)) != cudaSuccess) return IB_ERR_ALLOC;
-    c->work_cap = c->n_cells / (BT * BT * BT) + cap / 192 + 8;
+    {   // a tile with >= IB_SMALL_TILE points gives at most 4 runs of layers plus one piece per 192 points
+        const int64_t n_tiles = c->n_cells / (BT * BT * BT), dense = cap / IB_SMALL_TILE + 1;
+        c->work_cap = 4 * (dense < n_tiles ? dense : n_tiles) + cap / 192 + 8;
+    }
     if (cudaMalloc(&c->d_work, (size_t)c->work_cap * sizeof(int4)) != cudaSuccess) return IB_ERR_ALLOC;
     if (cudaMalloc(&c->d_small_rec, (size_t)cap * sizeof(int32_t)) != cudaSuccess) return IB_ERR_ALLOC;
     c->bin_cap = cap;

@@ -10,7 +10,9 @@
 #ifndef IB_SMALL_TILE
 #define IB_SMALL_TILE 96         // tiles with fewer points skip the tile kernel: their points go one by one (ib_point.cuh); 64/96/128/192 measured
 #endif
-#define IB_CHUNK 1920            // points per work item of the tile kernel (ib_bin.cu emits the work list)
+#ifndef IB_CHUNK
+#define IB_CHUNK 704             // points per work item of the tile kernel = records it stages in shared memory (ib_bin.cu emits the work list)
+#endif
 #define IB_SLAB0 4                // d_tile_count[IB_SLAB0 + k] = first work item of z-slab k (ib_tile_scan)
 #define IB_MAX_SLABS 32
 #define IB_SLABC0 40              // d_tile_count[IB_SLABC0 + k] = work counter of slab k
@@ -73,7 +75,7 @@ struct ib_ctx {
     int32_t *d_sid;            // [P] original point id of each record
     // host staging for the *_host entry point
     double *d_hx, *d_hu, *d_hv, *d_hw, *d_hfu, *d_hfv, *d_hfw, *d_hUn, *d_hB;
-    // status latch: [0] code, [1] first bad id
+    // status latch: one packed word (ib_latch)
     long long *d_status;
     cudaStream_t last_stream;
     cudaStream_t side;         // internal stream: work that needs only the positions overlaps the FE force
@@ -135,11 +137,18 @@ static inline unsigned ib_blocks(int64_t n, int per) { return (unsigned)((n + pe
 // ---------------------------------------------------------------------------------------------
 // device helpers
 // ---------------------------------------------------------------------------------------------
+// One word holds (code, id): code in the top 8 bits, 2^48-1 - id below, kept with atomicMax -- so the
+// reported pair is always one error: the highest code seen (OUT_OF_DOMAIN > NONFINITE > INVERTED) with the
+// smallest id that raised THAT code.  0 = no error.  ib_check unpacks it (ib_status_unpack).
+#define IB_STATUS_IDMASK 0xFFFFFFFFFFFFull
 __device__ __forceinline__ void ib_latch(long long *status, int code, long long id)
 {
-    // keep the smallest offending id; code of the first writer wins per id class
-    atomicMax((unsigned long long *)&status[0], (unsigned long long)code);
-    atomicMin(&status[1], id);
+    atomicMax((unsigned long long *)status, ((unsigned long long)code << 56) | (IB_STATUS_IDMASK - ((unsigned long long)id & IB_STATUS_IDMASK)));
+}
+static inline void ib_status_unpack(unsigned long long w, int *code, long long *id)
+{
+    *code = (int)(w >> 56);
+    *id = w ? (long long)(IB_STATUS_IDMASK - (w & IB_STATUS_IDMASK)) : -1;
 }
 
 // sqrt(a) for a in [1/64, 1/32] (the argument (1+4r-4r^2)/64 of the kernel): float rsqrt seed (~2^-22),

@@ -93,8 +93,7 @@ extern "C" const char *ib_status_string(ib_status s)
 
 static ib_status reset_status(ib_ctx *c, cudaStream_t st)
 {
-    long long init[2] = {0, LLONG_MAX};
-    IB_CUDA_TRY(cudaMemcpyAsync(c->d_status, init, sizeof(init), cudaMemcpyHostToDevice, st));
+    IB_CUDA_TRY(cudaMemsetAsync(c->d_status, 0, 2 * sizeof(long long), st));
     return IB_OK;
 }
 
@@ -145,6 +144,7 @@ extern "C" ib_status ib_create(ib_ctx **out, const ib_grid_desc *g, const ib_mes
     if (!(g->h > 0.0) || !std::isfinite(g->h) || !std::isfinite(g->x0) || !std::isfinite(g->y0) || !std::isfinite(g->z0))
         return IB_ERR_INVALID_ARG;
     if ((int64_t)g->nx * g->ny * g->nz > (int64_t)INT32_MAX) return IB_ERR_INVALID_ARG;
+    if (g->nx > 4096 || g->ny > 4096 || g->nz > 8192) return IB_ERR_UNSUPPORTED;      // tile coordinates are packed 10 + 10 + 11 bits in the work list
     if (m->n_nodes < 0 || m->n_elems < 0 || m->n_nodes > INT32_MAX || m->n_elems > INT32_MAX / 8) return IB_ERR_INVALID_ARG;
     if (m->n_elems > 0 && (!m->conn || !m->X_ref || !m->mats || m->n_mats <= 0)) return IB_ERR_INVALID_ARG;
     if (m->elem_type < IB_ELEM_HEX8 || m->elem_type > IB_ELEM_TET10) return IB_ERR_INVALID_ARG;
@@ -186,6 +186,9 @@ extern "C" ib_status ib_create(ib_ctx **out, const ib_grid_desc *g, const ib_mes
                 cnt[n]++;
             }
         }
+        if (m->nsub)                                      // a node of no element has lumped weight 0: 1/w_a would put NaN into Fhat and Un
+            for (int64_t n = 0; n < nn; ++n)
+                if (cnt[n] == 0) return IB_ERR_INVALID_ARG;
         if (npe != 8) {                                   // CSR: tets share nodes with any number of neighbours
             for (int64_t n = 0; n < nn; ++n) node_off[n + 1] = node_off[n] + cnt[n];
             node_slot.resize((size_t)ne * npe + 1);
@@ -243,10 +246,10 @@ extern "C" ib_status ib_create(ib_ctx **out, const ib_grid_desc *g, const ib_mes
         TRY(dev_alloc((void **)&c->d_Up, P * 3 * sizeof(double)));
     }
     const int n_tiles = (int)(c->n_cells / 64);          // 4x4x4-cell tiles of the tiled path
-    TRY(dev_alloc((void **)&c->d_tile_cur, (size_t)(n_tiles + 4) * sizeof(int32_t)));
-    TRY(dev_alloc((void **)&c->d_tile_start, (size_t)(n_tiles + 4) * sizeof(int32_t)));
+    TRY(dev_alloc((void **)&c->d_tile_cur, (size_t)(4 * n_tiles + 4) * sizeof(int32_t)));      // 4 z-layer bins per tile
+    TRY(dev_alloc((void **)&c->d_tile_start, (size_t)(4 * n_tiles + 4) * sizeof(int32_t)));
     TRY(dev_upload(&c->d_row_off, roff.data(), (size_t)ne + 1));
-    TRY(dev_alloc((void **)&c->d_tile_count, (size_t)(IB_TILE_HDR + 2 * (n_tiles / 4096 + 2)) * sizeof(int32_t)));
+    TRY(dev_alloc((void **)&c->d_tile_count, (size_t)(IB_TILE_HDR + 2 * (n_tiles / 1024 + 2)) * sizeof(int32_t)));
     TRY(dev_alloc((void **)&c->d_status, 2 * sizeof(long long)));
     if (s == IB_OK && (cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) != cudaSuccess ||
                        cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
@@ -272,9 +275,14 @@ extern "C" ib_status ib_create(ib_ctx **out, const ib_grid_desc *g, const ib_mes
     if (s == IB_OK && cudaDeviceSynchronize() != cudaSuccess) s = IB_ERR_CUDA;
 #undef TRY
     if (s == IB_OK) {
-        long long hs[2];
-        if (cudaMemcpy(hs, c->d_status, sizeof(hs), cudaMemcpyDeviceToHost) != cudaSuccess) s = IB_ERR_CUDA;
-        else if (hs[0] != 0) s = (ib_status)hs[0];                  // inverted reference element
+        unsigned long long hs = 0;
+        int code = 0;
+        long long id = -1;
+        if (cudaMemcpy(&hs, c->d_status, sizeof(hs), cudaMemcpyDeviceToHost) != cudaSuccess) s = IB_ERR_CUDA;
+        else {
+            ib_status_unpack(hs, &code, &id);
+            if (code != 0) s = (ib_status)code;                     // inverted reference element
+        }
     }
     if (s != IB_OK) { ib_destroy(c); return s; }
     *out = c;
@@ -303,8 +311,13 @@ static ib_status replace_ids(int32_t **dst, const int32_t *src, size_t n)
 extern "C" ib_status ib_set_tethers(ib_ctx *c, int64_t n, const int32_t *ids, double kappa)
 {
     if (!c || n < 0 || (n > 0 && !ids) || !std::isfinite(kappa)) return IB_ERR_INVALID_ARG;
-    for (int64_t k = 0; k < n; ++k)
-        if (ids[k] < 0 || ids[k] >= c->n_nodes) return IB_ERR_INVALID_ARG;
+    {
+        std::vector<unsigned char> seen((size_t)(c->n_nodes > 0 ? c->n_nodes : 1), 0);      // the kernel adds without atomics: ids must be distinct
+        for (int64_t k = 0; k < n; ++k) {
+            if (ids[k] < 0 || ids[k] >= c->n_nodes || seen[ids[k]]) return IB_ERR_INVALID_ARG;
+            seen[ids[k]] = 1;
+        }
+    }
     if (cudaSetDevice(c->device) != cudaSuccess) return IB_ERR_CUDA;
     cudaDeviceSynchronize();
     c->gstate = 0;
@@ -616,14 +629,8 @@ extern "C" ib_status ib_coupling_step(ib_ctx *c, const double *x, const double *
     return coupling_step_body(c, x, u, v, w, fu, fv, fw, Un, B, st);
 }
 
-// -DIB_HOST_TRACE (through IB_NVCC_EXTRA): time stamps of the pipelined host step on its three streams
-#ifdef IB_HOST_TRACE
-#include <cstdio>
-struct ib_trace { cudaEvent_t e[96]; const char *name[96]; int n; };
-#define IB_TR(STREAM, NAME) do { cudaEventCreate(&tr.e[tr.n]); cudaEventRecord(tr.e[tr.n], (STREAM)); tr.name[tr.n++] = (NAME); } while (0)
-#else
-#define IB_TR(STREAM, NAME) do { } while (0)
-#endif
+static ib_status host_step_pipelined(ib_ctx *c, const double *x_h, const double *u_h, const double *v_h, const double *w_h,
+                                     double *fu_h, double *fv_h, double *fw_h, double *Un_h, double *B_h, cudaStream_t st);
 
 extern "C" ib_status ib_coupling_step_host(ib_ctx *c, const double *x_h, const double *u_h, const double *v_h,
                                            const double *w_h, double *fu_h, double *fv_h, double *fw_h,
@@ -659,6 +666,22 @@ extern "C" ib_status ib_coupling_step_host(ib_ctx *c, const double *x_h, const d
         IB_CUDA_TRY(cudaStreamSynchronize(st));
         return IB_OK;
     }
+    s = host_step_pipelined(c, x_h, u_h, v_h, w_h, fu_h, fv_h, fw_h, Un_h, B_h, st);
+    if (s != IB_OK) {
+        // copies to and from the caller's host buffers may still be in flight on the internal streams: no
+        // return before they have drained
+        cudaStream_t all[5] = {st, c->side, c->side2, c->side3, c->side4};
+        for (cudaStream_t q : all) cudaStreamSynchronize(q);
+        cudaGetLastError();
+    }
+    return s;
+}
+
+static ib_status host_step_pipelined(ib_ctx *c, const double *x_h, const double *u_h, const double *v_h, const double *w_h,
+                                     double *fu_h, double *fv_h, double *fw_h, double *Un_h, double *B_h, cudaStream_t st)
+{
+    ib_status s = IB_OK;
+    const size_t nb = (size_t)c->n_nodes * 3 * sizeof(double), gb = (size_t)c->n_cells * sizeof(double);
     // Pipelined in z-slabs of the tile list (tiles are numbered z-major).  The force side of the step needs
     // only x, so it runs while u,v,w cross the bus, slab by slab, on a side stream.  The fused
     // spread + interpolate kernel of slab k needs the velocity layers of slab k and 2 more on either side
@@ -672,18 +695,13 @@ extern "C" ib_status ib_coupling_step_host(ib_ctx *c, const double *x_h, const d
     //   side3      :                                                        D2H f layers of slab 0 | slab 1 | ...
     cudaStream_t s2 = c->side, s3 = c->side3, s4 = c->side4, ss = c->side2;
     double *Bd = B_h ? c->d_hB : c->d_B;
-#ifdef IB_HOST_TRACE
-    ib_trace tr; tr.n = 0;
-#endif
     const int K = ib_slab_count(c), nz = c->grid.nz, zs = 4 * ib_slab_layers(c);
     const size_t plane = (size_t)c->grid.nx * c->grid.ny, pb = plane * sizeof(double);
     const int z_first = nz < 4 ? nz : 4;          // wrap margin: the last z_first layers come first, the first go back last
-    IB_TR(st, "start");
     // x first: the force side waits for it, and the copy engine serves the H2D copies of all streams in turn
     IB_CUDA_TRY(cudaMemcpyAsync(c->d_hx, x_h, nb, cudaMemcpyHostToDevice, st));
     IB_CUDA_TRY(cudaEventRecord(c->ev_fork, st));             // orders the side streams after x and earlier work on st
     IB_CUDA_TRY(cudaStreamWaitEvent(s2, c->ev_fork, 0));
-    IB_TR(st, "x on device");
     // zero-fill of f and the count pass of the binning beside the FE force, as in ib_coupling_step
     IB_CUDA_TRY(cudaStreamWaitEvent(ss, c->ev_fork, 0));
     IB_CUDA_TRY(cudaMemsetAsync(c->d_hfu, 0, gb, ss));
@@ -693,9 +711,7 @@ extern "C" ib_status ib_coupling_step_host(ib_ctx *c, const double *x_h, const d
     s = ibk_bin_reserve(c, c->n_points);
     if (s == IB_OK) s = ibk_bin_points(c, 1, nullptr, nullptr, c->n_points, c->d_hx, nullptr, nullptr, 1, ss);
     IB_CUDA_TRY(cudaEventRecord(c->ev_join, ss));
-    IB_TR(ss, "zero + count + scan");
     if (s == IB_OK) s = ibk_fe_force(c, c->d_hx, Bd, c->d_Fhat, st);
-    IB_TR(st, "FE force");
     if (s != IB_OK) return s;
     {
         const double *uh[3] = {u_h, v_h, w_h};
@@ -712,7 +728,6 @@ extern "C" ib_status ib_coupling_step_host(ib_ctx *c, const double *x_h, const d
                 IB_CUDA_TRY(cudaMemcpyAsync(ud[d] + z0 * plane, uh[d] + z0 * plane, (size_t)(z1 - z0) * pb,
                                             cudaMemcpyHostToDevice, s2));
             IB_CUDA_TRY(cudaEventRecord(c->ev_h2d[k], s2));
-            IB_TR(s2, "uvw slab on device");
         }
     }
     // While the device is busy with all that, the host finds the z-layers the structure can reach: the
@@ -740,11 +755,9 @@ extern "C" ib_status ib_coupling_step_host(ib_ctx *c, const double *x_h, const d
             IB_CUDA_TRY(cudaMemcpyAsync(fh[d], fd[d], (size_t)f_lo * pb, cudaMemcpyDeviceToHost, s3));
             IB_CUDA_TRY(cudaMemcpyAsync(fh[d] + f_hi * plane, fd[d] + f_hi * plane, (size_t)(nz - f_hi) * pb, cudaMemcpyDeviceToHost, s3));
         }
-        IB_TR(s3, "zero layers of f on host");
     }
     IB_CUDA_TRY(cudaStreamWaitEvent(st, c->ev_join, 0));
     if (s == IB_OK) s = ibk_bin_points(c, 1, nullptr, nullptr, c->n_points, c->d_hx, c->d_Fhat, c->d_Up, 2, st);
-    IB_TR(st, "scatter");
     // the sparse tiles are spread before the first slab: beside it they would find no free SM until it ends
     if (s == IB_OK) s = ibk_small_launch(c, c->n_points, 1, 0, nullptr, nullptr, nullptr, c->d_hfu, c->d_hfv, c->d_hfw, nullptr, st);
     if (s != IB_OK) return s;
@@ -760,7 +773,6 @@ extern "C" ib_status ib_coupling_step_host(ib_ctx *c, const double *x_h, const d
                                  c->d_Up, k, sk);
             if (s != IB_OK) return s;
             IB_CUDA_TRY(cudaEventRecord(c->ev_slab[k], sk));
-            IB_TR(sk, "spread + interp slab");
             int z_end = (k == K - 1) ? nz : zs * (k + 1) - 4;
             if (z_end > f_hi) z_end = f_hi;                   // f_hi = nz without a band
             if (z_end < z_done) z_end = z_done;
@@ -769,11 +781,9 @@ extern "C" ib_status ib_coupling_step_host(ib_ctx *c, const double *x_h, const d
                 IB_CUDA_TRY(cudaMemcpyAsync(fh[d] + z_done * plane, fd[d] + z_done * plane, (size_t)(z_end - z_done) * pb,
                                             cudaMemcpyDeviceToHost, s3));
             z_done = z_end;
-            IB_TR(s3, "f slab on host");
         }
         for (int d = 0; d < 3 && z_first > 0 && !band; ++d)
             IB_CUDA_TRY(cudaMemcpyAsync(fh[d], fd[d], z_first * pb, cudaMemcpyDeviceToHost, s3));
-        IB_TR(s3, "f on host");
     }
     IB_CUDA_TRY(cudaStreamWaitEvent(ss, c->ev_aux, 0));
     IB_CUDA_TRY(cudaStreamWaitEvent(ss, c->ev_h2d[K - 1], 0));
@@ -782,25 +792,13 @@ extern "C" ib_status ib_coupling_step_host(ib_ctx *c, const double *x_h, const d
     IB_CUDA_TRY(cudaEventRecord(c->ev_sfork, ss));            // the sparse tiles are interpolated
     IB_CUDA_TRY(cudaStreamWaitEvent(st, c->ev_sfork, 0));
     for (int k = 1; k < K; k += 2) IB_CUDA_TRY(cudaStreamWaitEvent(st, c->ev_slab[k], 0));
-    IB_TR(st, "all slabs");
     s = ibk_restrict(c, c->d_Up, c->d_hUn, st);
-    IB_TR(st, "restrict");
     if (s != IB_OK) return s;
     IB_CUDA_TRY(cudaMemcpyAsync(Un_h, c->d_hUn, nb, cudaMemcpyDeviceToHost, st));
     if (B_h) IB_CUDA_TRY(cudaMemcpyAsync(B_h, c->d_hB, nb, cudaMemcpyDeviceToHost, st));
-    IB_TR(st, "Un on host");
     IB_CUDA_TRY(cudaStreamSynchronize(st));
     IB_CUDA_TRY(cudaStreamSynchronize(s2));
     IB_CUDA_TRY(cudaStreamSynchronize(s3));
-#ifdef IB_HOST_TRACE
-    for (int i = 0; i < tr.n; ++i) {
-        float ms = 0.f;
-        cudaEventElapsedTime(&ms, tr.e[0], tr.e[i]);
-        fprintf(stderr, "[ib host trace] %8.3f ms  %s\n", ms, tr.name[i]);
-        if (i) cudaEventDestroy(tr.e[i]);
-    }
-    cudaEventDestroy(tr.e[0]);
-#endif
     return IB_OK;
 }
 
@@ -810,15 +808,18 @@ extern "C" ib_status ib_check(ib_ctx *c, int64_t *first_bad)
     if (cudaSetDevice(c->device) != cudaSuccess) return IB_ERR_CUDA;
     if (first_bad) *first_bad = -1;
     if (cudaStreamSynchronize(c->last_stream) != cudaSuccess) return IB_ERR_CUDA;
-    long long hs[2];
-    IB_CUDA_TRY(cudaMemcpy(hs, c->d_status, sizeof(hs), cudaMemcpyDeviceToHost));
+    unsigned long long hs = 0;
+    IB_CUDA_TRY(cudaMemcpy(&hs, c->d_status, sizeof(hs), cudaMemcpyDeviceToHost));
     if (cudaGetLastError() != cudaSuccess) return IB_ERR_CUDA;
-    if (hs[0] == 0) return IB_OK;
-    if (first_bad) *first_bad = hs[1] == LLONG_MAX ? -1 : hs[1];
+    int code = 0;
+    long long id = -1;
+    ib_status_unpack(hs, &code, &id);
+    if (code == 0) return IB_OK;
+    if (first_bad) *first_bad = id;
     ib_status r = reset_status(c, c->last_stream);
     if (r != IB_OK) return r;
     cudaStreamSynchronize(c->last_stream);
-    return (ib_status)hs[0];
+    return (ib_status)code;
 }
 
 // ---------------------------------------------------------------------------------------------

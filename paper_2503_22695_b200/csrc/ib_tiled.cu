@@ -1,23 +1,30 @@
 // ib_tiled.cu -- variant 1 of spread (Eq.(24)-(26)) and interpolation (Eq.(27)-(29)):
-// points grouped by 4x4x4-cell tile (ib_bin.cu); persistent CTAs pull chunks of one tile from a work
-// list, keep an 8x8x8 halo of u,v,w in shared memory and hold 4x4x4 stencil windows in registers.
+// points grouped by 4x4x4-cell tile (ib_bin.cu); persistent CTAs pull work items (runs of z-layers of one
+// tile, <= IB_CHUNK points) from a work list, keep an 8x8x8 halo of u,v,w in shared memory and hold the
+// stencil windows in registers.
 //
-// Per chunk the CTA stages the tile-relative scaled coordinates of the points in shared memory and
-// sorts them by half-cell ("octant", 8^3 per tile) with a shared-memory counting sort.  Why half-cells:
-// component c lives on its own staggered lattice (MAC grid, L205).  In the direction d == c the
-// 4-point support of a point is fixed by its cell; in the other two it is fixed by the cell of the
-// lattice shifted by h/2.  With the points ordered by half-cell every cell of every shifted lattice is
-// a union of <= 4 contiguous runs, so all points of one work item (shifted cell, component) share ONE
-// 4x4x4 window.
+// Per work item the CTA computes, one thread per point, the tile-relative scaled coordinates and from them
+// the six 1-D delta-weight sets of the point (3 directions x {face-aligned, centre-aligned}: component c
+// lives on its own staggered lattice, MAC grid L205), once, and stores them in shared memory in half-cell
+// order ("octant", 8^3 per tile; shared-memory counting sort).  Why half-cells: in the direction d == c the
+// 4-point support of a point is fixed by its cell; in the other two it is fixed by the cell of the lattice
+// shifted by h/2.  With the points ordered by half-cell every cell of every shifted lattice is a union of
+// <= 4 contiguous runs, so all points of one item (shifted cell, component) share ONE 4x4x4 window.
 //
-// Work item = (shifted cell, component); items are ordered by point count and pulled by the warps, 8
-// at a time.  A group of 4 lanes owns an item: lane q keeps the x-column q of the window -- 16
-// velocity values and 16 force accumulators -- in registers and loops over the item's points in quads.
-// Per point and lane: 21 DFMA for interpolation, 21 for spreading.  The delta weights of a quad are
-// computed by the 4 lanes (one point each, one branch-free sqrt per 1-D weight set) into a
-// double-buffered shared-memory record while the group consumes the previous quad; index, force and
-// id of the quad after that are already in flight.  Force is reduced in registers over all points of
-// the item and flushed with RED.ADD.F64 straight to the grid: the 4 lanes of a group hit 4 consecutive
+// A weight set is stored as the pair (a, q) it is made of: the Peskin 4-point weights of a point at
+// fraction r are  w0 = a - q, w1 = a + q, w2 = (1/2 - a) + q, w3 = (1/2 - a) - q  with a = 3/8 - r/4 and
+// q = sqrt(1 + 4r - 4r^2)/8 (ib_phi4).  They are affine in (a, q), so a 4-term contraction with them is a
+// 3-term one in the basis {1, a, q}:
+//     sum_i w_i u_i = S0 + a Sa + q Sq,   S0 = (u2+u3)/2,  Sa = u0+u1-u2-u3,  Sq = -u0+u1+u2-u3,
+// and the transpose for spreading: accumulate the moments M0 = sum g, Ma = sum g a, Mq = sum g q over the
+// points, then  f0 = Ma-Mq, f1 = Ma+Mq, f2 = M0/2-Ma+Mq, f3 = M0/2-Ma-Mq.  The y and z directions of a window
+// are kept in that basis (3x3 = 9 values instead of 4x4 = 16), x stays in weight form across 4 lanes.
+//
+// Items are ordered by point count and pulled by the warps, 8 at a time.  A group of 4 lanes owns an item:
+// lane q keeps the x-column q of the window -- 9 transformed velocity values and 9 force moments -- in
+// registers and loops over the item's points: per point and lane 9 DFMA for interpolation, 12 for
+// spreading, 2 for its own x-weight, against 21 + 21 in weight form.  The moments are transformed back once
+// per item and flushed with RED.ADD.F64 straight to the grid: the 4 lanes of a group hit 4 consecutive
 // faces (Blackwell has no native shared-memory fp64 add; the CAS loop measured 34 wavefronts each).
 // Tiles with fewer than IB_SMALL_TILE points skip all of this (ibk_small_tiles, ib_point.cuh).
 #include "ib_point.cuh"
@@ -27,16 +34,23 @@
 #define TH3 512
 #define NOC 512                 // half-cells per tile (8^3)
 #define NITEM 300               // 3 components x (4*5*5) shifted cells
-#define TB 192                  // threads per CTA (2 CTAs/SM at <= 168 registers)
+#ifndef TB
+#define TB 256                  // threads per CTA
+#endif
+#ifndef NCTA
 #define NCTA 2
+#endif
+#define NIT ((NITEM + TB - 1) / TB)   // items per thread in the counting pass
 #define NWARP (TB / 32)
-#define CH IB_CHUNK             // points staged per work item (9 per thread)
-#define REC 14                  // staging record: wx[4] wy[4] wz[4] G pad (doubles)
-#define GBUF 56                 // doubles per staging buffer of a group (4 records)
-#define GSTRIDE 120             // doubles per group: two buffers + pad (60 16-byte units = 4 mod 8: conflict-free STS.128)
+#define CH IB_CHUNK             // records staged per work item
+#define KPT ((CH + TB - 1) / TB)   // points per thread in the staging pass
 #define SZ 68                   // z-plane stride of the halo in doubles (64 + 4: the 4 lanes of a group hit distinct banks)
 #define SU3 (TH * SZ)           // one component of the halo
-#define NBIN 66
+#ifndef PCAP
+#define PCAP 32                 // an item with more points is cut into units of PCAP points (each with a window of its own)
+#endif
+#define NBIN (PCAP + 1)         // units are ordered by point count 0..PCAP
+#define NORD ((100 + IB_CHUNK / PCAP + 7) & ~7)   // units per component: one per item + IB_CHUNK / PCAP whole ones, in whole batches
 
 struct ib_tiled_params {
     const double *sx, *sG;      // [3][P] records grouped by tile
@@ -45,14 +59,14 @@ struct ib_tiled_params {
     const double *fld[3];
     double *frc[3];
     double *Up;
-    const int4 *work;           // {tile, first record, points, 0} per chunk
+    const int4 *work;           // {tile, first record, points, tile coordinates tx | ty << 10 | tz << 20} per work item
     int32_t *counters;          // [0] number of work items, [1] work counter, [3] zero, [IB_SLAB0 + k] first item of slab k
     int wb, we, wc;             // this launch covers the work items counters[wb] <= w < counters[we]; counters[wc] counts them
     ib_grid_desc g;
     double inv_h, ih3;
 };
 
-// decode a work item: component c, shifted-cell coordinates l[3]  (c*100 + (l2*ny + l1)*nx + l0 with
+// decode an item: component c, shifted-cell coordinates l[3]  (c*100 + (l2*ny + l1)*nx + l0 with
 // nx = 4 if c == 0 else 5, ny = 4 if c == 1 else 5; compile-time constant divisors only)
 __device__ __forceinline__ void ib_item_decode(int it, int &c, int l[3])
 {
@@ -66,18 +80,6 @@ __device__ __forceinline__ void ib_item_decode(int it, int &c, int l[3])
     const int q5 = rem / 5;
     l[1] = (c == 0) ? (rem >> 2) : q5;
     l[0] = (c == 0) ? (rem & 3) : rem - 5 * q5;
-}
-
-// the same, packed into 11 bits for the sorted item list (the item loop unpacks instead of dividing)
-__device__ __forceinline__ unsigned short ib_item_code(int it)
-{
-    int c, l[3];
-    ib_item_decode(it, c, l);
-    return (unsigned short)(c | (l[0] << 2) | (l[1] << 5) | (l[2] << 8));
-}
-__device__ __forceinline__ void ib_item_unpack(int code, int &c, int l[3])
-{
-    c = code & 3; l[0] = (code >> 2) & 7; l[1] = (code >> 5) & 7; l[2] = code >> 8;
 }
 
 // half-cell range [lo,hi] (clipped to the tile) covered by shifted cell l in direction d of comp c
@@ -99,16 +101,218 @@ __device__ __forceinline__ double ib_tile_coord(double x, double x0, double h, d
     return (ib_scaled(x, x0, h, inv_h) - fl) + (double)((long long)fl & (TT - 1));
 }
 
-__device__ __forceinline__ int ib_octant_key(double a, double b, double c)
-{
-    int hx = min(max((int)floor(2.0 * a), 0), 7), hy = min(max((int)floor(2.0 * b), 0), 7),
-        hz = min(max((int)floor(2.0 * c), 0), 7);
-    return (hz * 8 + hy) * 8 + hx;
-}
-
 __device__ __forceinline__ void ib_prefetch_l2(const void *p)
 {
     asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+}
+
+// (a, q) of the Peskin kernel at fraction r (see the header): w0..w3 = a-q, a+q, (1/2-a)+q, (1/2-a)-q
+__device__ __forceinline__ double2 ib_aq(double r)
+{
+    return make_double2(fma(-0.25, r, 0.375), ib_sqrt_seeded(fma(0.0625 * r, 1.0 - r, 0.015625)));
+}
+
+// 4 values along one direction of a window -> their 3 coefficients in the basis {1, a, q}
+__device__ __forceinline__ void ib_to_basis(double u0, double u1, double u2, double u3, double &s0, double &sa, double &sq)
+{
+    const double p = u2 + u3;
+    s0 = 0.5 * p;
+    sa = (u0 + u1) - p;
+    sq = (u1 - u0) + (u2 - u3);
+}
+
+// 3 moments along one direction -> the 4 face values (transpose of ib_to_basis)
+__device__ __forceinline__ void ib_from_basis(double m0, double ma, double mq, double f[4])
+{
+    const double t = fma(0.5, m0, -ma);
+    f[0] = ma - mq;
+    f[1] = ma + mq;
+    f[2] = t + mq;
+    f[3] = t - mq;
+}
+
+// shared-memory addresses (32-bit, shared window) of one work item's arrays, and per-lane constants.  They are
+// made opaque to the compiler once (ib_opaque): it otherwise re-derives them inside the point loop to save
+// registers (10 of 70 instructions per point in the SASS of the first version).
+struct ib_tile_smem {
+    unsigned su, sets, sGs, sids;    // [3][8][SZ] halo, [6][CH] (a,q) pairs, [3][CH] force, [CH] ids
+    const uint4 *item_runs;          // [NITEM + 1]
+    const unsigned *item_win;        // [NITEM + 1]
+};
+
+__device__ __forceinline__ void ib_opaque(unsigned &v) { asm volatile("" : "+r"(v)); }
+__device__ __forceinline__ void ib_opaque(double &v) { asm volatile("" : "+d"(v)); }
+__device__ __forceinline__ double2 ib_lds128(unsigned a)
+{
+    double2 v;
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ double ib_lds64(unsigned a)
+{
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ unsigned ib_lds32(unsigned a)
+{
+    unsigned v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a));
+    return v;
+}
+
+// record of virtual point index vi of an item made of <= 4 runs (rstart/rend: see the caller)
+__device__ __forceinline__ int ib_item_rec(int vi, const int rstart[4], const int rend[3])
+{
+    int off = rstart[0];
+    off = (vi >= rend[0]) ? rstart[1] : off;
+    off = (vi >= rend[1]) ? rstart[2] : off;
+    off = (vi >= rend[2]) ? rstart[3] : off;
+    return vi + off;
+}
+
+// One batch of 8 units of component C (the same for the whole warp): the group of 4 lanes owns the unit `part`
+// of item `it` (an empty slot of the batch gets the item NITEM, which has no points).  One instantiation serves
+// the three components: three copies of this loop do not fit the instruction cache of a scheduler (measured:
+// 1.9 "no instruction" stalls per issue).
+template <int DO_SPREAD, int DO_INTERP, int PER>
+__device__ __forceinline__ void ib_run_batch(int C, const ib_tiled_params &pr, const ib_tile_smem &sm, int it, int part, int q,
+                                             const int h0[3], const int n[3], double wsa, double wca, double wsg)
+{
+    const unsigned full = 0xffffffffu;
+    // runs of the half-cell order that make up this item
+    int rstart[4], rend[3], npts = 0;
+    {
+        const uint4 rn4 = sm.item_runs[it];
+        const unsigned rn[4] = {rn4.x, rn4.y, rn4.z, rn4.w};
+#pragma unroll
+        for (int rr = 0; rr < 4; ++rr) {
+            const int s0 = (int)(rn[rr] & 0xffffu), s1 = (int)(rn[rr] >> 16);
+            rstart[rr] = s0 - npts;          // record = rstart + virtual index
+            npts += s1 - s0;
+            if (rr < 3) rend[rr] = npts;     // virtual indices < rend belong to runs <= rr
+        }
+    }
+    // this group's unit: the virtual points [vlo, vlo + nun) of the item
+    const int vlo = part * PCAP, nun = min(PCAP, npts - vlo);       // <= 0 for the empty slot
+    int nmax = nun;
+#pragma unroll
+    for (int o = 16; o >= 4; o >>= 1) nmax = max(nmax, __shfl_xor_sync(full, nmax, o));
+    // window: offset of its origin in the halo (with the component), origin o3 = l + (d == C)
+    const unsigned win = sm.item_win[it];
+    // lane q owns x-column q of the window; y and z in the basis {1, a, q}: S[by][bz]
+    double S[3][3], M[3][3];
+    if (DO_INTERP) {
+        const unsigned suc = sm.su + ((win & 0xffffu) + q) * 8u;
+        double t[4][3];
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+            ib_to_basis(ib_lds64(suc + j * TH * 8), ib_lds64(suc + (j * TH + SZ) * 8), ib_lds64(suc + (j * TH + 2 * SZ) * 8),
+                        ib_lds64(suc + (j * TH + 3 * SZ) * 8), t[j][0], t[j][1], t[j][2]);
+#pragma unroll
+        for (int bz = 0; bz < 3; ++bz) ib_to_basis(t[0][bz], t[1][bz], t[2][bz], t[3][bz], S[0][bz], S[1][bz], S[2][bz]);
+    }
+#pragma unroll
+    for (int by = 0; by < 3; ++by)
+#pragma unroll
+        for (int bz = 0; bz < 3; ++bz) M[by][bz] = 0.0;
+    unsigned ax = sm.sets + (C != 0 ? CH * 16 : 0), ay = sm.sets + (C != 1 ? 3 * CH * 16 : 2 * CH * 16),
+             az = sm.sets + (C != 2 ? 5 * CH * 16 : 4 * CH * 16), ag = sm.sGs + C * (CH * 8);
+    double *Uc = DO_INTERP ? pr.Up + (int64_t)C * pr.P : nullptr;
+    unsigned qq = (unsigned)q;
+    ib_opaque(ax); ib_opaque(ay); ib_opaque(az); ib_opaque(ag); ib_opaque(qq);      // kept in registers, not re-derived per point
+    asm volatile("" : "+l"(Uc));
+
+    // 4 points per step: the x-sums of the 4 interpolated values are reduced across the 4 lanes in a
+    // transposing butterfly (3 shuffles instead of 8), which leaves point k's value in lane k -- one store
+    // instruction per 4 points
+    for (int v0 = 0; v0 < nmax; v0 += 4) {
+        double pv[4];
+        // two points in one straight line of code (their loads and dependent chains overlap); the second pair
+        // of a step only when the longest unit of the batch reaches it
+#pragma unroll
+        for (int kp = 0; kp < 4; kp += 2) {
+            pv[kp] = 0.0; pv[kp + 1] = 0.0;
+            if (kp == 0 || v0 + kp < nmax) {                  // warp-uniform
+                // all the loads of the pair first (the asm loads keep their order), then the arithmetic
+                bool valid[2];
+                double2 X[2], Y[2], Z[2];
+                double gl[2];
+#pragma unroll
+                for (int k = 0; k < 2; ++k) {
+                    valid[k] = v0 + kp + k < nun;
+                    const int rec = valid[k] ? ib_item_rec(vlo + v0 + kp + k, rstart, rend) : 0;   // padding: record 0 exists, its force is replaced by zero
+                    const unsigned r16 = (unsigned)rec << 4;
+                    X[k] = ib_lds128(ax + r16); Y[k] = ib_lds128(ay + r16); Z[k] = ib_lds128(az + r16);
+                    gl[k] = DO_SPREAD ? ib_lds64(ag + ((unsigned)rec << 3)) : 0.0;
+                }
+#pragma unroll
+                for (int k = 0; k < 2; ++k) {
+                    const double wx = fma(wsg, X[k].y, fma(wsa, X[k].x, wca));
+                    if (DO_INTERP) {
+                        const double c0 = fma(Z[k].y, S[0][2], fma(Z[k].x, S[0][1], S[0][0]));
+                        const double c1 = fma(Z[k].y, S[1][2], fma(Z[k].x, S[1][1], S[1][0]));
+                        const double c2 = fma(Z[k].y, S[2][2], fma(Z[k].x, S[2][1], S[2][0]));
+                        pv[kp + k] = fma(Y[k].y, c2, fma(Y[k].x, c1, c0)) * wx;
+                    }
+                    if (DO_SPREAD) {
+                        const double g0 = (valid[k] ? gl[k] : 0.0) * wx, g1 = g0 * Y[k].x, g2 = g0 * Y[k].y;
+                        M[0][0] += g0; M[0][1] = fma(g0, Z[k].x, M[0][1]); M[0][2] = fma(g0, Z[k].y, M[0][2]);
+                        M[1][0] += g1; M[1][1] = fma(g1, Z[k].x, M[1][1]); M[1][2] = fma(g1, Z[k].y, M[1][2]);
+                        M[2][0] += g2; M[2][1] = fma(g2, Z[k].x, M[2][1]); M[2][2] = fma(g2, Z[k].y, M[2][2]);
+                    }
+                }
+            }
+        }
+        if (DO_INTERP) {
+            const bool hi2 = (qq & 2u) != 0, hi1 = (qq & 1u) != 0;
+            double a0 = hi2 ? pv[2] : pv[0], a1 = hi2 ? pv[3] : pv[1];
+            const double s0 = hi2 ? pv[0] : pv[2], s1 = hi2 ? pv[1] : pv[3];
+            a0 += __shfl_xor_sync(full, s0, 2);
+            a1 += __shfl_xor_sync(full, s1, 2);
+            double tot = hi1 ? a1 : a0;
+            tot += __shfl_xor_sync(full, hi1 ? a0 : a1, 1);
+            // lane q holds the value of point v0 + q
+            if (v0 + (int)qq < nun) __stcs(Uc + ib_lds32(sm.sids + 4u * (unsigned)ib_item_rec(vlo + v0 + (int)qq, rstart, rend)), tot);
+        }
+    }
+    if (DO_SPREAD && nun > 0) {
+        // moments -> face values ff[y j][z i] of x-column q
+        double t[4][3], ff[4][4];
+#pragma unroll
+        for (int bz = 0; bz < 3; ++bz) {
+            double f4[4];
+            ib_from_basis(M[0][bz], M[1][bz], M[2][bz], f4);
+#pragma unroll
+            for (int j = 0; j < 4; ++j) t[j][bz] = f4[j];
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) ib_from_basis(t[j][0], t[j][1], t[j][2], ff[j]);
+        // lane q flushes x-column q: for every (y,z) the 4 lanes of the group hit 4 consecutive faces
+        // (bounded grid: faces outside 0..n-1 do not exist -- their share of the force is dropped, A26)
+        constexpr bool per = PER != 0;
+        int gi = h0[0] + (int)((win >> 16) & 15u) + q;
+        if (per) gi -= (gi >= n[0]) ? n[0] : 0;
+        const bool xin = per || (gi >= 0 && gi < n[0]);
+        const int j0 = h0[1] + (int)((win >> 20) & 15u), k0 = h0[2] + (int)((win >> 24) & 15u), nxy = n[0] * n[1];
+        unsigned ok[4], oj[4];                             // 32-bit face offsets (n_cells < 2^31)
+        bool jin[4], kin[4];
+#pragma unroll
+        for (int m = 0; m < 4; ++m) {
+            int gj = j0 + m, gk = k0 + m;
+            if (per) { gj -= (gj >= n[1]) ? n[1] : 0; gk -= (gk >= n[2]) ? n[2] : 0; }
+            jin[m] = per || (gj >= 0 && gj < n[1]);
+            kin[m] = per || (gk >= 0 && gk < n[2]);
+            oj[m] = (unsigned)(gj * n[0] + gi);
+            ok[m] = (unsigned)(gk * nxy);
+        }
+        double *fp = pr.frc[C];
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                if (xin && kin[i] && jin[j]) atomicAdd(fp + (ok[i] + oj[j]), ff[j][i]);
+    }
 }
 
 // PER: periodic grid (compile-time, so that the periodic kernel carries none of the wall predicates)
@@ -116,374 +320,262 @@ template <int DO_SPREAD, int DO_INTERP, int PER>
 __global__ void __launch_bounds__(TB, NCTA)
 ibk_tiled_kernel(ib_tiled_params pr)
 {
-    extern __shared__ __align__(16) double smem[];
-    double *su = smem;                                   // [3][8][SZ] halo of u,v,w
-    double *sxi = su + 3 * SU3;                          // [3][CH] tile-relative scaled coordinates
-    double *stg = sxi + 3 * CH;                          // [NWARP*8][GSTRIDE]
-    int *oc_cur = (int *)(stg + NWARP * 8 * GSTRIDE);    // [512]
-    int *bins = oc_cur + NOC;                            // [68]
-    unsigned short *oc_start = (unsigned short *)(bins + 68);   // [516]
-    unsigned short *item_cnt = oc_start + 516;           // [NITEM]
-    unsigned short *order = item_cnt + NITEM;            // [NITEM]
-    unsigned short *sidx = order + NITEM;                // [CH]
-    __shared__ int s_nitems, s_next;
-    __shared__ int4 s_work, s_nwk;
+    extern __shared__ __align__(16) unsigned char smraw[];
+    double *su = reinterpret_cast<double *>(smraw);                  // [3][8][SZ] halo of u,v,w
+    double2 *sets = reinterpret_cast<double2 *>(su + 3 * SU3);       // [6][CH] (a,q) of set 2 d + {0 face, 1 centre}, half-cell order
+    double *sGs = reinterpret_cast<double *>(sets + 6 * CH);         // [3][CH] force / h^3
+    uint4 *item_runs = reinterpret_cast<uint4 *>(sGs + 3 * CH);      // [NITEM + 1] the <= 4 runs [s, e) of records of an item, 16 bits each; item NITEM is empty
+    unsigned *item_win = reinterpret_cast<unsigned *>(item_runs + NITEM + 1);   // [NITEM + 3] window of an item: halo offset | o3x << 16 | o3y << 20 | o3z << 24
+    int *sids = reinterpret_cast<int *>(item_win + NITEM + 3);       // [CH] point id of the record
+    int *oc_cnt = sids + CH;                                         // [NOC] points per half-cell
+    int *bins = oc_cnt + NOC;                                        // [3][NBIN] items per component and point count
+    unsigned short *oc_start = reinterpret_cast<unsigned short *>(bins + 3 * NBIN + 2);   // [516] first record of a half-cell
+    unsigned short *order = oc_start + 516;                          // [3][NORD] units of a component by descending point count
+    __shared__ int s_next[2];
+    __shared__ int4 s_wk[2];                         // work item of the even / odd iteration
     __shared__ int wsum[NWARP];
 
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int grp = lane >> 2, q = lane & 3;
     const int n[3] = {pr.g.nx, pr.g.ny, pr.g.nz};
     const double org[3] = {pr.g.x0, pr.g.y0, pr.g.z0};
-    const int ntx = n[0] / TT, nty = n[1] / TT;
     const int64_t P = pr.P;
+    // lane q's own x-weight from (a, q):  w = sg q + (sa a + ca)
+    double wsa = q < 2 ? 1.0 : -1.0, wca = q < 2 ? 0.0 : 0.5, wsg = (q == 1 || q == 2) ? 1.0 : -1.0;
+    ib_opaque(wsa); ib_opaque(wca); ib_opaque(wsg);
+    ib_tile_smem sm;
+    sm.su = (unsigned)__cvta_generic_to_shared(su); sm.sets = (unsigned)__cvta_generic_to_shared(sets);
+    sm.sGs = (unsigned)__cvta_generic_to_shared(sGs); sm.sids = (unsigned)__cvta_generic_to_shared(sids);
+    ib_opaque(sm.su); ib_opaque(sm.sets); ib_opaque(sm.sGs); ib_opaque(sm.sids);
+    sm.item_runs = item_runs; sm.item_win = item_win;
+    // the windows of the items do not depend on the work item
+    for (int it = tid; it <= NITEM; it += TB) {
+        int c = 0, l[3] = {0, 0, 0};
+        if (it < NITEM) ib_item_decode(it, c, l);
+        const int o3[3] = {l[0] + (c == 0 ? 1 : 0), l[1] + (c == 1 ? 1 : 0), l[2] + (c == 2 ? 1 : 0)};
+        item_win[it] = (unsigned)(c * SU3 + o3[2] * SZ + o3[1] * TH + o3[0]) | (o3[0] << 16) | (o3[1] << 20) | (o3[2] << 24);
+        if (it == NITEM) item_runs[it] = make_uint4(0, 0, 0, 0);
+    }
+
+    // the records of a work item, one thread per point: coordinates, forces and ids are loaded, the tile
+    // coordinates and the half-cell of every point computed and counted.  Runs for work item k+1 as soon as a
+    // warp has no more items of work item k: nothing it touches (registers, oc_cnt) is used by the item loop.
+    double xi[KPT][3], Gr[KPT][3];
+    int ks[KPT], idr[KPT];
+    auto stage = [&](const int4 &wk) {
+        const int cb = wk.y, cn = wk.z;
+        double xr[KPT][3];
+#pragma unroll
+        for (int k = 0; k < KPT; ++k) {
+            const int i = tid + k * TB;
+#pragma unroll
+            for (int d = 0; d < 3; ++d) xr[k][d] = (i < cn) ? __ldcs(pr.sx + (int64_t)d * P + cb + i) : 0.0;
+        }
+#pragma unroll
+        for (int k = 0; k < KPT; ++k) {
+            const int i = tid + k * TB;
+            idr[k] = (DO_INTERP && i < cn) ? __ldcs(pr.sid + cb + i) : 0;
+#pragma unroll
+            for (int d = 0; d < 3; ++d) Gr[k][d] = (DO_SPREAD && i < cn) ? __ldcs(pr.sG + (int64_t)d * P + cb + i) : 0.0;
+        }
+#pragma unroll
+        for (int k = 0; k < KPT; ++k) {
+            const int i = tid + k * TB;
+            ks[k] = -1;
+            if (i < cn) {
+                int key = 0;
+#pragma unroll
+                for (int d = 2; d >= 0; --d) {
+                    xi[k][d] = ib_tile_coord(xr[k][d], org[d], pr.g.h, pr.inv_h);
+                    key = key * 8 + min(max((int)floor(2.0 * xi[k][d]), 0), 7);
+                }
+                ks[k] = key | (atomicAdd(&oc_cnt[key], 1) << 9);      // rank inside the half-cell
+            }
+        }
+    };
 
     if (tid == 0) {
         const int w = pr.counters[pr.wb] + atomicAdd(&pr.counters[pr.wc], 1);
-        s_work = (w < pr.counters[pr.we]) ? __ldg(pr.work + w) : make_int4(-1, 0, 0, 0);
-        s_next = 0;
+        s_wk[0] = (w < pr.counters[pr.we]) ? __ldg(pr.work + w) : make_int4(-1, 0, 0, 0);
+        s_next[0] = 0; s_next[1] = 0;
     }
-    for (int i = tid; i < NOC; i += TB) oc_cur[i] = 0;
-    for (int i = tid; i < 68; i += TB) bins[i] = 0;
+    for (int i = tid; i < NOC; i += TB) oc_cnt[i] = 0;
+    for (int i = tid; i < 3 * NBIN; i += TB) bins[i] = 0;
     __syncthreads();
-    for (;;) {
-        const int4 wk = s_work;                      // published by the barrier that ended the previous item
+    for (int iter = 0;; ++iter) {
+        // no barrier between the items of the previous work item and this: a warp that finds no more items goes
+        // on to the records of the next work item (its slot was written before the previous closing barrier)
+        const int4 wk = s_wk[iter & 1];
         if (wk.x < 0) break;
-        // the next work item is claimed and read now; its latency hides behind this item's processing
-        int4 nwk = make_int4(-1, 0, 0, 0);
+        stage(wk);
+        // the work item after this one is claimed now (slot of the other parity: the slow warps of the previous
+        // work item may still have to read this one's)
         if (tid == 0) {
             const int w = pr.counters[pr.wb] + atomicAdd(&pr.counters[pr.wc], 1);
-            if (w < pr.counters[pr.we]) nwk = __ldg(pr.work + w);
-            s_nwk = nwk;                                 // read behind the next barrier (prefetch of its records)
+            s_wk[(iter + 1) & 1] = (w < pr.counters[pr.we]) ? __ldg(pr.work + w) : make_int4(-1, 0, 0, 0);
         }
-        const int tile = wk.x, cb = wk.y, cn = wk.z;
-#ifndef IB_NO_PF
-        // this chunk's forces and ids are first needed after the staging and the sort: pull them into L2 now
-        // (one 128-byte line per 16 doubles / 32 ids; the item loop then waits on L2, not on DRAM)
-        if (16 * tid < cn) {
-            if (DO_SPREAD) {
-#pragma unroll
-                for (int d = 0; d < 3; ++d) ib_prefetch_l2(pr.sG + (int64_t)d * P + cb + 16 * tid);
-            }
-            if (DO_INTERP && 32 * tid < cn) ib_prefetch_l2(pr.sid + cb + 32 * tid);
-        }
-#endif
-        const int t3[3] = {tile % ntx, (tile / ntx) % nty, tile / (ntx * nty)};
+        const int t3[3] = {wk.w & 1023, (wk.w >> 10) & 1023, wk.w >> 20};     // tile coordinates, packed by ibk_tile_scan
         int h0[3];                                       // halo origin (global index of halo entry 0), wrapped
 #pragma unroll
         for (int d = 0; d < 3; ++d) h0[d] = PER ? ib_wrap(TT * t3[d] - 2, n[d]) : TT * t3[d] - 2;
-
-        // ---- halo load, zero the accumulators ---------------------------------------------------
-#ifndef IB_NO_HALO
+        __syncthreads();                             // every warp has left the items of the previous work item and counted its points of this one
+        if (tid == 0) s_next[(iter + 1) & 1] = 0;    // batch counter of the next work item
+        // ---- halo: asynchronous copies straight into shared memory, awaited before the items -------------
         if (DO_INTERP) {
+#pragma unroll
             for (int idx = tid; idx < 3 * TH3; idx += TB) {
                 int c = idx >> 9, r = idx & 511;
                 int i = h0[0] + (r & 7), j = h0[1] + ((r >> 3) & 7), k = h0[2] + (r >> 6);
-                double val = 0.0;                        // faces outside a bounded grid read as zero (never used: weight dropped)
                 if (PER) { i -= (i >= n[0]) ? n[0] : 0; j -= (j >= n[1]) ? n[1] : 0; k -= (k >= n[2]) ? n[2] : 0; }
-                if (PER || (i >= 0 && i < n[0] && j >= 0 && j < n[1] && k >= 0 && k < n[2]))
-                    val = __ldg(pr.fld[c] + ((int64_t)k * n[1] + j) * n[0] + i);
-                su[c * SU3 + (r >> 6) * SZ + (r & 63)] = val;
+                // faces outside a bounded grid read as zero (source size 0: their weight meets no force and no velocity)
+                const bool in = PER || (i >= 0 && i < n[0] && j >= 0 && j < n[1] && k >= 0 && k < n[2]);
+                const double *src = in ? pr.fld[c] + ((int64_t)k * n[1] + j) * n[0] + i : pr.fld[c];
+                const unsigned dst = (unsigned)__cvta_generic_to_shared(su + c * SU3 + (r >> 6) * SZ + (r & 63));
+                asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(dst), "l"(src), "r"(in ? 8 : 0) : "memory");
+            }
+            asm volatile("cp.async.commit_group;" ::: "memory");
+        }
+        {                                            // the next work item's coordinates -> L2 while this one is processed
+            const int4 nx4 = s_wk[(iter + 1) & 1];
+            if (nx4.x >= 0) {
+                for (int i = 16 * tid; i < 3 * CH; i += 16 * TB) {
+                    const int d = i / CH, o = i - d * CH;          // CH is a multiple of 16
+                    if (o < nx4.z) ib_prefetch_l2(pr.sx + (int64_t)d * P + nx4.y + o);
+                }
             }
         }
-#endif
-
-        {
-            // ---- stage the chunk, count points per half-cell -----------------------------------
-            {
-                double xr[CH / TB][3];                   // all loads of the chunk in flight at once
+        {                                            // exclusive scan of the 512 counts, SCK per thread
+            constexpr int SCK = (NOC + TB - 1) / TB;
+            int v[SCK], s = 0;
 #pragma unroll
-                for (int k = 0; k < CH / TB; ++k) {
-                    const int i = tid + k * TB;
-#pragma unroll
-                    for (int d = 0; d < 3; ++d)
-                        xr[k][d] = (i < cn) ? __ldcs(pr.sx + (int64_t)d * P + cb + i) : 0.0;
-                }
-#pragma unroll
-                for (int k = 0; k < CH / TB; ++k) {
-                    const int i = tid + k * TB;
-                    if (i < cn) {
-                        double xi[3];
-#pragma unroll
-                        for (int d = 0; d < 3; ++d) {
-                            xi[d] = ib_tile_coord(xr[k][d], org[d], pr.g.h, pr.inv_h);
-                            sxi[d * CH + i] = xi[d];
-                        }
-                        atomicAdd(&oc_cur[ib_octant_key(xi[0], xi[1], xi[2])], 1);
-                    }
-                }
+            for (int k = 0; k < SCK; ++k) {
+                v[k] = (SCK * tid + k < NOC) ? oc_cnt[SCK * tid + k] : 0;
+                s += v[k];
             }
+            int inc = s;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                int t = __shfl_up_sync(0xffffffffu, inc, o);
+                if (lane >= o) inc += t;
+            }
+            if (lane == 31) wsum[wid] = inc;
             __syncthreads();
-#ifndef IB_NO_PF
-            {                                            // the next chunk's coordinates -> L2 while this one is processed
-                const int4 nx4 = s_nwk;
-                if (nx4.x >= 0) {
-                    for (int i = 16 * tid; i < 3 * CH; i += 16 * TB) {
-                        const int d = i / CH, o = i - d * CH;          // CH is a multiple of 16
-                        if (o < nx4.z) ib_prefetch_l2(pr.sx + (int64_t)d * P + nx4.y + o);
-                    }
-                }
-            }
-#endif
-            {                                            // exclusive scan of the 512 counts, SCK per thread
-                constexpr int SCK = (NOC + TB - 1) / TB;
-                int v[SCK], s = 0;
+            int ex = inc - s;
+            for (int w = 0; w < wid; ++w) ex += wsum[w];
 #pragma unroll
-                for (int k = 0; k < SCK; ++k) {
-                    v[k] = (SCK * tid + k < NOC) ? oc_cur[SCK * tid + k] : 0;
-                    s += v[k];
+            for (int k = 0; k < SCK; ++k) {
+                if (SCK * tid + k < NOC) { oc_start[SCK * tid + k] = ex; oc_cnt[SCK * tid + k] = 0; }   // counts: ready for the next work item
+                ex += v[k];
+            }
+            if (tid == TB - 1) oc_start[NOC] = ex;
+        }
+        __syncthreads();
+        // ---- items: runs of records and point count; rank among the items of equal component and count ----
+        int my_nf[NIT], my_rf[NIT], my_rem[NIT], my_rr[NIT];     // whole units of the item and their first rank, points and rank of the last unit
+#pragma unroll
+        for (int j = 0; j < NIT; ++j) {
+            const int it = tid + j * TB;
+            my_nf[j] = 0; my_rf[j] = 0; my_rem[j] = 0; my_rr[j] = 0;
+            if (it < NITEM) {
+                int c, l[3], lo[3], hi[3];
+                ib_item_decode(it, c, l);
+#pragma unroll
+                for (int d = 0; d < 3; ++d) ib_half_range(c, d, l[d], lo[d], hi[d]);
+                unsigned rn[4];
+                int cnt = 0;
+#pragma unroll
+                for (int rr = 0; rr < 4; ++rr) {
+                    const int z2 = lo[2] + (rr >> 1), y2 = lo[1] + (rr & 1);
+                    const bool ok = z2 <= hi[2] && y2 <= hi[1];
+                    const int b = (z2 * 8 + y2) * 8;
+                    const unsigned s0 = ok ? oc_start[b + lo[0]] : 0, s1 = ok ? oc_start[b + hi[0] + 1] : 0;
+                    rn[rr] = s0 | (s1 << 16);
+                    cnt += (int)(s1 - s0);
                 }
-                int inc = s;
+                item_runs[it] = make_uint4(rn[0], rn[1], rn[2], rn[3]);
+                my_nf[j] = cnt / PCAP;
+                my_rem[j] = cnt - PCAP * my_nf[j];
+                if (my_nf[j] > 0) my_rf[j] = atomicAdd(&bins[c * NBIN + PCAP], my_nf[j]);
+                if (my_rem[j] > 0) my_rr[j] = atomicAdd(&bins[c * NBIN + my_rem[j]], 1);
+            }
+        }
+        // ---- the records, in half-cell order: six (a,q) sets, force / h^3, id ------------------------
+#pragma unroll
+        for (int k = 0; k < KPT; ++k) {
+            if (ks[k] >= 0) {
+                const int key = ks[k] & 511;
+                const int pos = oc_start[key] + (ks[k] >> 9);
+#pragma unroll
+                for (int d = 0; d < 3; ++d) {
+                    // face-aligned: cell hd >> 1; centre-aligned: shifted cell (hd + 1) >> 1 covers xi - 1/2 in [l-1, l).
+                    // r in [0,1] up to rounding at cell boundaries, where the formula continues phi smoothly (A19)
+                    const int hd = (key >> (3 * d)) & 7;
+                    sets[(2 * d) * CH + pos] = ib_aq(xi[k][d] - (double)(hd >> 1));
+                    sets[(2 * d + 1) * CH + pos] = ib_aq(xi[k][d] + 0.5 - (double)((hd + 1) >> 1));
+                }
+                if (DO_SPREAD) {
+#pragma unroll
+                    for (int d = 0; d < 3; ++d) sGs[d * CH + pos] = Gr[k][d] * pr.ih3;
+                }
+                if (DO_INTERP) sids[pos] = idr[k];
+            }
+        }
+        if (DO_INTERP) asm volatile("cp.async.wait_group 0;" ::: "memory");      // this thread's part of the halo has landed
+        __syncthreads();
+        // ---- order the units by component, then by point count (descending): every warp scans the 3 x PCAP
+        // bins for itself (lane l: the units of PCAP - l points).  Unit k of component c goes to order[c][k] as
+        // item | part << 9; batch b of the item loop is the 8 units 8 (b / 3) ... of component b % 3, so that the
+        // batches come in roughly descending size whatever their component (longest first keeps the warps level
+        // at the end of the work item).
+        int ncomp[3], nbatch;
+        {
+            int pre[3];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const int v = lane < PCAP ? bins[c * NBIN + PCAP - lane] : 0;
+                int inc = v;
 #pragma unroll
                 for (int o = 1; o < 32; o <<= 1) {
                     int t = __shfl_up_sync(0xffffffffu, inc, o);
                     if (lane >= o) inc += t;
                 }
-                if (lane == 31) wsum[wid] = inc;
-                __syncthreads();
-                int ex = inc - s;
-                for (int w = 0; w < wid; ++w) ex += wsum[w];
-#pragma unroll
-                for (int k = 0; k < SCK; ++k) {
-                    if (SCK * tid + k < NOC) { oc_start[SCK * tid + k] = ex; oc_cur[SCK * tid + k] = ex; }
-                    ex += v[k];
-                }
-                if (tid == TB - 1) oc_start[NOC] = ex;
+                pre[c] = inc - v;
+                ncomp[c] = __shfl_sync(0xffffffffu, inc, 31);
             }
-            __syncthreads();
-#ifndef IB_NO_PASS2
-            for (int i = tid; i < cn; i += TB) {
-                int key = ib_octant_key(sxi[i], sxi[CH + i], sxi[2 * CH + i]);
-                sidx[atomicAdd(&oc_cur[key], 1)] = (unsigned short)i;
-            }
-#endif
-            // ---- points per work item, order items by count (descending) -----------------------
-            for (int it = tid; it < NITEM; it += TB) {
-                int c, l[3], lo[3], hi[3];
-                ib_item_decode(it, c, l);
+            static_assert(PCAP <= 32 && PCAP % 4 == 0, "one lane per unit size; the item loop steps by 4 points");
+            nbatch = 3 * ((max(ncomp[0], max(ncomp[1], ncomp[2])) + 7) >> 3);
 #pragma unroll
-                for (int d = 0; d < 3; ++d) ib_half_range(c, d, l[d], lo[d], hi[d]);
-                int cnt = 0;
-                for (int z2 = lo[2]; z2 <= hi[2]; ++z2)
-                    for (int y2 = lo[1]; y2 <= hi[1]; ++y2) {
-                        int b = (z2 * 8 + y2) * 8;
-                        cnt += oc_start[b + hi[0] + 1] - oc_start[b + lo[0]];
-                    }
-                item_cnt[it] = cnt;
-                atomicAdd(&bins[min(cnt, NBIN - 1)], 1);
-            }
-            __syncthreads();
-            if (wid == 0) {                       // descending exclusive scan of the bins (bin 0 dropped)
-                int carry = 0;
-                for (int b0 = NBIN - 1; b0 >= 1; b0 -= 32) {
-                    int b = b0 - lane;
-                    int v = (b >= 1) ? bins[b] : 0, inc = v;
-#pragma unroll
-                    for (int o = 1; o < 32; o <<= 1) {
-                        int t = __shfl_up_sync(0xffffffffu, inc, o);
-                        if (lane >= o) inc += t;
-                    }
-                    if (b >= 1) bins[b] = carry + inc - v;
-                    carry += __shfl_sync(0xffffffffu, inc, 31);
-                }
-                if (lane == 0) s_nitems = carry;
-            }
-            __syncthreads();
-            for (int it = tid; it < NITEM; it += TB) {
-                int cnt = item_cnt[it];
-                if (cnt > 0) order[atomicAdd(&bins[min(cnt, NBIN - 1)], 1)] = ib_item_code(it);
-            }
-            __syncthreads();
-            const int nitems = s_nitems;
-            // the half-cell cursors and the count bins are dead from here on: reset them for the next
-            // work item (their next use lies behind the barriers that end this one)
-            for (int i = tid; i < NOC; i += TB) oc_cur[i] = 0;
-            for (int i = tid; i < 68; i += TB) bins[i] = 0;
-
-            // ---- the items --------------------------------------------------------------------------
-            double *mystg = stg + (wid * 8 + grp) * GSTRIDE;
-            for (;;) {
-                int base = 0;
-                if (lane == 0) base = atomicAdd(&s_next, 8);     // warps pull 8 items at a time (largest first)
-                base = __shfl_sync(0xffffffffu, base, 0);
-                if (base >= nitems) break;
-#ifdef IB_NO_ITEMS
-                if (base >= 0) break;
-#endif
-                const int wi = base + grp;
-                const bool have = wi < nitems;
-                int c = 0, l[3] = {0, 0, 0};
-                if (have) ib_item_unpack(order[wi], c, l);
-                // runs of the half-cell order that make up this item
-                int rstart[4], rend[4], npts = 0;
-                {
-                    int lo[3], hi[3];
-#pragma unroll
-                    for (int d = 0; d < 3; ++d) ib_half_range(c, d, l[d], lo[d], hi[d]);
-#pragma unroll
-                    for (int rr = 0; rr < 4; ++rr) {
-                        int z2 = lo[2] + (rr >> 1), y2 = lo[1] + (rr & 1);
-                        bool ok = have && z2 <= hi[2] && y2 <= hi[1];
-                        int b = (z2 * 8 + y2) * 8;
-                        int s0 = ok ? oc_start[b + lo[0]] : 0, s1 = ok ? oc_start[b + hi[0] + 1] : 0;
-                        rstart[rr] = s0 - npts;          // rank = rstart + virtual index
-                        npts += s1 - s0;
-                        rend[rr] = npts;                 // virtual indices < rend belong to runs <= rr
-                    }
-                }
-                int nmax = npts;
-#pragma unroll
-                for (int o = 16; o >= 4; o >>= 1) nmax = max(nmax, __shfl_xor_sync(0xffffffffu, nmax, o));
-                // window origin inside the halo; base3[d] = scaled coordinate of the point minus
-                // base3 is r in [0,1): d == c: cell l; d != c: shifted cell covers xi-1/2 in [l-1,l)
-                int o3[3];
-                double base3[3];
-#pragma unroll
-                for (int d = 0; d < 3; ++d) {
-                    o3[d] = l[d] + ((d == c) ? 1 : 0);
-                    base3[d] = (d == c) ? (double)l[d] : (double)l[d] - 0.5;
-                }
-                const double *suc = su + c * SU3 + o3[2] * SZ + o3[1] * TH + o3[0] + q;   // lane q owns x-column q
-                double uu[4][4], ff[4][4];
-#pragma unroll
-                for (int j = 0; j < 4; ++j)
-#pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        uu[j][i] = DO_INTERP ? suc[i * SZ + j * TH] : 0.0;            // [y j][z i]
-                        ff[j][i] = 0.0;
-                    }
-                const double *Gc = DO_SPREAD ? pr.sG + (int64_t)c * P + cb : nullptr;
-                double *Uc = DO_INTERP ? pr.Up + (int64_t)c * P : nullptr;
-
-                // Software pipeline over quads of 4 points: while the group consumes quad k from one staging
-                // buffer, lane q computes the delta weights of its point of quad k+1 into the other buffer and
-                // the index / force / id of its point of quad k+2 are in flight.  One __syncwarp per quad.
-                int si1, id0 = 0, id1 = 0;
-                bool valid0, valid1;
-                double G1 = 0.0;
-#define IB_FETCH(R0, SI, GV, ID, VALID)                                                                      \
-    {                                                                                                        \
-        const int vi = (R0) + q;                                                                             \
-        VALID = vi < npts;                                                                                   \
-        int rank = vi + ((vi < rend[0]) ? rstart[0] : (vi < rend[1]) ? rstart[1] : (vi < rend[2]) ? rstart[2] : rstart[3]); \
-        SI = VALID ? (int)sidx[rank] : 0;                                                                    \
-        GV = (DO_SPREAD && VALID) ? __ldcs(Gc + SI) : 0.0;                                                   \
-        if (DO_INTERP && VALID) ID = __ldcs(pr.sid + cb + SI);                                               \
-    }
-#define IB_WEIGHTS(BUF, SI, GV, VALID)                                                                       \
-    {                                                                                                        \
-        double wgt[3][4];                                                                                    \
-        _Pragma("unroll") for (int d = 0; d < 3; ++d) {                                                      \
-            /* r in [0,1] up to rounding at cell boundaries, where the formula continues phi smoothly (A19) */ \
-            ib_phi4((VALID) ? sxi[d * CH + SI] - base3[d] : 0.0, wgt[d]); /* padding lanes: any r in range */ \
-        }                                                                                                    \
-        if (!(VALID)) { _Pragma("unroll") for (int m = 0; m < 4; ++m) wgt[2][m] = 0.0; }                     \
-        double *rec = mystg + (BUF) * GBUF + q * REC;                                                        \
-        *reinterpret_cast<double2 *>(rec + 0) = make_double2(wgt[0][0], wgt[0][1]);                          \
-        *reinterpret_cast<double2 *>(rec + 2) = make_double2(wgt[0][2], wgt[0][3]);                          \
-        *reinterpret_cast<double2 *>(rec + 4) = make_double2(wgt[1][0], wgt[1][1]);                          \
-        *reinterpret_cast<double2 *>(rec + 6) = make_double2(wgt[1][2], wgt[1][3]);                          \
-        *reinterpret_cast<double2 *>(rec + 8) = make_double2(wgt[2][0], wgt[2][1]);                          \
-        *reinterpret_cast<double2 *>(rec + 10) = make_double2(wgt[2][2], wgt[2][3]);                         \
-        rec[12] = (GV) * pr.ih3;                                                                             \
-    }
-                {
-                    int si0;
-                    double G0 = 0.0;
-                    IB_FETCH(0, si0, G0, id0, valid0)
-                    IB_WEIGHTS(0, si0, G0, valid0)
-                }
-                IB_FETCH(4, si1, G1, id1, valid1)
-                __syncwarp();
-                int buf = 0;
-#ifdef IB_NO_MAIN
-                nmax = 0;
-#endif
-                for (int r0 = 0; r0 < nmax; r0 += 4, buf ^= 1) {
-                    // -- weights of quad r0+4 into the other buffer, fetch quad r0+8
-                    int si2 = 0, id2 = 0;
-                    bool valid2 = false;
-                    double G2 = 0.0;
-                    if (r0 + 4 < nmax) {
-                        IB_WEIGHTS(buf ^ 1, si1, G1, valid1)
-                        IB_FETCH(r0 + 8, si2, G2, id2, valid2)
-                    }
-                    // -- consume quad r0
-                    const double *cur = mystg + buf * GBUF;
-                    double mine = 0.0;
-#pragma unroll
-                    for (int jp = 0; jp < 4; ++jp) {
-                        const double *rj = cur + jp * REC;
-                        double2 a0 = *reinterpret_cast<const double2 *>(rj + 4), a1 = *reinterpret_cast<const double2 *>(rj + 6);
-                        double2 b0 = *reinterpret_cast<const double2 *>(rj + 8), b1 = *reinterpret_cast<const double2 *>(rj + 10);
-                        const double wy[4] = {a0.x, a0.y, a1.x, a1.y}, wz[4] = {b0.x, b0.y, b1.x, b1.y};
-                        const double wx = rj[q];
-                        if (DO_INTERP) {
-                            double rr[4];
-#pragma unroll
-                            for (int j = 0; j < 4; ++j) {
-                                rr[j] = uu[j][0] * wz[0];
-                                rr[j] = fma(uu[j][1], wz[1], rr[j]);
-                                rr[j] = fma(uu[j][2], wz[2], rr[j]);
-                                rr[j] = fma(uu[j][3], wz[3], rr[j]);
-                            }
-                            double pv = fma(rr[0], wy[0], rr[1] * wy[1]) + fma(rr[2], wy[2], rr[3] * wy[3]);
-                            pv *= wx;
-                            pv += __shfl_xor_sync(0xffffffffu, pv, 1);
-                            pv += __shfl_xor_sync(0xffffffffu, pv, 2);
-                            if (q == jp) mine = pv;
-                        }
-                        if (DO_SPREAD) {
-                            double gx = rj[12] * wx;
-#pragma unroll
-                            for (int j = 0; j < 4; ++j) {
-                                double gj = gx * wy[j];
-#pragma unroll
-                                for (int i = 0; i < 4; ++i) ff[j][i] = fma(gj, wz[i], ff[j][i]);
-                            }
-                        }
-                    }
-                    if (DO_INTERP && valid0) __stcs(Uc + id0, mine);
-                    valid0 = valid1; id0 = id1;
-                    si1 = si2; G1 = G2; id1 = id2; valid1 = valid2;
-                    __syncwarp();
-                }
-#undef IB_FETCH
-#undef IB_WEIGHTS
-#ifdef IB_NO_FLUSH
-                if (DO_SPREAD && have && ff[0][0] == 123.456) {
-#else
-                if (DO_SPREAD && have) {
-#endif
-                    // lane q flushes x-column q: for every (y,z) the 4 lanes of the group hit 4 consecutive faces
-                    // (bounded grid: faces outside 0..n-1 do not exist -- their share of the force is dropped, A26)
-                    constexpr bool per = PER != 0;
-                    int gi = h0[0] + o3[0] + q;
-                    if (per) gi -= (gi >= n[0]) ? n[0] : 0;
-                    const bool xin = per || (gi >= 0 && gi < n[0]);
-                    int gj[4], gk[4];
-                    bool jin[4], kin[4];
-#pragma unroll
-                    for (int m = 0; m < 4; ++m) {
-                        gj[m] = h0[1] + o3[1] + m; gk[m] = h0[2] + o3[2] + m;
-                        if (per) { gj[m] -= (gj[m] >= n[1]) ? n[1] : 0; gk[m] -= (gk[m] >= n[2]) ? n[2] : 0; }
-                        jin[m] = per || (gj[m] >= 0 && gj[m] < n[1]);
-                        kin[m] = per || (gk[m] >= 0 && gk[m] < n[2]);
-                    }
-                    double *fp = pr.frc[c] + gi;
-                    int ok[4], oj[4];                                  // 32-bit face offsets (n_cells < 2^31)
-#pragma unroll
-                    for (int m = 0; m < 4; ++m) { ok[m] = gk[m] * n[1] * n[0]; oj[m] = gj[m] * n[0]; }
-#pragma unroll
-                    for (int i = 0; i < 4; ++i)
-#pragma unroll
-                        for (int j = 0; j < 4; ++j)
-                            if (xin && kin[i] && jin[j]) atomicAdd(fp + (ok[i] + oj[j]), ff[j][i]);
+            for (int j = 0; j < NIT; ++j) {
+                if (wid * 32 + j * TB < NITEM) {                // warp-uniform: some lane of this warp has an item
+                    const int it = tid + j * TB;
+                    const int c = it >= 200 ? 2 : (it >= 100 ? 1 : 0);
+                    // the owner lane of the size cannot know the asker's component, so all three prefixes travel
+                    const int owner = PCAP - max(my_rem[j], 1);
+                    const int a0 = __shfl_sync(0xffffffffu, pre[0], owner), a1 = __shfl_sync(0xffffffffu, pre[1], owner),
+                              a2 = __shfl_sync(0xffffffffu, pre[2], owner);
+                    unsigned short *oc = order + c * NORD;
+                    for (int pp = 0; pp < my_nf[j]; ++pp) oc[my_rf[j] + pp] = (unsigned short)(it | (pp << 9));   // units of PCAP points come first
+                    if (my_rem[j] > 0) oc[(c == 0 ? a0 : (c == 1 ? a1 : a2)) + my_rr[j]] = (unsigned short)(it | (my_nf[j] << 9));
                 }
             }
         }
-        __syncthreads();                              // every warp has left the item loop and read s_work
-        if (tid == 0) { s_work = nwk; s_next = 0; }
-        __syncthreads();                              // buffers are reused by the next work item
+        __syncthreads();
+        for (int i = tid; i < 3 * NBIN; i += TB) bins[i] = 0;        // next use: behind the barriers that end this work item
+
+        // ---- the items, in batches of 8 of one component ----------------------------------------------
+        // the next batch is claimed one batch ahead: the shared-memory atomic and its broadcast are out of the way
+        int bnext = 0;
+        if (lane == 0) bnext = atomicAdd(&s_next[iter & 1], 1);
+        for (;;) {
+            const int b = __shfl_sync(0xffffffffu, bnext, 0);
+            if (b >= nbatch) break;
+            if (lane == 0) bnext = atomicAdd(&s_next[iter & 1], 1);   // warps pull one batch at a time
+            const int c = b % 3, k8 = (b / 3) * 8;                                 // warp-uniform
+            const int nc = c == 0 ? ncomp[0] : (c == 1 ? ncomp[1] : ncomp[2]);
+            if (k8 >= nc) continue;                                                // this component has fewer batches
+            const int un = k8 + grp < nc ? (int)order[c * NORD + k8 + grp] : NITEM;      // empty slot: the item without points
+            ib_run_batch<DO_SPREAD, DO_INTERP, PER>(c, pr, sm, un & 511, un >> 9, q, h0, n, wsa, wca, wsg);
+        }
     }
 }
 
@@ -531,9 +623,9 @@ static ib_status launch_tiled_p(ib_ctx *c, const ib_tiled_params &pr, bool with_
     static unsigned char configured[64] = {0};           // per device: function attributes belong to the device's context
     static int sm_count[64] = {0};
     const int dv = c->device & 63;
-    const size_t smem = (size_t)(3 * SU3 + 3 * CH + NWARP * 8 * GSTRIDE) * sizeof(double) +
-                        (NOC + 68) * sizeof(int) + (516 + 2 * NITEM + CH) * sizeof(unsigned short);
-    static_assert(CH % TB == 0, "chunk must be a whole number of points per thread");
+    const size_t smem = (size_t)(3 * SU3 + 12 * CH + 3 * CH) * sizeof(double) + (NITEM + 1) * sizeof(uint4) +
+                        (NITEM + 3 + CH + NOC + 3 * NBIN + 2) * sizeof(int) + (516 + 3 * NORD) * sizeof(unsigned short);
+    static_assert(CH % 16 == 0, "staging layout");
     if (!configured[dv]) {
         IB_CUDA_TRY(cudaFuncSetAttribute(ibk_tiled_kernel<S, I, PER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         configured[dv] = 1;
