@@ -133,17 +133,30 @@ def whole_job_value(units_per_rank_per_step, steps, t_rank_s, world, device=None
     return world * units_per_rank_per_step * steps / t, t
 
 
+def kernel_source_sha():
+    """sha256 over the sources of the dominant kernel: the stamp of an ncu capture (profiles/*_traffic.json)."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in ("ib_tiled.cu", "ib_common.cuh", "ib_point.cuh"):
+        h.update(open(os.path.join(ROOT, "paper_2503_22695_b200", "csrc", f), "rb").read())
+    return h.hexdigest()[:16]
+
+
 def ncu_traffic_bytes(workload_name):
-    """DRAM bytes per launch of the dominant kernel from the committed ncu capture
-    (profiles/r01_traffic.txt: '<workload> <bytes>' lines), or None."""
-    path = os.path.join(ROOT, "profiles", "r01_traffic.txt")
-    if not os.path.exists(path):
-        return None
-    for line in open(path):
-        parts = line.split()
-        if len(parts) >= 2 and parts[0] == workload_name:
-            return int(parts[1])
-    return None
+    """(DRAM bytes per launch of the dominant kernel, source) from the newest committed ncu capture
+    profiles/r*_traffic.json -- only if it was taken on THESE kernel sources (the file carries their
+    sha256); otherwise (None, why): a stale capture is not a measurement of this build."""
+    import glob
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_traffic.json")))
+    if not files:
+        return None, "no ncu capture committed"
+    rec = json.load(open(files[-1]))
+    if rec.get("kernel_source_sha256_16") != kernel_source_sha():
+        return None, f"{os.path.basename(files[-1])} was captured on other kernel sources"
+    v = rec.get("dram_bytes_per_launch", {}).get(workload_name)
+    if v is None:
+        return None, f"{os.path.basename(files[-1])} has no capture of {workload_name}"
+    return int(v), f"ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum ({os.path.basename(files[-1])}, same kernel sources)"
 
 
 # ----------------------------------------------------------------------------------------------
@@ -161,7 +174,7 @@ def cpu_sample(wl, frac):
                 n_points=int(np.prod(wl.nsub[:ne].astype(np.int64), axis=1).sum()), n_elems=ne)
 
 
-def time_oracle(wl, frac, reps=1):
+def time_oracle(wl, frac, reps=1, omp=False):
     import oracle
     s = cpu_sample(wl, frac)
     g = oracle.make_grid(wl.nx, wl.ny, wl.nz, wl.h, wl.origin)
@@ -169,7 +182,7 @@ def time_oracle(wl, frac, reps=1):
     for _ in range(reps):
         t0 = time.perf_counter()
         oracle.coupling_step(g, s["conn"], s["X"], s["fibers"], s["mat_id"], s["nsub"], wl.mats, s["x"],
-                             wl.u, wl.v, wl.w)
+                             wl.u, wl.v, wl.w, omp=omp)
         dt = time.perf_counter() - t0
         best = dt if best is None else min(best, dt)
     return s, best
@@ -204,6 +217,37 @@ def run_reference(args):
 
 
 # ----------------------------------------------------------------------------------------------
+def relaunch(n):
+    """`python bench.py --gpus N` without torchrun: start the N replica processes ourselves, one per GPU, the
+    way the driver does (python -m torch.distributed.run, rendezvous on 127.0.0.1)."""
+    import socket
+    import subprocess
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
+
+
+def run_dry(args):
+    """The launch and whole-job arithmetic of run_ours with no GPU: every rank 'processes' the workload's
+    points in 1 + rank/10 seconds; rank 0 prints the line."""
+    import torch.distributed as dist
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    if world > 1:
+        dist.init_process_group("gloo")
+    units = 1000
+    value, t = whole_job_value(units, args.steps, 1.0 + 0.1 * rank, world, None)
+    if rank == 0:
+        print(json.dumps({"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                          "dry_run": True, "slowest_rank_s": t}))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -324,8 +368,11 @@ def run_ours(args):
         step_ms = 1e3 * t_dev / args.steps
         abytes = algorithmic_bytes(wl)
         dfma_peak, _ = ibcouple.probe_dfma(local)
-        # dominant kernel: points' 72 B + grid 48 B/cell of the algorithmic bytes belong to it
-        dom_bytes = 72 * wl.n_points + 48 * wl.n_cells
+        # dominant kernel: the points' 72 B and the 24 B/cell of u,v,w belong to it; the other 24 B/cell of the
+        # SURVEY.md §8(d) figure (f out, incl. its zero-fill) are the zero phase's -- a memset on another
+        # stream -- so that the fraction cannot exceed 1 on sparsely filled grids
+        dom_bytes = 72 * wl.n_points + 24 * wl.n_cells
+        traffic, traffic_src = ncu_traffic_bytes(wl.name)
         # The dominant kernel is bound by the plain fp64 ALUs, not by HBM: the top-level
         # roofline is the ALU one -- algorithmic flops = 2 x 600 DFMA slots per force point (SURVEY.md
         # §8(d): weights 100 + interpolation 252 + spreading 252), peak derived from the unit count and
@@ -338,7 +385,7 @@ def run_ours(args):
         dom_tf = 2.0 * dom_slots / (dom_ms * 1e-3) / 1e12
         roofline = {"bound": "alu", "kernel": "spread+interp (" + ("tiled" if args.variant else "per-point") + ")",
                     "achieved": dom_tf, "peak": alu_peak_tf, "unit": "TFLOP/s", "frac": dom_tf / alu_peak_tf,
-                    "traffic": ncu_traffic_bytes(wl.name),
+                    "traffic": traffic, "traffic_source": traffic_src,
                     "peak_source": f"derived: 64 DFMA/clk/SM x {sms} SMs x {sm_hz / 1e6:.0f} MHz x 2 flop (fp64 vector pipe); "
                                    f"ib_probe_dfma measured {2 * dfma_peak / 1e12:.1f} TFLOP/s in this run",
                     "kernel_ms": dom_ms, "algorithmic_flops_per_launch": 2 * dom_slots,
@@ -354,6 +401,9 @@ def run_ours(args):
         s, dt = time_oracle(wl, args.cpu_frac)
         sample = (f"first {s['n_elems']} of {wl.n_elems} elements ({s['n_points']} force points) of {wl.name}, "
                   f"full grid, one oracle_coupling_step, {dt:.1f} s")
+        # all-core leg (SURVEY.md §8(d) "Oracle timing (ii)"): the same source built with -fopenmp, 4x the sample
+        cores = len(os.sched_getaffinity(0))
+        s_all, dt_all = time_oracle(wl, min(1.0, 4 * args.cpu_frac), omp=True)
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": max(args.warmup, 3), "ms_per_step": step_ms, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -371,7 +421,10 @@ def run_ours(args):
                 "run_to_run": {"runs": 3, "max_abs_dev_over_max_abs": dev_rr},
                 "roofline": roofline,
                 "cpu_baseline": {"value": s["n_points"] / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
-                                 "sample": sample}}
+                                 "sample": sample,
+                                 "all_cores": {"value": s_all["n_points"] / dt_all, "unit": UNIT, "cores": cores,
+                                               "kind": "oracle built with -fopenmp (spread: private grid per thread; interpolation over points; FE force serial)",
+                                               "sample": f"first {s_all['n_elems']} elements ({s_all['n_points']} force points), {dt_all:.1f} s"}}}
         print(json.dumps(line))
     ctx.close()
     if world > 1:
@@ -388,9 +441,15 @@ def main():
     ap.add_argument("--workload", default="C3")
     ap.add_argument("--variant", type=int, default=1)
     ap.add_argument("--cpu-frac", type=float, default=1.0 / 16, dest="cpu_frac")
+    ap.add_argument("--dry-run", action="store_true", dest="dry_run",
+                    help="launch and timing plumbing only, on CPU with gloo (tests/test_bench_replicas.py)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return relaunch(args.gpus)
+    if args.dry_run:
+        return run_dry(args)
     return run_ours(args)
 
 

@@ -15,7 +15,9 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "ib_oracle.c")
 _SO = os.path.join(_HERE, "liboracle.so")
+_SO_OMP = os.path.join(_HERE, "liboracle_omp.so")      # same source with -fopenmp: bench.py's all-core timing leg only
 _lib = None
+_lib_omp = None
 
 
 class Material(C.Structure):
@@ -38,14 +40,33 @@ def build(force=False):
     return _SO
 
 
-def lib():
-    global _lib
+def build_omp(force=False):
+    """The same source with -fopenmp (spreading with one private grid per thread, interpolation over the
+    points): the all-core timing leg of bench.py.  Parity always uses the single-thread build."""
+    if force or (not os.path.exists(_SO_OMP)) or os.path.getmtime(_SO_OMP) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-ffp-contract=off", "-fno-fast-math", "-fopenmp",
+               "-o", _SO_OMP, _SRC, "-lm"]
+        subprocess.check_call(cmd)
+    return _SO_OMP
+
+
+def _declare(L):
+    L.oracle_phi.restype = C.c_double
+    L.oracle_phi.argtypes = [C.c_double]
+    L.oracle_num_points.restype = C.c_int64
+    return L
+
+
+def lib(omp=False):
+    global _lib, _lib_omp
+    if omp:
+        if _lib_omp is None:
+            build_omp()
+            _lib_omp = _declare(C.CDLL(_SO_OMP))
+        return _lib_omp
     if _lib is None:
         build()
-        _lib = C.CDLL(_SO)
-        _lib.oracle_phi.restype = C.c_double
-        _lib.oracle_phi.argtypes = [C.c_double]
-        _lib.oracle_num_points.restype = C.c_int64
+        _lib = _declare(C.CDLL(_SO))
     return _lib
 
 
@@ -218,8 +239,8 @@ def bin_sort(grid, xp, inv_h=None):
     return key, perm
 
 
-def coupling_step(grid, conn, X, fibers, mat_id, nsub, mats, x, u, v, w):
-    """dict(fu, fv, fw, Un, B)."""
+def coupling_step(grid, conn, X, fibers, mat_id, nsub, mats, x, u, v, w, omp=False):
+    """dict(fu, fv, fw, Un, B).  omp=True: the OpenMP build (timing only; sums in another order)."""
     conn, nsub, mat_id = _i32(conn), _i32(nsub), _i32(mat_id)
     X, x, u, v, w = _f64(X), _f64(x), _f64(u), _f64(v), _f64(w)
     fibers = None if fibers is None else _f64(fibers)
@@ -228,7 +249,7 @@ def coupling_step(grid, conn, X, fibers, mat_id, nsub, mats, x, u, v, w):
     fu, fv, fw = np.zeros(n), np.zeros(n), np.zeros(n)
     Un, B = np.empty((3, nn)), np.empty((3, nn))
     bad = C.c_int64(-1)
-    rc = lib().oracle_coupling_step(C.byref(grid), C.c_int64(nn), C.c_int64(ne), _p(conn, C.c_int32),
+    rc = lib(omp).oracle_coupling_step(C.byref(grid), C.c_int64(nn), C.c_int64(ne), _p(conn, C.c_int32),
                                     _p(X), _p(fibers), _p(mat_id, C.c_int32), _p(nsub, C.c_int32),
                                     make_materials(mats), _p(x), _p(u), _p(v), _p(w),
                                     _p(fu), _p(fv), _p(fw), _p(Un), _p(B), C.byref(bad))

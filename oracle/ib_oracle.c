@@ -730,6 +730,22 @@ static void support(const oracle_grid *g, int c, const ld xpt[3], int64_t i0[3],
     }
 }
 
+/* one point's share of component c, Eq.(24)-(26): acc[face] += G_c phi phi phi / h^3 over its 4x4x4 support */
+static void spread_point(const oracle_grid *g, int c, int64_t P, int64_t p, const double *xp, const double *Gp, ld h3, ld *acc)
+{
+    ld xpt[3] = {xp[p], xp[P + p], xp[2 * P + p]}, wt[3][4];
+    int64_t i0[3];
+    support(g, c, xpt, i0, wt);
+    ld G = Gp[c * P + p];
+    for (int m3 = 0; m3 < 4; ++m3)
+        for (int m2 = 0; m2 < 4; ++m2)
+            for (int m1 = 0; m1 < 4; ++m1) {
+                int64_t i = facei(g, i0[0] + m1, g->nx), j = facei(g, i0[1] + m2, g->ny), k = facei(g, i0[2] + m3, g->nz);
+                if (i < 0 || j < 0 || k < 0) continue;
+                acc[(k * g->ny + j) * g->nx + i] += G * wt[0][m1] * wt[1][m2] * wt[2][m3] / h3;
+            }
+}
+
 void oracle_spread(const oracle_grid *g, int64_t P, const double *xp, const double *Gp,
                    double *fu, double *fv, double *fw, int32_t accumulate)
 {
@@ -739,19 +755,19 @@ void oracle_spread(const oracle_grid *g, int64_t P, const double *xp, const doub
     for (int c = 0; c < 3; ++c) {
         ld *acc = (ld *)calloc((size_t)ncell, sizeof(ld));
         if (accumulate) for (int64_t i = 0; i < ncell; ++i) acc[i] = f[c][i];
-        for (int64_t p = 0; p < P; ++p) {
-            ld xpt[3] = {xp[p], xp[P + p], xp[2 * P + p]}, wt[3][4];
-            int64_t i0[3];
-            support(g, c, xpt, i0, wt);
-            ld G = Gp[c * P + p];
-            for (int m3 = 0; m3 < 4; ++m3)
-                for (int m2 = 0; m2 < 4; ++m2)
-                    for (int m1 = 0; m1 < 4; ++m1) {
-                        int64_t i = facei(g, i0[0] + m1, g->nx), j = facei(g, i0[1] + m2, g->ny), k = facei(g, i0[2] + m3, g->nz);
-                        if (i < 0 || j < 0 || k < 0) continue;
-                        acc[(k * g->ny + j) * g->nx + i] += G * wt[0][m1] * wt[1][m2] * wt[2][m3] / h3;
-                    }
+#ifdef _OPENMP            /* timing leg only (liboracle_omp.so): one private grid per thread, summed at the end */
+#pragma omp parallel
+        {
+            ld *mine = (ld *)calloc((size_t)ncell, sizeof(ld));
+#pragma omp for schedule(static)
+            for (int64_t p = 0; p < P; ++p) spread_point(g, c, P, p, xp, Gp, h3, mine);
+#pragma omp critical
+            for (int64_t i = 0; i < ncell; ++i) acc[i] += mine[i];
+            free(mine);
         }
+#else
+        for (int64_t p = 0; p < P; ++p) spread_point(g, c, P, p, xp, Gp, h3, acc);
+#endif
         for (int64_t i = 0; i < ncell; ++i) f[c][i] = (double)acc[i];
         free(acc);
     }
@@ -762,6 +778,9 @@ void oracle_interp(const oracle_grid *g, int64_t P, const double *xp, const doub
 {
     const double *f[3] = {u, v, w};
     for (int c = 0; c < 3; ++c)
+#ifdef _OPENMP            /* timing leg only (liboracle_omp.so): points are independent */
+#pragma omp parallel for schedule(static)
+#endif
         for (int64_t p = 0; p < P; ++p) {
             ld xpt[3] = {xp[p], xp[P + p], xp[2 * P + p]}, wt[3][4];
             int64_t i0[3];

@@ -11,7 +11,7 @@ CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libibcouple.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-         "-Xcompiler", "-fPIC", "-shared", "--fmad=true", "-Xptxas", "-v"]
+         "-Xcompiler", "-fPIC", "-shared", "--fmad=true", "-Xptxas", "-v", "-ldl"]
 
 
 def sources():
@@ -27,10 +27,9 @@ def needs_build():
 
 
 def build(force=False, verbose=False):
-    extra = os.environ.get("IB_NVCC_EXTRA", "").split()          # e.g. -D switches for kernel experiments
-    if not force and not extra and not needs_build():
+    if not force and not needs_build():
         return SO
-    cmd = [NVCC] + FLAGS + extra + ["-o", SO] + sources()
+    cmd = [NVCC] + FLAGS + ["-o", SO] + sources()
     r = subprocess.run(cmd, capture_output=True, text=True)
     log = r.stdout + r.stderr
     with open(os.path.join(HERE, "build.log"), "w") as f:

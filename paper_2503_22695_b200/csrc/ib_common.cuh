@@ -87,6 +87,8 @@ struct ib_ctx {
     cudaEvent_t ev_slab[IB_MAX_SLABS], ev_h2d[IB_MAX_SLABS];
     cudaEvent_t ev_zero;       // ... f has been zero-filled
     int64_t launches;
+    unsigned char tiled_cfg[8];  // ibk_tiled_kernel<S,I,PER>: dynamic shared memory size has been set
+    int sm_count;
     // NEXT-4 boundary loads (ib_set_tethers / ib_set_surface / ib_set_loads)
     int32_t *d_teth_ids, *d_faces;
     int64_t n_teth, n_faces;

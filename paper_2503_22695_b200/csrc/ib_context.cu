@@ -5,6 +5,7 @@
 #include <cstring>
 #include <new>
 #include <vector>
+#include <nvtx3/nvToolsExt.h>
 #include "ib_common.cuh"
 
 #define ST(s) ((cudaStream_t)(s))
@@ -28,8 +29,14 @@ static ib_status dev_upload(T **dst, const T *src, size_t n)
 struct ib_prof_rec { int phase; cudaEvent_t e0, e1; };
 typedef std::vector<ib_prof_rec> ib_prof_vec;
 
+// Every phase of a step is an NVTX range on the calling thread (names a timeline of the three streams; costs a
+// function-pointer check when no tool is attached) and, with ib_profile_enable, a pair of CUDA events.
+static const char *const ib_phase_name[IB_PHASE_COUNT] = {"ib:fe_force", "ib:points(count+scan)", "ib:sort(scatter)",
+                                                          "ib:spread+interp", "ib:restrict", "ib:zero f"};
+
 void ib_prof_begin(ib_ctx *c, int phase, cudaStream_t st)
 {
+    nvtxRangePushA(ib_phase_name[phase]);
     if (!c->profile) return;
     ib_prof_vec *v = (ib_prof_vec *)c->prof;
     ib_prof_rec r;
@@ -42,6 +49,7 @@ void ib_prof_begin(ib_ctx *c, int phase, cudaStream_t st)
 
 void ib_prof_end(ib_ctx *c, int phase, cudaStream_t st)
 {
+    nvtxRangePop();
     if (!c->profile) return;
     ib_prof_vec *v = (ib_prof_vec *)c->prof;
     for (size_t i = v->size(); i-- > 0;)

@@ -620,18 +620,17 @@ static int ib_small_blocks(int64_t nsmall_max, int sms)
 template <int S, int I, int PER>
 static ib_status launch_tiled_p(ib_ctx *c, const ib_tiled_params &pr, bool with_small, cudaStream_t st)
 {
-    static unsigned char configured[64] = {0};           // per device: function attributes belong to the device's context
-    static int sm_count[64] = {0};
-    const int dv = c->device & 63;
     const size_t smem = (size_t)(3 * SU3 + 12 * CH + 3 * CH) * sizeof(double) + (NITEM + 1) * sizeof(uint4) +
                         (NITEM + 3 + CH + NOC + 3 * NBIN + 2) * sizeof(int) + (516 + 3 * NORD) * sizeof(unsigned short);
     static_assert(CH % 16 == 0, "staging layout");
-    if (!configured[dv]) {
+    // per context (a context belongs to one device and, by the header's contract, to one thread at a time)
+    unsigned char &configured = c->tiled_cfg[S * 4 + I * 2 + PER];
+    if (!configured) {
         IB_CUDA_TRY(cudaFuncSetAttribute(ibk_tiled_kernel<S, I, PER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured[dv] = 1;
+        configured = 1;
     }
-    if (!sm_count[dv]) IB_CUDA_TRY(cudaDeviceGetAttribute(&sm_count[dv], cudaDevAttrMultiProcessorCount, c->device));
-    const int sms = sm_count[dv];
+    if (!c->sm_count) IB_CUDA_TRY(cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device));
+    const int sms = c->sm_count;
     // the few points of sparsely filled tiles go one by one on a second stream, beside the tile kernel
     const int64_t nsmall_max = min((int64_t)pr.P, (c->n_cells / (TT * TT * TT)) * (int64_t)(IB_SMALL_TILE - 1));
     const bool beside = !c->profile && with_small;

@@ -41,4 +41,22 @@ def test_single_rank_needs_no_process_group():
     sys.path.insert(0, ROOT)
     import bench
     assert bench.whole_job_value(10, 3, 0.5, 1) == (60.0, 0.5)
-    assert bench.ncu_traffic_bytes("no-such-workload") is None
+    v, why = bench.ncu_traffic_bytes("no-such-workload")
+    assert v is None and isinstance(why, str)               # never a stale or foreign capture
+
+
+def test_gpus_flag_starts_the_replicas_itself():
+    """`python bench.py --gpus 2` with WORLD_SIZE unset (how the driver may call it) must start two replica
+    processes and report n_gpus 2: the launcher re-executes bench.py under torch.distributed.run.  --dry-run
+    keeps the GPU out of it (gloo; every rank 'takes' 1 + rank/10 s for 1000 units per step)."""
+    import json
+    import subprocess
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--dry-run", "--steps", "3"],
+                       capture_output=True, text=True, env=env, timeout=300)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1                                   # rank 0 alone prints
+    d = json.loads(lines[0])
+    assert d["n_gpus"] == 2 and d["slowest_rank_s"] == 1.1
+    assert abs(d["value"] - 2 * 1000 * 3 / 1.1) < 1e-9

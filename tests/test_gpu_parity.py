@@ -311,6 +311,59 @@ def test_step_eq16_matches_oracle_composition(ib, orc, name, nodal, variant):
     ctx.close()
 
 
+@pytest.mark.parametrize("name,nodal", [("LV-small", False), ("C1", True)])
+def test_step_eq16_three_steps_with_positions_fed_back(ib, orc, name, nodal):
+    """NEXT-1's multi-step driver (Eq.(16)) with a frozen velocity field: three calls of
+    ib_step_eq16, x_new of one step being x of the next, against the oracle's operators composed in the
+    same order over the same three steps (the oracle advances its own positions)."""
+    import torch
+    wl = CONFIGS[name]()
+    dt = 2e-3 * wl.h
+    g = _grid(orc, wl)
+
+    def oracle_step(x):
+        if nodal:
+            Un = orc.interp(g, x, wl.u, wl.v, wl.w)
+            xn = x + dt * Un
+            B = orc.fe_force(wl.conn, wl.X, xn, wl.fibers, wl.mat_id, wl.mats)["B"]
+            return xn, Un, B, orc.spread(g, x, B)
+        xp, Wp, wa = orc.points(wl.conn, wl.X, x, wl.nsub)
+        Un = orc.restrict(wl.conn, wl.nsub, wa, Wp, orc.interp(g, xp, wl.u, wl.v, wl.w))
+        xn = x + dt * Un
+        B = orc.fe_force(wl.conn, wl.X, xn, wl.fibers, wl.mat_id, wl.mats)["B"]
+        return xn, Un, B, orc.spread(g, xp, orc.prolong(wl.conn, wl.nsub, wa, Wp, B))
+
+    ctx = ib.Context.from_workload(wl, nodal=nodal)
+    f = [torch.full((wl.n_cells,), 5.0, dtype=torch.float64, device="cuda") for _ in range(3)]
+    Un, B = (torch.empty((3, wl.n_nodes), dtype=torch.float64, device="cuda") for _ in range(2))
+    xa, xb = _t(wl.x), torch.empty((3, wl.n_nodes), dtype=torch.float64, device="cuda")
+    u, v, w = _t(wl.u), _t(wl.v), _t(wl.w)
+    x_r = wl.x.copy()
+    for step in range(3):
+        ctx.ib_step_eq16(xa, u, v, w, dt, xb, *f, Un, B)
+        ctx.check()
+        x_r, Un_r, B_r, f_r = oracle_step(x_r)
+        _close(xb, x_r, f"step {step} x_new")
+        _close(Un, Un_r, f"step {step} Un")
+        # the stiffness kappa amplifies the 1e-16 differences of the positions in B and f: compare those
+        # with the oracle at the GPU's own positions, and the two oracle runs to conditioning
+        B_g = orc.fe_force(wl.conn, wl.X, xb.cpu().numpy(), wl.fibers, wl.mat_id, wl.mats)["B"]
+        _close(B, B_g, f"step {step} B")
+        assert rel_l2(B_g, B_r) < 1e-8
+        x_old = xa.cpu().numpy()
+        if nodal:
+            f_g = orc.spread(g, x_old, B_g)
+        else:
+            xp_g, Wp_g, wa_g = orc.points(wl.conn, wl.X, x_old, wl.nsub)
+            f_g = orc.spread(g, xp_g, orc.prolong(wl.conn, wl.nsub, wa_g, Wp_g, B_g))
+        for c in range(3):
+            _close(f[c], f_g[c], f"step {step} f{c}")
+            assert rel_l2(f_g[c], f_r[c]) < 1e-8, (step, c)
+        xa, xb = xb, xa                                            # x_new becomes x
+    assert np.max(np.abs(x_r - wl.x)) > 1e-4 * wl.h                # the structure did move
+    ctx.close()
+
+
 def test_fe_force_next2_laws_and_active_stress(ib, orc):
     """NEXT-2: Eq.(7), Eq.(8)-(9) as an HO special case, Eq.(10)-(11), and the active stress of L317-331,
     mixed element by element on a distorted block."""

@@ -261,6 +261,25 @@ def test_points_weights_prolong_restrict(orc):
     assert abs(wq.sum() - 0.3 * 0.3 * 0.2) < 1e-15
 
 
+def test_nodal_weights_node_by_node_on_a_regular_block(orc):
+    """w_q = int phi_q dX on an undistorted n1 x n2 x n3 block of bricks d1 x d2 x d3: the
+    trilinear hat of a node integrates to d1 d2 d3 / 8 over each brick it belongs to, so w_q = V_brick
+    k_q / 8 with k_q = number of bricks at the node: 8 inside, 4 on a face, 2 on an edge, 1 at a corner.
+    A weight assigned to the wrong node fails this; the sum alone would not."""
+    n1, n2, n3 = 3, 4, 2
+    conn, (N1, N2, N3) = W.block_connectivity(n1, n2, n3)
+    d = np.array([0.11, 0.07, 0.13])
+    k, j, i = np.meshgrid(np.arange(N3), np.arange(N2), np.arange(N1), indexing="ij")
+    X = np.stack([0.2 + i.ravel() * d[0], 0.3 + j.ravel() * d[1], 0.1 + k.ravel() * d[2]])
+    wq = orc.nodal_weights(conn.astype(np.int32), X)
+    per_axis = lambda idx, n: np.where((idx == 0) | (idx == n), 1, 2)          # bricks along one axis at the node
+    kq = per_axis(i.ravel(), n1) * per_axis(j.ravel(), n2) * per_axis(k.ravel(), n3)
+    assert np.max(np.abs(wq - d.prod() * kq / 8.0)) < 1e-16
+    # and on a sheared block (affine map A): every weight scales by det A, node by node
+    A = np.array([[1.0, 0.3, -0.1], [0.0, 0.9, 0.2], [0.05, 0.0, 1.1]])
+    assert np.max(np.abs(orc.nodal_weights(conn.astype(np.int32), A @ X) - np.linalg.det(A) * wq)) < 1e-16
+
+
 def test_coupling_step_composition_and_node_level_adjointness(orc):
     conn, X, x, fib = distorted_block(3, 3, 2, size=(0.3, 0.3, 0.2), origin=(0.35, 0.3, 0.4), seed=4)
     ne, nn = conn.shape[0], X.shape[1]
