@@ -11,7 +11,7 @@ CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libibcouple.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-         "-Xcompiler", "-fPIC", "-shared", "--fmad=true", "-Xptxas", "-v", "-ldl"]
+         "-Xcompiler", "-fPIC", "-shared", "--fmad=true", "-DNDEBUG", "-Xptxas", "-v", "-ldl"]       # NDEBUG: the device-side assert()s of csrc/ are for checked test builds
 
 
 def sources():

@@ -15,6 +15,7 @@
 //           so the element-ordered xp/Gp arrays never touch HBM in ib_coupling_step.
 // The cell of a point is the binning formula of A21 (IEEE double, no contraction); positions are
 // computed with explicit __fma_rn/__dmul_rn so that the count and scatter passes agree bit for bit.
+#include <cassert>
 #include "ib_common.cuh"
 
 #define BT 4                       // tile edge in cells
@@ -265,6 +266,7 @@ ibk_bin_mesh(ib_bin_params pr)
         }
         if (SCATTER && valid) {
             const int64_t P = pr.P;
+            assert(pos >= 0 && pos < P);
             // streaming stores: the records (325 MB for C3) exceed L2 and are read once, oldest first,
             // so keeping them out of L2 leaves room for the grid halos (measured -0.6 % on the step)
 #define IB_ST(PTR, V) __stcs((PTR), (V))
@@ -368,7 +370,7 @@ ibk_tile_partials(const int32_t *__restrict__ tile_cur, int n_tiles, int chunk, 
 __global__ void __launch_bounds__(SCT)
 ibk_tile_scan(int32_t *__restrict__ tile_cur, int n_tiles, int chunk, const int2 *__restrict__ partial,
               int32_t *__restrict__ tile_start, int4 *__restrict__ work, int32_t *__restrict__ small_rec,
-              int32_t *__restrict__ counters, int slab_tiles, int ntx, int nty)
+              int32_t *__restrict__ counters, int slab_tiles, int ntx, int nty, int work_cap)
 {
     __shared__ int ws[33], wl[33];
     __shared__ int base_s, base_l, base_m;
@@ -394,6 +396,7 @@ ibk_tile_scan(int32_t *__restrict__ tile_cur, int n_tiles, int chunk, const int2
         const int4 st = make_int4(s, s + c.x, s + c.x + c.y, s + c.x + c.y + c.z);
         *reinterpret_cast<int4 *>(tile_start + 4 * t) = st;
         *reinterpret_cast<int4 *>(tile_cur + 4 * t) = st;
+        assert(l + ib_tile_chunks<0>(c, chunk, t, 0, nullptr, 0, 1, 1) <= work_cap);
         ib_tile_chunks<1>(c, chunk, t, s, work, l, ntx, nty);
     }
     {   // records of sparsely filled tiles: a compact list (order across CTAs is whatever the atomic gives)
@@ -445,7 +448,7 @@ ib_status ibk_bin_points(ib_ctx *c, int mesh, const double *xp, const double *Gp
         chunk = chunk < 192 ? 192 : (chunk > IB_CHUNK ? IB_CHUNK : chunk);
         if (nsb > 1) ibk_tile_partials<<<nsb, SCT, 0, st>>>(c->d_tile_cur, n_tiles, chunk, partial);   // one CTA needs no partial sums
         ibk_tile_scan<<<nsb, SCT, 0, st>>>(c->d_tile_cur, n_tiles, chunk, partial, c->d_tile_start, c->d_work, c->d_small_rec, c->d_tile_count,
-                                           ib_slab_tiles(c), c->grid.nx / BT, c->grid.ny / BT);
+                                           ib_slab_tiles(c), c->grid.nx / BT, c->grid.ny / BT, (int)c->work_cap);
         c->launches += 3;
     }
     if (phases & 2) {

@@ -27,6 +27,7 @@
 // per item and flushed with RED.ADD.F64 straight to the grid: the 4 lanes of a group hit 4 consecutive
 // faces (Blackwell has no native shared-memory fp64 add; the CAS loop measured 34 wavefronts each).
 // Tiles with fewer than IB_SMALL_TILE points skip all of this (ibk_small_tiles, ib_point.cuh).
+#include <cassert>
 #include "ib_point.cuh"
 
 #define TT 4                    // tile edge in cells
@@ -34,16 +35,12 @@
 #define TH3 512
 #define NOC 512                 // half-cells per tile (8^3)
 #define NITEM 300               // 3 components x (4*5*5) shifted cells
-#ifndef TB
-#define TB 256                  // threads per CTA
-#endif
-#ifndef NCTA
-#define NCTA 2
-#endif
-#define NIT ((NITEM + TB - 1) / TB)   // items per thread in the counting pass
+#define TB 512                  // threads per CTA: one CTA per SM, 16 warps
 #define NWARP (TB / 32)
+#ifndef IB_TILED_PRODUCER_WARPS
+#define IB_TILED_PRODUCER_WARPS 8   // of the 16 warps (the others run the items); 4 / 5 / 6 measured
+#endif
 #define CH IB_CHUNK             // records staged per work item
-#define KPT ((CH + TB - 1) / TB)   // points per thread in the staging pass
 #define SZ 68                   // z-plane stride of the halo in doubles (64 + 4: the 4 lanes of a group hit distinct banks)
 #define SU3 (TH * SZ)           // one component of the halo
 #ifndef PCAP
@@ -195,6 +192,7 @@ __device__ __forceinline__ void ib_run_batch(int C, const ib_tiled_params &pr, c
     }
     // this group's unit: the virtual points [vlo, vlo + nun) of the item
     const int vlo = part * PCAP, nun = min(PCAP, npts - vlo);       // <= 0 for the empty slot
+    assert(it <= NITEM && npts <= CH && (it == NITEM || nun > 0));
     int nmax = nun;
 #pragma unroll
     for (int o = 16; o >= 4; o >>= 1) nmax = max(nmax, __shfl_xor_sync(full, nmax, o));
@@ -242,6 +240,7 @@ __device__ __forceinline__ void ib_run_batch(int C, const ib_tiled_params &pr, c
                 for (int k = 0; k < 2; ++k) {
                     valid[k] = v0 + kp + k < nun;
                     const int rec = valid[k] ? ib_item_rec(vlo + v0 + kp + k, rstart, rend) : 0;   // padding: record 0 exists, its force is replaced by zero
+                    assert(rec >= 0 && rec < CH);
                     const unsigned r16 = (unsigned)rec << 4;
                     X[k] = ib_lds128(ax + r16); Y[k] = ib_lds128(ay + r16); Z[k] = ib_lds128(az + r16);
                     gl[k] = DO_SPREAD ? ib_lds64(ag + ((unsigned)rec << 3)) : 0.0;
@@ -315,266 +314,357 @@ __device__ __forceinline__ void ib_run_batch(int C, const ib_tiled_params &pr, c
     }
 }
 
+// ---- warp-specialised persistent kernel ----------------------------------------------------------------
+// One CTA per SM, 16 warps: NPW "producer" warps turn work items into shared-memory records (coordinates ->
+// half-cell sort -> (a,q) sets, runs and ordered units of the items, halo), NCW "consumer" warps run the
+// batches of units.  Two record buffers: the producers fill buffer k+1 while the consumers work through
+// buffer k.  full[b] / empty[b] are mbarriers (producers -> consumers: one arrival; consumers -> producers:
+// one per consumer warp).  No barrier ever joins the two groups: a consumer warp that finds no more batches
+// in a buffer moves on to the next, the producers wait only for the buffer they are about to overwrite.
+// (The first version had all warps walk through the phases of a work item together: a quarter of the warp
+// time went to the barriers between the phases and to the tail of the item loop.)
+#define NPW IB_TILED_PRODUCER_WARPS
+#define NCW (NWARP - NPW)
+#define TBP (NPW * 32)                                  // producer threads
+#define KPT ((CH + TBP - 1) / TBP)                      // points per producer thread
+#define NIT ((NITEM + TBP - 1) / TBP)                   // items per producer thread in the counting pass
+#define SCK ((NOC + TBP - 1) / TBP)                     // half-cell counters per producer thread in the scan
+
+// byte offsets inside one record buffer
+#define OFF_SU 0
+#define OFF_SETS (OFF_SU + 3 * SU3 * 8)
+#define OFF_SG (OFF_SETS + 6 * CH * 16)
+#define OFF_RUNS (OFF_SG + 3 * CH * 8)
+#define OFF_SIDS (OFF_RUNS + (NITEM + 1) * 16)
+#define OFF_ORDER (OFF_SIDS + CH * 4)
+#define OFF_CTL (OFF_ORDER + ((3 * NORD * 2 + 15) & ~15))
+#define BUF_BYTES (OFF_CTL + 32)                        // ctl: {nbatch, ncomp[3], next, h0[3]}
+// after the two buffers: producer-private scratch and the static window table
+#define OFF_OCCNT (2 * BUF_BYTES)
+#define OFF_BINS (OFF_OCCNT + NOC * 4)
+#define OFF_OCSTART (OFF_BINS + ((3 * NBIN * 4 + 15) & ~15))
+#define OFF_WIN (OFF_OCSTART + ((516 * 2 + 15) & ~15))
+#define OFF_MISC (OFF_WIN + ((NITEM + 1) * 4 + 15) / 16 * 16)      // wsum[NPW], work slots int4[2], mbarriers
+#define TILED_SMEM_BYTES (OFF_MISC + 16 * 4 + 2 * 16 + 4 * 8)
+
+__device__ __forceinline__ void ib_mbar_init(unsigned a, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(a), "r"(count) : "memory");
+}
+__device__ __forceinline__ void ib_mbar_arrive(unsigned a)
+{
+    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}" ::"r"(a) : "memory");
+}
+__device__ __forceinline__ void ib_mbar_wait(unsigned a, unsigned parity)
+{
+    asm volatile("{\n\t.reg .pred p;\n"
+                 "IB_MBAR_WAIT:\n\t"
+                 "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, 0x989680;\n\t"
+                 "@p bra IB_MBAR_DONE;\n\t"
+                 "bra IB_MBAR_WAIT;\n"
+                 "IB_MBAR_DONE:\n\t}" ::"r"(a), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void ib_producer_sync()
+{
+    asm volatile("bar.sync 1, %0;" ::"n"(TBP) : "memory");
+}
+
 // PER: periodic grid (compile-time, so that the periodic kernel carries none of the wall predicates)
 template <int DO_SPREAD, int DO_INTERP, int PER>
-__global__ void __launch_bounds__(TB, NCTA)
+__global__ void __launch_bounds__(TB, 1)
 ibk_tiled_kernel(ib_tiled_params pr)
 {
     extern __shared__ __align__(16) unsigned char smraw[];
-    double *su = reinterpret_cast<double *>(smraw);                  // [3][8][SZ] halo of u,v,w
-    double2 *sets = reinterpret_cast<double2 *>(su + 3 * SU3);       // [6][CH] (a,q) of set 2 d + {0 face, 1 centre}, half-cell order
-    double *sGs = reinterpret_cast<double *>(sets + 6 * CH);         // [3][CH] force / h^3
-    uint4 *item_runs = reinterpret_cast<uint4 *>(sGs + 3 * CH);      // [NITEM + 1] the <= 4 runs [s, e) of records of an item, 16 bits each; item NITEM is empty
-    unsigned *item_win = reinterpret_cast<unsigned *>(item_runs + NITEM + 1);   // [NITEM + 3] window of an item: halo offset | o3x << 16 | o3y << 20 | o3z << 24
-    int *sids = reinterpret_cast<int *>(item_win + NITEM + 3);       // [CH] point id of the record
-    int *oc_cnt = sids + CH;                                         // [NOC] points per half-cell
-    int *bins = oc_cnt + NOC;                                        // [3][NBIN] items per component and point count
-    unsigned short *oc_start = reinterpret_cast<unsigned short *>(bins + 3 * NBIN + 2);   // [516] first record of a half-cell
-    unsigned short *order = oc_start + 516;                          // [3][NORD] units of a component by descending point count
-    __shared__ int s_next[2];
-    __shared__ int4 s_wk[2];                         // work item of the even / odd iteration
-    __shared__ int wsum[NWARP];
+    int *oc_cnt = reinterpret_cast<int *>(smraw + OFF_OCCNT);                       // [NOC] points per half-cell
+    int *bins = reinterpret_cast<int *>(smraw + OFF_BINS);                          // [3][NBIN] units per component and point count
+    unsigned short *oc_start = reinterpret_cast<unsigned short *>(smraw + OFF_OCSTART);   // [516] first record of a half-cell
+    unsigned *item_win = reinterpret_cast<unsigned *>(smraw + OFF_WIN);             // [NITEM + 1] window of an item: halo offset | o3x << 16 | o3y << 20 | o3z << 24
+    int *wsum = reinterpret_cast<int *>(smraw + OFF_MISC);                          // [16]
+    int4 *s_wk = reinterpret_cast<int4 *>(smraw + OFF_MISC + 64);                   // work item of the even / odd iteration
+    const unsigned mbar = (unsigned)__cvta_generic_to_shared(smraw + OFF_MISC + 96);   // full[0], full[1], empty[0], empty[1]
 
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-    const int grp = lane >> 2, q = lane & 3;
     const int n[3] = {pr.g.nx, pr.g.ny, pr.g.nz};
-    const double org[3] = {pr.g.x0, pr.g.y0, pr.g.z0};
     const int64_t P = pr.P;
-    // lane q's own x-weight from (a, q):  w = sg q + (sa a + ca)
-    double wsa = q < 2 ? 1.0 : -1.0, wca = q < 2 ? 0.0 : 0.5, wsg = (q == 1 || q == 2) ? 1.0 : -1.0;
-    ib_opaque(wsa); ib_opaque(wca); ib_opaque(wsg);
-    ib_tile_smem sm;
-    sm.su = (unsigned)__cvta_generic_to_shared(su); sm.sets = (unsigned)__cvta_generic_to_shared(sets);
-    sm.sGs = (unsigned)__cvta_generic_to_shared(sGs); sm.sids = (unsigned)__cvta_generic_to_shared(sids);
-    ib_opaque(sm.su); ib_opaque(sm.sets); ib_opaque(sm.sGs); ib_opaque(sm.sids);
-    sm.item_runs = item_runs; sm.item_win = item_win;
-    // the windows of the items do not depend on the work item
+
+    if (tid == 0) {
+        ib_mbar_init(mbar + 0, 1); ib_mbar_init(mbar + 8, 1);
+        ib_mbar_init(mbar + 16, NCW); ib_mbar_init(mbar + 24, NCW);
+        const int w = pr.counters[pr.wb] + atomicAdd(&pr.counters[pr.wc], 1);
+        s_wk[0] = (w < pr.counters[pr.we]) ? __ldg(pr.work + w) : make_int4(-1, 0, 0, 0);
+    }
+    for (int i = tid; i < NOC; i += TB) oc_cnt[i] = 0;
+    for (int i = tid; i < 3 * NBIN; i += TB) bins[i] = 0;
+    // the windows of the items do not depend on the work item; item NITEM (in both buffers) has no points
     for (int it = tid; it <= NITEM; it += TB) {
         int c = 0, l[3] = {0, 0, 0};
         if (it < NITEM) ib_item_decode(it, c, l);
         const int o3[3] = {l[0] + (c == 0 ? 1 : 0), l[1] + (c == 1 ? 1 : 0), l[2] + (c == 2 ? 1 : 0)};
         item_win[it] = (unsigned)(c * SU3 + o3[2] * SZ + o3[1] * TH + o3[0]) | (o3[0] << 16) | (o3[1] << 20) | (o3[2] << 24);
-        if (it == NITEM) item_runs[it] = make_uint4(0, 0, 0, 0);
     }
+    if (tid < 2) reinterpret_cast<uint4 *>(smraw + tid * BUF_BYTES + OFF_RUNS)[NITEM] = make_uint4(0, 0, 0, 0);
+    __syncthreads();                                 // the only CTA-wide barrier of the kernel
 
-    // the records of a work item, one thread per point: coordinates, forces and ids are loaded, the tile
-    // coordinates and the half-cell of every point computed and counted.  Runs for work item k+1 as soon as a
-    // warp has no more items of work item k: nothing it touches (registers, oc_cnt) is used by the item loop.
-    double xi[KPT][3], Gr[KPT][3];
-    int ks[KPT], idr[KPT];
-    auto stage = [&](const int4 &wk) {
-        const int cb = wk.y, cn = wk.z;
-        double xr[KPT][3];
-#pragma unroll
-        for (int k = 0; k < KPT; ++k) {
-            const int i = tid + k * TB;
-#pragma unroll
-            for (int d = 0; d < 3; ++d) xr[k][d] = (i < cn) ? __ldcs(pr.sx + (int64_t)d * P + cb + i) : 0.0;
-        }
-#pragma unroll
-        for (int k = 0; k < KPT; ++k) {
-            const int i = tid + k * TB;
-            idr[k] = (DO_INTERP && i < cn) ? __ldcs(pr.sid + cb + i) : 0;
-#pragma unroll
-            for (int d = 0; d < 3; ++d) Gr[k][d] = (DO_SPREAD && i < cn) ? __ldcs(pr.sG + (int64_t)d * P + cb + i) : 0.0;
-        }
-#pragma unroll
-        for (int k = 0; k < KPT; ++k) {
-            const int i = tid + k * TB;
-            ks[k] = -1;
-            if (i < cn) {
-                int key = 0;
-#pragma unroll
-                for (int d = 2; d >= 0; --d) {
-                    xi[k][d] = ib_tile_coord(xr[k][d], org[d], pr.g.h, pr.inv_h);
-                    key = key * 8 + min(max((int)floor(2.0 * xi[k][d]), 0), 7);
+    if (wid < NPW) {
+        // =================================== producers ==========================================================
+        const double org[3] = {pr.g.x0, pr.g.y0, pr.g.z0};
+        for (int iter = 0;; ++iter) {
+            const int b = iter & 1;
+            unsigned char *buf = smraw + b * BUF_BYTES;
+            const int4 wk = s_wk[b];
+            // the work item after this one is claimed now (the other slot: every producer has read it, before
+            // the last barrier of the previous iteration at the latest)
+            if (tid == 0) {
+                const int w = pr.counters[pr.wb] + atomicAdd(&pr.counters[pr.wc], 1);
+                s_wk[b ^ 1] = (w < pr.counters[pr.we]) ? __ldg(pr.work + w) : make_int4(-1, 0, 0, 0);
+            }
+            if (wk.x < 0) {
+                // no more work: an empty buffer with nbatch < 0 tells the consumers to stop
+                if (tid == 0) {
+                    if (iter >= 2) ib_mbar_wait(mbar + 16 + 8 * b, ((iter >> 1) - 1) & 1);
+                    reinterpret_cast<int *>(buf + OFF_CTL)[0] = -1;
+                    ib_mbar_arrive(mbar + 8 * b);
                 }
-                ks[k] = key | (atomicAdd(&oc_cnt[key], 1) << 9);      // rank inside the half-cell
+                break;
             }
-        }
-    };
-
-    if (tid == 0) {
-        const int w = pr.counters[pr.wb] + atomicAdd(&pr.counters[pr.wc], 1);
-        s_wk[0] = (w < pr.counters[pr.we]) ? __ldg(pr.work + w) : make_int4(-1, 0, 0, 0);
-        s_next[0] = 0; s_next[1] = 0;
-    }
-    for (int i = tid; i < NOC; i += TB) oc_cnt[i] = 0;
-    for (int i = tid; i < 3 * NBIN; i += TB) bins[i] = 0;
-    __syncthreads();
-    for (int iter = 0;; ++iter) {
-        // no barrier between the items of the previous work item and this: a warp that finds no more items goes
-        // on to the records of the next work item (its slot was written before the previous closing barrier)
-        const int4 wk = s_wk[iter & 1];
-        if (wk.x < 0) break;
-        stage(wk);
-        // the work item after this one is claimed now (slot of the other parity: the slow warps of the previous
-        // work item may still have to read this one's)
-        if (tid == 0) {
-            const int w = pr.counters[pr.wb] + atomicAdd(&pr.counters[pr.wc], 1);
-            s_wk[(iter + 1) & 1] = (w < pr.counters[pr.we]) ? __ldg(pr.work + w) : make_int4(-1, 0, 0, 0);
-        }
-        const int t3[3] = {wk.w & 1023, (wk.w >> 10) & 1023, wk.w >> 20};     // tile coordinates, packed by ibk_tile_scan
-        int h0[3];                                       // halo origin (global index of halo entry 0), wrapped
+            const int cb = wk.y, cn = wk.z;
+            // ---- coordinates of the records, one thread per point: tile coordinates, half-cell, rank inside it.
+            // Nothing here touches the record buffers: it overlaps the consumers' work on both of them.
+            double xi[KPT][3];
+            int ks[KPT];
+            {
+                double xr[KPT][3];
 #pragma unroll
-        for (int d = 0; d < 3; ++d) h0[d] = PER ? ib_wrap(TT * t3[d] - 2, n[d]) : TT * t3[d] - 2;
-        __syncthreads();                             // every warp has left the items of the previous work item and counted its points of this one
-        if (tid == 0) s_next[(iter + 1) & 1] = 0;    // batch counter of the next work item
-        // ---- halo: asynchronous copies straight into shared memory, awaited before the items -------------
-        if (DO_INTERP) {
+                for (int k = 0; k < KPT; ++k) {
+                    const int i = tid + k * TBP;
 #pragma unroll
-            for (int idx = tid; idx < 3 * TH3; idx += TB) {
-                int c = idx >> 9, r = idx & 511;
-                int i = h0[0] + (r & 7), j = h0[1] + ((r >> 3) & 7), k = h0[2] + (r >> 6);
-                if (PER) { i -= (i >= n[0]) ? n[0] : 0; j -= (j >= n[1]) ? n[1] : 0; k -= (k >= n[2]) ? n[2] : 0; }
-                // faces outside a bounded grid read as zero (source size 0: their weight meets no force and no velocity)
-                const bool in = PER || (i >= 0 && i < n[0] && j >= 0 && j < n[1] && k >= 0 && k < n[2]);
-                const double *src = in ? pr.fld[c] + ((int64_t)k * n[1] + j) * n[0] + i : pr.fld[c];
-                const unsigned dst = (unsigned)__cvta_generic_to_shared(su + c * SU3 + (r >> 6) * SZ + (r & 63));
-                asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(dst), "l"(src), "r"(in ? 8 : 0) : "memory");
-            }
-            asm volatile("cp.async.commit_group;" ::: "memory");
-        }
-        {                                            // the next work item's coordinates -> L2 while this one is processed
-            const int4 nx4 = s_wk[(iter + 1) & 1];
-            if (nx4.x >= 0) {
-                for (int i = 16 * tid; i < 3 * CH; i += 16 * TB) {
-                    const int d = i / CH, o = i - d * CH;          // CH is a multiple of 16
-                    if (o < nx4.z) ib_prefetch_l2(pr.sx + (int64_t)d * P + nx4.y + o);
+                    for (int d = 0; d < 3; ++d) xr[k][d] = (i < cn) ? __ldcs(pr.sx + (int64_t)d * P + cb + i) : 0.0;
+                }
+#pragma unroll
+                for (int k = 0; k < KPT; ++k) {
+                    const int i = tid + k * TBP;
+                    ks[k] = -1;
+                    if (i < cn) {
+                        int key = 0;
+#pragma unroll
+                        for (int d = 2; d >= 0; --d) {
+                            xi[k][d] = ib_tile_coord(xr[k][d], org[d], pr.g.h, pr.inv_h);
+                            key = key * 8 + min(max((int)floor(2.0 * xi[k][d]), 0), 7);
+                        }
+                        ks[k] = key | (atomicAdd(&oc_cnt[key], 1) << 9);
+                    }
                 }
             }
-        }
-        {                                            // exclusive scan of the 512 counts, SCK per thread
-            constexpr int SCK = (NOC + TB - 1) / TB;
-            int v[SCK], s = 0;
-#pragma unroll
-            for (int k = 0; k < SCK; ++k) {
-                v[k] = (SCK * tid + k < NOC) ? oc_cnt[SCK * tid + k] : 0;
-                s += v[k];
-            }
-            int inc = s;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                int t = __shfl_up_sync(0xffffffffu, inc, o);
-                if (lane >= o) inc += t;
-            }
-            if (lane == 31) wsum[wid] = inc;
-            __syncthreads();
-            int ex = inc - s;
-            for (int w = 0; w < wid; ++w) ex += wsum[w];
-#pragma unroll
-            for (int k = 0; k < SCK; ++k) {
-                if (SCK * tid + k < NOC) { oc_start[SCK * tid + k] = ex; oc_cnt[SCK * tid + k] = 0; }   // counts: ready for the next work item
-                ex += v[k];
-            }
-            if (tid == TB - 1) oc_start[NOC] = ex;
-        }
-        __syncthreads();
-        // ---- items: runs of records and point count; rank among the items of equal component and count ----
-        int my_nf[NIT], my_rf[NIT], my_rem[NIT], my_rr[NIT];     // whole units of the item and their first rank, points and rank of the last unit
-#pragma unroll
-        for (int j = 0; j < NIT; ++j) {
-            const int it = tid + j * TB;
-            my_nf[j] = 0; my_rf[j] = 0; my_rem[j] = 0; my_rr[j] = 0;
-            if (it < NITEM) {
-                int c, l[3], lo[3], hi[3];
-                ib_item_decode(it, c, l);
-#pragma unroll
-                for (int d = 0; d < 3; ++d) ib_half_range(c, d, l[d], lo[d], hi[d]);
-                unsigned rn[4];
-                int cnt = 0;
-#pragma unroll
-                for (int rr = 0; rr < 4; ++rr) {
-                    const int z2 = lo[2] + (rr >> 1), y2 = lo[1] + (rr & 1);
-                    const bool ok = z2 <= hi[2] && y2 <= hi[1];
-                    const int b = (z2 * 8 + y2) * 8;
-                    const unsigned s0 = ok ? oc_start[b + lo[0]] : 0, s1 = ok ? oc_start[b + hi[0] + 1] : 0;
-                    rn[rr] = s0 | (s1 << 16);
-                    cnt += (int)(s1 - s0);
+            ib_producer_sync();
+            for (int i = tid; i < 3 * NBIN; i += TBP) bins[i] = 0;      // read last before the closing barrier of the previous iteration
+            {                                            // the next work item's records -> L2 while this one is processed
+                const int4 nx4 = s_wk[b ^ 1];
+                if (nx4.x >= 0) {
+                    for (int i = 16 * tid; i < 3 * CH; i += 16 * TBP) {
+                        const int d = i / CH, o = i - d * CH;          // CH is a multiple of 16: one 128-byte line per 16 doubles
+                        if (o < nx4.z) {
+                            ib_prefetch_l2(pr.sx + (int64_t)d * P + nx4.y + o);
+                            if (DO_SPREAD) ib_prefetch_l2(pr.sG + (int64_t)d * P + nx4.y + o);
+                        }
+                    }
+                    if (DO_INTERP && 32 * tid < nx4.z) ib_prefetch_l2(pr.sid + nx4.y + 32 * tid);
                 }
-                item_runs[it] = make_uint4(rn[0], rn[1], rn[2], rn[3]);
-                my_nf[j] = cnt / PCAP;
-                my_rem[j] = cnt - PCAP * my_nf[j];
-                if (my_nf[j] > 0) my_rf[j] = atomicAdd(&bins[c * NBIN + PCAP], my_nf[j]);
-                if (my_rem[j] > 0) my_rr[j] = atomicAdd(&bins[c * NBIN + my_rem[j]], 1);
             }
-        }
-        // ---- the records, in half-cell order: six (a,q) sets, force / h^3, id ------------------------
+            {                                            // exclusive scan of the 512 counts
+                int v[SCK], s = 0;
 #pragma unroll
-        for (int k = 0; k < KPT; ++k) {
-            if (ks[k] >= 0) {
-                const int key = ks[k] & 511;
-                const int pos = oc_start[key] + (ks[k] >> 9);
-#pragma unroll
-                for (int d = 0; d < 3; ++d) {
-                    // face-aligned: cell hd >> 1; centre-aligned: shifted cell (hd + 1) >> 1 covers xi - 1/2 in [l-1, l).
-                    // r in [0,1] up to rounding at cell boundaries, where the formula continues phi smoothly (A19)
-                    const int hd = (key >> (3 * d)) & 7;
-                    sets[(2 * d) * CH + pos] = ib_aq(xi[k][d] - (double)(hd >> 1));
-                    sets[(2 * d + 1) * CH + pos] = ib_aq(xi[k][d] + 0.5 - (double)((hd + 1) >> 1));
+                for (int k = 0; k < SCK; ++k) {
+                    v[k] = (SCK * tid + k < NOC) ? oc_cnt[SCK * tid + k] : 0;
+                    s += v[k];
                 }
-                if (DO_SPREAD) {
-#pragma unroll
-                    for (int d = 0; d < 3; ++d) sGs[d * CH + pos] = Gr[k][d] * pr.ih3;
-                }
-                if (DO_INTERP) sids[pos] = idr[k];
-            }
-        }
-        if (DO_INTERP) asm volatile("cp.async.wait_group 0;" ::: "memory");      // this thread's part of the halo has landed
-        __syncthreads();
-        // ---- order the units by component, then by point count (descending): every warp scans the 3 x PCAP
-        // bins for itself (lane l: the units of PCAP - l points).  Unit k of component c goes to order[c][k] as
-        // item | part << 9; batch b of the item loop is the 8 units 8 (b / 3) ... of component b % 3, so that the
-        // batches come in roughly descending size whatever their component (longest first keeps the warps level
-        // at the end of the work item).
-        int ncomp[3], nbatch;
-        {
-            int pre[3];
-#pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                const int v = lane < PCAP ? bins[c * NBIN + PCAP - lane] : 0;
-                int inc = v;
+                int inc = s;
 #pragma unroll
                 for (int o = 1; o < 32; o <<= 1) {
                     int t = __shfl_up_sync(0xffffffffu, inc, o);
                     if (lane >= o) inc += t;
                 }
-                pre[c] = inc - v;
-                ncomp[c] = __shfl_sync(0xffffffffu, inc, 31);
+                if (lane == 31) wsum[wid] = inc;
+                ib_producer_sync();
+                int ex = inc - s;
+                for (int w = 0; w < wid; ++w) ex += wsum[w];
+#pragma unroll
+                for (int k = 0; k < SCK; ++k) {
+                    if (SCK * tid + k < NOC) { oc_start[SCK * tid + k] = ex; oc_cnt[SCK * tid + k] = 0; }   // counts: ready for the next work item
+                    ex += v[k];
+                }
+                if (tid == TBP - 1) oc_start[NOC] = ex;
             }
-            static_assert(PCAP <= 32 && PCAP % 4 == 0, "one lane per unit size; the item loop steps by 4 points");
-            nbatch = 3 * ((max(ncomp[0], max(ncomp[1], ncomp[2])) + 7) >> 3);
+            ib_producer_sync();
+            // ---- from here on the record buffer is written: the consumers must have left its previous contents
+            if (iter >= 2) ib_mbar_wait(mbar + 16 + 8 * b, ((iter >> 1) - 1) & 1);
+            double *su = reinterpret_cast<double *>(buf + OFF_SU);
+            double2 *sets = reinterpret_cast<double2 *>(buf + OFF_SETS);
+            double *sGs = reinterpret_cast<double *>(buf + OFF_SG);
+            uint4 *item_runs = reinterpret_cast<uint4 *>(buf + OFF_RUNS);
+            int *sids = reinterpret_cast<int *>(buf + OFF_SIDS);
+            unsigned short *order = reinterpret_cast<unsigned short *>(buf + OFF_ORDER);
+            int *ctl = reinterpret_cast<int *>(buf + OFF_CTL);
+            const int t3[3] = {wk.w & 1023, (wk.w >> 10) & 1023, wk.w >> 20};     // tile coordinates, packed by ibk_tile_scan
+            int h0[3];                                       // halo origin (global index of halo entry 0), wrapped
+#pragma unroll
+            for (int d = 0; d < 3; ++d) h0[d] = PER ? ib_wrap(TT * t3[d] - 2, n[d]) : TT * t3[d] - 2;
+            // ---- halo: asynchronous copies straight into shared memory
+            if (DO_INTERP) {
+                for (int idx = tid; idx < 3 * TH3; idx += TBP) {
+                    int c = idx >> 9, r = idx & 511;
+                    int i = h0[0] + (r & 7), j = h0[1] + ((r >> 3) & 7), k = h0[2] + (r >> 6);
+                    if (PER) { i -= (i >= n[0]) ? n[0] : 0; j -= (j >= n[1]) ? n[1] : 0; k -= (k >= n[2]) ? n[2] : 0; }
+                    // faces outside a bounded grid read as zero (source size 0: their weight meets no force and no velocity)
+                    const bool in = PER || (i >= 0 && i < n[0] && j >= 0 && j < n[1] && k >= 0 && k < n[2]);
+                    const double *src = in ? pr.fld[c] + ((int64_t)k * n[1] + j) * n[0] + i : pr.fld[c];
+                    const unsigned dst = (unsigned)__cvta_generic_to_shared(su + c * SU3 + (r >> 6) * SZ + (r & 63));
+                    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(dst), "l"(src), "r"(in ? 8 : 0) : "memory");
+                }
+                asm volatile("cp.async.commit_group;" ::: "memory");
+            }
+            // ---- items: runs of records and point count; rank among the units of equal component and count ----
+            int my_nf[NIT], my_rf[NIT], my_rem[NIT], my_rr[NIT];     // whole units of the item and their first rank, points and rank of the last unit
 #pragma unroll
             for (int j = 0; j < NIT; ++j) {
-                if (wid * 32 + j * TB < NITEM) {                // warp-uniform: some lane of this warp has an item
-                    const int it = tid + j * TB;
-                    const int c = it >= 200 ? 2 : (it >= 100 ? 1 : 0);
-                    // the owner lane of the size cannot know the asker's component, so all three prefixes travel
-                    const int owner = PCAP - max(my_rem[j], 1);
-                    const int a0 = __shfl_sync(0xffffffffu, pre[0], owner), a1 = __shfl_sync(0xffffffffu, pre[1], owner),
-                              a2 = __shfl_sync(0xffffffffu, pre[2], owner);
-                    unsigned short *oc = order + c * NORD;
-                    for (int pp = 0; pp < my_nf[j]; ++pp) oc[my_rf[j] + pp] = (unsigned short)(it | (pp << 9));   // units of PCAP points come first
-                    if (my_rem[j] > 0) oc[(c == 0 ? a0 : (c == 1 ? a1 : a2)) + my_rr[j]] = (unsigned short)(it | (my_nf[j] << 9));
+                const int it = tid + j * TBP;
+                my_nf[j] = 0; my_rf[j] = 0; my_rem[j] = 0; my_rr[j] = 0;
+                if (it < NITEM) {
+                    int c, l[3], lo[3], hi[3];
+                    ib_item_decode(it, c, l);
+#pragma unroll
+                    for (int d = 0; d < 3; ++d) ib_half_range(c, d, l[d], lo[d], hi[d]);
+                    unsigned rn[4];
+                    int cnt = 0;
+#pragma unroll
+                    for (int rr = 0; rr < 4; ++rr) {
+                        const int z2 = lo[2] + (rr >> 1), y2 = lo[1] + (rr & 1);
+                        const bool ok = z2 <= hi[2] && y2 <= hi[1];
+                        const int bb = (z2 * 8 + y2) * 8;
+                        const unsigned s0 = ok ? oc_start[bb + lo[0]] : 0, s1 = ok ? oc_start[bb + hi[0] + 1] : 0;
+                        rn[rr] = s0 | (s1 << 16);
+                        cnt += (int)(s1 - s0);
+                    }
+                    item_runs[it] = make_uint4(rn[0], rn[1], rn[2], rn[3]);
+                    my_nf[j] = cnt / PCAP;
+                    my_rem[j] = cnt - PCAP * my_nf[j];
+                    if (my_nf[j] > 0) my_rf[j] = atomicAdd(&bins[c * NBIN + PCAP], my_nf[j]);
+                    if (my_rem[j] > 0) my_rr[j] = atomicAdd(&bins[c * NBIN + my_rem[j]], 1);
                 }
             }
+            // ---- the records, in half-cell order: six (a,q) sets, force / h^3, id ------------------------
+#pragma unroll
+            for (int k = 0; k < KPT; ++k) {
+                if (ks[k] >= 0) {
+                    const int i = tid + k * TBP;
+                    double Gr[3] = {0.0, 0.0, 0.0};
+                    int idr = 0;
+                    if (DO_INTERP) idr = __ldcs(pr.sid + cb + i);
+                    if (DO_SPREAD) {
+#pragma unroll
+                        for (int d = 0; d < 3; ++d) Gr[d] = __ldcs(pr.sG + (int64_t)d * P + cb + i);
+                    }
+                    const int key = ks[k] & 511;
+                    const int pos = oc_start[key] + (ks[k] >> 9);
+                    assert(pos >= 0 && pos < cn && cn <= CH);
+#pragma unroll
+                    for (int d = 0; d < 3; ++d) {
+                        // face-aligned: cell hd >> 1; centre-aligned: shifted cell (hd + 1) >> 1 covers xi - 1/2 in [l-1, l).
+                        // r in [0,1] up to rounding at cell boundaries, where the formula continues phi smoothly (A19)
+                        const int hd = (key >> (3 * d)) & 7;
+                        sets[(2 * d) * CH + pos] = ib_aq(xi[k][d] - (double)(hd >> 1));
+                        sets[(2 * d + 1) * CH + pos] = ib_aq(xi[k][d] + 0.5 - (double)((hd + 1) >> 1));
+                    }
+                    if (DO_SPREAD) {
+#pragma unroll
+                        for (int d = 0; d < 3; ++d) sGs[d * CH + pos] = Gr[d] * pr.ih3;
+                    }
+                    if (DO_INTERP) sids[pos] = idr;
+                }
+            }
+            if (DO_INTERP) asm volatile("cp.async.wait_group 0;" ::: "memory");      // this thread's part of the halo has landed
+            ib_producer_sync();
+            // ---- order the units by component, then by point count (descending): every warp scans the 3 x PCAP
+            // bins for itself (lane l: the units of PCAP - l points).  Unit k of component c goes to order[c][k] as
+            // item | part << 9; batch b of the item loop is the 8 units 8 (b / 3) ... of component b % 3, so that the
+            // batches come in roughly descending size whatever their component (longest first keeps the warps level
+            // at the end of the work item).
+            {
+                int pre[3], ncomp[3];
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    const int v = lane < PCAP ? bins[c * NBIN + PCAP - lane] : 0;
+                    int inc = v;
+#pragma unroll
+                    for (int o = 1; o < 32; o <<= 1) {
+                        int t = __shfl_up_sync(0xffffffffu, inc, o);
+                        if (lane >= o) inc += t;
+                    }
+                    pre[c] = inc - v;
+                    ncomp[c] = __shfl_sync(0xffffffffu, inc, 31);
+                }
+                static_assert(PCAP <= 32 && PCAP % 4 == 0, "one lane per unit size; the item loop steps by 4 points");
+#pragma unroll
+                for (int j = 0; j < NIT; ++j) {
+                    if (wid * 32 + j * TBP < NITEM) {                // warp-uniform: some lane of this warp has an item
+                        const int it = tid + j * TBP;
+                        const int c = it >= 200 ? 2 : (it >= 100 ? 1 : 0);
+                        // the owner lane of the size cannot know the asker's component, so all three prefixes travel
+                        const int owner = PCAP - max(my_rem[j], 1);
+                        const int a0 = __shfl_sync(0xffffffffu, pre[0], owner), a1 = __shfl_sync(0xffffffffu, pre[1], owner),
+                                  a2 = __shfl_sync(0xffffffffu, pre[2], owner);
+                        unsigned short *oc = order + c * NORD;
+                        assert(ncomp[c] <= NORD && my_rf[j] + my_nf[j] <= ncomp[c]);
+                        for (int pp = 0; pp < my_nf[j]; ++pp) oc[my_rf[j] + pp] = (unsigned short)(it | (pp << 9));   // units of PCAP points come first
+                        if (my_rem[j] > 0) oc[(c == 0 ? a0 : (c == 1 ? a1 : a2)) + my_rr[j]] = (unsigned short)(it | (my_nf[j] << 9));
+                    }
+                }
+                if (tid == 0) {
+                    ctl[1] = ncomp[0]; ctl[2] = ncomp[1]; ctl[3] = ncomp[2];
+                    ctl[4] = 0;                                  // batch counter
+                    ctl[5] = h0[0]; ctl[6] = h0[1]; ctl[7] = h0[2];
+                    ctl[0] = 3 * ((max(ncomp[0], max(ncomp[1], ncomp[2])) + 7) >> 3);
+                }
+            }
+            ib_producer_sync();                              // every producer's records and units are written ...
+            if (tid == 0) ib_mbar_arrive(mbar + 8 * b);      // ... and, through this arrival, visible to the consumers
         }
-        __syncthreads();
-        for (int i = tid; i < 3 * NBIN; i += TB) bins[i] = 0;        // next use: behind the barriers that end this work item
-
-        // ---- the items, in batches of 8 of one component ----------------------------------------------
-        // the next batch is claimed one batch ahead: the shared-memory atomic and its broadcast are out of the way
-        int bnext = 0;
-        if (lane == 0) bnext = atomicAdd(&s_next[iter & 1], 1);
-        for (;;) {
-            const int b = __shfl_sync(0xffffffffu, bnext, 0);
-            if (b >= nbatch) break;
-            if (lane == 0) bnext = atomicAdd(&s_next[iter & 1], 1);   // warps pull one batch at a time
-            const int c = b % 3, k8 = (b / 3) * 8;                                 // warp-uniform
-            const int nc = c == 0 ? ncomp[0] : (c == 1 ? ncomp[1] : ncomp[2]);
-            if (k8 >= nc) continue;                                                // this component has fewer batches
-            const int un = k8 + grp < nc ? (int)order[c * NORD + k8 + grp] : NITEM;      // empty slot: the item without points
-            ib_run_batch<DO_SPREAD, DO_INTERP, PER>(c, pr, sm, un & 511, un >> 9, q, h0, n, wsa, wca, wsg);
+    } else {
+        // =================================== consumers ==========================================================
+        const int grp = lane >> 2, q = lane & 3;
+        // lane q's own x-weight from (a, q):  w = sg q + (sa a + ca)
+        double wsa = q < 2 ? 1.0 : -1.0, wca = q < 2 ? 0.0 : 0.5, wsg = (q == 1 || q == 2) ? 1.0 : -1.0;
+        ib_opaque(wsa); ib_opaque(wca); ib_opaque(wsg);
+        for (int iter = 0;; ++iter) {
+            const int b = iter & 1;
+            unsigned char *buf = smraw + b * BUF_BYTES;
+            ib_mbar_wait(mbar + 8 * b, (iter >> 1) & 1);
+            int *ctl = reinterpret_cast<int *>(buf + OFF_CTL);
+            const int nbatch = ctl[0];
+            if (nbatch < 0) break;
+            const int ncomp[3] = {ctl[1], ctl[2], ctl[3]};
+            const int h0[3] = {ctl[5], ctl[6], ctl[7]};
+            const unsigned short *order = reinterpret_cast<const unsigned short *>(buf + OFF_ORDER);
+            ib_tile_smem sm;
+            sm.su = (unsigned)__cvta_generic_to_shared(buf + OFF_SU); sm.sets = (unsigned)__cvta_generic_to_shared(buf + OFF_SETS);
+            sm.sGs = (unsigned)__cvta_generic_to_shared(buf + OFF_SG); sm.sids = (unsigned)__cvta_generic_to_shared(buf + OFF_SIDS);
+            ib_opaque(sm.su); ib_opaque(sm.sets); ib_opaque(sm.sGs); ib_opaque(sm.sids);
+            sm.item_runs = reinterpret_cast<const uint4 *>(buf + OFF_RUNS); sm.item_win = item_win;
+            // batches of 8 units of one component; the next batch is claimed one batch ahead: the shared-memory
+            // atomic and its broadcast are out of the way
+            int bnext = 0;
+            if (lane == 0) bnext = atomicAdd(&ctl[4], 1);
+            for (;;) {
+                const int bt = __shfl_sync(0xffffffffu, bnext, 0);
+                if (bt >= nbatch) break;
+                if (lane == 0) bnext = atomicAdd(&ctl[4], 1);
+                const int c = bt % 3, k8 = (bt / 3) * 8;                                 // warp-uniform
+                const int nc = c == 0 ? ncomp[0] : (c == 1 ? ncomp[1] : ncomp[2]);
+                if (k8 >= nc) continue;                                                // this component has fewer batches
+                const int un = k8 + grp < nc ? (int)order[c * NORD + k8 + grp] : NITEM;      // empty slot: the item without points
+                ib_run_batch<DO_SPREAD, DO_INTERP, PER>(c, pr, sm, un & 511, un >> 9, q, h0, n, wsa, wca, wsg);
+            }
+            __syncwarp();
+            if (lane == 0) ib_mbar_arrive(mbar + 16 + 8 * b);    // this warp has left the buffer
         }
     }
 }
@@ -620,9 +710,8 @@ static int ib_small_blocks(int64_t nsmall_max, int sms)
 template <int S, int I, int PER>
 static ib_status launch_tiled_p(ib_ctx *c, const ib_tiled_params &pr, bool with_small, cudaStream_t st)
 {
-    const size_t smem = (size_t)(3 * SU3 + 12 * CH + 3 * CH) * sizeof(double) + (NITEM + 1) * sizeof(uint4) +
-                        (NITEM + 3 + CH + NOC + 3 * NBIN + 2) * sizeof(int) + (516 + 3 * NORD) * sizeof(unsigned short);
-    static_assert(CH % 16 == 0, "staging layout");
+    const size_t smem = TILED_SMEM_BYTES;
+    static_assert(CH % 16 == 0 && TILED_SMEM_BYTES <= 227 * 1024, "staging layout");
     // per context (a context belongs to one device and, by the header's contract, to one thread at a time)
     unsigned char &configured = c->tiled_cfg[S * 4 + I * 2 + PER];
     if (!configured) {
@@ -641,7 +730,7 @@ static ib_status launch_tiled_p(ib_ctx *c, const ib_tiled_params &pr, bool with_
     }
     if (with_small) ibk_small_tiles<S, I><<<ib_small_blocks(nsmall_max, sms), 128, 0, s3>>>(pr, c->d_small_rec, c->d_tile_count);
     if (beside) IB_CUDA_TRY(cudaEventRecord(c->ev_sjoin, s3));
-    ibk_tiled_kernel<S, I, PER><<<sms * NCTA, TB, smem, st>>>(pr);
+    ibk_tiled_kernel<S, I, PER><<<sms, TB, smem, st>>>(pr);
     if (beside) IB_CUDA_TRY(cudaStreamWaitEvent(st, c->ev_sjoin, 0));
     c->launches += with_small ? 2 : 1;
     return IB_OK;
