@@ -178,6 +178,13 @@ ib_status ib_coupling_step_host(ib_ctx *ctx, const double *x_host, const double 
                                 double *fv_host, double *fw_host, double *Un_host, double *B_host,
                                 void *stream);
 
+/* The same with the three velocity components, and the three force components, each in ONE host array
+ * [3][n_cells] (u then v then w; fu then fv then fw): every slab then crosses the bus as one copy per direction
+ * instead of three (three small copies in flight in both directions measured 40 GB/s where one gets 55).
+ * (Three separate arrays that happen to be adjacent do not qualify: one copy cannot span allocations.) */
+ib_status ib_coupling_step_host3(ib_ctx *ctx, const double *x_host, const double *uvw_host, double *f_host,
+                                 double *Un_host, double *B_host, void *stream);
+
 /* Synchronise the last used stream and report the latched device status. first_bad_index (may be
  * NULL) receives the smallest offending element or node id, or -1. Clears the latch. */
 ib_status ib_check(ib_ctx *ctx, int64_t *first_bad_index);

@@ -128,10 +128,16 @@ static inline int ib_slab_count(const ib_ctx *c)
 void ib_prof_begin(ib_ctx *c, int phase, cudaStream_t st);
 void ib_prof_end(ib_ctx *c, int phase, cudaStream_t st);
 
+#ifdef NDEBUG
+#define IB_CUDA_WHERE(e) ((void)0)
+#else            /* checked test builds say which call failed */
+#include <cstdio>
+#define IB_CUDA_WHERE(e) fprintf(stderr, "[ibcouple] %s at %s:%d\n", cudaGetErrorString(e), __FILE__, __LINE__)
+#endif
 #define IB_CUDA_TRY(expr)                                   \
     do {                                                    \
         cudaError_t _e = (expr);                            \
-        if (_e != cudaSuccess) return IB_ERR_CUDA;          \
+        if (_e != cudaSuccess) { IB_CUDA_WHERE(_e); return IB_ERR_CUDA; } \
     } while (0)
 
 static inline unsigned ib_blocks(int64_t n, int per) { return (unsigned)((n + per - 1) / per); }

@@ -113,7 +113,7 @@ extern "C" ib_status ib_destroy(ib_ctx *c)
                     c->d_Wp, c->d_wa, c->d_geo, c->d_node_off, c->d_node_slot, c->d_teth_ids, c->d_faces, c->d_Ce, c->d_Fhat, c->d_B, c->d_xp, c->d_Gp, c->d_Up, c->d_key[0],
                     c->d_key[1], c->d_val[0], c->d_val[1], c->d_hist, c->d_tile_cur, c->d_tile_start, c->d_work, c->d_small_rec,
                     c->d_row_off, c->d_sx, c->d_sG, c->d_sid,
-                    c->d_tile_count, c->d_hx, c->d_hu, c->d_hv, c->d_hw, c->d_hfu, c->d_hfv, c->d_hfw,
+                    c->d_tile_count, c->d_hx, c->d_hu, c->d_hfu,
                     c->d_hUn, c->d_hB, c->d_status};
     for (void *p : ptrs)
         if (p) cudaFree(p);
@@ -638,11 +638,19 @@ extern "C" ib_status ib_coupling_step(ib_ctx *c, const double *x, const double *
 }
 
 static ib_status host_step_pipelined(ib_ctx *c, const double *x_h, const double *u_h, const double *v_h, const double *w_h,
-                                     double *fu_h, double *fv_h, double *fw_h, double *Un_h, double *B_h, cudaStream_t st);
+                                     double *fu_h, double *fv_h, double *fw_h, double *Un_h, double *B_h, int packed, cudaStream_t st);
+static ib_status host_step(ib_ctx *c, const double *x_h, const double *u_h, const double *v_h, const double *w_h, double *fu_h,
+                           double *fv_h, double *fw_h, double *Un_h, double *B_h, int packed, void *stream);
 
 extern "C" ib_status ib_coupling_step_host(ib_ctx *c, const double *x_h, const double *u_h, const double *v_h,
                                            const double *w_h, double *fu_h, double *fv_h, double *fw_h,
                                            double *Un_h, double *B_h, void *stream)
+{
+    return host_step(c, x_h, u_h, v_h, w_h, fu_h, fv_h, fw_h, Un_h, B_h, 0, stream);
+}
+
+static ib_status host_step(ib_ctx *c, const double *x_h, const double *u_h, const double *v_h, const double *w_h, double *fu_h,
+                           double *fv_h, double *fw_h, double *Un_h, double *B_h, int packed, void *stream)
 {
     ib_status s = enter(c, stream);
     if (s != IB_OK) return s;
@@ -653,9 +661,13 @@ extern "C" ib_status ib_coupling_step_host(ib_ctx *c, const double *x_h, const d
         ib_status a = IB_OK;
         double **bufs[] = {&c->d_hx, &c->d_hUn, &c->d_hB};
         for (auto b : bufs) if (a == IB_OK) a = dev_alloc((void **)b, nb);
-        double **gbufs[] = {&c->d_hu, &c->d_hv, &c->d_hw, &c->d_hfu, &c->d_hfv, &c->d_hfw};
-        for (auto b : gbufs) if (a == IB_OK) a = dev_alloc((void **)b, gb);
+        // u,v,w and fu,fv,fw are one [3][n_cells] block each: a caller whose host arrays are laid out the same way
+        // (ib_coupling_step_host3) gets one copy per slab and direction instead of three
+        if (a == IB_OK) a = dev_alloc((void **)&c->d_hu, 3 * gb);
+        if (a == IB_OK) a = dev_alloc((void **)&c->d_hfu, 3 * gb);
         if (a != IB_OK) return a;
+        c->d_hv = c->d_hu + c->n_cells; c->d_hw = c->d_hu + 2 * c->n_cells;
+        c->d_hfv = c->d_hfu + c->n_cells; c->d_hfw = c->d_hfu + 2 * c->n_cells;
     }
     const bool pipelined = c->variant == 1 && !c->nodal && !c->profile && c->n_points > 0;
     if (!pipelined) {
@@ -674,7 +686,7 @@ extern "C" ib_status ib_coupling_step_host(ib_ctx *c, const double *x_h, const d
         IB_CUDA_TRY(cudaStreamSynchronize(st));
         return IB_OK;
     }
-    s = host_step_pipelined(c, x_h, u_h, v_h, w_h, fu_h, fv_h, fw_h, Un_h, B_h, st);
+    s = host_step_pipelined(c, x_h, u_h, v_h, w_h, fu_h, fv_h, fw_h, Un_h, B_h, packed, st);
     if (s != IB_OK) {
         // copies to and from the caller's host buffers may still be in flight on the internal streams: no
         // return before they have drained
@@ -685,8 +697,16 @@ extern "C" ib_status ib_coupling_step_host(ib_ctx *c, const double *x_h, const d
     return s;
 }
 
+extern "C" ib_status ib_coupling_step_host3(ib_ctx *c, const double *x_h, const double *uvw_h, double *f_h, double *Un_h,
+                                            double *B_h, void *stream)
+{
+    if (!c || !uvw_h || !f_h) return IB_ERR_INVALID_ARG;
+    return host_step(c, x_h, uvw_h, uvw_h + c->n_cells, uvw_h + 2 * c->n_cells, f_h, f_h + c->n_cells, f_h + 2 * c->n_cells, Un_h,
+                     B_h, 1, stream);
+}
+
 static ib_status host_step_pipelined(ib_ctx *c, const double *x_h, const double *u_h, const double *v_h, const double *w_h,
-                                     double *fu_h, double *fv_h, double *fw_h, double *Un_h, double *B_h, cudaStream_t st)
+                                     double *fu_h, double *fv_h, double *fw_h, double *Un_h, double *B_h, int packed, cudaStream_t st)
 {
     ib_status s = IB_OK;
     const size_t nb = (size_t)c->n_nodes * 3 * sizeof(double), gb = (size_t)c->n_cells * sizeof(double);
@@ -706,15 +726,39 @@ static ib_status host_step_pipelined(ib_ctx *c, const double *x_h, const double 
     const int K = ib_slab_count(c), nz = c->grid.nz, zs = 4 * ib_slab_layers(c);
     const size_t plane = (size_t)c->grid.nx * c->grid.ny, pb = plane * sizeof(double);
     const int z_first = nz < 4 ? nz : 4;          // wrap margin: the last z_first layers come first, the first go back last
+    // z-layers [z0, z0 + nl) of the three components: one 2-D copy (3 rows, pitch n_cells) when the host arrays
+    // are one [3][n_cells] block like the device's, else three copies
+    // (only on the caller's word -- ib_coupling_step_host3: three arrays that merely happen to be adjacent may be
+    // separate allocations, which one copy cannot span)
+    const bool upack = packed != 0, fpack = packed != 0;
+    auto h2d3 = [&](int z0, int nl, cudaStream_t q) -> cudaError_t {
+        if (nl <= 0) return cudaSuccess;
+        if (upack) return cudaMemcpy2DAsync(c->d_hu + z0 * plane, gb, u_h + z0 * plane, gb, (size_t)nl * pb, 3, cudaMemcpyHostToDevice, q);
+        const double *uh[3] = {u_h, v_h, w_h};
+        double *ud[3] = {c->d_hu, c->d_hv, c->d_hw};
+        for (int d = 0; d < 3; ++d) {
+            cudaError_t e = cudaMemcpyAsync(ud[d] + z0 * plane, uh[d] + z0 * plane, (size_t)nl * pb, cudaMemcpyHostToDevice, q);
+            if (e != cudaSuccess) return e;
+        }
+        return cudaSuccess;
+    };
+    auto d2h3 = [&](int z0, int nl, cudaStream_t q) -> cudaError_t {
+        if (nl <= 0) return cudaSuccess;
+        if (fpack) return cudaMemcpy2DAsync(fu_h + z0 * plane, gb, c->d_hfu + z0 * plane, gb, (size_t)nl * pb, 3, cudaMemcpyDeviceToHost, q);
+        double *fh[3] = {fu_h, fv_h, fw_h}, *fd[3] = {c->d_hfu, c->d_hfv, c->d_hfw};
+        for (int d = 0; d < 3; ++d) {
+            cudaError_t e = cudaMemcpyAsync(fh[d] + z0 * plane, fd[d] + z0 * plane, (size_t)nl * pb, cudaMemcpyDeviceToHost, q);
+            if (e != cudaSuccess) return e;
+        }
+        return cudaSuccess;
+    };
     // x first: the force side waits for it, and the copy engine serves the H2D copies of all streams in turn
     IB_CUDA_TRY(cudaMemcpyAsync(c->d_hx, x_h, nb, cudaMemcpyHostToDevice, st));
     IB_CUDA_TRY(cudaEventRecord(c->ev_fork, st));             // orders the side streams after x and earlier work on st
     IB_CUDA_TRY(cudaStreamWaitEvent(s2, c->ev_fork, 0));
     // zero-fill of f and the count pass of the binning beside the FE force, as in ib_coupling_step
     IB_CUDA_TRY(cudaStreamWaitEvent(ss, c->ev_fork, 0));
-    IB_CUDA_TRY(cudaMemsetAsync(c->d_hfu, 0, gb, ss));
-    IB_CUDA_TRY(cudaMemsetAsync(c->d_hfv, 0, gb, ss));
-    IB_CUDA_TRY(cudaMemsetAsync(c->d_hfw, 0, gb, ss));
+    IB_CUDA_TRY(cudaMemsetAsync(c->d_hfu, 0, 3 * gb, ss));
     IB_CUDA_TRY(cudaEventRecord(c->ev_zero, ss));             // f is zero
     s = ibk_bin_reserve(c, c->n_points);
     if (s == IB_OK) s = ibk_bin_points(c, 1, nullptr, nullptr, c->n_points, c->d_hx, nullptr, nullptr, 1, ss);
@@ -722,19 +766,13 @@ static ib_status host_step_pipelined(ib_ctx *c, const double *x_h, const double 
     if (s == IB_OK) s = ibk_fe_force(c, c->d_hx, Bd, c->d_Fhat, st);
     if (s != IB_OK) return s;
     {
-        const double *uh[3] = {u_h, v_h, w_h};
-        double *ud[3] = {c->d_hu, c->d_hv, c->d_hw};
-        for (int d = 0; d < 3 && K > 1; ++d)
-            IB_CUDA_TRY(cudaMemcpyAsync(ud[d] + (nz - z_first) * plane, uh[d] + (nz - z_first) * plane, z_first * pb,
-                                        cudaMemcpyHostToDevice, s2));
+        if (K > 1) IB_CUDA_TRY(h2d3(nz - z_first, z_first, s2));
         // copy k ends 4 layers into slab k+1: with the wrap layers it is all that the kernel of slab k reads
         const int z_last = K > 1 ? nz - z_first : nz;
         for (int k = 0; k < K; ++k) {
             const int z0 = k == 0 ? 0 : (zs * k + 4 < z_last ? zs * k + 4 : z_last);
             const int z1 = (k == K - 1 || zs * (k + 1) + 4 > z_last) ? z_last : zs * (k + 1) + 4;
-            for (int d = 0; d < 3 && z1 > z0; ++d)
-                IB_CUDA_TRY(cudaMemcpyAsync(ud[d] + z0 * plane, uh[d] + z0 * plane, (size_t)(z1 - z0) * pb,
-                                            cudaMemcpyHostToDevice, s2));
+            IB_CUDA_TRY(h2d3(z0, z1 - z0, s2));
             IB_CUDA_TRY(cudaEventRecord(c->ev_h2d[k], s2));
         }
     }
@@ -757,12 +795,9 @@ static ib_status host_step_pipelined(ib_ctx *c, const double *x_h, const double 
         }
     }
     if (band) {
-        double *fh[3] = {fu_h, fv_h, fw_h}, *fd[3] = {c->d_hfu, c->d_hfv, c->d_hfw};
         IB_CUDA_TRY(cudaStreamWaitEvent(s3, c->ev_zero, 0));
-        for (int d = 0; d < 3; ++d) {
-            IB_CUDA_TRY(cudaMemcpyAsync(fh[d], fd[d], (size_t)f_lo * pb, cudaMemcpyDeviceToHost, s3));
-            IB_CUDA_TRY(cudaMemcpyAsync(fh[d] + f_hi * plane, fd[d] + f_hi * plane, (size_t)(nz - f_hi) * pb, cudaMemcpyDeviceToHost, s3));
-        }
+        IB_CUDA_TRY(d2h3(0, f_lo, s3));
+        IB_CUDA_TRY(d2h3(f_hi, nz - f_hi, s3));
     }
     IB_CUDA_TRY(cudaStreamWaitEvent(st, c->ev_join, 0));
     if (s == IB_OK) s = ibk_bin_points(c, 1, nullptr, nullptr, c->n_points, c->d_hx, c->d_Fhat, c->d_Up, 2, st);
@@ -772,7 +807,6 @@ static ib_status host_step_pipelined(ib_ctx *c, const double *x_h, const double 
     IB_CUDA_TRY(cudaEventRecord(c->ev_aux, st));              // the records are binned
     IB_CUDA_TRY(cudaStreamWaitEvent(s4, c->ev_aux, 0));
     {
-        double *fh[3] = {fu_h, fv_h, fw_h}, *fd[3] = {c->d_hfu, c->d_hfv, c->d_hfw};
         int z_done = band ? f_lo : z_first;
         for (int k = 0; k < K; ++k) {
             cudaStream_t sk = (k & 1) ? s4 : st;
@@ -785,13 +819,10 @@ static ib_status host_step_pipelined(ib_ctx *c, const double *x_h, const double 
             if (z_end > f_hi) z_end = f_hi;                   // f_hi = nz without a band
             if (z_end < z_done) z_end = z_done;
             IB_CUDA_TRY(cudaStreamWaitEvent(s3, c->ev_slab[k], 0));
-            for (int d = 0; d < 3 && z_end > z_done; ++d)
-                IB_CUDA_TRY(cudaMemcpyAsync(fh[d] + z_done * plane, fd[d] + z_done * plane, (size_t)(z_end - z_done) * pb,
-                                            cudaMemcpyDeviceToHost, s3));
+            IB_CUDA_TRY(d2h3(z_done, z_end - z_done, s3));
             z_done = z_end;
         }
-        for (int d = 0; d < 3 && z_first > 0 && !band; ++d)
-            IB_CUDA_TRY(cudaMemcpyAsync(fh[d], fd[d], z_first * pb, cudaMemcpyDeviceToHost, s3));
+        if (!band) IB_CUDA_TRY(d2h3(0, z_first, s3));
     }
     IB_CUDA_TRY(cudaStreamWaitEvent(ss, c->ev_aux, 0));
     IB_CUDA_TRY(cudaStreamWaitEvent(ss, c->ev_h2d[K - 1], 0));

@@ -20,7 +20,7 @@ STATUS = {0: "IB_OK", 1: "IB_ERR_INVALID_ARG", 2: "IB_ERR_UNSUPPORTED", 3: "IB_E
 
 EXPORTS = ["ib_create", "ib_destroy", "ib_num_points", "ib_num_nodes", "ib_num_elems", "ib_fe_force",
            "ib_points", "ib_restrict", "ib_bin_sort", "ib_spread", "ib_interp", "ib_coupling_step",
-           "ib_coupling_step_host", "ib_step_eq16", "ib_check", "ib_launch_count", "ib_set_variant", "ib_set_graph", "ib_set_tethers", "ib_set_surface", "ib_set_loads", "ib_probe_dfma",
+           "ib_coupling_step_host", "ib_coupling_step_host3", "ib_step_eq16", "ib_check", "ib_launch_count", "ib_set_variant", "ib_set_graph", "ib_set_tethers", "ib_set_surface", "ib_set_loads", "ib_probe_dfma",
            "ib_profile_enable", "ib_profile_read",
            "ib_status_string"]
 
@@ -69,6 +69,7 @@ def lib():
         L.ib_interp.argtypes = [vp, vp, i64, vp, vp, vp, vp, vp]
         L.ib_coupling_step.argtypes = [vp] * 11
         L.ib_coupling_step_host.argtypes = [vp] * 11
+        L.ib_coupling_step_host3.argtypes = [vp] * 7
         L.ib_step_eq16.argtypes = [vp] * 5 + [C.c_double] + [vp] * 7
         L.ib_check.argtypes = [vp, C.POINTER(i64)]
         L.ib_set_variant.argtypes = [vp, i32]
@@ -226,6 +227,11 @@ class Context:
         """All tensors are (pinned) HOST tensors."""
         _chk(lib().ib_coupling_step_host(self._h, _dp(x), _dp(u), _dp(v), _dp(w), _dp(fu), _dp(fv), _dp(fw),
                                          _dp(Un), _dp(B), _stream(stream)), "ib_coupling_step_host")
+
+    def ib_coupling_step_host3(self, x, uvw, f, Un, B=None, stream=None):
+        """All tensors are (pinned) HOST tensors; uvw and f are [3][n_cells]."""
+        _chk(lib().ib_coupling_step_host3(self._h, _dp(x), _dp(uvw), _dp(f), _dp(Un), _dp(B), _stream(stream)),
+             "ib_coupling_step_host3")
 
     def ib_check(self):
         """Synchronise and return (status code, first bad id)."""

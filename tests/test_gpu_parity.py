@@ -222,7 +222,7 @@ def test_host_entry_point_matches_device_path(ib, name, variant):
     ctx.close()
 
 
-@pytest.mark.parametrize("case", ["wrap", "bounded", "one-slab", "pageable", "non-cubic"])
+@pytest.mark.parametrize("case", ["wrap", "bounded", "one-slab", "pageable", "non-cubic", "packed"])
 def test_host_step_slabs_against_oracle(ib, orc, case):
     """ib_coupling_step_host cuts the step into z-slabs (copies of u,v,w and f overlap the tile kernel):
     a structure across the periodic z wrap (first and last slab share points), a bounded grid with the
@@ -236,8 +236,8 @@ def test_host_step_slabs_against_oracle(ib, orc, case):
     elif case == "bounded":
         shift = org - wl.X.min(axis=1) + 0.3 * wl.h
         periodic = 0
-    elif case == "pageable":                      # plain (unpinned) host memory: slower copies, same answer
-        shift = np.zeros(3)
+    elif case in ("pageable", "packed"):          # plain (unpinned) host memory: slower copies, same answer;
+        shift = np.zeros(3)                       # packed: ib_coupling_step_host3, one [3][n_cells] array per direction
     elif case == "non-cubic":                     # 24 x 16 x 40 cells: 5 slabs of 2 tile layers, the slab tilted across them
         shift = np.zeros(3)
     else:
@@ -264,8 +264,14 @@ def test_host_step_slabs_against_oracle(ib, orc, case):
           (lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory())
     outs = [pin(np.full(ncell, 9.0)) for _ in range(3)]
     Un, B = pin(np.empty((3, wl.n_nodes))), pin(np.empty((3, wl.n_nodes)))
-    for _ in range(2):
-        ctx.ib_coupling_step_host(pin(x), pin(u), pin(v), pin(w), *outs, Un, B)
+    if case == "packed":
+        f3 = pin(np.full((3, ncell), 9.0))
+        outs = [f3[0], f3[1], f3[2]]
+        for _ in range(2):
+            ctx.ib_coupling_step_host3(pin(x), pin(np.stack([u, v, w])), f3, Un, B)
+    else:
+        for _ in range(2):
+            ctx.ib_coupling_step_host(pin(x), pin(u), pin(v), pin(w), *outs, Un, B)
     ctx.check()
     for k, t in (("B", B), ("fu", outs[0]), ("fv", outs[1]), ("fw", outs[2]), ("Un", Un)):
         _close(t.numpy(), ref[k], f"host slabs {case} {k}")

@@ -94,6 +94,17 @@ def test_c3_host_step_matches_oracle(ib, orc):
         ctx.check()
         for k, t in (("B", B), ("fu", outs[0]), ("fv", outs[1]), ("fw", outs[2]), ("Un", Un)):
             _close(t.numpy(), ref[k], f"C3 host step call {it} {k}")
+    # the packed entry point bench.py times: one [3][n_cells] host array per direction
+    uvw = pin(np.stack([wl.u, wl.v, wl.w]))
+    f3 = torch.full((3, wl.n_cells), 7.0, dtype=torch.float64).pin_memory()
+    for it in range(2):
+        f3.fill_(7.0 + it)
+        ctx.ib_coupling_step_host3(x, uvw, f3, Un, B)
+        ctx.check()
+        for c, k in enumerate(("fu", "fv", "fw")):
+            _close(f3[c].numpy(), ref[k], f"C3 host3 call {it} {k}")
+        _close(Un.numpy(), ref["Un"], f"C3 host3 call {it} Un")
+        _close(B.numpy(), ref["B"], f"C3 host3 call {it} B")
     ctx.close()
 
 
