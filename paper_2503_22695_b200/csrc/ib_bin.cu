@@ -36,8 +36,7 @@ struct ib_bin_params {
     double inv_h;
     // bins
     int32_t *tile_cur;             // count pass: counts; scatter pass: running cursors
-    double *sx, *sG;               // [3][P] sorted records
-    int32_t *sid;                  // [P] original point id
+    double *rec;                   // [P][8] records: {x, y, z, id | G0, G1, G2, -} (two 32-byte halves)
     double *Up;                    // non-finite points get Up = 0 (scatter pass), may be NULL
     long long *status;
 };
@@ -49,25 +48,57 @@ __device__ __forceinline__ int ib_tile_of(double x, double y, double z, const ib
     return ((((cz >> 2) * (g.ny / BT) + (cy >> 2)) * (g.nx / BT) + (cx >> 2)) << 2) | (cz & 3);
 }
 
-// warp-aggregated count / slot allocation; every lane of the warp must call (valid may differ)
-template <int SCATTER>
-__device__ __forceinline__ int ib_bin_slot(bool valid, int tile, int32_t *tile_cur)
+// The points of a CTA are neighbours in space (rows of the same few elements) and fall into a handful of bins:
+// they are counted per CTA in a small shared-memory hash table (native 32-bit shared atomics), and the CTA then
+// makes ONE global atomic per distinct bin -- instead of a warp match and a global atomic per point and warp,
+// whose returned slot every store of the scatter pass had to wait for.
+#define HT 128
+struct ib_bin_hash { int key[HT], cnt[HT], base[HT]; };
+#define IB_CODE_NONE (-1)          // no record (invalid point)
+
+__device__ __forceinline__ void ib_hash_clear(ib_bin_hash &h)
 {
-    const unsigned full = 0xffffffffu;
-    const int lane = threadIdx.x & 31;
-    unsigned act = __ballot_sync(full, valid);
-    int pos = -1;
-    if (valid) {
-        unsigned peers = __match_any_sync(act, tile);
-        int leader = __ffs(peers) - 1;
-        int base = 0;
-        if (lane == leader) base = atomicAdd(&tile_cur[tile], __popc(peers));
-        if (SCATTER) {
-            base = __shfl_sync(peers, base, leader);
-            pos = base + __popc(peers & ((1u << lane) - 1u));
-        }
+    for (int i = threadIdx.x; i < HT; i += blockDim.x) { h.key[i] = -1; h.cnt[i] = 0; }
+}
+// count the point in; returns slot | rank << 8, or (table full after 32 probes: clouds scattered all over the
+// grid) INT_MIN | the global slot taken at once
+template <int SCATTER>
+__device__ __forceinline__ int ib_hash_insert(ib_bin_hash &h, int bin, int32_t *tile_cur)
+{
+    unsigned s = ((unsigned)bin * 2654435761u) >> 25;
+    for (int t = 0; t < 32; ++t) {
+        const int k = atomicCAS(&h.key[s], -1, bin);
+        if (k == -1 || k == bin) return (int)s | (atomicAdd(&h.cnt[s], 1) << 8);
+        s = (s + 1) & (HT - 1);
     }
-    return pos;
+    const int pos = atomicAdd(&tile_cur[bin], 1);
+    return SCATTER ? (int)(0x80000000u | (unsigned)pos) : IB_CODE_NONE;
+}
+// one global atomic per distinct bin of the CTA; barriers inside: every thread of the CTA must call
+template <int SCATTER>
+__device__ __forceinline__ void ib_hash_flush(ib_bin_hash &h, int32_t *tile_cur)
+{
+    __syncthreads();
+    for (int i = threadIdx.x; i < HT; i += blockDim.x)
+        if (h.key[i] >= 0) {
+            const int b = atomicAdd(&tile_cur[h.key[i]], h.cnt[i]);
+            if (SCATTER) h.base[i] = b;
+        }
+    if (SCATTER) __syncthreads();
+}
+__device__ __forceinline__ int ib_hash_pos(const ib_bin_hash &h, int code)
+{
+    return code < 0 ? (int)((unsigned)code & 0x7fffffffu) : h.base[code & 255] + (code >> 8);
+}
+
+// one record: two 32-byte stores, streaming (the records exceed L2 and are read once, oldest first, so keeping
+// them out of L2 leaves room for the grid halos)
+__device__ __forceinline__ void ib_store_rec(double *rec, int pos, double x, double y, double z, int id,
+                                             bool with_g, double g0, double g1, double g2)
+{
+    double *r = rec + (size_t)pos * 8;
+    asm volatile("st.global.cs.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(r), "d"(x), "d"(y), "d"(z), "d"(__longlong_as_double((long long)id)) : "memory");
+    if (with_g) asm volatile("st.global.cs.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(r + 4), "d"(g0), "d"(g1), "d"(g2), "d"(0.0) : "memory");
 }
 
 // ---- cloud source ------------------------------------------------------------------------------
@@ -75,6 +106,9 @@ template <int SCATTER>
 __global__ void __launch_bounds__(256)
 ibk_bin_cloud(ib_bin_params pr)
 {
+    __shared__ ib_bin_hash h;
+    ib_hash_clear(h);
+    __syncthreads();
     const int64_t P = pr.P;
     int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     bool valid = p < P;
@@ -95,14 +129,14 @@ ibk_bin_cloud(ib_bin_params pr)
             valid = false;
         }
     }
-    int tile = valid ? ib_tile_of(x, y, z, pr.g, pr.inv_h) : 0;
-    int pos = ib_bin_slot<SCATTER>(valid, tile, pr.tile_cur);
+    const int code = valid ? ib_hash_insert<SCATTER>(h, ib_tile_of(x, y, z, pr.g, pr.inv_h), pr.tile_cur) : IB_CODE_NONE;
+    ib_hash_flush<SCATTER>(h, pr.tile_cur);
     if (SCATTER && valid) {
-        pr.sx[pos] = x; pr.sx[P + pos] = y; pr.sx[2 * P + pos] = z;
-        pr.sid[pos] = (int32_t)p;
-        if (pr.Gp) {
-            pr.sG[pos] = __ldg(pr.Gp + p); pr.sG[P + pos] = __ldg(pr.Gp + P + p); pr.sG[2 * P + pos] = __ldg(pr.Gp + 2 * P + p);
-        }
+        const int pos = ib_hash_pos(h, code);
+        assert(pos >= 0 && pos < P);
+        const bool wg = pr.Gp != nullptr;
+        ib_store_rec(pr.rec, pos, x, y, z, (int)p, wg, wg ? __ldg(pr.Gp + p) : 0.0, wg ? __ldg(pr.Gp + P + p) : 0.0,
+                     wg ? __ldg(pr.Gp + 2 * P + p) : 0.0);
     }
 }
 
@@ -131,8 +165,10 @@ template <int SCATTER, int STAGE>
 __global__ void __launch_bounds__(256, 4)
 ibk_bin_mesh(ib_bin_params pr)
 {
-    const unsigned full = 0xffffffffu;
     __shared__ double s_nd[STAGE ? 16 * 8 * 6 : 1];       // [element of the CTA][local node][x0 x1 x2 F0 F1 F2]
+    __shared__ ib_bin_hash h;
+    ib_hash_clear(h);
+    if (!STAGE) __syncthreads();
     if (STAGE) {
         const int rpe = pr.un2 * pr.un3, epc = 256 / rpe;
         const int64_t e_first = (int64_t)blockIdx.x * epc;
@@ -215,68 +251,41 @@ ibk_bin_mesh(ib_bin_params pr)
             live = false;
         }
     }
-    const int nmax = __reduce_max_sync(full, live ? n1 : 0);
+    // ---- the n1 points of the row: position, bin, count in the CTA's table ------------------------------
     const double rn1 = 1.0 / (double)(n1 > 0 ? n1 : 1);
-    // fast path: every live row of the warp lies inside one tile (a row of sub-points spans a
-    // fraction of a cell) -> one aggregated atomic per distinct tile for the whole row
-    int tile0 = 0;
-    bool same = true;
-    if (live) {
-        for (int j = 0; j < n1; ++j) {
-            double t = ((double)j + 0.5) * rn1;
-            const double xj = __fma_rn(t, D[0], L[0]), yj = __fma_rn(t, D[1], L[1]), zj = __fma_rn(t, D[2], L[2]);
-            int tl = ib_tile_of(xj, yj, zj, pr.g, pr.inv_h);
-            if (j == 0) tile0 = tl;
-            same = same && (tl == tile0) && (pr.g.periodic || ib_in_box(xj, yj, zj, pr.g, pr.inv_h));
-        }
-    }
-    const bool warp_same = __all_sync(full, same) && __all_sync(full, !live || n1 == nmax);
-    int base = -1, pstride = 0;
-    if (warp_same) {
-        unsigned act = __ballot_sync(full, live);
-        if (live) {
-            unsigned peers = __match_any_sync(act, tile0);
-            int leader = __ffs(peers) - 1;
-            const int lane = threadIdx.x & 31;
-            int b0 = 0;
-            if (lane == leader) b0 = atomicAdd(&pr.tile_cur[tile0], __popc(peers) * n1);
-            if (SCATTER) {
-                b0 = __shfl_sync(peers, b0, leader);
-                base = b0 + __popc(peers & ((1u << lane) - 1u));      // slot j of the row: base + j*pstride
-                pstride = __popc(peers);
-            }
-        }
-    }
-    for (int j = 0; j < nmax; ++j) {
-        bool valid = live && j < n1;
-        double t = ((double)j + 0.5) * rn1;
-        double x = __fma_rn(t, D[0], L[0]), y = __fma_rn(t, D[1], L[1]), z = __fma_rn(t, D[2], L[2]);
-        int pos;
-        if (warp_same) pos = base + j * pstride;
-        else {
-            if (valid && !pr.g.periodic && !ib_in_box(x, y, z, pr.g, pr.inv_h)) {      // outside a bounded grid
+    int code[8];                                   // nsub <= 8 (ib_create)
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+        code[j] = IB_CODE_NONE;
+        if (live && j < n1) {
+            const double t = ((double)j + 0.5) * rn1;
+            const double x = __fma_rn(t, D[0], L[0]), y = __fma_rn(t, D[1], L[1]), z = __fma_rn(t, D[2], L[2]);
+            if (!pr.g.periodic && !ib_in_box(x, y, z, pr.g, pr.inv_h)) {      // outside a bounded grid
                 if (SCATTER) {
                     ib_latch(pr.status, IB_ERR_OUT_OF_DOMAIN, e);
                     if (pr.Up) { pr.Up[p0 + j] = 0.0; pr.Up[pr.P + p0 + j] = 0.0; pr.Up[2 * pr.P + p0 + j] = 0.0; }
                 }
-                valid = false;
+            } else {
+                const int c = ib_hash_insert<SCATTER>(h, ib_tile_of(x, y, z, pr.g, pr.inv_h), pr.tile_cur);
+                code[j] = SCATTER ? c : 0;
             }
-            int tile = valid ? ib_tile_of(x, y, z, pr.g, pr.inv_h) : 0;
-            pos = ib_bin_slot<SCATTER>(valid, tile, pr.tile_cur);
         }
-        if (SCATTER && valid) {
-            const int64_t P = pr.P;
-            assert(pos >= 0 && pos < P);
-            // streaming stores: the records (325 MB for C3) exceed L2 and are read once, oldest first,
-            // so keeping them out of L2 leaves room for the grid halos (measured -0.6 % on the step)
-#define IB_ST(PTR, V) __stcs((PTR), (V))
-            IB_ST(pr.sx + pos, x); IB_ST(pr.sx + P + pos, y); IB_ST(pr.sx + 2 * P + pos, z);
-            IB_ST(pr.sid + pos, (int32_t)(p0 + j));
-            if (pr.Fhat) {
-                double W = __ldg(pr.Wp + p0 + j);
-                IB_ST(pr.sG + pos, W * fma(t, DF[0], LF[0]));
-                IB_ST(pr.sG + P + pos, W * fma(t, DF[1], LF[1]));
-                IB_ST(pr.sG + 2 * P + pos, W * fma(t, DF[2], LF[2]));
+    }
+    ib_hash_flush<SCATTER>(h, pr.tile_cur);
+    if (SCATTER) {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            if (live && j < n1 && code[j] != IB_CODE_NONE) {
+                const double t = ((double)j + 0.5) * rn1;
+                const double x = __fma_rn(t, D[0], L[0]), y = __fma_rn(t, D[1], L[1]), z = __fma_rn(t, D[2], L[2]);
+                const int pos = ib_hash_pos(h, code[j]);
+                assert(pos >= 0 && pos < pr.P);
+                double g0 = 0.0, g1 = 0.0, g2 = 0.0;
+                if (pr.Fhat) {
+                    const double W = __ldg(pr.Wp + p0 + j);
+                    g0 = W * fma(t, DF[0], LF[0]); g1 = W * fma(t, DF[1], LF[1]); g2 = W * fma(t, DF[2], LF[2]);
+                }
+                ib_store_rec(pr.rec, pos, x, y, z, (int)(p0 + j), pr.Fhat != nullptr, g0, g1, g2);
             }
         }
     }
@@ -430,7 +439,7 @@ ib_status ibk_bin_points(ib_ctx *c, int mesh, const double *xp, const double *Gp
     pr.nsub = c->d_nsub; pr.pt_off = c->d_pt_off; pr.row_off = c->d_row_off; pr.conn = c->d_conn;
     pr.x = x; pr.Fhat = Fhat; pr.Wp = c->d_Wp;
     pr.g = c->grid; pr.inv_h = c->inv_h;
-    pr.tile_cur = c->d_tile_cur; pr.sx = c->d_sx; pr.sG = c->d_sG; pr.sid = c->d_sid;
+    pr.tile_cur = c->d_tile_cur; pr.rec = c->d_rec;
     pr.Up = Up; pr.status = c->d_status;
     const int64_t nthr = mesh ? c->n_rows : P;
     const int rpe = c->un[1] * c->un[2];
@@ -465,18 +474,14 @@ ib_status ibk_bin_reserve(ib_ctx *c, int64_t P)
 {
     if (P <= c->bin_cap) return IB_OK;
     c->gstate = 0;                                  // a captured step holds the old buffers
-    if (c->d_sx) cudaFree(c->d_sx);
-    if (c->d_sG) cudaFree(c->d_sG);
-    if (c->d_sid) cudaFree(c->d_sid);
+    if (c->d_rec) cudaFree(c->d_rec);
     if (c->d_work) cudaFree(c->d_work);
     if (c->d_small_rec) cudaFree(c->d_small_rec);
     c->d_small_rec = nullptr;
-    c->d_sx = c->d_sG = nullptr; c->d_sid = nullptr; c->d_work = nullptr;
+    c->d_rec = nullptr; c->d_work = nullptr;
     c->bin_cap = 0;
     int64_t cap = P + P / 8 + 1024;
-    if (cudaMalloc(&c->d_sx, (size_t)cap * 3 * sizeof(double)) != cudaSuccess) return IB_ERR_ALLOC;
-    if (cudaMalloc(&c->d_sG, (size_t)cap * 3 * sizeof(double)) != cudaSuccess) return IB_ERR_ALLOC;
-    if (cudaMalloc(&c->d_sid, (size_t)cap * sizeof(int32_t)) != cudaSuccess) return IB_ERR_ALLOC;
+    if (cudaMalloc(&c->d_rec, (size_t)cap * 8 * sizeof(double)) != cudaSuccess) return IB_ERR_ALLOC;
     {   // a tile with >= IB_SMALL_TILE points gives at most 4 runs of layers plus one piece per 192 points
         const int64_t n_tiles = c->n_cells / (BT * BT * BT), dense = cap / IB_SMALL_TILE + 1;
         c->work_cap = 4 * (dense < n_tiles ? dense : n_tiles) + cap / 192 + 8;

@@ -71,8 +71,7 @@ struct ib_ctx {
     int32_t *d_small_rec;      // records of tiles with < IB_SMALL_TILE points (count in d_tile_count[2])
     int32_t *d_tile_count;     // [0] number of non-empty tiles, [1] work counter
     int64_t bin_cap;
-    double *d_sx, *d_sG;       // [3][P] point records grouped by tile
-    int32_t *d_sid;            // [P] original point id of each record
+    double *d_rec;             // [P][8] point records grouped by bin: {x, y, z, id | G0, G1, G2, -}
     // host staging for the *_host entry point
     double *d_hx, *d_hu, *d_hv, *d_hw, *d_hfu, *d_hfv, *d_hfw, *d_hUn, *d_hB;
     // status latch: one packed word (ib_latch)

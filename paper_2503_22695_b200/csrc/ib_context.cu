@@ -112,7 +112,7 @@ extern "C" ib_status ib_destroy(ib_ctx *c)
     void *ptrs[] = {c->d_conn, c->d_X, c->d_fib, c->d_mat_id, c->d_nsub, c->d_pt_off, c->d_mats, c->d_adj,
                     c->d_Wp, c->d_wa, c->d_geo, c->d_node_off, c->d_node_slot, c->d_teth_ids, c->d_faces, c->d_Ce, c->d_Fhat, c->d_B, c->d_xp, c->d_Gp, c->d_Up, c->d_key[0],
                     c->d_key[1], c->d_val[0], c->d_val[1], c->d_hist, c->d_tile_cur, c->d_tile_start, c->d_work, c->d_small_rec,
-                    c->d_row_off, c->d_sx, c->d_sG, c->d_sid,
+                    c->d_row_off, c->d_rec,
                     c->d_tile_count, c->d_hx, c->d_hu, c->d_hfu,
                     c->d_hUn, c->d_hB, c->d_status};
     for (void *p : ptrs)

@@ -50,8 +50,7 @@
 #define NORD ((100 + IB_CHUNK / PCAP + 7) & ~7)   // units per component: one per item + IB_CHUNK / PCAP whole ones, in whole batches
 
 struct ib_tiled_params {
-    const double *sx, *sG;      // [3][P] records grouped by tile
-    const int32_t *sid;         // [P] point id of record
+    const double *rec;          // [P][8] records grouped by bin: {x, y, z, id | G0, G1, G2, -} (ib_bin.cu)
     int64_t P;
     const double *fld[3];
     double *frc[3];
@@ -101,6 +100,12 @@ __device__ __forceinline__ double ib_tile_coord(double x, double x0, double h, d
 __device__ __forceinline__ void ib_prefetch_l2(const void *p)
 {
     asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+}
+
+// one 32-byte half of a record, streaming
+__device__ __forceinline__ void ib_load_rec(const double *p, double v[4])
+{
+    asm volatile("ld.global.cs.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(v[0]), "=d"(v[1]), "=d"(v[2]), "=d"(v[3]) : "l"(p));
 }
 
 // (a, q) of the Peskin kernel at fraction r (see the header): w0..w3 = a-q, a+q, (1/2-a)+q, (1/2-a)-q
@@ -385,7 +390,6 @@ ibk_tiled_kernel(ib_tiled_params pr)
 
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int n[3] = {pr.g.nx, pr.g.ny, pr.g.nz};
-    const int64_t P = pr.P;
 
     if (tid == 0) {
         ib_mbar_init(mbar + 0, 1); ib_mbar_init(mbar + 8, 1);
@@ -431,14 +435,15 @@ ibk_tiled_kernel(ib_tiled_params pr)
             // ---- coordinates of the records, one thread per point: tile coordinates, half-cell, rank inside it.
             // Nothing here touches the record buffers: it overlaps the consumers' work on both of them.
             double xi[KPT][3];
-            int ks[KPT];
+            int ks[KPT], idr[KPT];
             {
-                double xr[KPT][3];
+                double xr[KPT][4];
 #pragma unroll
                 for (int k = 0; k < KPT; ++k) {
                     const int i = tid + k * TBP;
-#pragma unroll
-                    for (int d = 0; d < 3; ++d) xr[k][d] = (i < cn) ? __ldcs(pr.sx + (int64_t)d * P + cb + i) : 0.0;
+                    xr[k][0] = xr[k][1] = xr[k][2] = xr[k][3] = 0.0;
+                    if (i < cn) ib_load_rec(pr.rec + (size_t)(cb + i) * 8, xr[k]);
+                    idr[k] = (int)__double_as_longlong(xr[k][3]);
                 }
 #pragma unroll
                 for (int k = 0; k < KPT; ++k) {
@@ -459,16 +464,8 @@ ibk_tiled_kernel(ib_tiled_params pr)
             for (int i = tid; i < 3 * NBIN; i += TBP) bins[i] = 0;      // read last before the closing barrier of the previous iteration
             {                                            // the next work item's records -> L2 while this one is processed
                 const int4 nx4 = s_wk[b ^ 1];
-                if (nx4.x >= 0) {
-                    for (int i = 16 * tid; i < 3 * CH; i += 16 * TBP) {
-                        const int d = i / CH, o = i - d * CH;          // CH is a multiple of 16: one 128-byte line per 16 doubles
-                        if (o < nx4.z) {
-                            ib_prefetch_l2(pr.sx + (int64_t)d * P + nx4.y + o);
-                            if (DO_SPREAD) ib_prefetch_l2(pr.sG + (int64_t)d * P + nx4.y + o);
-                        }
-                    }
-                    if (DO_INTERP && 32 * tid < nx4.z) ib_prefetch_l2(pr.sid + nx4.y + 32 * tid);
-                }
+                if (nx4.x >= 0)
+                    for (int i = 2 * tid; i < nx4.z; i += 2 * TBP) ib_prefetch_l2(pr.rec + (size_t)(nx4.y + i) * 8);   // two records per 128-byte line
             }
             {                                            // exclusive scan of the 512 counts
                 int v[SCK], s = 0;
@@ -556,13 +553,8 @@ ibk_tiled_kernel(ib_tiled_params pr)
             for (int k = 0; k < KPT; ++k) {
                 if (ks[k] >= 0) {
                     const int i = tid + k * TBP;
-                    double Gr[3] = {0.0, 0.0, 0.0};
-                    int idr = 0;
-                    if (DO_INTERP) idr = __ldcs(pr.sid + cb + i);
-                    if (DO_SPREAD) {
-#pragma unroll
-                        for (int d = 0; d < 3; ++d) Gr[d] = __ldcs(pr.sG + (int64_t)d * P + cb + i);
-                    }
+                    double Gr[4] = {0.0, 0.0, 0.0, 0.0};
+                    if (DO_SPREAD) ib_load_rec(pr.rec + (size_t)(cb + i) * 8 + 4, Gr);
                     const int key = ks[k] & 511;
                     const int pos = oc_start[key] + (ks[k] >> 9);
                     assert(pos >= 0 && pos < cn && cn <= CH);
@@ -578,7 +570,7 @@ ibk_tiled_kernel(ib_tiled_params pr)
 #pragma unroll
                         for (int d = 0; d < 3; ++d) sGs[d * CH + pos] = Gr[d] * pr.ih3;
                     }
-                    if (DO_INTERP) sids[pos] = idr;
+                    if (DO_INTERP) sids[pos] = idr[k];
                 }
             }
             if (DO_INTERP) asm volatile("cp.async.wait_group 0;" ::: "memory");      // this thread's part of the halo has landed
@@ -690,10 +682,11 @@ ibk_small_tiles(ib_tiled_params pr, const int32_t *__restrict__ small_rec, const
     for (int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 2; i < n; i += stride) {
         const int r = __ldg(small_rec + i);
         double G[3] = {0, 0, 0}, U[3];
-        if (DO_SPREAD) { G[0] = pr.sG[r] * pr.ih3; G[1] = pr.sG[P + r] * pr.ih3; G[2] = pr.sG[2 * P + r] * pr.ih3; }
-        ib_point_quad<DO_SPREAD, DO_INTERP>(pr.sx[r], pr.sx[P + r], pr.sx[2 * P + r], G, pr.fld, pr.frc, pr.g, pr.inv_h, q, qmask, U);
+        const double *rc = pr.rec + (size_t)r * 8;
+        if (DO_SPREAD) { G[0] = rc[4] * pr.ih3; G[1] = rc[5] * pr.ih3; G[2] = rc[6] * pr.ih3; }
+        ib_point_quad<DO_SPREAD, DO_INTERP>(rc[0], rc[1], rc[2], G, pr.fld, pr.frc, pr.g, pr.inv_h, q, qmask, U);
         if (DO_INTERP && q == 0) {
-            const int id = pr.sid[r];
+            const int id = (int)__double_as_longlong(rc[3]);
             pr.Up[id] = U[0]; pr.Up[P + id] = U[1]; pr.Up[2 * P + id] = U[2];
         }
     }
@@ -763,7 +756,7 @@ ib_status ibk_tiled_spread_interp(ib_ctx *c, int mesh, const double *xp, const d
 static void fill_params(ib_ctx *c, ib_tiled_params &pr, int64_t P, const double *u, const double *v, const double *w,
                         double *fu, double *fv, double *fw, double *Up, int slab)
 {
-    pr.sx = c->d_sx; pr.sG = c->d_sG; pr.sid = c->d_sid; pr.P = P;
+    pr.rec = c->d_rec; pr.P = P;
     pr.fld[0] = u; pr.fld[1] = v; pr.fld[2] = w;
     pr.frc[0] = fu; pr.frc[1] = fv; pr.frc[2] = fw;
     pr.Up = Up;
