@@ -445,8 +445,7 @@ ib_status ibk_bin_points(ib_ctx *c, int mesh, const double *xp, const double *Gp
     const int rpe = c->un[1] * c->un[2];
     const bool stage = c->un[0] > 0 && rpe >= 16 && 256 % rpe == 0;     // <= 16 elements per CTA fit the staging array
     if (phases & 1) {
-        IB_CUDA_TRY(cudaMemsetAsync(c->d_tile_cur, 0, (size_t)n_tiles * 4 * sizeof(int32_t), st));
-        IB_CUDA_TRY(cudaMemsetAsync(c->d_tile_count, 0, 4 * sizeof(int32_t), st));
+        IB_CUDA_TRY(cudaMemsetAsync(c->d_tile_count, 0, ((size_t)c->tile_hdr + (size_t)n_tiles * 4) * sizeof(int32_t), st));   // counters and bins
         if (mesh && stage) ibk_bin_mesh<0, 1><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
         else if (mesh) ibk_bin_mesh<0, 0><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
         else ibk_bin_cloud<0><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);

@@ -69,7 +69,8 @@ struct ib_ctx {
     int4 *d_work;              // work list of the tile kernel: {tile, first record, points, 0} per chunk
     int64_t work_cap;
     int32_t *d_small_rec;      // records of tiles with < IB_SMALL_TILE points (count in d_tile_count[2])
-    int32_t *d_tile_count;     // [0] number of non-empty tiles, [1] work counter
+    int32_t *d_tile_count;     // [0] number of non-empty tiles, [1] work counter; d_tile_cur follows it in the same block
+    int tile_hdr;              // ints of d_tile_count before d_tile_cur
     int64_t bin_cap;
     double *d_rec;             // [P][8] point records grouped by bin: {x, y, z, id | G0, G1, G2, -}
     // host staging for the *_host entry point

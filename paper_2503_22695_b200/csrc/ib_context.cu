@@ -111,7 +111,7 @@ extern "C" ib_status ib_destroy(ib_ctx *c)
     cudaSetDevice(c->device);
     void *ptrs[] = {c->d_conn, c->d_X, c->d_fib, c->d_mat_id, c->d_nsub, c->d_pt_off, c->d_mats, c->d_adj,
                     c->d_Wp, c->d_wa, c->d_geo, c->d_node_off, c->d_node_slot, c->d_teth_ids, c->d_faces, c->d_Ce, c->d_Fhat, c->d_B, c->d_xp, c->d_Gp, c->d_Up, c->d_key[0],
-                    c->d_key[1], c->d_val[0], c->d_val[1], c->d_hist, c->d_tile_cur, c->d_tile_start, c->d_work, c->d_small_rec,
+                    c->d_key[1], c->d_val[0], c->d_val[1], c->d_hist, c->d_tile_start, c->d_work, c->d_small_rec,
                     c->d_row_off, c->d_rec,
                     c->d_tile_count, c->d_hx, c->d_hu, c->d_hfu,
                     c->d_hUn, c->d_hB, c->d_status};
@@ -254,10 +254,12 @@ extern "C" ib_status ib_create(ib_ctx **out, const ib_grid_desc *g, const ib_mes
         TRY(dev_alloc((void **)&c->d_Up, P * 3 * sizeof(double)));
     }
     const int n_tiles = (int)(c->n_cells / 64);          // 4x4x4-cell tiles of the tiled path
-    TRY(dev_alloc((void **)&c->d_tile_cur, (size_t)(4 * n_tiles + 4) * sizeof(int32_t)));      // 4 z-layer bins per tile
+    // counters + scan partials, then the bins (4 z-layer bins per tile): one block, zeroed by one memset per step
+    c->tile_hdr = (IB_TILE_HDR + 2 * (n_tiles / 1024 + 2) + 3) & ~3;
+    TRY(dev_alloc((void **)&c->d_tile_count, (size_t)(c->tile_hdr + 4 * n_tiles + 4) * sizeof(int32_t)));
+    if (s == IB_OK) c->d_tile_cur = c->d_tile_count + c->tile_hdr;
     TRY(dev_alloc((void **)&c->d_tile_start, (size_t)(4 * n_tiles + 4) * sizeof(int32_t)));
     TRY(dev_upload(&c->d_row_off, roff.data(), (size_t)ne + 1));
-    TRY(dev_alloc((void **)&c->d_tile_count, (size_t)(IB_TILE_HDR + 2 * (n_tiles / 1024 + 2)) * sizeof(int32_t)));
     TRY(dev_alloc((void **)&c->d_status, 2 * sizeof(long long)));
     if (s == IB_OK && (cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) != cudaSuccess ||
                        cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
@@ -491,11 +493,15 @@ static ib_status coupling_step_body(ib_ctx *c, const double *x, const double *u,
             IB_CUDA_TRY(cudaEventRecord(c->ev_fork, st));
             IB_CUDA_TRY(cudaStreamWaitEvent(s2, c->ev_fork, 0));
         }
+        // the zero-fill of f is a branch of its own (third stream): neither the force nor the binning waits for it
+        cudaStream_t sz = overlap ? c->side2 : st;
+        if (overlap) IB_CUDA_TRY(cudaStreamWaitEvent(sz, c->ev_fork, 0));
         ib_prof_begin(c, IB_PHASE_ZERO, st);
-        IB_CUDA_TRY(cudaMemsetAsync(fu, 0, gb, s2));
-        IB_CUDA_TRY(cudaMemsetAsync(fv, 0, gb, s2));
-        IB_CUDA_TRY(cudaMemsetAsync(fw, 0, gb, s2));
+        IB_CUDA_TRY(cudaMemsetAsync(fu, 0, gb, sz));
+        IB_CUDA_TRY(cudaMemsetAsync(fv, 0, gb, sz));
+        IB_CUDA_TRY(cudaMemsetAsync(fw, 0, gb, sz));
         ib_prof_end(c, IB_PHASE_ZERO, st);
+        if (overlap) IB_CUDA_TRY(cudaEventRecord(c->ev_zero, sz));
         if (c->n_points > 0) {
             s = ibk_bin_reserve(c, c->n_points);
             if (s != IB_OK) return s;
@@ -509,7 +515,10 @@ static ib_status coupling_step_body(ib_ctx *c, const double *x, const double *u,
         s = ibk_fe_force(c, x, Bd, c->d_Fhat, st);
         ib_prof_end(c, IB_PHASE_FE_FORCE, st);
         if (s != IB_OK) return s;
-        if (overlap) IB_CUDA_TRY(cudaStreamWaitEvent(st, c->ev_join, 0));
+        if (overlap) {
+            IB_CUDA_TRY(cudaStreamWaitEvent(st, c->ev_join, 0));
+            IB_CUDA_TRY(cudaStreamWaitEvent(st, c->ev_zero, 0));
+        }
         if (c->n_points > 0)
             s = ibk_tiled_spread_interp(c, 1, nullptr, nullptr, c->n_points, x, c->d_Fhat, u, v, w, fu, fv, fw,
                                         c->d_Up, 1, st);

@@ -781,7 +781,7 @@ ib_status ibk_tiled_launch(ib_ctx *c, int64_t P, int do_spread, int do_interp,
     ib_tiled_params pr;
     fill_params(c, pr, P, u, v, w, fu, fv, fw, Up, slab);
     const bool with_small = slab < 0;
-    IB_CUDA_TRY(cudaMemsetAsync(c->d_tile_count + pr.wc, 0, sizeof(int32_t), st));
+    if (slab >= 0) IB_CUDA_TRY(cudaMemsetAsync(c->d_tile_count + pr.wc, 0, sizeof(int32_t), st));   // slab < 0: ibk_tile_scan has just reset counters[1]
     ib_prof_begin(c, IB_PHASE_SPREAD_INTERP, st);
     if (do_spread && do_interp) rs = launch_tiled<1, 1>(c, pr, with_small, st);
     else if (do_spread) rs = launch_tiled<1, 0>(c, pr, with_small, st);
