@@ -189,6 +189,13 @@ __device__ __forceinline__ void ib_phi4(double r, double w[4])
     w[3] = b - q;
 }
 
+// The same as the pair (a, q) the four weights are made of:  w0 = a - q, w1 = a + q, w2 = (1/2 - a) + q,
+// w3 = (1/2 - a) - q  with a = 3/8 - r/4, q = sqrt(1 + 4r - 4r^2)/8.
+__device__ __forceinline__ double2 ib_aq(double r)
+{
+    return make_double2(fma(-0.25, r, 0.375), ib_sqrt_seeded(fma(0.0625 * r, 1.0 - r, 0.015625)));
+}
+
 // scaled coordinate s = (x - x0)/h, computed as a product with 1/h plus one residual correction
 // so that it agrees with true division to ~1 ulp.
 __device__ __forceinline__ double ib_scaled(double x, double x0, double h, double inv_h)

@@ -108,12 +108,6 @@ __device__ __forceinline__ void ib_load_rec(const double *p, double v[4])
     asm volatile("ld.global.cs.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(v[0]), "=d"(v[1]), "=d"(v[2]), "=d"(v[3]) : "l"(p));
 }
 
-// (a, q) of the Peskin kernel at fraction r (see the header): w0..w3 = a-q, a+q, (1/2-a)+q, (1/2-a)-q
-__device__ __forceinline__ double2 ib_aq(double r)
-{
-    return make_double2(fma(-0.25, r, 0.375), ib_sqrt_seeded(fma(0.0625 * r, 1.0 - r, 0.015625)));
-}
-
 // 4 values along one direction of a window -> their 3 coefficients in the basis {1, a, q}
 __device__ __forceinline__ void ib_to_basis(double u0, double u1, double u2, double u3, double &s0, double &sa, double &sq)
 {
@@ -662,14 +656,14 @@ ibk_tiled_kernel(ib_tiled_params pr)
 }
 
 
-// Points of tiles with fewer than IB_SMALL_TILE points are not worth a halo and a sort: one thread per
-// point of the compact list written by ibk_tile_scan, every point treated directly against the grid.
-// 8 resident CTAs = 64 registers, 32 warps per SM: the kernel waits on dependent loads and REDs, not on issue slots,
-// so the few spilled values (<= 170 B) cost less than the warps gain (5/6/8/10/12/16 CTAs measured: DESIGN.md s.9)
+// Points of tiles with fewer than IB_SMALL_TILE points are not worth a halo and a sort: 4 lanes per point of
+// the compact list written by ibk_tile_scan, every point treated directly against the grid (ib_point_quad).
+// The spreading half is bound by the L2 reduction units (48 sectors per point), the rest by dependent loads:
+// 6 resident CTAs = 80 registers measured best on the sparse workloads (4 / 6 / 8: DESIGN.md)
 #ifndef IB_SMALL_MINB
-#define IB_SMALL_MINB 8
+#define IB_SMALL_MINB 6
 #endif
-template <int DO_SPREAD, int DO_INTERP>
+template <int DO_SPREAD, int DO_INTERP, int PER>
 __global__ void __launch_bounds__(128, IB_SMALL_MINB)
 ibk_small_tiles(ib_tiled_params pr, const int32_t *__restrict__ small_rec, const int32_t *__restrict__ counters)
 {
@@ -684,7 +678,7 @@ ibk_small_tiles(ib_tiled_params pr, const int32_t *__restrict__ small_rec, const
         double G[3] = {0, 0, 0}, U[3];
         const double *rc = pr.rec + (size_t)r * 8;
         if (DO_SPREAD) { G[0] = rc[4] * pr.ih3; G[1] = rc[5] * pr.ih3; G[2] = rc[6] * pr.ih3; }
-        ib_point_quad<DO_SPREAD, DO_INTERP>(rc[0], rc[1], rc[2], G, pr.fld, pr.frc, pr.g, pr.inv_h, q, qmask, U);
+        ib_point_quad<DO_SPREAD, DO_INTERP, PER>(rc[0], rc[1], rc[2], G, pr.fld, pr.frc, pr.g, pr.inv_h, q, qmask, U);
         if (DO_INTERP && q == 0) {
             const int id = (int)__double_as_longlong(rc[3]);
             pr.Up[id] = U[0]; pr.Up[P + id] = U[1]; pr.Up[2 * P + id] = U[2];
@@ -721,7 +715,7 @@ static ib_status launch_tiled_p(ib_ctx *c, const ib_tiled_params &pr, bool with_
         IB_CUDA_TRY(cudaEventRecord(c->ev_sfork, st));
         IB_CUDA_TRY(cudaStreamWaitEvent(s3, c->ev_sfork, 0));
     }
-    if (with_small) ibk_small_tiles<S, I><<<ib_small_blocks(nsmall_max, sms), 128, 0, s3>>>(pr, c->d_small_rec, c->d_tile_count);
+    if (with_small) ibk_small_tiles<S, I, PER><<<ib_small_blocks(nsmall_max, sms), 128, 0, s3>>>(pr, c->d_small_rec, c->d_tile_count);
     if (beside) IB_CUDA_TRY(cudaEventRecord(c->ev_sjoin, s3));
     ibk_tiled_kernel<S, I, PER><<<sms, TB, smem, st>>>(pr);
     if (beside) IB_CUDA_TRY(cudaStreamWaitEvent(st, c->ev_sjoin, 0));
@@ -801,9 +795,17 @@ ib_status ibk_small_launch(ib_ctx *c, int64_t P, int do_spread, int do_interp,
     fill_params(c, pr, P, u, v, w, fu, fv, fw, Up, -1);
     const int64_t nsmall_max = min((int64_t)P, (c->n_cells / (TT * TT * TT)) * (int64_t)(IB_SMALL_TILE - 1));
     const int nb = ib_small_blocks(nsmall_max, 0);
-    if (do_spread && do_interp) ibk_small_tiles<1, 1><<<nb, 128, 0, st>>>(pr, c->d_small_rec, c->d_tile_count);
-    else if (do_spread) ibk_small_tiles<1, 0><<<nb, 128, 0, st>>>(pr, c->d_small_rec, c->d_tile_count);
-    else ibk_small_tiles<0, 1><<<nb, 128, 0, st>>>(pr, c->d_small_rec, c->d_tile_count);
+    const bool per = c->grid.periodic != 0;
+    if (do_spread && do_interp) {
+        if (per) ibk_small_tiles<1, 1, 1><<<nb, 128, 0, st>>>(pr, c->d_small_rec, c->d_tile_count);
+        else ibk_small_tiles<1, 1, 0><<<nb, 128, 0, st>>>(pr, c->d_small_rec, c->d_tile_count);
+    } else if (do_spread) {
+        if (per) ibk_small_tiles<1, 0, 1><<<nb, 128, 0, st>>>(pr, c->d_small_rec, c->d_tile_count);
+        else ibk_small_tiles<1, 0, 0><<<nb, 128, 0, st>>>(pr, c->d_small_rec, c->d_tile_count);
+    } else {
+        if (per) ibk_small_tiles<0, 1, 1><<<nb, 128, 0, st>>>(pr, c->d_small_rec, c->d_tile_count);
+        else ibk_small_tiles<0, 1, 0><<<nb, 128, 0, st>>>(pr, c->d_small_rec, c->d_tile_count);
+    }
     c->launches += 1;
     IB_CUDA_TRY(cudaGetLastError());
     return IB_OK;
