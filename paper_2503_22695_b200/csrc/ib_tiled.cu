@@ -1,9 +1,9 @@
 // ib_tiled.cu -- variant 1 of spread (Eq.(24)-(26)) and interpolation (Eq.(27)-(29)):
-// points grouped by 4x4x4-cell tile (ib_bin.cu); persistent CTAs pull work items (runs of z-layers of one
-// tile, <= IB_CHUNK points) from a work list, keep an 8x8x8 halo of u,v,w in shared memory and hold the
-// stencil windows in registers.
+// points grouped by 4x4x4-cell tile (ib_bin.cu); one persistent, warp-specialised CTA per SM pulls work items
+// (runs of z-layers of one tile, <= IB_CHUNK points) from a work list, keeps an 8x8x8 halo of u,v,w in shared
+// memory and holds the stencil windows in registers (the producer / consumer split is described at the kernel).
 //
-// Per work item the CTA computes, one thread per point, the tile-relative scaled coordinates and from them
+// Per work item the producer warps compute, one thread per point, the tile-relative scaled coordinates and from them
 // the six 1-D delta-weight sets of the point (3 directions x {face-aligned, centre-aligned}: component c
 // lives on its own staggered lattice, MAC grid L205), once, and stores them in shared memory in half-cell
 // order ("octant", 8^3 per tile; shared-memory counting sort).  Why half-cells: in the direction d == c the
@@ -20,11 +20,11 @@
 // points, then  f0 = Ma-Mq, f1 = Ma+Mq, f2 = M0/2-Ma+Mq, f3 = M0/2-Ma-Mq.  The y and z directions of a window
 // are kept in that basis (3x3 = 9 values instead of 4x4 = 16), x stays in weight form across 4 lanes.
 //
-// Items are ordered by point count and pulled by the warps, 8 at a time.  A group of 4 lanes owns an item:
-// lane q keeps the x-column q of the window -- 9 transformed velocity values and 9 force moments -- in
-// registers and loops over the item's points: per point and lane 9 DFMA for interpolation, 12 for
+// Items are cut into units of <= PCAP points, ordered by point count and pulled by the consumer warps in
+// batches of 8 units of one component.  A group of 4 lanes owns a unit: lane q keeps the x-column q of the window -- 9 transformed velocity values and 9 force moments -- in
+// registers and loops over the unit's points: per point and lane 9 DFMA for interpolation, 12 for
 // spreading, 2 for its own x-weight, against 21 + 21 in weight form.  The moments are transformed back once
-// per item and flushed with RED.ADD.F64 straight to the grid: the 4 lanes of a group hit 4 consecutive
+// per unit and flushed with RED.ADD.F64 straight to the grid: the 4 lanes of a group hit 4 consecutive
 // faces (Blackwell has no native shared-memory fp64 add; the CAS loop measured 34 wavefronts each).
 // Tiles with fewer than IB_SMALL_TILE points skip all of this (ibk_small_tiles, ib_point.cuh).
 #include <cassert>
