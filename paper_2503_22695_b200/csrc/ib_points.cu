@@ -90,13 +90,19 @@ ibk_elem_node_sums(int64_t n_elems, int64_t P, const int32_t *__restrict__ nsub,
     double s1 = (a & 1) ? 1.0 : -1.0, s2 = (a & 2) ? 1.0 : -1.0, s3 = (a & 4) ? 1.0 : -1.0;
     double acc0 = 0.0, acc1 = 0.0, acc2 = 0.0;
     int s = 0;
+    // N_a along one direction at xi = -1 + (2m+1)/n:  1/2 (1 + s xi) = 1/2 (1 - s) + s (2m+1)/(2n) = base + m step
+    // (no division inside the loops)
+    const double r1 = 1.0 / (double)n1, r2 = 1.0 / (double)n2, r3 = 1.0 / (double)n3;
+    const double b1 = fma(0.5 * s1, r1, 0.5 - 0.5 * s1), b2 = fma(0.5 * s2, r2, 0.5 - 0.5 * s2), b3 = fma(0.5 * s3, r3, 0.5 - 0.5 * s3);
+    const double t1 = s1 * r1, t2 = s2 * r2, t3 = s3 * r3;
     for (int m3 = 0; m3 < n3; ++m3) {
-        double f3 = 0.5 * fma(s3, ib_subxi(m3, n3), 1.0);
+        const double f3 = fma((double)m3, t3, b3);
         for (int m2 = 0; m2 < n2; ++m2) {
-            double f23 = f3 * 0.5 * fma(s2, ib_subxi(m2, n2), 1.0);
+            const double f23 = f3 * fma((double)m2, t2, b2);
+#pragma unroll 4
             for (int m1 = 0; m1 < n1; ++m1, ++s) {
-                double Na = f23 * 0.5 * fma(s1, ib_subxi(m1, n1), 1.0);
-                double wn = __ldg(Wp + p0 + s) * Na;
+                const double Na = f23 * fma((double)m1, t1, b1);
+                const double wn = __ldg(Wp + p0 + s) * Na;
                 if (WITH_U) {
                     acc0 = fma(wn, __ldg(Up + p0 + s), acc0);
                     acc1 = fma(wn, __ldg(Up + P + p0 + s), acc1);
