@@ -142,7 +142,7 @@ def kernel_source_sha():
     return h.hexdigest()[:16]
 
 
-def ncu_traffic_bytes(workload_name):
+def ncu_traffic_bytes(workload_name, n_points=None):
     """(DRAM bytes per launch of the dominant kernel, source) from the newest committed ncu capture
     profiles/r*_traffic.json -- only if it was taken on THESE kernel sources (the file carries their
     sha256); otherwise (None, why): a stale capture is not a measurement of this build."""
@@ -153,9 +153,10 @@ def ncu_traffic_bytes(workload_name):
     rec = json.load(open(files[-1]))
     if rec.get("kernel_source_sha256_16") != kernel_source_sha():
         return None, f"{os.path.basename(files[-1])} was captured on other kernel sources"
-    v = rec.get("dram_bytes_per_launch", {}).get(workload_name)
+    key = workload_name if n_points is None else f"{workload_name}:{n_points}"
+    v = rec.get("dram_bytes_per_launch", {}).get(key)
     if v is None:
-        return None, f"{os.path.basename(files[-1])} has no capture of {workload_name}"
+        return None, f"{os.path.basename(files[-1])} has no capture of {key}"
     return int(v), f"ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum ({os.path.basename(files[-1])}, same kernel sources)"
 
 
@@ -372,7 +373,7 @@ def run_ours(args):
         # SURVEY.md §8(d) figure (f out, incl. its zero-fill) are the zero phase's -- a memset on another
         # stream -- so that the fraction cannot exceed 1 on sparsely filled grids
         dom_bytes = 72 * wl.n_points + 24 * wl.n_cells
-        traffic, traffic_src = ncu_traffic_bytes(wl.name)
+        traffic, traffic_src = ncu_traffic_bytes(wl.name, wl.n_points)
         # The dominant kernel is bound by the plain fp64 ALUs, not by HBM: the top-level
         # roofline is the ALU one -- algorithmic flops = 2 x 600 DFMA slots per force point (SURVEY.md
         # §8(d): weights 100 + interpolation 252 + spreading 252), peak derived from the unit count and
