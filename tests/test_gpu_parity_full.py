@@ -76,6 +76,40 @@ def test_c3_graph_replay_on_private_stream_matches_oracle(ib, orc):
     ctx.close()
 
 
+@pytest.mark.parametrize("name", ["C3", "C5-L2-s3"])
+def test_step_is_stable_over_many_replays(ib, orc, name):
+    """The tile kernel's two warp groups hand record buffers to each other through mbarriers, and no race
+    detector is available on this pool (profiles/r02_sanitizer.md): replay the captured step 300 times and
+    compare every result on the device with the first one -- B and Un bit for bit (no atomics feed them
+    except through Up, which is written once per point), f to the order of its REDs -- and the last one
+    with the oracle.  A lost update, a stale record or a buffer handed over too early shows at 1e-3."""
+    import torch
+    wl, ref = _workload(name), _oracle_step(orc, name)
+    ctx = ib.Context.from_workload(wl)
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        x, u, v, w = _t(wl.x), _t(wl.u), _t(wl.v), _t(wl.w)
+        out = [torch.empty(wl.n_cells, dtype=torch.float64, device="cuda") for _ in range(3)]
+        out += [torch.empty((3, wl.n_nodes), dtype=torch.float64, device="cuda") for _ in range(2)]     # Un, B
+        first, worst = None, 0.0
+        for it in range(300):
+            ctx.ib_coupling_step(x, u, v, w, *out, st)
+            if first is None:
+                ctx.check()
+                first = [t.clone() for t in out]
+                scale = [float(t.abs().max()) for t in first]
+                continue
+            assert torch.equal(out[3], first[3]) and torch.equal(out[4], first[4]), f"replay {it}: Un or B changed"
+            for c in range(3):
+                worst = max(worst, float((out[c] - first[c]).abs().max()) / scale[c])
+        ctx.check()
+        assert worst <= 1e-12, worst
+        for k, t in zip(("fu", "fv", "fw", "Un", "B"), out):
+            _close(t, ref[k], f"{name} after 300 replays {k}")
+    st.synchronize()
+    ctx.close()
+
+
 def test_c3_host_step_matches_oracle(ib, orc):
     """The end-to-end number of bench.py: ib_coupling_step_host at C3 (8 z-slabs of 4 tile layers, the band
     shortcut for the layers the shell cannot reach), pinned host buffers, against the oracle."""
