@@ -50,7 +50,8 @@ typedef enum {
     IB_ERR_CUDA = 4,             /* a CUDA runtime call failed (no device, launch error)                */
     IB_ERR_INVERTED_ELEMENT = 5, /* det J0 <= 0 or J <= 0 at a Gauss point (reported by ib_check)       */
     IB_ERR_NONFINITE = 6,        /* NaN/Inf position (reported by ib_check)                             */
-    IB_ERR_OUT_OF_DOMAIN = 7     /* point outside a bounded (periodic == 0) grid (reported by ib_check) */
+    IB_ERR_OUT_OF_DOMAIN = 7,    /* point outside a bounded (periodic == 0) grid (reported by ib_check) */
+    IB_ERR_TOO_LARGE = 8         /* ib_bin_sort_static: more points than its fixed scratch area holds  */
 } ib_status;
 
 /* Uniform MAC grid. periodic = 1: indices wrap in all three directions (the configs).
@@ -132,6 +133,28 @@ ib_status ib_restrict(ib_ctx *ctx, const double *Up, double *Un, void *stream);
  * Bit-exact against the definition. key_out or perm_out may be NULL. P <= 2^31-1. */
 ib_status ib_bin_sort(ib_ctx *ctx, const double *xp, int64_t P, int64_t *key_out, int32_t *perm_out,
                       void *stream);
+
+/* The same bin sort (same definition, same kernels, bit-identical key_out / perm_out) for callers that must
+ * not allocate: code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.  It takes
+ * no context and calls no cudaMalloc / cudaFree or allocating library routine: its scratch (two key and two
+ * id buffers, the digit histograms of the radix sort, the status word) lives in ONE file-scope
+ * `static __device__` array of the library, 4,260,352 bytes, which every GPU that loads the library holds
+ * until the process exits.  Hence the limit: P <= IB_BIN_SORT_STATIC_MAX_POINTS, beyond it the call returns
+ * IB_ERR_TOO_LARGE and does nothing.
+ *   grid   HOST pointer; validated like ib_create's (dimensions multiples of 8, h > 0, ...): IB_ERR_INVALID_ARG.
+ *   xp     DEVICE [3][P] (may be NULL iff P == 0); key_out DEVICE [P] or NULL; perm_out DEVICE [P] or NULL.
+ *   stream the cudaStream_t to enqueue on (NULL: the default stream); it must belong to the CURRENT device,
+ *          whose copy of the scratch array is used.
+ *   check  0: asynchronous, like ib_bin_sort.  A non-finite coordinate is binned at the grid origin (as by
+ *          ib_bin_sort) and only latched in the scratch array.  != 0: the call also synchronises the stream and
+ *          returns IB_ERR_NONFINITE if a coordinate was NaN/Inf (key_out / perm_out are still written).
+ * All calls on one device share the array, which keeps the last call's contents (the call clears the status
+ * word; every other word it reads it has written first).  Two calls that overlap on the GPU -- different
+ * streams, or two host threads -- RACE on it: serialise them (one stream, or events).  Calls on different
+ * devices are independent. */
+#define IB_BIN_SORT_STATIC_MAX_POINTS 262144
+ib_status ib_bin_sort_static(const ib_grid_desc *grid, const double *xp, int64_t P, int64_t *key_out,
+                             int32_t *perm_out, int32_t check, void *stream);
 
 /* (2) Spread, Eq.(24)-(26): f_c[face] (+)= sum_s Gp_{s,c} delta_h(x_face - xp_s), delta_h =
  * h^-3 phi phi phi on component c's own staggered lattice. accumulate == 0 zero-fills fu,fv,fw

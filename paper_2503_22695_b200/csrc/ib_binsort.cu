@@ -286,3 +286,104 @@ ib_status ibk_bin_sort(ib_ctx *c, const double *xp, int64_t P, int64_t *key_out,
     IB_CUDA_TRY(cudaGetLastError());
     return IB_OK;
 }
+
+// ---- ib_bin_sort_static: the same sort without a context and without any allocation ------------------------
+// (include/ibcouple.h).  The kernels are the ones above; the scratch that ibk_sort_reserve takes from cudaMalloc
+// is ONE file-scope device array here, sized for IB_BIN_SORT_STATIC_MAX_POINTS points.  Every GPU that loads
+// the library holds it until the process exits; all calls on a device share it.
+#include <cmath>
+#include <mutex>
+
+#define IBS_MAXP IB_BIN_SORT_STATIC_MAX_POINTS
+#define IBS_NB ((IBS_MAXP + RS_TILE - 1) / RS_TILE)            // blocks of the histogram / scatter kernels at the limit
+#define IBS_HL (256 * IBS_NB)                                  // histogram entries
+#define IBS_NSUM ((IBS_HL + SC_TILE - 1) / SC_TILE)            // block sums of the scan
+// layout, in 32-bit words; every part starts on a 256-byte boundary
+#define IBS_OFF_STATUS 0                                       // 2 x 64 bit: the status latch (ib_latch)
+#define IBS_OFF_KEY 64                                         // [2][IBS_MAXP] keys, ping and pong
+#define IBS_OFF_VAL (IBS_OFF_KEY + 2 * IBS_MAXP)               // [2][IBS_MAXP] point ids
+#define IBS_OFF_HIST (IBS_OFF_VAL + 2 * IBS_MAXP)              // [256][blocks] digit counts
+#define IBS_OFF_SUMS (IBS_OFF_HIST + IBS_HL)                   // [IBS_NSUM]
+#define IBS_WORDS (IBS_OFF_SUMS + ((IBS_NSUM + 63) & ~63))
+static_assert(IBS_MAXP % 64 == 0 && IBS_HL % 64 == 0, "parts of the scratch array stay 256-byte aligned");
+static_assert(IBS_WORDS * 4ll == 4260352ll, "include/ibcouple.h and README.md state this size");
+
+static __device__ __align__(256) uint32_t ib_static_scratch[IBS_WORDS];
+
+// In host code `ib_static_scratch` is a stand-in for the symbol, not a device address: the address comes from
+// cudaGetSymbolAddress, once per device, with that device current.
+#define IBS_MAX_DEVICES 64
+static std::mutex ibs_mutex;
+static uint32_t *ibs_dev_ptr[IBS_MAX_DEVICES];
+
+static ib_status ibs_scratch(uint32_t **out)
+{
+    int dev = -1;
+    IB_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= IBS_MAX_DEVICES) return IB_ERR_UNSUPPORTED;
+    std::lock_guard<std::mutex> lock(ibs_mutex);
+    if (!ibs_dev_ptr[dev]) {
+        void *p = nullptr;
+        IB_CUDA_TRY(cudaGetSymbolAddress(&p, ib_static_scratch));
+        if (!p) return IB_ERR_CUDA;
+        ibs_dev_ptr[dev] = static_cast<uint32_t *>(p);
+    }
+    *out = ibs_dev_ptr[dev];
+    return IB_OK;
+}
+
+extern "C" ib_status ib_bin_sort_static(const ib_grid_desc *g, const double *xp, int64_t P, int64_t *key_out,
+                                        int32_t *perm_out, int32_t check, void *stream)
+{
+    if (!g || P < 0 || (P > 0 && !xp)) return IB_ERR_INVALID_ARG;
+    if (g->nx <= 0 || g->ny <= 0 || g->nz <= 0 || (g->nx % IB_TILE) || (g->ny % IB_TILE) || (g->nz % IB_TILE))
+        return IB_ERR_INVALID_ARG;
+    if (!(g->h > 0.0) || !std::isfinite(g->h) || !std::isfinite(g->x0) || !std::isfinite(g->y0) || !std::isfinite(g->z0))
+        return IB_ERR_INVALID_ARG;
+    const int64_t n_cells = (int64_t)g->nx * g->ny * g->nz;
+    if (n_cells > (int64_t)INT32_MAX) return IB_ERR_INVALID_ARG;
+    if (P > (int64_t)IBS_MAXP) return IB_ERR_TOO_LARGE;        // the scratch array holds no more
+    uint32_t *scr = nullptr;
+    ib_status rs = ibs_scratch(&scr);
+    if (rs != IB_OK) return rs;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    long long *status = reinterpret_cast<long long *>(scr + IBS_OFF_STATUS);
+    uint32_t *key[2] = {scr + IBS_OFF_KEY, scr + IBS_OFF_KEY + IBS_MAXP};
+    int32_t *val[2] = {reinterpret_cast<int32_t *>(scr + IBS_OFF_VAL), reinterpret_cast<int32_t *>(scr + IBS_OFF_VAL + IBS_MAXP)};
+    uint32_t *hist = scr + IBS_OFF_HIST, *sums = scr + IBS_OFF_SUMS;
+    // the array keeps the last call's contents.  The status word must start at zero; everything else that is
+    // read below is written first (keys and ids [0, P), all 256 x nb histogram entries, all nsum block sums)
+    IB_CUDA_TRY(cudaMemsetAsync(status, 0, 2 * sizeof(long long), st));
+    if (P > 0) {
+        ibk_keys<<<ib_blocks(P, 256), 256, 0, st>>>(P, xp, *g, 1.0 / g->h, key[0], key_out, status);
+        int bits = 1;
+        while ((1ll << bits) < n_cells) ++bits;
+        const int passes = (bits + 7) / 8;
+        const int nb = (int)((P + RS_TILE - 1) / RS_TILE);
+        const int64_t hl = 256ll * nb;
+        const int nsum = (int)((hl + SC_TILE - 1) / SC_TILE);
+        int cur = 0;
+        for (int ps = 0; ps < passes; ++ps) {
+            const int shift = 8 * ps;
+            ibk_radix_hist<<<nb, RS_THREADS, 0, st>>>(key[cur], P, shift, hist, nb);
+            ibk_scan_reduce<<<nsum, SC_THREADS, 0, st>>>(hist, hl, sums);
+            ibk_scan_sums<<<1, 1024, 0, st>>>(sums, nsum);
+            ibk_scan_apply<<<nsum, SC_THREADS, 0, st>>>(hist, hl, sums);
+            ibk_radix_scatter<<<nb, RS_THREADS, 0, st>>>(key[cur], ps == 0 ? nullptr : val[cur], key[cur ^ 1], val[cur ^ 1],
+                                                         P, shift, hist, nb);
+            cur ^= 1;
+        }
+        if (perm_out) ibk_copy_perm<<<ib_blocks(P, 256), 256, 0, st>>>(val[cur], perm_out, P);
+        IB_CUDA_TRY(cudaGetLastError());
+    }
+    if (check) {
+        unsigned long long w[2] = {0, 0};
+        IB_CUDA_TRY(cudaMemcpyAsync(w, status, sizeof(w), cudaMemcpyDeviceToHost, st));
+        IB_CUDA_TRY(cudaStreamSynchronize(st));
+        int code = 0;
+        long long id = -1;
+        ib_status_unpack(w[0], &code, &id);
+        if (code != 0) return static_cast<ib_status>(code);
+    }
+    return IB_OK;
+}

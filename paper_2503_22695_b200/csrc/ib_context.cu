@@ -95,6 +95,7 @@ extern "C" const char *ib_status_string(ib_status s)
     case IB_ERR_INVERTED_ELEMENT: return "IB_ERR_INVERTED_ELEMENT";
     case IB_ERR_NONFINITE: return "IB_ERR_NONFINITE";
     case IB_ERR_OUT_OF_DOMAIN: return "IB_ERR_OUT_OF_DOMAIN";
+    case IB_ERR_TOO_LARGE: return "IB_ERR_TOO_LARGE";
     }
     return "IB_ERR_UNKNOWN";
 }

@@ -16,10 +16,10 @@ _SO = os.path.join(_HERE, "libibcouple.so")
 _lib = None
 
 STATUS = {0: "IB_OK", 1: "IB_ERR_INVALID_ARG", 2: "IB_ERR_UNSUPPORTED", 3: "IB_ERR_ALLOC", 4: "IB_ERR_CUDA",
-          5: "IB_ERR_INVERTED_ELEMENT", 6: "IB_ERR_NONFINITE", 7: "IB_ERR_OUT_OF_DOMAIN"}
+          5: "IB_ERR_INVERTED_ELEMENT", 6: "IB_ERR_NONFINITE", 7: "IB_ERR_OUT_OF_DOMAIN", 8: "IB_ERR_TOO_LARGE"}
 
 EXPORTS = ["ib_create", "ib_destroy", "ib_num_points", "ib_num_nodes", "ib_num_elems", "ib_fe_force",
-           "ib_points", "ib_restrict", "ib_bin_sort", "ib_spread", "ib_interp", "ib_coupling_step",
+           "ib_points", "ib_restrict", "ib_bin_sort", "ib_bin_sort_static", "ib_spread", "ib_interp", "ib_coupling_step",
            "ib_coupling_step_host", "ib_coupling_step_host3", "ib_step_eq16", "ib_check", "ib_launch_count", "ib_set_variant", "ib_set_graph", "ib_set_tethers", "ib_set_surface", "ib_set_loads", "ib_probe_dfma",
            "ib_profile_enable", "ib_profile_read",
            "ib_status_string"]
@@ -65,6 +65,7 @@ def lib():
         L.ib_points.argtypes = [vp, vp, vp, vp, vp, vp]
         L.ib_restrict.argtypes = [vp, vp, vp, vp]
         L.ib_bin_sort.argtypes = [vp, vp, i64, vp, vp, vp]
+        L.ib_bin_sort_static.argtypes = [C.POINTER(GridDesc), vp, i64, vp, vp, i32, vp]
         L.ib_spread.argtypes = [vp, vp, vp, i64, vp, vp, vp, i32, vp]
         L.ib_interp.argtypes = [vp, vp, i64, vp, vp, vp, vp, vp]
         L.ib_coupling_step.argtypes = [vp] * 11
@@ -104,6 +105,18 @@ def _stream(stream):
     if stream is None:
         stream = torch.cuda.current_stream()
     return C.c_void_p(stream.cuda_stream)
+
+
+BIN_SORT_STATIC_MAX_POINTS = 262144      # IB_BIN_SORT_STATIC_MAX_POINTS of include/ibcouple.h
+
+
+def ib_bin_sort_static(grid, xp, P, key_out, perm_out, check=0, stream=None):
+    """ib_bin_sort without a context and without any allocation (fixed scratch area inside the library);
+    grid = (nx, ny, nz, h, (x0, y0, z0), periodic).  Raises IbError (IB_ERR_TOO_LARGE beyond the limit)."""
+    nx, ny, nz, h, org, periodic = grid
+    g = GridDesc(int(nx), int(ny), int(nz), float(h), float(org[0]), float(org[1]), float(org[2]), int(periodic))
+    _chk(lib().ib_bin_sort_static(C.byref(g), _dp(xp), int(P), _dp(key_out), _dp(perm_out), int(check), _stream(stream)),
+         "ib_bin_sort_static")
 
 
 def probe_dfma(device=0):
