@@ -28,6 +28,7 @@
 // faces (Blackwell has no native shared-memory fp64 add; the CAS loop measured 34 wavefronts each).
 // Tiles with fewer than IB_SMALL_TILE points skip all of this (ibk_small_tiles, ib_point.cuh).
 #include <cassert>
+#include <cuda.h>               // CUtensorMap and its enums only: the encoder is fetched through the runtime, libcuda is not linked
 #include "ib_point.cuh"
 
 #define TT 4                    // tile edge in cells
@@ -38,10 +39,10 @@
 #define TB 512                  // threads per CTA: one CTA per SM, 16 warps
 #define NWARP (TB / 32)
 #ifndef IB_TILED_PRODUCER_WARPS
-#define IB_TILED_PRODUCER_WARPS 8   // of the 16 warps (the others run the items); 4 / 5 / 6 measured
+#define IB_TILED_PRODUCER_WARPS 6   // of the 16 warps (the others run the items); 5 / 7 / 8 measured
 #endif
 #define CH IB_CHUNK             // records staged per work item
-#define SZ 68                   // z-plane stride of the halo in doubles (64 + 4: the 4 lanes of a group hit distinct banks)
+#define SZ 64                   // z-plane stride of the halo in doubles: dense 8 x 8 x 8, the layout a TMA box load writes
 #define SU3 (TH * SZ)           // one component of the halo
 #ifndef PCAP
 #define PCAP 32                 // an item with more points is cut into units of PCAP points (each with a window of its own)
@@ -60,6 +61,8 @@ struct ib_tiled_params {
     int wb, we, wc;             // this launch covers the work items counters[wb] <= w < counters[we]; counters[wc] counts them
     ib_grid_desc g;
     double inv_h, ih3;
+    int use_tma;                // tm[] are valid: the halo of a tile that does not wrap comes by one TMA box load per component
+    alignas(64) CUtensorMap tm[3];   // u, v, w as 3-D fp64 tensors (nx, ny, nz), box 8 x 8 x 8, out-of-range elements read as zero
 };
 
 // decode an item: component c, shifted-cell coordinates l[3]  (c*100 + (l2*ny + l1)*nx + l0 with
@@ -315,7 +318,8 @@ __device__ __forceinline__ void ib_run_batch(int C, const ib_tiled_params &pr, c
 
 // ---- warp-specialised persistent kernel ----------------------------------------------------------------
 // One CTA per SM, 16 warps: NPW "producer" warps turn work items into shared-memory records (coordinates ->
-// half-cell sort -> (a,q) sets, runs and ordered units of the items, halo), NCW "consumer" warps run the
+// half-cell sort -> (a,q) sets, runs and ordered units of the items; one thread starts the TMA box loads of the
+// halo, whose bytes the consumers await on a barrier of their own), NCW "consumer" warps run the
 // batches of units.  Two record buffers: the producers fill buffer k+1 while the consumers work through
 // buffer k.  full[b] / empty[b] are mbarriers (producers -> consumers: one arrival; consumers -> producers:
 // one per consumer warp).  No barrier ever joins the two groups: a consumer warp that finds no more batches
@@ -337,14 +341,14 @@ __device__ __forceinline__ void ib_run_batch(int C, const ib_tiled_params &pr, c
 #define OFF_SIDS (OFF_RUNS + (NITEM + 1) * 16)
 #define OFF_ORDER (OFF_SIDS + CH * 4)
 #define OFF_CTL (OFF_ORDER + ((3 * NORD * 2 + 15) & ~15))
-#define BUF_BYTES (OFF_CTL + 32)                        // ctl: {nbatch, ncomp[3], next, h0[3]}
+#define BUF_BYTES ((OFF_CTL + 48 + 127) & ~127)          // ctl: {nbatch, ncomp[3], next, h0[3], halo barrier phase + 1 or 0}; the halo of the next buffer stays 128-byte aligned
 // after the two buffers: producer-private scratch and the static window table
 #define OFF_OCCNT (2 * BUF_BYTES)
 #define OFF_BINS (OFF_OCCNT + NOC * 4)
 #define OFF_OCSTART (OFF_BINS + ((3 * NBIN * 4 + 15) & ~15))
 #define OFF_WIN (OFF_OCSTART + ((516 * 2 + 15) & ~15))
 #define OFF_MISC (OFF_WIN + ((NITEM + 1) * 4 + 15) / 16 * 16)      // wsum[NPW], work slots int4[2], mbarriers
-#define TILED_SMEM_BYTES (OFF_MISC + 16 * 4 + 2 * 16 + 4 * 8)
+#define TILED_SMEM_BYTES (OFF_MISC + 16 * 4 + 2 * 16 + 6 * 8)
 
 __device__ __forceinline__ void ib_mbar_init(unsigned a, unsigned count)
 {
@@ -363,6 +367,16 @@ __device__ __forceinline__ void ib_mbar_wait(unsigned a, unsigned parity)
                  "bra IB_MBAR_WAIT;\n"
                  "IB_MBAR_DONE:\n\t}" ::"r"(a), "r"(parity) : "memory");
 }
+__device__ __forceinline__ void ib_mbar_expect_tx(unsigned a, unsigned bytes)
+{
+    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n\t}" ::"r"(a), "r"(bytes) : "memory");
+}
+// one 8 x 8 x 8 box of a 3-D tensor -> shared memory; elements outside the tensor arrive as zeros
+__device__ __forceinline__ void ib_tma_box(unsigned dst, const CUtensorMap *tm, int x, int y, int z, unsigned bar)
+{
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+                 ::"r"(dst), "l"(tm), "r"(x), "r"(y), "r"(z), "r"(bar) : "memory");
+}
 __device__ __forceinline__ void ib_producer_sync()
 {
     asm volatile("bar.sync 1, %0;" ::"n"(TBP) : "memory");
@@ -371,16 +385,16 @@ __device__ __forceinline__ void ib_producer_sync()
 // PER: periodic grid (compile-time, so that the periodic kernel carries none of the wall predicates)
 template <int DO_SPREAD, int DO_INTERP, int PER>
 __global__ void __launch_bounds__(TB, 1)
-ibk_tiled_kernel(ib_tiled_params pr)
+ibk_tiled_kernel(const __grid_constant__ ib_tiled_params pr)
 {
-    extern __shared__ __align__(16) unsigned char smraw[];
+    extern __shared__ __align__(1024) unsigned char smraw[];
     int *oc_cnt = reinterpret_cast<int *>(smraw + OFF_OCCNT);                       // [NOC] points per half-cell
     int *bins = reinterpret_cast<int *>(smraw + OFF_BINS);                          // [3][NBIN] units per component and point count
     unsigned short *oc_start = reinterpret_cast<unsigned short *>(smraw + OFF_OCSTART);   // [516] first record of a half-cell
     unsigned *item_win = reinterpret_cast<unsigned *>(smraw + OFF_WIN);             // [NITEM + 1] window of an item: halo offset | o3x << 16 | o3y << 20 | o3z << 24
     int *wsum = reinterpret_cast<int *>(smraw + OFF_MISC);                          // [16]
     int4 *s_wk = reinterpret_cast<int4 *>(smraw + OFF_MISC + 64);                   // work item of the even / odd iteration
-    const unsigned mbar = (unsigned)__cvta_generic_to_shared(smraw + OFF_MISC + 96);   // full[0], full[1], empty[0], empty[1]
+    const unsigned mbar = (unsigned)__cvta_generic_to_shared(smraw + OFF_MISC + 96);   // full[0], full[1], empty[0], empty[1], halo[0], halo[1]
 
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int n[3] = {pr.g.nx, pr.g.ny, pr.g.nz};
@@ -388,6 +402,8 @@ ibk_tiled_kernel(ib_tiled_params pr)
     if (tid == 0) {
         ib_mbar_init(mbar + 0, 1); ib_mbar_init(mbar + 8, 1);
         ib_mbar_init(mbar + 16, NCW); ib_mbar_init(mbar + 24, NCW);
+        ib_mbar_init(mbar + 32, 1); ib_mbar_init(mbar + 40, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");      // the TMA unit sees the initialised barriers
         const int w = pr.counters[pr.wb] + atomicAdd(&pr.counters[pr.wc], 1);
         s_wk[0] = (w < pr.counters[pr.we]) ? __ldg(pr.work + w) : make_int4(-1, 0, 0, 0);
     }
@@ -406,6 +422,7 @@ ibk_tiled_kernel(ib_tiled_params pr)
     if (wid < NPW) {
         // =================================== producers ==========================================================
         const double org[3] = {pr.g.x0, pr.g.y0, pr.g.z0};
+        unsigned halo_phase = 0;                         // bit b: phase of halo[b] that the next TMA load into buffer b completes
         for (int iter = 0;; ++iter) {
             const int b = iter & 1;
             unsigned char *buf = smraw + b * BUF_BYTES;
@@ -499,8 +516,29 @@ ibk_tiled_kernel(ib_tiled_params pr)
             int h0[3];                                       // halo origin (global index of halo entry 0), wrapped
 #pragma unroll
             for (int d = 0; d < 3; ++d) h0[d] = PER ? ib_wrap(TT * t3[d] - 2, n[d]) : TT * t3[d] - 2;
-            // ---- halo: asynchronous copies straight into shared memory
+            // ---- halo: one TMA box load per component (8 x 8 x 8 doubles; what lies outside a bounded grid arrives as
+            // zeros, which is what A26 asks for); the halo of a tile at the edge of a periodic grid wraps around, which a
+            // box cannot: it is put together from asynchronous 8-byte copies, as is every halo when there are no tensor maps
+            bool tma = false;
             if (DO_INTERP) {
+                tma = pr.use_tma != 0;
+                if (PER) {
+#pragma unroll
+                    for (int d = 0; d < 3; ++d) tma = tma && t3[d] > 0 && TT * t3[d] + 6 <= n[d];
+                }
+            }
+            int halo_tag = 0;                                // phase of halo[b] + 1 for the consumers to wait on; 0: none
+            if (DO_INTERP && tma) {
+                halo_tag = 1 + (int)((halo_phase >> b) & 1u);
+                halo_phase ^= 1u << b;
+                if (tid == 0) {
+                    const unsigned hb = mbar + 32 + 8 * b, dst = (unsigned)__cvta_generic_to_shared(su);
+                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // earlier generic-proxy accesses to the buffer come first
+                    ib_mbar_expect_tx(hb, 3 * TH3 * 8);
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) ib_tma_box(dst + c * (SU3 * 8), &pr.tm[c], TT * t3[0] - 2, TT * t3[1] - 2, TT * t3[2] - 2, hb);
+                }
+            } else if (DO_INTERP) {
                 for (int idx = tid; idx < 3 * TH3; idx += TBP) {
                     int c = idx >> 9, r = idx & 511;
                     int i = h0[0] + (r & 7), j = h0[1] + ((r >> 3) & 7), k = h0[2] + (r >> 6);
@@ -608,6 +646,7 @@ ibk_tiled_kernel(ib_tiled_params pr)
                     ctl[1] = ncomp[0]; ctl[2] = ncomp[1]; ctl[3] = ncomp[2];
                     ctl[4] = 0;                                  // batch counter
                     ctl[5] = h0[0]; ctl[6] = h0[1]; ctl[7] = h0[2];
+                    ctl[8] = halo_tag;
                     ctl[0] = 3 * ((max(ncomp[0], max(ncomp[1], ncomp[2])) + 7) >> 3);
                 }
             }
@@ -629,6 +668,7 @@ ibk_tiled_kernel(ib_tiled_params pr)
             if (nbatch < 0) break;
             const int ncomp[3] = {ctl[1], ctl[2], ctl[3]};
             const int h0[3] = {ctl[5], ctl[6], ctl[7]};
+            if (DO_INTERP && ctl[8] != 0) ib_mbar_wait(mbar + 32 + 8 * b, (unsigned)(ctl[8] - 1));      // the halo came by TMA: wait for its bytes
             const unsigned short *order = reinterpret_cast<const unsigned short *>(buf + OFF_ORDER);
             ib_tile_smem sm;
             sm.su = (unsigned)__cvta_generic_to_shared(buf + OFF_SU); sm.sets = (unsigned)__cvta_generic_to_shared(buf + OFF_SETS);
@@ -747,9 +787,46 @@ ib_status ibk_tiled_spread_interp(ib_ctx *c, int mesh, const double *xp, const d
     return ibk_tiled_launch(c, P, spread, Up != nullptr, u, v, w, fu, fv, fw, Up, -1, st);
 }
 
+// cuTensorMapEncodeTiled of the driver, through the runtime's entry-point query (the library does not link libcuda)
+typedef CUresult (*ib_tma_encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                     const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                     CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static ib_tma_encode_fn ib_tma_encoder()
+{
+    static ib_tma_encode_fn fn = []() -> ib_tma_encode_fn {
+        void *f = nullptr;
+        cudaDriverEntryPointQueryResult q = cudaDriverEntryPointSymbolNotFound;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess) {
+            (void)cudaGetLastError();
+            return nullptr;
+        }
+        return reinterpret_cast<ib_tma_encode_fn>(f);
+    }();
+    return fn;
+}
+
+// u, v, w as 3-D tensors for the halo loads of the tile kernel.  Returns false (the kernel then copies every halo
+// element by element) when the driver has no encoder or refuses the arrays: a pointer that is not 16-byte aligned.
+static bool ib_halo_maps(const ib_grid_desc &g, const double *const fld[3], CUtensorMap tm[3])
+{
+    ib_tma_encode_fn enc = ib_tma_encoder();
+    if (!enc) return false;
+    const cuuint64_t dims[3] = {(cuuint64_t)g.nx, (cuuint64_t)g.ny, (cuuint64_t)g.nz};
+    const cuuint64_t strides[2] = {(cuuint64_t)g.nx * 8, (cuuint64_t)g.nx * g.ny * 8};
+    const cuuint32_t box[3] = {TH, TH, TH}, estr[3] = {1, 1, 1};
+    for (int c = 0; c < 3; ++c) {
+        if (!fld[c] || (reinterpret_cast<uintptr_t>(fld[c]) & 15u)) return false;
+        if (enc(&tm[c], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<double *>(fld[c]), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+            return false;
+    }
+    return true;
+}
+
 static void fill_params(ib_ctx *c, ib_tiled_params &pr, int64_t P, const double *u, const double *v, const double *w,
                         double *fu, double *fv, double *fw, double *Up, int slab)
 {
+    memset(&pr, 0, sizeof(pr));
     pr.rec = c->d_rec; pr.P = P;
     pr.fld[0] = u; pr.fld[1] = v; pr.fld[2] = w;
     pr.frc[0] = fu; pr.frc[1] = fv; pr.frc[2] = fw;
@@ -759,6 +836,7 @@ static void fill_params(ib_ctx *c, ib_tiled_params &pr, int64_t P, const double 
     pr.we = slab < 0 ? 0 : IB_SLAB0 + slab + 1;
     pr.wc = slab < 0 ? 1 : IB_SLABC0 + slab;
     pr.g = c->grid; pr.inv_h = c->inv_h; pr.ih3 = c->inv_h * c->inv_h * c->inv_h;
+    pr.use_tma = (u && v && w && Up) ? (ib_halo_maps(c->grid, pr.fld, pr.tm) ? 1 : 0) : 0;
 }
 
 // The tile kernel (and the direct path of the sparse tiles) over records that are already binned.

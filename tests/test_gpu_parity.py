@@ -156,6 +156,42 @@ def test_spread_interp_generic_cloud(ib, orc, variant):
     ctx.close()
 
 
+@pytest.mark.parametrize("periodic", [1, 0])
+def test_interp_halo_by_tma_and_by_copies_agree(ib, orc, periodic):
+    """The tile kernel loads the 8^3 velocity halo of a tile by TMA box loads (zero fill outside a bounded grid)
+    and falls back to element copies for tiles at the wrap of a periodic grid and for arrays that are not
+    16-byte aligned: both must give the same bits, and the oracle's values."""
+    import torch
+    n, h, org = (32, 24, 40), 0.1, (0.3, -0.2, 1.0)
+    ctx = ib.Context(*n, h, org, np.zeros((0, 8), np.int32), np.zeros((3, 0)), None, None, None, [], periodic=periodic)
+    g = orc.make_grid(*n, h, org, periodic=periodic)
+    rng = np.random.default_rng(77 + periodic)
+    L = np.array(n) * h
+    P = 150001                                                 # ~5 points per cell: every tile goes through the tile kernel
+    lo, hi = (-0.1, 1.1) if periodic else (0.0, 1.0)
+    xp = np.asarray(org)[:, None] + rng.uniform(lo, hi, (3, P)) * L[:, None]
+    if not periodic:
+        xp = np.minimum(xp, (np.asarray(org) + L * (1 - 1e-12))[:, None])
+    ncell = n[0] * n[1] * n[2]
+    uvw = rng.normal(size=(3, ncell))
+    x_d = _t(xp)
+    Up = torch.empty((3, P), dtype=torch.float64, device="cuda")
+    ctx.ib_interp(x_d, P, _t(uvw[0]), _t(uvw[1]), _t(uvw[2]), Up)                   # aligned arrays: TMA where the tile allows
+    ctx.check()
+    _close(Up, orc.interp(g, xp, *uvw), "interp, aligned arrays")
+    shifted = []
+    for c in range(3):                                                              # the same values at an address = 8 mod 16
+        big = torch.empty(ncell + 1, dtype=torch.float64, device="cuda")
+        big[1:] = _t(uvw[c])
+        assert big[1:].data_ptr() % 16 == 8
+        shifted.append(big[1:])
+    Up2 = torch.empty((3, P), dtype=torch.float64, device="cuda")
+    ctx.ib_interp(x_d, P, *shifted, Up2)
+    ctx.check()
+    assert torch.equal(Up, Up2)
+    ctx.close()
+
+
 def test_bin_sort_bit_exact(ib, orc):
     import torch
     for n, P in (((16, 8, 24), 0), ((16, 8, 24), 1), ((16, 8, 24), 5000), ((64, 64, 64), 300007)):
