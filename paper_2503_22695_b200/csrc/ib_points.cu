@@ -211,6 +211,69 @@ ibk_restrict_rows(int64_t n_rows, int64_t P, int n1r, int n2, int n3, const doub
     }
 }
 
+// The restriction for a uniform nsub whose rows-per-element n2*n3 is NOT a power of two (3^3, 5^3, 6^3 ...): a
+// butterfly over the rows of an element does not close, so the rows meet in shared memory.  A CTA takes
+// 256 / (n2 n3) whole elements; phase 1: one thread per row (e, m2, m3), coalesced reads of W_s and Up, the sum over
+// m1 against the two x-shape functions (6 values per row); phase 2: 6 threads per element -- (x-side of the node, component)
+// -- add the rows up in fixed order with the y and z shape functions, four nodes each.  Same sums as ibk_elem_node_sums in another
+// order, one pass over the points instead of eight.
+__global__ void __launch_bounds__(256)
+ibk_restrict_rows_smem(int64_t n_elems, int64_t P, int n1, int n2, int n3, const double *__restrict__ Wp,
+                       const double *__restrict__ Up, double *__restrict__ Ce, int64_t ne8)
+{
+    __shared__ double sA[256 * 7];                     // [row of the CTA][A0[3], A1[3], pad]
+    const int rpe = n2 * n3, epc = 256 / rpe;
+    const int tid = threadIdx.x;
+    const int64_t e0 = (int64_t)blockIdx.x * epc;
+    if (tid < epc * rpe) {
+        const int64_t e = e0 + tid / rpe;
+        double A0[3] = {0, 0, 0}, A1[3] = {0, 0, 0};
+        if (e < n_elems) {
+            const int64_t p0 = (e0 * rpe + tid) * (int64_t)n1;
+            const double rn = 1.0 / (double)n1;
+            for (int j = 0; j < n1; ++j) {
+                const double t = ((double)j + 0.5) * rn;           // 1/2 (1 + xi_j)
+                const double W = __ldg(Wp + p0 + j);
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    const double wu = W * __ldg(Up + (int64_t)c * P + p0 + j);
+                    A1[c] = fma(wu, t, A1[c]);
+                    A0[c] = fma(wu, 1.0 - t, A0[c]);
+                }
+            }
+        }
+#pragma unroll
+        for (int c = 0; c < 3; ++c) { sA[tid * 7 + c] = A0[c]; sA[tid * 7 + 3 + c] = A1[c]; }
+    }
+    __syncthreads();
+    // phase 2: thread = (element, x-side ia, component); it walks the element's rows once and forms the four
+    // (ja, ka) sums of its column of nodes together
+    if (tid < epc * 6) {
+        const int el = tid / 6, k = tid - el * 6, ia = k / 3, c = k - ia * 3;
+        const int64_t e = e0 + el;
+        if (e >= n_elems) return;
+        const double r2 = 1.0 / (double)n2, r3 = 1.0 / (double)n3;
+        const double *row = sA + (el * rpe) * 7 + ia * 3 + c;
+        double acc[2][2] = {{0.0, 0.0}, {0.0, 0.0}};      // [ka][ja]
+        double t3 = 0.5 * r3;
+        for (int m3 = 0; m3 < n3; ++m3, t3 += r3) {
+            double p0 = 0.0, p1 = 0.0, t2 = 0.5 * r2;
+            for (int m2 = 0; m2 < n2; ++m2, t2 += r2) {
+                const double v = row[(m3 * n2 + m2) * 7];
+                p1 = fma(t2, v, p1);
+                p0 = fma(1.0 - t2, v, p0);
+            }
+            acc[0][0] = fma(1.0 - t3, p0, acc[0][0]); acc[0][1] = fma(1.0 - t3, p1, acc[0][1]);
+            acc[1][0] = fma(t3, p0, acc[1][0]); acc[1][1] = fma(t3, p1, acc[1][1]);
+        }
+        double *out = Ce + c * ne8 + e * 8 + ia;
+#pragma unroll
+        for (int ka = 0; ka < 2; ++ka)
+#pragma unroll
+            for (int ja = 0; ja < 2; ++ja) out[2 * ja + 4 * ka] = acc[ka][ja];
+    }
+}
+
 // per node gather of Ce; mode 0: w_a = sum ; mode 1: Un_c = sum_c / w_a
 template <int WITH_U>
 __global__ void __launch_bounds__(256)
@@ -315,6 +378,12 @@ ib_status ibk_restrict(ib_ctx *c, const double *Up, double *Un, cudaStream_t st)
         else
             ibk_restrict_rows<0><<<ib_blocks(c->n_rows, 256), 256, 0, st>>>(c->n_rows, c->n_points, c->un[0], c->un[1],
                                                                           c->un[2], c->d_Wp, Up, c->d_Ce, c->n_elems * 8);
+    }
+    else if (c->un[0] > 0 && rpe <= 256)
+    {
+        const int epc = 256 / rpe;
+        ibk_restrict_rows_smem<<<ib_blocks(c->n_elems, epc), 256, 0, st>>>(c->n_elems, c->n_points, c->un[0], c->un[1], c->un[2],
+                                                                          c->d_Wp, Up, c->d_Ce, c->n_elems * 8);
     }
     else
         ibk_elem_node_sums<1><<<ib_blocks(c->n_elems * 8, 256), 256, 0, st>>>(

@@ -117,6 +117,37 @@ def test_fe_force_pieces_and_determinism(ib, orc):
     ctx.close()
 
 
+@pytest.mark.parametrize("sub", [(3, 3, 3), (5, 5, 5), (6, 6, 6), (2, 3, 5), (7, 8, 8), (4, 4, 4), (3, 4, 2), (1, 1, 1)])
+def test_restrict_uniform_subpoint_counts(ib, orc, sub):
+    """ib_restrict takes one of three kernels by the sub-point rule: rows-per-element a power of
+    two (shuffles), any other uniform rule (rows meet in shared memory; CTAs of 256 / (n2 n3) elements -- 59 elements
+    leave a ragged last CTA for every rule here), ragged rules (test_fe_force_pieces_and_determinism)."""
+    import torch
+    conn, X, x, fib = distorted_block(5, 4, 3, seed=21)
+    conn, fib = conn[:59], fib[:, :59]                           # 59 elements: not a multiple of any CTA's element count
+    ne, nn = conn.shape[0], X.shape[1]
+    used = np.unique(conn)
+    remap = -np.ones(nn, np.int64); remap[used] = np.arange(used.size)
+    conn, X, x = remap[conn].astype(np.int32), X[:, used], x[:, used]
+    nn = X.shape[1]
+    nsub = np.tile(np.array(sub, np.int32), (ne, 1))
+    mats = [W.material(W.LAW_NEOHOOKEAN, a=1e4, kappa=1e6)]
+    ctx = ib.Context(16, 16, 16, 1 / 16, (0, 0, 0), conn, X, fib, np.zeros(ne, np.int32), nsub, mats)
+    xp_r, Wp_r, wa_r = orc.points(conn, X, x, nsub)
+    P = ctx.n_points
+    assert P == ne * sub[0] * sub[1] * sub[2]
+    rng = np.random.default_rng(5)
+    Up = rng.normal(size=(3, P))
+    Un = torch.empty((3, nn), dtype=torch.float64, device="cuda")
+    ctx.ib_restrict(_t(Up), Un)
+    ctx.check()
+    _close(Un, orc.restrict(conn, nsub, wa_r, Wp_r, Up), f"Un {sub}")
+    Un2 = torch.empty_like(Un)
+    ctx.ib_restrict(_t(Up), Un2)
+    assert torch.equal(Un, Un2)                                   # fixed summation order: bit-reproducible
+    ctx.close()
+
+
 @pytest.mark.parametrize("variant", [0, 1])
 def test_spread_interp_generic_cloud(ib, orc, variant):
     import torch
