@@ -294,6 +294,7 @@ ibk_bin_mesh(ib_bin_params pr)
 // ---- scan over the tiles (two small kernels, one thread per tile = 4 bins): start offsets, cursors, work
 // list, compact list of the records of sparsely filled tiles ------------------------------------------
 #define SCT 1024
+#define IB_MIN_CHUNK 128           // smallest work item of the tile kernel (points) that the work list is cut into
 
 __device__ __forceinline__ void ib_block_scan2(int &a, int &b, int *ws, int *wl, int &ta, int &tb)
 {
@@ -451,9 +452,12 @@ ib_status ibk_bin_points(ib_ctx *c, int mesh, const double *xp, const double *Gp
         else ibk_bin_cloud<0><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
         const int nsb = (n_tiles + SCT - 1) / SCT;
         int2 *partial = reinterpret_cast<int2 *>(c->d_tile_count + IB_TILE_HDR);
-        // ~4 work items per resident CTA of the tile kernel when the cloud is small
-        int chunk = (int)((P / 1200 + 63) / 64 * 64);
-        chunk = chunk < 192 ? 192 : (chunk > IB_CHUNK ? IB_CHUNK : chunk);
+        // a small cloud is cut into about one work item per SM (measured at C2, 65 k points: 66 us per step against
+        // 76 with four items per SM -- every work item has a fixed cost, and a CTA with one item has nothing to
+        // overlap anyway); from 704 points per SM on the items have the tile kernel's full staging capacity
+        if (!c->sm_count) IB_CUDA_TRY(cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device));
+        int chunk = (int)((P / (c->sm_count > 0 ? c->sm_count : 148) + 31) / 32 * 32);
+        chunk = chunk < IB_MIN_CHUNK ? IB_MIN_CHUNK : (chunk > IB_CHUNK ? IB_CHUNK : chunk);
         if (nsb > 1) ibk_tile_partials<<<nsb, SCT, 0, st>>>(c->d_tile_cur, n_tiles, chunk, partial);   // one CTA needs no partial sums
         ibk_tile_scan<<<nsb, SCT, 0, st>>>(c->d_tile_cur, n_tiles, chunk, partial, c->d_tile_start, c->d_work, c->d_small_rec, c->d_tile_count,
                                            ib_slab_tiles(c), c->grid.nx / BT, c->grid.ny / BT, (int)c->work_cap);
@@ -481,9 +485,9 @@ ib_status ibk_bin_reserve(ib_ctx *c, int64_t P)
     c->bin_cap = 0;
     int64_t cap = P + P / 8 + 1024;
     if (cudaMalloc(&c->d_rec, (size_t)cap * 8 * sizeof(double)) != cudaSuccess) return IB_ERR_ALLOC;
-    {   // a tile with >= IB_SMALL_TILE points gives at most 4 runs of layers plus one piece per 192 points
+    {   // a tile with >= IB_SMALL_TILE points gives at most 4 runs of layers plus one piece per IB_MIN_CHUNK points
         const int64_t n_tiles = c->n_cells / (BT * BT * BT), dense = cap / IB_SMALL_TILE + 1;
-        c->work_cap = 4 * (dense < n_tiles ? dense : n_tiles) + cap / 192 + 8;
+        c->work_cap = 4 * (dense < n_tiles ? dense : n_tiles) + cap / IB_MIN_CHUNK + 8;
     }
     if (cudaMalloc(&c->d_work, (size_t)c->work_cap * sizeof(int4)) != cudaSuccess) return IB_ERR_ALLOC;
     if (cudaMalloc(&c->d_small_rec, (size_t)cap * sizeof(int32_t)) != cudaSuccess) return IB_ERR_ALLOC;
