@@ -8,7 +8,7 @@
 #define IB_TILE 8              // tile edge of the binning key (A21)
 #define IB_TILE_CELLS 512
 #ifndef IB_SMALL_TILE
-#define IB_SMALL_TILE 96         // tiles with fewer points skip the tile kernel: their points go one by one (ib_point.cuh); 64/96/128/192 measured
+#define IB_SMALL_TILE 64         // tiles with fewer points skip the tile kernel: their points go one by one (ib_point.cuh); 32/48/80/96/128/192 measured
 #endif
 #ifndef IB_CHUNK
 #define IB_CHUNK 704             // points per work item of the tile kernel = records it stages in shared memory (ib_bin.cu emits the work list)
@@ -66,7 +66,7 @@ struct ib_ctx {
     int64_t *d_row_off;        // [n_elems+1]
     int32_t *d_tile_cur;       // [n_tiles] counts, then running cursors
     int32_t *d_tile_start;     // [n_tiles+1]
-    int4 *d_work;              // work list of the tile kernel: {tile, first record, points, 0} per chunk
+    int4 *d_work;              // work list of the tile kernel: {tile, first record, points, packed tile coordinates} per work item
     int64_t work_cap;
     int32_t *d_small_rec;      // records of tiles with < IB_SMALL_TILE points (count in d_tile_count[2])
     int32_t *d_tile_count;     // [0] number of non-empty tiles, [1] work counter; d_tile_cur follows it in the same block

@@ -698,10 +698,11 @@ ibk_tiled_kernel(const __grid_constant__ ib_tiled_params pr)
 
 // Points of tiles with fewer than IB_SMALL_TILE points are not worth a halo and a sort: 4 lanes per point of
 // the compact list written by ibk_tile_scan, every point treated directly against the grid (ib_point_quad).
-// The spreading half is bound by the L2 reduction units (48 sectors per point), the rest by dependent loads:
-// 6 resident CTAs = 80 registers measured best on the sparse workloads (4 / 6 / 8: DESIGN.md)
+// The spreading half is bound by the L2 reduction units (48 sectors per point), the rest by dependent loads.
+// 3 resident CTAs of 128 threads per SM measured best on the sparse workloads (2 / 4 / 5 / 6 / 8: DESIGN.md): the
+// compiler keeps all offsets and weights of a component in registers, and the kernel leaves the L2 more room
 #ifndef IB_SMALL_MINB
-#define IB_SMALL_MINB 6
+#define IB_SMALL_MINB 3
 #endif
 template <int DO_SPREAD, int DO_INTERP, int PER>
 __global__ void __launch_bounds__(128, IB_SMALL_MINB)
