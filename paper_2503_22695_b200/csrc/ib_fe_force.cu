@@ -129,7 +129,9 @@ ibk_fe_geometry(int64_t n_elems, int64_t n_nodes, const int32_t *__restrict__ co
 }
 
 // One thread per Gauss point; lanes 8g..8g+7 of a warp hold the 8 Gauss points of one element.
-__global__ void __launch_bounds__(256, 2)
+#define IB_FE_TB 128             // 3 CTAs of 128 threads per SM (168 registers, no spills) measured best: 256 x 2 (128 registers, spilling) +5 %,
+                                 // 128 x 4 / 64 x 8 +3 %, 128 x 5 +15 %
+__global__ void __launch_bounds__(IB_FE_TB, 3)
 ibk_fe_gauss(int64_t n_elems, int64_t n_nodes, const int32_t *__restrict__ conn,
              const double *__restrict__ geo, const double *__restrict__ x,
              const double *__restrict__ fib, const int32_t *__restrict__ mat_id,
@@ -625,7 +627,7 @@ ib_status ibk_fe_force(ib_ctx *c, const double *x, double *B, double *Fhat, cuda
     }
     if (c->n_elems > 0) {
         int64_t nt = c->n_elems * 8;
-        ibk_fe_gauss<<<ib_blocks(nt, 256), 256, 0, st>>>(c->n_elems, c->n_nodes, c->d_conn, c->d_geo, x,
+        ibk_fe_gauss<<<ib_blocks(nt, IB_FE_TB), IB_FE_TB, 0, st>>>(c->n_elems, c->n_nodes, c->d_conn, c->d_geo, x,
                                                          c->d_fib, c->d_mat_id, c->d_mats, c->d_Ce,
                                                          c->d_status);
         c->launches++;
