@@ -704,8 +704,9 @@ ibk_tiled_kernel(const __grid_constant__ ib_tiled_params pr)
 #ifndef IB_SMALL_MINB
 #define IB_SMALL_MINB 3
 #endif
+#define IB_SMALL_TB 128
 template <int DO_SPREAD, int DO_INTERP, int PER>
-__global__ void __launch_bounds__(128, IB_SMALL_MINB)
+__global__ void __launch_bounds__(IB_SMALL_TB, IB_SMALL_MINB)
 ibk_small_tiles(ib_tiled_params pr, const int32_t *__restrict__ small_rec, const int32_t *__restrict__ counters)
 {
     // 4 lanes per point (ib_point_quad); the list length is known on the device only, so the grid is sized for
@@ -727,11 +728,12 @@ ibk_small_tiles(ib_tiled_params pr, const int32_t *__restrict__ small_rec, const
     }
 }
 
-// blocks of the sparse-tile kernel: enough for the longest possible list, at most 16 per SM (grid stride)
+// blocks of the sparse-tile kernel: enough for the longest possible list, at most 64 per SM (grid stride; 3 are
+// resident -- many short CTAs level the end of the kernel: 3 / 6 / 16 / 256 / 2048 per SM measured)
 static int ib_small_blocks(int64_t nsmall_max, int sms)
 {
-    const int64_t need = (nsmall_max * 4 + 127) / 128;
-    const int64_t cap = (int64_t)(sms > 0 ? sms : 148) * 16;
+    const int64_t need = (nsmall_max * 4 + IB_SMALL_TB - 1) / IB_SMALL_TB;
+    const int64_t cap = (int64_t)(sms > 0 ? sms : 148) * 64;
     return (int)(need < 1 ? 1 : (need < cap ? need : cap));
 }
 
@@ -756,7 +758,7 @@ static ib_status launch_tiled_p(ib_ctx *c, const ib_tiled_params &pr, bool with_
         IB_CUDA_TRY(cudaEventRecord(c->ev_sfork, st));
         IB_CUDA_TRY(cudaStreamWaitEvent(s3, c->ev_sfork, 0));
     }
-    if (with_small) ibk_small_tiles<S, I, PER><<<ib_small_blocks(nsmall_max, sms), 128, 0, s3>>>(pr, c->d_small_rec, c->d_tile_count);
+    if (with_small) ibk_small_tiles<S, I, PER><<<ib_small_blocks(nsmall_max, sms), IB_SMALL_TB, 0, s3>>>(pr, c->d_small_rec, c->d_tile_count);
     if (beside) IB_CUDA_TRY(cudaEventRecord(c->ev_sjoin, s3));
     ibk_tiled_kernel<S, I, PER><<<sms, TB, smem, st>>>(pr);
     if (beside) IB_CUDA_TRY(cudaStreamWaitEvent(st, c->ev_sjoin, 0));
@@ -876,14 +878,14 @@ ib_status ibk_small_launch(ib_ctx *c, int64_t P, int do_spread, int do_interp,
     const int nb = ib_small_blocks(nsmall_max, 0);
     const bool per = c->grid.periodic != 0;
     if (do_spread && do_interp) {
-        if (per) ibk_small_tiles<1, 1, 1><<<nb, 128, 0, st>>>(pr, c->d_small_rec, c->d_tile_count);
-        else ibk_small_tiles<1, 1, 0><<<nb, 128, 0, st>>>(pr, c->d_small_rec, c->d_tile_count);
+        if (per) ibk_small_tiles<1, 1, 1><<<nb, IB_SMALL_TB, 0, st>>>(pr, c->d_small_rec, c->d_tile_count);
+        else ibk_small_tiles<1, 1, 0><<<nb, IB_SMALL_TB, 0, st>>>(pr, c->d_small_rec, c->d_tile_count);
     } else if (do_spread) {
-        if (per) ibk_small_tiles<1, 0, 1><<<nb, 128, 0, st>>>(pr, c->d_small_rec, c->d_tile_count);
-        else ibk_small_tiles<1, 0, 0><<<nb, 128, 0, st>>>(pr, c->d_small_rec, c->d_tile_count);
+        if (per) ibk_small_tiles<1, 0, 1><<<nb, IB_SMALL_TB, 0, st>>>(pr, c->d_small_rec, c->d_tile_count);
+        else ibk_small_tiles<1, 0, 0><<<nb, IB_SMALL_TB, 0, st>>>(pr, c->d_small_rec, c->d_tile_count);
     } else {
-        if (per) ibk_small_tiles<0, 1, 1><<<nb, 128, 0, st>>>(pr, c->d_small_rec, c->d_tile_count);
-        else ibk_small_tiles<0, 1, 0><<<nb, 128, 0, st>>>(pr, c->d_small_rec, c->d_tile_count);
+        if (per) ibk_small_tiles<0, 1, 1><<<nb, IB_SMALL_TB, 0, st>>>(pr, c->d_small_rec, c->d_tile_count);
+        else ibk_small_tiles<0, 1, 0><<<nb, IB_SMALL_TB, 0, st>>>(pr, c->d_small_rec, c->d_tile_count);
     }
     c->launches += 1;
     IB_CUDA_TRY(cudaGetLastError());
