@@ -161,10 +161,14 @@ __device__ __forceinline__ double ib_face_lerp(double w00, double w10, double w0
 // STAGE: uniform nsub with 4 <= n2*n3 dividing 256 -- the CTA's 256 rows are 256/(n2 n3) whole elements,
 // whose node positions (and force coefficients) are staged once in shared memory instead of being
 // gathered by every row.
-template <int SCATTER, int STAGE>
+// N1: the number of sub-points of a row when the rule is uniform with 2 or 4 of them (the loops over the points of a
+// row are unrolled for registers: 8 copies of which a 4-point rule skips half -- the code of the generic kernel is
+// 5,900 instructions long and a row executes 1,100 of them, which the instruction cache does not like); 0: any rule
+template <int SCATTER, int STAGE, int N1>
 __global__ void __launch_bounds__(256, 4)
 ibk_bin_mesh(ib_bin_params pr)
 {
+    constexpr int NJ = N1 > 0 ? N1 : 8;
     __shared__ double s_nd[STAGE ? 16 * 8 * 6 : 1];       // [element of the CTA][local node][x0 x1 x2 F0 F1 F2]
     __shared__ ib_bin_hash h;
     ib_hash_clear(h);
@@ -192,7 +196,7 @@ ibk_bin_mesh(ib_bin_params pr)
     if (live) {
         int r;
         if (pr.un1 > 0) {
-            n1 = pr.un1; n2 = pr.un2; n3 = pr.un3;
+            n1 = N1 > 0 ? N1 : pr.un1; n2 = pr.un2; n3 = pr.un3;
             int rpe = n2 * n3;
             e = row / rpe;
             r = (int)(row - e * rpe);
@@ -253,9 +257,9 @@ ibk_bin_mesh(ib_bin_params pr)
     }
     // ---- the n1 points of the row: position, bin, count in the CTA's table ------------------------------
     const double rn1 = 1.0 / (double)(n1 > 0 ? n1 : 1);
-    int code[8];                                   // nsub <= 8 (ib_create)
+    int code[NJ];                                  // nsub <= 8 (ib_create)
 #pragma unroll
-    for (int j = 0; j < 8; ++j) {
+    for (int j = 0; j < NJ; ++j) {
         code[j] = IB_CODE_NONE;
         if (live && j < n1) {
             const double t = ((double)j + 0.5) * rn1;
@@ -274,7 +278,7 @@ ibk_bin_mesh(ib_bin_params pr)
     ib_hash_flush<SCATTER>(h, pr.tile_cur);
     if (SCATTER) {
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
+        for (int j = 0; j < NJ; ++j) {
             if (live && j < n1 && code[j] != IB_CODE_NONE) {
                 const double t = ((double)j + 0.5) * rn1;
                 const double x = __fma_rn(t, D[0], L[0]), y = __fma_rn(t, D[1], L[1]), z = __fma_rn(t, D[2], L[2]);
@@ -447,8 +451,10 @@ ib_status ibk_bin_points(ib_ctx *c, int mesh, const double *xp, const double *Gp
     const bool stage = c->un[0] > 0 && rpe >= 16 && 256 % rpe == 0;     // <= 16 elements per CTA fit the staging array
     if (phases & 1) {
         IB_CUDA_TRY(cudaMemsetAsync(c->d_tile_count, 0, ((size_t)c->tile_hdr + (size_t)n_tiles * 4) * sizeof(int32_t), st));   // counters and bins
-        if (mesh && stage) ibk_bin_mesh<0, 1><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
-        else if (mesh) ibk_bin_mesh<0, 0><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
+        if (mesh && stage && c->un[0] == 4) ibk_bin_mesh<0, 1, 4><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
+        else if (mesh && stage && c->un[0] == 2) ibk_bin_mesh<0, 1, 2><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
+        else if (mesh && stage) ibk_bin_mesh<0, 1, 0><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
+        else if (mesh) ibk_bin_mesh<0, 0, 0><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
         else ibk_bin_cloud<0><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
         const int nsb = (n_tiles + SCT - 1) / SCT;
         int2 *partial = reinterpret_cast<int2 *>(c->d_tile_count + IB_TILE_HDR);
@@ -464,8 +470,10 @@ ib_status ibk_bin_points(ib_ctx *c, int mesh, const double *xp, const double *Gp
         c->launches += 3;
     }
     if (phases & 2) {
-        if (mesh && stage) ibk_bin_mesh<1, 1><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
-        else if (mesh) ibk_bin_mesh<1, 0><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
+        if (mesh && stage && c->un[0] == 4) ibk_bin_mesh<1, 1, 4><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
+        else if (mesh && stage && c->un[0] == 2) ibk_bin_mesh<1, 1, 2><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
+        else if (mesh && stage) ibk_bin_mesh<1, 1, 0><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
+        else if (mesh) ibk_bin_mesh<1, 0, 0><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
         else ibk_bin_cloud<1><<<ib_blocks(nthr, 256), 256, 0, st>>>(pr);
         c->launches += 1;
     }
