@@ -159,19 +159,26 @@ static inline void ib_status_unpack(unsigned long long w, int *code, long long *
     *id = w ? (long long)(IB_STATUS_IDMASK - (w & IB_STATUS_IDMASK)) : -1;
 }
 
-// sqrt(a) for a in [1/64, 1/32] (the argument (1+4r-4r^2)/64 of the kernel): float rsqrt seed (~2^-22),
-// one Goldschmidt step (~2^-43) and one residual correction (~2^-85, i.e. rounding level) -- no special
+// sqrt(a) for a in [1/64, 1/32] (the argument (1+4r-4r^2)/64 of the kernel): reciprocal-square-root seed
+// from the upper word (MUFU.RSQ64H, ~2^-20; the float route costs two conversions more on the same unit),
+// one Goldschmidt step (~2^-39) and one residual correction (~2^-77, i.e. rounding level) -- no special
 // cases, no branches, 7 fp64 operations.
 __device__ __forceinline__ double ib_sqrt_seeded(double a)
 {
-    float yf;
-    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(yf) : "f"((float)a));       // one MUFU.RSQ
-    double y = (double)yf;
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a));               // one MUFU.RSQ64H
     double g = a * y, h = 0.5 * y;
     double r = fma(-g, h, 0.5);
     g = fma(g, r, g);
     h = fma(h, r, h);
     return fma(fma(-g, g, a), h, g);
+}
+
+// (double)v for |v| < 2^31 without the conversion unit: the integer goes into the low word of 2^52 + 2^31 + v
+// (exact), one fp64 subtraction takes the offset out again
+__device__ __forceinline__ double ib_i2d(int v)
+{
+    return __hiloint2double(0x43300000, v ^ (int)0x80000000) - 4503601774854144.0;
 }
 
 // Peskin 4-point kernel (PAPER.md L52 -> ref.1): the four weights of the support that starts at
@@ -215,9 +222,10 @@ __device__ __forceinline__ int ib_wrap(int i, int n)
 // Binning cell index of A21: floor((x - x0) * inv_h) mod n, in IEEE double with NO contraction.
 __device__ __forceinline__ int ib_cell(double x, double x0, double inv_h, int n)
 {
-    double fl = floor(__dmul_rn(__dsub_rn(x, x0), inv_h));
-    if (fl >= 0.0 && fl < (double)n) return (int)fl;      // inside the box: no wrap, no 64-bit modulo
-    long long c = (long long)fl;
+    const double sc = __dmul_rn(__dsub_rn(x, x0), inv_h);
+    const int ci = __double2int_rd(sc);                   // floor in one conversion (saturates far outside)
+    if ((unsigned)ci < (unsigned)n) return ci;            // inside the box: no wrap, no 64-bit modulo
+    long long c = (long long)floor(sc);
     c %= n;
     if (c < 0) c += n;
     return (int)c;

@@ -93,11 +93,10 @@ __device__ __forceinline__ void ib_half_range(int c, int d, int l, int &lo, int 
 // part comes from that formula and only the fraction from s.
 __device__ __forceinline__ double ib_tile_coord(double x, double x0, double h, double inv_h)
 {
-    double sc = __dmul_rn(__dsub_rn(x, x0), inv_h);
-    double fl = floor(sc);
+    const int ci = __double2int_rd(__dmul_rn(__dsub_rn(x, x0), inv_h));       // floor: the cell of A21 before the wrap
     // grid dims are multiples of 8, so the periodically wrapped cell index is congruent to the
-    // unwrapped one modulo the tile edge 4
-    return (ib_scaled(x, x0, h, inv_h) - fl) + (double)((long long)fl & (TT - 1));
+    // unwrapped one modulo the tile edge 4.  s - fl is exact, so (s - fl) + (ci & 3) = s - (fl - (ci & 3)) in one rounding
+    return ib_scaled(x, x0, h, inv_h) - ib_i2d(ci & ~(TT - 1));
 }
 
 __device__ __forceinline__ void ib_prefetch_l2(const void *p)
@@ -465,7 +464,7 @@ ibk_tiled_kernel(const __grid_constant__ ib_tiled_params pr)
 #pragma unroll
                         for (int d = 2; d >= 0; --d) {
                             xi[k][d] = ib_tile_coord(xr[k][d], org[d], pr.g.h, pr.inv_h);
-                            key = key * 8 + min(max((int)floor(2.0 * xi[k][d]), 0), 7);
+                            key = key * 8 + min(max(__double2int_rd(2.0 * xi[k][d]), 0), 7);
                         }
                         ks[k] = key | (atomicAdd(&oc_cnt[key], 1) << 9);
                     }
@@ -595,8 +594,8 @@ ibk_tiled_kernel(const __grid_constant__ ib_tiled_params pr)
                         // face-aligned: cell hd >> 1; centre-aligned: shifted cell (hd + 1) >> 1 covers xi - 1/2 in [l-1, l).
                         // r in [0,1] up to rounding at cell boundaries, where the formula continues phi smoothly (A19)
                         const int hd = (key >> (3 * d)) & 7;
-                        sets[(2 * d) * CH + pos] = ib_aq(xi[k][d] - (double)(hd >> 1));
-                        sets[(2 * d + 1) * CH + pos] = ib_aq(xi[k][d] + 0.5 - (double)((hd + 1) >> 1));
+                        sets[(2 * d) * CH + pos] = ib_aq(xi[k][d] - ib_i2d(hd >> 1));
+                        sets[(2 * d + 1) * CH + pos] = ib_aq(xi[k][d] + 0.5 - ib_i2d((hd + 1) >> 1));
                     }
                     if (DO_SPREAD) {
 #pragma unroll
