@@ -27,6 +27,10 @@ struct ib_bin_params {
     // mesh source
     int64_t n_rows, n_elems, n_nodes;
     int un1, un2, un3;             // uniform nsub (un1 == 0: per-element nsub / row_off / pt_off)
+    // uniform nsub: what every row would otherwise divide for (host: ib_bin_uniform)
+    int rpe, epc;                  // rows per element n2 n3; elements per CTA of 256 rows when rpe divides 256
+    unsigned rpe_m16, n2_m16;      // ceil(2^16 / rpe), ceil(2^16 / n2): a / d = (a * m16) >> 16 for a < 512
+    double rn2, rn3;               // 1.0 / n2, 1.0 / n3 (IEEE division, the value the device would form)
     const int32_t *nsub;
     const int64_t *pt_off, *row_off;
     const int32_t *conn;
@@ -171,10 +175,17 @@ ibk_bin_mesh(ib_bin_params pr)
     constexpr int NJ = N1 > 0 ? N1 : 8;
     __shared__ double s_nd[STAGE ? 16 * 8 * 6 : 1];       // [element of the CTA][local node][x0 x1 x2 F0 F1 F2]
     __shared__ ib_bin_hash h;
+    __shared__ long long s_e0;                            // uniform rule, rows not staged: element and row inside it of the CTA's first row
+    __shared__ int s_r0;
     ib_hash_clear(h);
+    if (!STAGE && threadIdx.x == 0 && pr.un1 > 0) {       // one 64-bit division per CTA instead of one per row
+        const long long base = (long long)blockIdx.x * blockDim.x;
+        s_e0 = base / pr.rpe;
+        s_r0 = (int)(base - s_e0 * pr.rpe);
+    }
     if (!STAGE) __syncthreads();
     if (STAGE) {
-        const int rpe = pr.un2 * pr.un3, epc = 256 / rpe;
+        const int epc = pr.epc;
         const int64_t e_first = (int64_t)blockIdx.x * epc;
         for (int i = threadIdx.x; i < epc * 8; i += 256) {
             const int64_t ee = e_first + (i >> 3);
@@ -197,9 +208,14 @@ ibk_bin_mesh(ib_bin_params pr)
         int r;
         if (pr.un1 > 0) {
             n1 = N1 > 0 ? N1 : pr.un1; n2 = pr.un2; n3 = pr.un3;
-            int rpe = n2 * n3;
-            e = row / rpe;
-            r = (int)(row - e * rpe);
+            const int rpe = pr.rpe;
+            // row = 256 blockIdx + thread: the element comes from the CTA's first row and a division of a number
+            // below 512 by rpe <= 64, which is a multiplication (exact: a (m16 d - 2^16) < 2^16 for a < 512, d <= 64)
+            const int rr = (STAGE ? 0 : s_r0) + (int)threadIdx.x;
+            const int el = (int)(((unsigned)rr * pr.rpe_m16) >> 16);
+            e = (STAGE ? (int64_t)blockIdx.x * pr.epc : (int64_t)s_e0) + el;
+            r = rr - el * rpe;
+            assert(e == row / rpe && r == (int)(row - e * rpe));
             p0 = e * (int64_t)(n1 * rpe) + (int64_t)r * n1;
         } else {
             e = ib_find_row_elem(pr.row_off, pr.n_elems, row);
@@ -207,7 +223,9 @@ ibk_bin_mesh(ib_bin_params pr)
             r = (int)(row - __ldg(pr.row_off + e));
             p0 = __ldg(pr.pt_off + e) + (int64_t)r * n1;
         }
-        m2 = r % n2; m3 = r / n2;
+        if (pr.un1 > 0) { m3 = (int)(((unsigned)r * pr.n2_m16) >> 16); m2 = r - m3 * n2; }
+        else { m2 = r % n2; m3 = r / n2; }
+        assert(m3 == r / n2 && m2 == r % n2);
     }
     double L[3] = {0, 0, 0}, D[3] = {0, 0, 0}, LF[3] = {0, 0, 0}, DF[3] = {0, 0, 0};
     bool finite = true;
@@ -215,7 +233,7 @@ ibk_bin_mesh(ib_bin_params pr)
         int nd[8] = {0, 0, 0, 0, 0, 0, 0, 0};
         const double *sn = s_nd;
         if (STAGE) {
-            sn = s_nd + (int)(e - (int64_t)blockIdx.x * (256 / (pr.un2 * pr.un3))) * 48;
+            sn = s_nd + (int)(e - (int64_t)blockIdx.x * pr.epc) * 48;
         } else {
             const int4 *cp = reinterpret_cast<const int4 *>(pr.conn + e * 8);
             int4 c0 = __ldg(cp), c1 = __ldg(cp + 1);
@@ -223,7 +241,8 @@ ibk_bin_mesh(ib_bin_params pr)
             nd[4] = c1.x; nd[5] = c1.y; nd[6] = c1.z; nd[7] = c1.w;
         }
         // N-weights of the row: 1/2 (1 +- xi) with xi = -1 + (2m+1)/n  ->  (m + 1/2)/n and its complement
-        double b1 = ((double)m2 + 0.5) * (1.0 / (double)n2), g1 = ((double)m3 + 0.5) * (1.0 / (double)n3);
+        const double rn2 = pr.un1 > 0 ? pr.rn2 : 1.0 / (double)n2, rn3 = pr.un1 > 0 ? pr.rn3 : 1.0 / (double)n3;
+        double b1 = ((double)m2 + 0.5) * rn2, g1 = ((double)m3 + 0.5) * rn3;
         double b0 = 1.0 - b1, g0 = 1.0 - g1;
         double w00 = __dmul_rn(b0, g0), w10 = __dmul_rn(b1, g0), w01 = __dmul_rn(b0, g1), w11 = __dmul_rn(b1, g1);
 #pragma unroll
@@ -441,6 +460,14 @@ ib_status ibk_bin_points(ib_ctx *c, int mesh, const double *xp, const double *Gp
     pr.P = P; pr.xp = xp; pr.Gp = Gp;
     pr.n_rows = c->n_rows; pr.n_elems = c->n_elems; pr.n_nodes = c->n_nodes;
     pr.un1 = c->un[0]; pr.un2 = c->un[1]; pr.un3 = c->un[2];
+    if (pr.un1 > 0) {
+        pr.rpe = pr.un2 * pr.un3;
+        pr.epc = 256 / pr.rpe;
+        pr.rpe_m16 = (65536u + (unsigned)pr.rpe - 1u) / (unsigned)pr.rpe;
+        pr.n2_m16 = (65536u + (unsigned)pr.un2 - 1u) / (unsigned)pr.un2;
+        pr.rn2 = 1.0 / (double)pr.un2;
+        pr.rn3 = 1.0 / (double)pr.un3;
+    }
     pr.nsub = c->d_nsub; pr.pt_off = c->d_pt_off; pr.row_off = c->d_row_off; pr.conn = c->d_conn;
     pr.x = x; pr.Fhat = Fhat; pr.Wp = c->d_Wp;
     pr.g = c->grid; pr.inv_h = c->inv_h;
