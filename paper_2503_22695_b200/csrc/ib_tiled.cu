@@ -421,17 +421,13 @@ ibk_tiled_kernel(const __grid_constant__ ib_tiled_params pr)
     if (wid < NPW) {
         // =================================== producers ==========================================================
         const double org[3] = {pr.g.x0, pr.g.y0, pr.g.z0};
+        int wfirst = 0, wlast = 0, wnext = 0;            // thread 0: the launch's range of work items, the index claimed for the next one
+        if (tid == 0) { wfirst = pr.counters[pr.wb]; wlast = pr.counters[pr.we]; wnext = wfirst + atomicAdd(&pr.counters[pr.wc], 1); }
         unsigned halo_phase = 0;                         // bit b: phase of halo[b] that the next TMA load into buffer b completes
         for (int iter = 0;; ++iter) {
             const int b = iter & 1;
             unsigned char *buf = smraw + b * BUF_BYTES;
             const int4 wk = s_wk[b];
-            // the work item after this one is claimed now (the other slot: every producer has read it, before
-            // the last barrier of the previous iteration at the latest)
-            if (tid == 0) {
-                const int w = pr.counters[pr.wb] + atomicAdd(&pr.counters[pr.wc], 1);
-                s_wk[b ^ 1] = (w < pr.counters[pr.we]) ? __ldg(pr.work + w) : make_int4(-1, 0, 0, 0);
-            }
             if (wk.x < 0) {
                 // no more work: an empty buffer with nbatch < 0 tells the consumers to stop
                 if (tid == 0) {
@@ -442,6 +438,13 @@ ibk_tiled_kernel(const __grid_constant__ ib_tiled_params pr)
                 break;
             }
             const int cb = wk.y, cn = wk.z;
+            // Work items are claimed two ahead, so that thread 0 never waits for a round trip to the L2 (the atomic on
+            // the one counter of all CTAs takes about 2000 cycles, the load of the work item 700 more): the atomic
+            // issued now names the item after the next one and is not looked at before the next iteration; the
+            // index it returned last time is used now, and the work item loaded with it is stored into the other slot
+            // (every producer has read that one at the top of the previous iteration) inside the scan
+            int wnn = 0;
+            if (tid == 0) wnn = wfirst + atomicAdd(&pr.counters[pr.wc], 1);
             // ---- coordinates of the records, one thread per point: tile coordinates, half-cell, rank inside it.
             // Nothing here touches the record buffers: it overlaps the consumers' work on both of them.
             double xi[KPT][3];
@@ -470,13 +473,10 @@ ibk_tiled_kernel(const __grid_constant__ ib_tiled_params pr)
                     }
                 }
             }
+            int4 wk_next = make_int4(-1, 0, 0, 0);
+            if (tid == 0 && wnext < wlast) wk_next = __ldg(pr.work + wnext);
             ib_producer_sync();
             for (int i = tid; i < 3 * NBIN; i += TBP) bins[i] = 0;      // read last before the closing barrier of the previous iteration
-            {                                            // the next work item's records -> L2 while this one is processed
-                const int4 nx4 = s_wk[b ^ 1];
-                if (nx4.x >= 0)
-                    for (int i = 2 * tid; i < nx4.z; i += 2 * TBP) ib_prefetch_l2(pr.rec + (size_t)(nx4.y + i) * 8);   // two records per 128-byte line
-            }
             {                                            // exclusive scan of the 512 counts
                 int v[SCK], s = 0;
 #pragma unroll
@@ -491,6 +491,7 @@ ibk_tiled_kernel(const __grid_constant__ ib_tiled_params pr)
                     if (lane >= o) inc += t;
                 }
                 if (lane == 31) wsum[wid] = inc;
+                if (tid == 0) { s_wk[b ^ 1] = wk_next; wnext = wnn; }
                 ib_producer_sync();
                 int ex = inc - s;
                 for (int w = 0; w < wid; ++w) ex += wsum[w];
@@ -500,6 +501,11 @@ ibk_tiled_kernel(const __grid_constant__ ib_tiled_params pr)
                     ex += v[k];
                 }
                 if (tid == TBP - 1) oc_start[NOC] = ex;
+            }
+            {                                            // the next work item's records -> L2 while this one is processed
+                const int4 nx4 = s_wk[b ^ 1];
+                if (nx4.x >= 0)
+                    for (int i = 2 * tid; i < nx4.z; i += 2 * TBP) ib_prefetch_l2(pr.rec + (size_t)(nx4.y + i) * 8);   // two records per 128-byte line
             }
             ib_producer_sync();
             // ---- from here on the record buffer is written: the consumers must have left its previous contents
