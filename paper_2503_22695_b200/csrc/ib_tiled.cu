@@ -225,7 +225,17 @@ __device__ __forceinline__ void ib_run_batch(int C, const ib_tiled_params &pr, c
     // 4 points per step: the x-sums of the 4 interpolated values are reduced across the 4 lanes in a
     // transposing butterfly (3 shuffles instead of 8), which leaves point k's value in lane k -- one store
     // instruction per 4 points
+    double ra0 = 0.0, ra1 = 0.0, rs0 = 0.0, rs1 = 0.0;                      // the reduction of a step is finished in the next one (its second shuffle and the
+                                                       // store run beside the loads of the next four points)
     for (int v0 = 0; v0 < nmax; v0 += 4) {
+        if (DO_INTERP && v0 > 0) {
+            const bool hi1 = (qq & 1u) != 0;
+            ra0 += __shfl_xor_sync(full, rs0, 2);
+            ra1 += __shfl_xor_sync(full, rs1, 2);
+            double tot = hi1 ? ra1 : ra0;
+            tot += __shfl_xor_sync(full, hi1 ? ra0 : ra1, 1);
+            if (v0 - 4 + (int)qq < nun) __stcs(Uc + ib_lds32(sm.sids + 4u * (unsigned)ib_item_rec(vlo + v0 - 4 + (int)qq, rstart, rend)), tot);
+        }
         double pv[4];
         // two points in one straight line of code (their loads and dependent chains overlap); the second pair
         // of a step only when the longest unit of the batch reaches it
@@ -265,16 +275,21 @@ __device__ __forceinline__ void ib_run_batch(int C, const ib_tiled_params &pr, c
             }
         }
         if (DO_INTERP) {
-            const bool hi2 = (qq & 2u) != 0, hi1 = (qq & 1u) != 0;
-            double a0 = hi2 ? pv[2] : pv[0], a1 = hi2 ? pv[3] : pv[1];
-            const double s0 = hi2 ? pv[0] : pv[2], s1 = hi2 ? pv[1] : pv[3];
-            a0 += __shfl_xor_sync(full, s0, 2);
-            a1 += __shfl_xor_sync(full, s1, 2);
-            double tot = hi1 ? a1 : a0;
-            tot += __shfl_xor_sync(full, hi1 ? a0 : a1, 1);
-            // lane q holds the value of point v0 + q
-            if (v0 + (int)qq < nun) __stcs(Uc + ib_lds32(sm.sids + 4u * (unsigned)ib_item_rec(vlo + v0 + (int)qq, rstart, rend)), tot);
+            const bool hi2 = (qq & 2u) != 0;
+            rs0 = hi2 ? pv[0] : pv[2]; rs1 = hi2 ? pv[1] : pv[3];
+            ra0 = hi2 ? pv[2] : pv[0];
+            ra1 = hi2 ? pv[3] : pv[1];
         }
+    }
+    if (DO_INTERP && nmax > 0) {
+        // the last step of the batch; lane q holds the value of point v0 + q
+        const int v0 = (nmax - 1) & ~3;
+        const bool hi1 = (qq & 1u) != 0;
+        ra0 += __shfl_xor_sync(full, rs0, 2);
+        ra1 += __shfl_xor_sync(full, rs1, 2);
+        double tot = hi1 ? ra1 : ra0;
+        tot += __shfl_xor_sync(full, hi1 ? ra0 : ra1, 1);
+        if (v0 + (int)qq < nun) __stcs(Uc + ib_lds32(sm.sids + 4u * (unsigned)ib_item_rec(vlo + v0 + (int)qq, rstart, rend)), tot);
     }
     if (DO_SPREAD && nun > 0) {
         // moments -> face values ff[y j][z i] of x-column q
