@@ -266,6 +266,45 @@ def test_error_latch_inverted_element_and_nan(ib):
 
 
 @pytest.mark.parametrize("variant", [0, 1])
+def test_step_with_nonfinite_node_latches_and_recovers(ib, orc, variant):
+    """A NaN node position inside the whole step (FE force, on-the-fly sub-points, binning, tile kernel): the step
+    ends, the latch reads IB_ERR_NONFINITE, nothing hangs or faults; the same context then gives the oracle's
+    result for clean positions, on the default stream and on a private one (graph replay)."""
+    import torch
+    wl = W.config1()
+    ctx = ib.Context.from_workload(wl)
+    ctx.ib_set_variant(variant)
+    u, v, w = _t(wl.u), _t(wl.v), _t(wl.w)
+    fu, fv, fw = (torch.empty((wl.n_cells,), dtype=torch.float64, device="cuda") for _ in range(3))
+    Un = torch.empty((3, wl.n_nodes), dtype=torch.float64, device="cuda")
+    B = torch.empty((3, wl.n_nodes), dtype=torch.float64, device="cuda")
+    xn = wl.x.copy()
+    xn[2, wl.n_nodes // 2] = np.nan
+    ctx.ib_coupling_step(_t(xn), u, v, w, fu, fv, fw, Un, B)
+    code, bad = ctx.ib_check()
+    assert code == 6 and bad >= 0
+    ref = orc.coupling_step(_grid(orc, wl), wl.conn, wl.X, wl.fibers, wl.mat_id, wl.nsub, wl.mats, wl.x, wl.u, wl.v, wl.w)
+    x = _t(wl.x)
+    st = torch.cuda.Stream()
+    for stream in (None, st, st, st):
+        for t in (fu, fv, fw, Un, B):
+            t.fill_(3.0)
+        torch.cuda.synchronize()
+        if stream is None:
+            ctx.ib_coupling_step(x, u, v, w, fu, fv, fw, Un, B)
+        else:
+            with torch.cuda.stream(stream):
+                ctx.ib_coupling_step(x, u, v, w, fu, fv, fw, Un, B, stream)
+        assert ctx.ib_check()[0] == 0                                # latch was cleared
+        torch.cuda.synchronize()
+        _close(B, ref["B"], "B after a non-finite step")
+        for k, t in zip(("fu", "fv", "fw"), (fu, fv, fw)):
+            _close(t, ref[k], f"{k} after a non-finite step")
+        _close(Un, ref["Un"], "Un after a non-finite step")
+    ctx.close()
+
+
+@pytest.mark.parametrize("variant", [0, 1])
 @pytest.mark.parametrize("name", ["C1", "LV-small"])
 def test_host_entry_point_matches_device_path(ib, name, variant):
     """ib_coupling_step_host (variant 1: spread and interpolation pipelined around the host copies on two
