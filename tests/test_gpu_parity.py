@@ -760,3 +760,54 @@ def test_bounded_grid_cloud_and_mesh(ib, orc, variant):
     for k, t in (("B", B), ("fu", fo[0]), ("fv", fo[1]), ("fw", fo[2]), ("Un", Un)):
         _close(t, ref[k], f"bounded step v{variant} {k}")
     ctx.close()
+
+
+def test_create_and_setters_reject_bad_input(ib):
+    """What ib_create and the setters refuse (include/ibcouple.h: error behaviour): each case names the status code
+    the header states, and a refused creation leaves no context behind."""
+    conn, X, x, fib = distorted_block(3, 3, 2, seed=3)
+    ne, nn = conn.shape[0], X.shape[1]
+    mats = [W.material(0, a=1.0, kappa=10.0)]
+    sub = np.full((ne, 3), 2, np.int32)
+    good = lambda **kw: dict(dict(nx=16, ny=16, nz=16, h=1 / 16, origin=(0, 0, 0), conn=conn, X=X, fibers=fib,
+                                  mat_id=None, nsub=sub, mats=mats), **kw)
+    ib.Context(**good()).close()                                            # the unmodified case is accepted
+    INVALID, UNSUPPORTED = 1, 2
+
+    def refused(code, **kw):
+        with pytest.raises(ib.IbError) as e:
+            ib.Context(**good(**kw))
+        assert e.value.code == code, (kw.keys(), e.value)
+
+    refused(INVALID, nx=12)                                                 # grid edge not a multiple of the tile edge
+    refused(INVALID, h=0.0)
+    refused(INVALID, h=float("nan"))
+    refused(UNSUPPORTED, nx=4104, ny=8, nz=8)                               # tile coordinates are packed in 10 + 10 + 11 bits
+    bad = conn.copy(); bad[2, 5] = nn
+    refused(INVALID, conn=bad)                                              # node id out of range
+    bad = conn.copy(); bad[2, 5] = -1
+    refused(INVALID, conn=bad)
+    s9 = sub.copy(); s9[1, 2] = 9
+    refused(INVALID, nsub=s9)                                               # at most 8 sub-points per direction
+    s0 = sub.copy(); s0[0, 0] = 0
+    refused(INVALID, nsub=s0)
+    refused(INVALID, mat_id=np.full(ne, 1, np.int32))                       # material index beyond the table
+    Xo = np.concatenate([X, X[:, :1] + 5.0], axis=1)
+    refused(INVALID, X=Xo)                                                  # a node of no element has lumped weight 0 (A13)
+    ib.Context(**good(X=Xo, nsub=None)).close()                             # ... which the nodal rule does not need
+    law9 = [dict(mats[0], law=9)]
+    refused(INVALID, mats=law9)
+    # nine elements at one node: the ELL adjacency holds eight
+    star = np.concatenate([conn, conn[:1]], axis=0)
+    refused(UNSUPPORTED, conn=star, nsub=np.full((ne + 1, 3), 2, np.int32),
+            fibers=None if fib is None else np.concatenate([fib, fib[:, :1]], axis=1))
+
+    ctx = ib.Context(**good())
+    for call, args in ((ctx.ib_set_variant, (2,)), (ctx.ib_set_tethers, ([0, 1, 1], 10.0)),
+                       (ctx.ib_set_tethers, ([nn], 10.0)), (ctx.ib_set_tethers, ([0], float("inf"))),
+                       (ctx.ib_set_surface, (np.array([[0, 1, 2, nn]], np.int32),))):
+        with pytest.raises(ib.IbError) as e:
+            call(*args)
+        assert e.value.code == INVALID, (call.__name__, args)
+    ctx.ib_set_tethers([0, 1, 2], 10.0)                                     # and the context still works
+    ctx.close()
