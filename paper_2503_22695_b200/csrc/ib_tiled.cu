@@ -45,7 +45,7 @@
 #define SZ 64                   // z-plane stride of the halo in doubles: dense 8 x 8 x 8, the layout a TMA box load writes
 #define SU3 (TH * SZ)           // one component of the halo
 #ifndef PCAP
-#define PCAP 32                 // an item with more points is cut into units of PCAP points (each with a window of its own)
+#define PCAP 24                 // an item with more points is cut into units of PCAP points (each with a window of its own); 16 / 20 / 24 / 28 / 32 measured on the final kernel
 #endif
 #define NBIN (PCAP + 1)         // units are ordered by point count 0..PCAP
 #define NORD ((100 + IB_CHUNK / PCAP + 7) & ~7)   // units per component: one per item + IB_CHUNK / PCAP whole ones, in whole batches
