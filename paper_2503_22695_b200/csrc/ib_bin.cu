@@ -492,7 +492,7 @@ ib_status ibk_bin_points(ib_ctx *c, int mesh, const double *xp, const double *Gp
         int2 *partial = reinterpret_cast<int2 *>(c->d_tile_count + IB_TILE_HDR);
         // a small cloud is cut into about one work item per SM (measured at C2, 65 k points: 66 us per step against
         // 76 with four items per SM -- every work item has a fixed cost, and a CTA with one item has nothing to
-        // overlap anyway); from 704 points per SM on the items have the tile kernel's full staging capacity
+        // overlap anyway); from IB_CHUNK points per SM on the items have the tile kernel's full staging capacity
         if (!c->sm_count) IB_CUDA_TRY(cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device));
         int chunk = (int)((P / (c->sm_count > 0 ? c->sm_count : 148) + 31) / 32 * 32);
         chunk = chunk < IB_MIN_CHUNK ? IB_MIN_CHUNK : (chunk > IB_CHUNK ? IB_CHUNK : chunk);

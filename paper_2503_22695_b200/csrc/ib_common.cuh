@@ -11,7 +11,7 @@
 #define IB_SMALL_TILE 64         // tiles with fewer points skip the tile kernel: their points go one by one (ib_point.cuh); 32/48/80/96/128/192 measured
 #endif
 #ifndef IB_CHUNK
-#define IB_CHUNK 704             // points per work item of the tile kernel = records it stages in shared memory (ib_bin.cu emits the work list)
+#define IB_CHUNK 768             // points per work item of the tile kernel = records it stages in shared memory (ib_bin.cu emits the work list); the largest that two record buffers leave room for (576 ... 768 measured: the larger the better)
 #endif
 #define IB_SLAB0 4                // d_tile_count[IB_SLAB0 + k] = first work item of z-slab k (ib_tile_scan)
 #define IB_MAX_SLABS 32
